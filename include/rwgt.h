@@ -1,0 +1,109 @@
+/* include/rwgt.h — C ABI of the B200-native LO event-reweighting hot path.
+ *
+ * What it computes (arXiv 2312.07440; citations are /root/reference/PAPER.md lines):
+ *   for every stored event, the tree-level squared matrix element |M|^2 under the
+ *   original parameter set and |M'|^2 under the modified one, and the new weight
+ *        W' = W * |M'|^2 / |M|^2                      (§2.2 eq. 3)
+ *   i.e. steps 3-6 of the reweighting procedure of PAPER.md:87 (§3.2), fused into ONE
+ *   kernel launch per call.  |M|^2 is a helicity-amplitude evaluation (PAPER.md:66,
+ *   §3.1): external wavefunctions, vertex/propagator recursion, colour-flow amplitudes,
+ *   colour quadratic form J^dagger C J, helicity sum.  The paper prints none of those
+ *   formulas; the conventions are the readings listed in DESIGN.md ("Readings", from
+ *   SURVEY.md §8(c) C1-C8), and they are binding because the modified model of the
+ *   configs (ggg/gggg couplings rescaled, qqg not) is not gauge invariant (reading Q1).
+ *
+ * Plain C: no exceptions, no C++/torch types cross this boundary.  All event buffers
+ * are DEVICE pointers unless a function says HOST.
+ */
+#ifndef RWGT_H
+#define RWGT_H
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct rwgt_handle rwgt_handle; /* opaque; owned by the library */
+
+/* One physics parameter set (PAPER.md:87 steps 1 and 4: "Input reweight parameters",
+ * "Overwrite physics parameters with new values").  POD, copied by value at create. */
+typedef struct {
+  double alpha_em;    /* electromagnetic coupling, e = sqrt(4 pi alpha_em)               */
+  double alpha_s;     /* strong coupling, g_s = sqrt(4 pi alpha_s)                       */
+  double mZ;          /* Z mass, GeV                                                     */
+  double GammaZ;      /* Z width, GeV (fixed-width Breit-Wigner s - mZ^2 + i mZ GammaZ)  */
+  double sin2_thetaW; /* direct input; cos^2 = 1 - sin^2                                 */
+  double mt;          /* top mass, GeV (used in spinors and propagators)                 */
+  double Gamma_t;     /* top width, GeV; must be 0 (no config uses it; reading Q7)       */
+  double ggg_scale;   /* multiplies the 3-gluon coupling: g_3 = g_s * ggg_scale          */
+  double gggg_scale;  /* multiplies the 4-gluon coupling: g_4 = g_s^2 * gggg_scale       */
+} rwgt_params;
+
+/* Precision modes of rwgt_set_precision. I/O buffers are FP64 in every mode. */
+#define RWGT_FP64 0  /* all arithmetic in double (default)                               */
+#define RWGT_FP32 1  /* all per-event arithmetic in float                                */
+#define RWGT_MIXED 2 /* float vertex algebra; momentum sums, propagator denominators,
+                        helicity/colour accumulation in double                           */
+
+/* Create a handle for one process and one (old, new) pair of parameter sets.
+ *   process: "epem_mupmum" | "gg_ttx" | "gg_ttxg" | "gg_ttxgg" | "gg_ttxggg"
+ *            leg order in `momenta`: [e+,e-,mu+,mu-] resp. [g,g,t,tbar,(g,(g,(g)))];
+ *            legs 0,1 incoming, all momenta physical (E>0).
+ * Builds the per-process tables (ordered-current schedule, colour matrix) on the host and
+ * copies them and the couplings to the CURRENT device.  Returns NULL on error (unknown
+ * process, non-positive alpha, sin2_thetaW outside (0,1), Gamma_t != 0, no CUDA device);
+ * rwgt_last_error() then describes it.  PAPER.md:87 restricts reweighting to parameters
+ * "that can be modified at runtime": old and new share the process. */
+rwgt_handle* rwgt_create(const char* process, const rwgt_params* params_old, const rwgt_params* params_new);
+
+/* 0 on success, -1 on bad handle/mode or a mode the process does not support
+ * (epem_mupmum and gg_ttx are FP64 only). */
+int rwgt_set_precision(rwgt_handle* h, int mode);
+
+/* Number of external legs (4..7), so callers can size `momenta`; -1 on bad handle. */
+int rwgt_n_external(const rwgt_handle* h);
+
+/* Exact count of double- (or single-) precision FMA-pipe instructions per event of the
+ * schedule the kernel executes for this handle in its current mode (FMA, MUL, ADD each
+ * count 1; both parameter sets).  Used for the roofline. */
+double rwgt_flops_per_event(const rwgt_handle* h);
+
+/* The hot path: a1-a7 of SURVEY.md §8(a) in one kernel launch on `stream`.
+ *   momenta   DEVICE, SoA double [n_ext][4][n_events]: momenta[(ip*4+mu)*n_events + ievt],
+ *             mu = (E,px,py,pz), GeV
+ *   weights   DEVICE double [n_events]              original weights W
+ *   out_me_old, out_me_new  DEVICE double [n_events] |M|^2, |M'|^2, summed over helicities
+ *             and colours, averaged over initial helicities/colours and divided by the
+ *             identical-particle factor (reading Q3)
+ *   out_w_new DEVICE double [n_events]              W' of eq. 3
+ *   stream    a cudaStream_t (NULL = default stream).  Work is enqueued; the call does not
+ *             synchronise, allocate, or copy between host and device.
+ * Outputs must not alias inputs or each other.  Caller owns all buffers.
+ * If |M|^2 == 0 (outside the validity condition of PAPER.md:46) the IEEE result of
+ * W * (|M'|^2 / |M|^2) is written (inf/nan); no error is raised.
+ * Returns 0 on success (n_events == 0 is a no-op), -1 on bad argument (NULL pointer,
+ * n_events < 0), otherwise the positive cudaError_t of the launch. */
+int rwgt_run(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old,
+             double* out_me_new, double* out_w_new, long long n_events, void* stream);
+
+/* Same computation with HOST buffers (pageable or pinned): copies the inputs to device
+ * scratch owned by the handle (grown on demand), runs the kernel, copies the three outputs
+ * back and synchronises `stream`.  This is the end-to-end path of bench.py's `e2e` key
+ * (host<->device transfer is part of what a user pays).  Same return codes. */
+int rwgt_run_host(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old,
+                  double* out_me_new, double* out_w_new, long long n_events, void* stream);
+
+/* Frees device tables and scratch. 0 on success, -1 on NULL. */
+int rwgt_destroy(rwgt_handle* h);
+
+/* Thread-local, static storage; never NULL. */
+const char* rwgt_last_error(void);
+
+/* HOST: writes the n! x n! colour matrix C (row-major, permutations of the gluon labels in
+ * lexicographic order) the library uses for a process with n_gluons in 2..5; computed with
+ * the SU(3) Fierz identity in exact integer arithmetic.  Returns n! or -1. */
+int rwgt_colour_matrix(int n_gluons, double* out);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RWGT_H */

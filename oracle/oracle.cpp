@@ -107,9 +107,11 @@ static void chi2(const double p[4], int lam, cd out[2]) {
     if (lam > 0) { out[0] = 0; out[1] = 1; } else { out[0] = -1; out[1] = 0; }
     return;
   }
-  double N = 1.0 / std::sqrt(2.0 * pabs * (pabs + pz));
-  if (lam > 0) { out[0] = N * (pabs + pz); out[1] = N * cd(px, py); }
-  else         { out[0] = N * cd(-px, py); out[1] = N * (pabs + pz); }
+  // |p|+p_z without cancellation for backward legs (SURVEY §7 "exact-axis legs": use the light-cone form)
+  double ppz = (pz >= 0.0) ? pabs + pz : pt2 / (pabs - pz);
+  double N = 1.0 / std::sqrt(2.0 * pabs * ppz);
+  if (lam > 0) { out[0] = N * ppz; out[1] = N * cd(px, py); }
+  else         { out[0] = N * cd(-px, py); out[1] = N * ppz; }
 }
 // u(p,lambda) in the Dirac representation: ( sqrt(E+m) chi_l , l sqrt(E-m) chi_l )
 static Sp spinor_u(const double p[4], double m, int lam) {

@@ -1,0 +1,152 @@
+"""Thin ctypes binding of include/rwgt.h — argument marshalling only; every step of the hot path
+runs in the CUDA kernels of librwgt.so.  Fails loudly when the library is missing or cannot load:
+there is no CPU fallback."""
+from __future__ import annotations
+
+import ctypes as C
+import math
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "librwgt.so")
+
+RWGT_FP64, RWGT_FP32, RWGT_MIXED = 0, 1, 2
+PRECISIONS = {"fp64": RWGT_FP64, "fp32": RWGT_FP32, "mixed": RWGT_MIXED}
+
+EXPORTS = ("rwgt_create", "rwgt_set_precision", "rwgt_n_external", "rwgt_flops_per_event", "rwgt_run",
+           "rwgt_run_host", "rwgt_destroy", "rwgt_last_error", "rwgt_colour_matrix")
+
+
+class rwgt_params(C.Structure):
+    _fields_ = [(k, C.c_double) for k in ("alpha_em", "alpha_s", "mZ", "GammaZ", "sin2_thetaW", "mt",
+                                          "Gamma_t", "ggg_scale", "gggg_scale")]
+
+
+_lib = None
+
+
+def lib():
+    """Load librwgt.so (built by `python -m paper_2312_07440_b200.build` / __graft_entry__.build())."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} not built: run `python paper_2312_07440_b200/build.py` "
+                               "(the reweighting path has no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        vp, dp = C.c_void_p, C.c_void_p
+        L.rwgt_create.argtypes = [C.c_char_p, C.POINTER(rwgt_params), C.POINTER(rwgt_params)]
+        L.rwgt_create.restype = vp
+        L.rwgt_set_precision.argtypes = [vp, C.c_int]
+        L.rwgt_n_external.argtypes = [vp]
+        L.rwgt_flops_per_event.argtypes = [vp]
+        L.rwgt_flops_per_event.restype = C.c_double
+        L.rwgt_run.argtypes = [vp, dp, dp, dp, dp, dp, C.c_longlong, vp]
+        L.rwgt_run_host.argtypes = [vp, dp, dp, dp, dp, dp, C.c_longlong, vp]
+        L.rwgt_destroy.argtypes = [vp]
+        L.rwgt_last_error.restype = C.c_char_p
+        L.rwgt_colour_matrix.argtypes = [C.c_int, dp]
+        _lib = L
+    return _lib
+
+
+def _params(p) -> rwgt_params:
+    if isinstance(p, rwgt_params):
+        return p
+    return rwgt_params(*[float(x) for x in p])
+
+
+def rwgt_last_error() -> str:
+    return lib().rwgt_last_error().decode()
+
+
+def rwgt_create(process: str, params_old, params_new):
+    po, pn = _params(params_old), _params(params_new)
+    h = lib().rwgt_create(process.encode(), C.byref(po), C.byref(pn))
+    if not h:
+        raise RuntimeError(rwgt_last_error())
+    return h
+
+
+def rwgt_set_precision(h, mode) -> None:
+    mode = PRECISIONS.get(mode, mode)
+    if lib().rwgt_set_precision(h, int(mode)) != 0:
+        raise RuntimeError(rwgt_last_error())
+
+
+def rwgt_n_external(h) -> int:
+    return lib().rwgt_n_external(h)
+
+
+def rwgt_flops_per_event(h) -> float:
+    return lib().rwgt_flops_per_event(h)
+
+
+def rwgt_run(h, momenta_ptr: int, weights_ptr: int, out_me_old_ptr: int, out_me_new_ptr: int,
+             out_w_new_ptr: int, n_events: int, stream: int = 0) -> None:
+    """Device pointers (ints, e.g. torch.Tensor.data_ptr()) and a cudaStream_t handle."""
+    rc = lib().rwgt_run(h, momenta_ptr, weights_ptr, out_me_old_ptr, out_me_new_ptr, out_w_new_ptr,
+                        int(n_events), stream or None)
+    if rc != 0:
+        raise RuntimeError(f"rwgt_run rc={rc}: {rwgt_last_error()}")
+
+
+def rwgt_run_host(h, momenta: np.ndarray, weights: np.ndarray, out_me_old: np.ndarray,
+                  out_me_new: np.ndarray, out_w_new: np.ndarray, stream: int = 0) -> None:
+    """Host numpy buffers (float64, C-contiguous); copies in/out inside the call."""
+    n = weights.shape[0]
+    for a in (momenta, weights, out_me_old, out_me_new, out_w_new):
+        assert a.dtype == np.float64 and a.flags.c_contiguous
+    rc = lib().rwgt_run_host(h, momenta.ctypes.data, weights.ctypes.data, out_me_old.ctypes.data,
+                             out_me_new.ctypes.data, out_w_new.ctypes.data, int(n), stream or None)
+    if rc != 0:
+        raise RuntimeError(f"rwgt_run_host rc={rc}: {rwgt_last_error()}")
+
+
+def rwgt_destroy(h) -> None:
+    lib().rwgt_destroy(h)
+
+
+def rwgt_colour_matrix(n_gluons: int) -> np.ndarray:
+    f = math.factorial(n_gluons)
+    out = np.empty((f, f), dtype=np.float64)
+    if lib().rwgt_colour_matrix(n_gluons, out.ctypes.data) != f:
+        raise RuntimeError("rwgt_colour_matrix: bad n_gluons")
+    return out
+
+
+class Reweighter:
+    """Convenience wrapper: one handle, torch device tensors in, torch device tensors out."""
+
+    def __init__(self, process: str, params_old, params_new, precision="fp64"):
+        self.h = rwgt_create(process, params_old, params_new)
+        self.process = process
+        self.n_ext = rwgt_n_external(self.h)
+        rwgt_set_precision(self.h, precision)
+
+    def flops_per_event(self) -> float:
+        return rwgt_flops_per_event(self.h)
+
+    def run(self, momenta, weights, out=None):
+        import torch
+        n = weights.shape[0]
+        assert momenta.is_cuda and momenta.dtype == torch.float64 and momenta.is_contiguous()
+        assert momenta.shape == (self.n_ext, 4, n) and weights.dtype == torch.float64
+        if out is None:
+            out = torch.empty((3, n), dtype=torch.float64, device=momenta.device)
+        st = torch.cuda.current_stream(momenta.device).cuda_stream
+        rwgt_run(self.h, momenta.data_ptr(), weights.data_ptr(), out[0].data_ptr(), out[1].data_ptr(),
+                 out[2].data_ptr(), n, st)
+        return out
+
+    def close(self):
+        if self.h:
+            rwgt_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,30 @@
+"""Build paper_2312_07440_b200/librwgt.so (the C-ABI library of include/rwgt.h) for sm_100a, in-tree."""
+import os
+import subprocess
+import sys
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+CSRC = os.path.join(HERE, "csrc")
+LIB = os.path.join(HERE, "librwgt.so")
+SOURCES = [os.path.join(CSRC, "rwgt_api.cu")]
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("rwgt_math.cuh", "kernels_small.cuh", "bg_engine.cuh")] + [
+    os.path.join(os.path.dirname(HERE), "include", "rwgt.h")]
+NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
+              "-Xcompiler", "-fPIC", "-shared", "--fmad=true"]
+
+
+def up_to_date() -> bool:
+    return os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in DEPS)
+
+
+def build(force: bool = False, verbose: bool = False) -> str:
+    if not force and up_to_date():
+        return LIB
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SOURCES
+    subprocess.check_call(cmd)
+    return LIB
+
+
+if __name__ == "__main__":
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -1,0 +1,141 @@
+// kernels_small.cuh — one-event-per-thread FP64 kernels for the two 2->2 processes.
+//   cfg 1  e+ e- -> gamma/Z -> mu+ mu-   (2 diagrams, ncol = 1)
+//   cfg 2  g g -> t tbar                 (SURVEY §8(c) C5/C6 with n = 2; 3 diagrams, ncol = 2)
+// Steps a1-a7 of SURVEY §8(a) in one launch: coalesced SoA loads, external wavefunctions,
+// vertices, colour form, helicity sum, eq. 3, three coalesced stores.
+#pragma once
+#include "rwgt_math.cuh"
+
+namespace rwgt {
+
+// ------------------------------------------------------------------------------------- cfg 1
+struct EpemSet {          // per parameter set, prepared on the host
+  double e2;              // e^2 = 4 pi alpha
+  double gz2;             // g_Z^2 = e^2 / (sW^2 cW^2)
+  double gL, gR;          // -1/2 + sW^2, sW^2
+  double mZ2, mZGZ;       // mZ^2, mZ*GammaZ
+};
+struct EpemParams { EpemSet set[2]; };
+
+// chi_a^dagger sigma^mu chi_b (bar=false) or chi_a^dagger sigmabar^mu chi_b (bar=true)
+__device__ __forceinline__ vec4<double> bilinear2(const cx<double>* a, const cx<double>* b, bool barred) {
+  cx<double> a0 = conj(a[0]), a1 = conj(a[1]);
+  cx<double> t00 = a0 * b[0], t11 = a1 * b[1], t01 = a0 * b[1], t10 = a1 * b[0];
+  vec4<double> r; double s = barred ? -1.0 : 1.0;
+  r.c[0] = t00 + t11;
+  r.c[1] = s * (t01 + t10);                                   // sigma_x
+  cx<double> d = t01 - t10; r.c[2] = s * mk<double>(d.im, -d.re);   // sigma_y: -i t01 + i t10
+  r.c[3] = s * (t00 - t11);                                   // sigma_z
+  return r;
+}
+
+// Massless leptons: only the 4 helicity combinations with opposite helicities on each fermion line
+// are non-zero (tests check the oracle's full 16-term sum against this, reading Q5).
+__global__ void __launch_bounds__(256) epem_mupmum_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
+                                                          double* __restrict__ me_old, double* __restrict__ me_new,
+                                                          double* __restrict__ w_new, long long n, EpemParams P) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double p[4][4];
+#pragma unroll
+  for (int ip = 0; ip < 4; ip++)
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) p[ip][mu] = __ldg(mom + (size_t)(ip * 4 + mu) * n + i);
+  double W = __ldg(wgt + i);
+  double q[4] = {p[0][0] + p[1][0], p[0][1] + p[1][1], p[0][2] + p[1][2], p[0][3] + p[1][3]};
+  double s = mdot_rr(q, q);
+  chi_pair<double> x1 = make_chi(p[0][1], p[0][2], p[0][3]), x2 = make_chi(p[1][1], p[1][2], p[1][3]);
+  chi_pair<double> x3 = make_chi(p[2][1], p[2][2], p[2][3]), x4 = make_chi(p[3][1], p[3][2], p[3][3]);
+  // massless: sqrt(E+|p|) with |p| from the 3-momentum (mass parameter 0, reading Q8)
+  double ce = sqrt((p[0][0] + x1.pabs) * (p[1][0] + x2.pabs)), cm = sqrt((p[2][0] + x3.pabs) * (p[3][0] + x4.pabs));
+  // electron line vbar(p1) gamma^mu u(p2): L = (lam1,lam2) = (+,-), R = (-,+)
+  vec4<double> JeL = bilinear2(x1.m, x2.m, true), JeR = bilinear2(x1.p, x2.p, false);
+  // muon line ubar(p4) gamma^mu v(p3): L = (lam3,lam4) = (+,-), R = (-,+)
+  vec4<double> JmL = bilinear2(x4.m, x3.m, true), JmR = bilinear2(x4.p, x3.p, false);
+  double c2 = ce * cm; c2 *= c2;
+  double dLL = norm2(mdot_cc(JeL, JmL)) * c2, dLR = norm2(mdot_cc(JeL, JmR)) * c2;
+  double dRL = norm2(mdot_cc(JeR, JmL)) * c2, dRR = norm2(mdot_cc(JeR, JmR)) * c2;
+  double me[2];
+#pragma unroll
+  for (int k = 0; k < 2; k++) {
+    const EpemSet& S = P.set[k];
+    // photon e^2/s (Q_e Q_mu = +1) plus Z g_Z^2 g_a g_b / (s - mZ^2 + i mZ GammaZ)
+    double dr = s - S.mZ2, di = S.mZGZ, inv = 1.0 / (dr * dr + di * di);
+    double zr = S.gz2 * dr * inv, zi = -S.gz2 * di * inv, ph = S.e2 / s;
+    double fLL = norm2(mk<double>(ph + S.gL * S.gL * zr, S.gL * S.gL * zi));
+    double fLR = norm2(mk<double>(ph + S.gL * S.gR * zr, S.gL * S.gR * zi));
+    double fRR = norm2(mk<double>(ph + S.gR * S.gR * zr, S.gR * S.gR * zi));
+    me[k] = 0.25 * (fLL * dLL + fLR * (dLR + dRL) + fRR * dRR);
+  }
+  me_old[i] = me[0]; me_new[i] = me[1]; w_new[i] = W * (me[1] / me[0]);
+}
+
+// ------------------------------------------------------------------------------------- cfg 2
+struct GGttxParams {
+  double mt[2];           // top mass per set
+  double fac[2];          // g_s^4 / 256 per set (averaging denominator D = 4*64)
+  double s3[2];           // ggg_scale per set
+  int two_pass;           // masses differ: evaluate each set with its own mass
+};
+
+// Helicity-summed colour forms for ONE mass and two values of the ggg scale.
+//   M = i g_s^2 [ (T^a T^b)(X12 + s3 Y) + (T^b T^a)(X21 - s3 Y) ]
+//   X12 = ubar e1-slash Psi(2), Psi(i) = -(q_i-slash + m) e_i-slash v / (q_i^2 - m^2), q_i = k_i - p_tbar
+//   Y   = -(1/s) ubar L3-slash(e1,k1;e2,k2) v
+// Parity (|M_{-h}|^2 = |M_h|^2, tests/test_oracle_pins.py) halves the helicity loop: lam1 = +1 only, x2.
+__device__ __forceinline__ void ggttx_sums(const double (*p)[4], double m, double sa, double sb, double& sum_a, double& sum_b) {
+  const double* k1 = p[0]; const double* k2 = p[1];
+  double q1[4], q2[4], kk[4];
+#pragma unroll
+  for (int mu = 0; mu < 4; mu++) { q1[mu] = k1[mu] - p[3][mu]; q2[mu] = k2[mu] - p[3][mu]; kk[mu] = k1[mu] + k2[mu]; }
+  double m2 = m * m;
+  double d1 = -1.0 / (mdot_rr(q1, q1) - m2), d2 = -1.0 / (mdot_rr(q2, q2) - m2), ds = -1.0 / mdot_rr(kk, kk);
+  chi_pair<double> xt = make_chi(p[2][1], p[2][2], p[2][3]), xb = make_chi(p[3][1], p[3][2], p[3][3]);
+  sum_a = 0; sum_b = 0;
+  const int l1 = +1;
+  vec4<double> e1 = polvec(k1[1], k1[2], k1[3], l1);
+#pragma unroll
+  for (int i2 = 0; i2 < 2; i2++) {
+    int l2 = i2 ? -1 : +1;
+    vec4<double> e2 = polvec(k2[1], k2[2], k2[3], l2);
+    vec4<double> l3; for (int mu = 0; mu < 4; mu++) l3.c[mu] = mk<double>(0, 0);
+    L3_acc(l3, ds, e1, k1, e2, k2);
+#pragma unroll
+    for (int ib = 0; ib < 2; ib++) {
+      spn<double> v = spinor_v(xb, p[3][0], m, ib ? -1 : +1);
+      spn<double> psi1 = slash_r_plus_m(q1, m, slash_c(e1, v)), psi2 = slash_r_plus_m(q2, m, slash_c(e2, v));
+      spn<double> c12 = slash_c(e1, psi2), c21 = slash_c(e2, psi1), cy = slash_c(l3, v);
+#pragma unroll
+      for (int it = 0; it < 2; it++) {
+        spn<double> ub = bar(spinor_u(xt, p[2][0], m, it ? -1 : +1));
+        cx<double> X12 = d2 * rowcol(ub, c12), X21 = d1 * rowcol(ub, c21), Y = rowcol(ub, cy);
+        cx<double> A1 = X12, A2 = X21; rfma(A1, sa, Y); rfma(A2, -sa, Y);
+        sum_a += 16.0 * (norm2(A1) + norm2(A2)) - 4.0 * (A1.re * A2.re + A1.im * A2.im);
+        cx<double> B1 = X12, B2 = X21; rfma(B1, sb, Y); rfma(B2, -sb, Y);
+        sum_b += 16.0 * (norm2(B1) + norm2(B2)) - 4.0 * (B1.re * B2.re + B1.im * B2.im);
+      }
+    }
+  }
+  // colour matrix (16,-2;-2,16)/3, parity factor 2
+  sum_a *= 2.0 / 3.0; sum_b *= 2.0 / 3.0;
+}
+
+__global__ void __launch_bounds__(128) gg_ttx_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
+                                                     double* __restrict__ me_old, double* __restrict__ me_new,
+                                                     double* __restrict__ w_new, long long n, GGttxParams P) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double p[4][4];
+#pragma unroll
+  for (int ip = 0; ip < 4; ip++)
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) p[ip][mu] = __ldg(mom + (size_t)(ip * 4 + mu) * n + i);
+  double W = __ldg(wgt + i);
+  double a, b;
+  if (!P.two_pass) ggttx_sums(p, P.mt[0], P.s3[0], P.s3[1], a, b);
+  else { double t; ggttx_sums(p, P.mt[0], P.s3[0], P.s3[0], a, t); ggttx_sums(p, P.mt[1], P.s3[1], P.s3[1], t, b); }
+  a *= P.fac[0]; b *= P.fac[1];
+  me_old[i] = a; me_new[i] = b; w_new[i] = W * (b / a);
+}
+
+}  // namespace rwgt

@@ -1,0 +1,187 @@
+// rwgt_api.cu — C ABI of include/rwgt.h: handle management, parameter preparation, kernel dispatch.
+#include <cuda_runtime.h>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/rwgt.h"
+#include "kernels_small.cuh"
+#include "bg_engine.cuh"
+
+namespace {
+
+thread_local char g_err[512] = "";
+void set_err(const char* fmt, const char* a = "") { std::snprintf(g_err, sizeof(g_err), fmt, a); }
+
+enum Proc { P_EPEM = 0, P_GG_TTX = 1, P_BG = 2 };
+const double PI = 3.14159265358979323846;
+
+}  // namespace
+
+struct rwgt_handle {
+  int proc;
+  int n_ext;
+  int n_gluons;
+  int precision;
+  int device;
+  rwgt_params po, pn;
+  rwgt::EpemParams epem;
+  rwgt::GGttxParams ggttx;
+  rwgt::BgProcess* bg;        // ordered-current engine (n_gluons >= 3, or gg_ttx when forced)
+  // device scratch for rwgt_run_host
+  double* scratch;
+  size_t scratch_bytes;
+};
+
+static bool valid_params(const rwgt_params* p) {
+  if (!p) return false;
+  if (!(p->alpha_em > 0) || !(p->alpha_s > 0)) return false;
+  if (!(p->sin2_thetaW > 0 && p->sin2_thetaW < 1)) return false;
+  if (!(p->mZ > 0) || !(p->GammaZ >= 0) || !(p->mt >= 0)) return false;
+  if (p->Gamma_t != 0.0) return false;
+  if (!std::isfinite(p->ggg_scale) || !std::isfinite(p->gggg_scale)) return false;
+  return true;
+}
+
+static rwgt::EpemSet make_epem(const rwgt_params& p) {
+  rwgt::EpemSet s;
+  s.e2 = 4.0 * PI * p.alpha_em;
+  s.gz2 = s.e2 / (p.sin2_thetaW * (1.0 - p.sin2_thetaW));
+  s.gL = -0.5 + p.sin2_thetaW;
+  s.gR = p.sin2_thetaW;
+  s.mZ2 = p.mZ * p.mZ;
+  s.mZGZ = p.mZ * p.GammaZ;
+  return s;
+}
+
+extern "C" {
+
+const char* rwgt_last_error(void) { return g_err; }
+
+rwgt_handle* rwgt_create(const char* process, const rwgt_params* params_old, const rwgt_params* params_new) {
+  if (!process || !params_old || !params_new) { set_err("rwgt_create: NULL argument"); return nullptr; }
+  if (!valid_params(params_old) || !valid_params(params_new)) { set_err("rwgt_create: invalid parameter set for %s", process); return nullptr; }
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); set_err("rwgt_create: no CUDA device (this library has no CPU path)"); return nullptr; }
+  rwgt_handle* h = new (std::nothrow) rwgt_handle();
+  if (!h) { set_err("rwgt_create: out of memory"); return nullptr; }
+  h->proc = -1; h->po = *params_old; h->pn = *params_new; h->precision = RWGT_FP64; h->bg = nullptr; h->scratch = nullptr; h->scratch_bytes = 0;
+  cudaGetDevice(&h->device);
+  std::string p(process);
+  // "@bg" suffix routes gg_ttx through the generic ordered-current engine (used by the tests to cross-check it)
+  bool force_bg = false;
+  if (p.size() > 3 && p.compare(p.size() - 3, 3, "@bg") == 0) { force_bg = true; p.resize(p.size() - 3); }
+  int ng = -1;
+  if (p == "epem_mupmum") { h->proc = P_EPEM; h->n_ext = 4; h->n_gluons = 0; }
+  else if (p == "gg_ttx") { ng = 2; }
+  else if (p == "gg_ttxg") { ng = 3; }
+  else if (p == "gg_ttxgg") { ng = 4; }
+  else if (p == "gg_ttxggg") { ng = 5; }
+  else { set_err("rwgt_create: unknown process '%s'", process); delete h; return nullptr; }
+  if (h->proc == P_EPEM) {
+    h->epem.set[0] = make_epem(h->po); h->epem.set[1] = make_epem(h->pn);
+    return h;
+  }
+  h->n_gluons = ng; h->n_ext = ng + 2;
+  if (ng == 2 && !force_bg) {
+    h->proc = P_GG_TTX;
+    const rwgt_params* ps[2] = {&h->po, &h->pn};
+    for (int k = 0; k < 2; k++) {
+      double gs2 = 4.0 * PI * ps[k]->alpha_s;
+      h->ggttx.mt[k] = ps[k]->mt; h->ggttx.fac[k] = gs2 * gs2 / 256.0; h->ggttx.s3[k] = ps[k]->ggg_scale;
+    }
+    h->ggttx.two_pass = (h->po.mt != h->pn.mt) ? 1 : 0;
+    return h;
+  }
+  h->proc = P_BG;
+  std::string err;
+  h->bg = rwgt::bg_create(ng, h->po, h->pn, err);
+  if (!h->bg) { set_err("rwgt_create: %s", err.c_str()); delete h; return nullptr; }
+  return h;
+}
+
+int rwgt_set_precision(rwgt_handle* h, int mode) {
+  if (!h || mode < 0 || mode > 2) { set_err("rwgt_set_precision: bad argument"); return -1; }
+  if (h->proc != P_BG && mode != RWGT_FP64) { set_err("rwgt_set_precision: this process is FP64 only"); return -1; }
+  h->precision = mode;
+  return 0;
+}
+
+int rwgt_n_external(const rwgt_handle* h) { return h ? h->n_ext : -1; }
+
+double rwgt_flops_per_event(const rwgt_handle* h) {
+  if (!h) return -1.0;
+  if (h->proc == P_EPEM) return 330.0;      // counted from the SASS of epem_mupmum_kernel
+  if (h->proc == P_GG_TTX) return h->ggttx.two_pass ? 2.0 * 2150.0 : 2150.0;
+  return rwgt::bg_flops_per_event(h->bg, h->precision);
+}
+
+int rwgt_run(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old, double* out_me_new,
+             double* out_w_new, long long n_events, void* stream) {
+  if (!h || n_events < 0) { set_err("rwgt_run: bad handle or n_events < 0"); return -1; }
+  if (n_events == 0) return 0;
+  if (!momenta || !weights || !out_me_old || !out_me_new || !out_w_new) { set_err("rwgt_run: NULL buffer"); return -1; }
+  cudaStream_t st = (cudaStream_t)stream;
+  if (h->proc == P_EPEM) {
+    int bs = 256; long long nb = (n_events + bs - 1) / bs;
+    rwgt::epem_mupmum_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n_events, h->epem);
+  } else if (h->proc == P_GG_TTX) {
+    int bs = 128; long long nb = (n_events + bs - 1) / bs;
+    rwgt::gg_ttx_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n_events, h->ggttx);
+  } else {
+    int rc = rwgt::bg_run(h->bg, h->precision, momenta, weights, out_me_old, out_me_new, out_w_new, n_events, st);
+    if (rc != 0) { set_err("rwgt_run: engine launch failed"); return rc; }
+  }
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { set_err("rwgt_run: %s", cudaGetErrorString(e)); return (int)e; }
+  return 0;
+}
+
+int rwgt_run_host(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old, double* out_me_new,
+                  double* out_w_new, long long n_events, void* stream) {
+  if (!h || n_events < 0) { set_err("rwgt_run_host: bad handle or n_events < 0"); return -1; }
+  if (n_events == 0) return 0;
+  if (!momenta || !weights || !out_me_old || !out_me_new || !out_w_new) { set_err("rwgt_run_host: NULL buffer"); return -1; }
+  cudaStream_t st = (cudaStream_t)stream;
+  size_t n = (size_t)n_events, nin = (size_t)h->n_ext * 4 * n, need = (nin + 4 * n) * sizeof(double);
+  cudaError_t e;
+  if (need > h->scratch_bytes) {
+    if (h->scratch) cudaFree(h->scratch);
+    h->scratch = nullptr; h->scratch_bytes = 0;
+    e = cudaMalloc((void**)&h->scratch, need);
+    if (e != cudaSuccess) { set_err("rwgt_run_host: %s", cudaGetErrorString(e)); return (int)e; }
+    h->scratch_bytes = need;
+  }
+  double* d_mom = h->scratch; double* d_w = d_mom + nin; double* d_a = d_w + n; double* d_b = d_a + n; double* d_o = d_b + n;
+  cudaMemcpyAsync(d_mom, momenta, nin * sizeof(double), cudaMemcpyHostToDevice, st);
+  cudaMemcpyAsync(d_w, weights, n * sizeof(double), cudaMemcpyHostToDevice, st);
+  int rc = rwgt_run(h, d_mom, d_w, d_a, d_b, d_o, n_events, stream);
+  if (rc != 0) return rc;
+  cudaMemcpyAsync(out_me_old, d_a, n * sizeof(double), cudaMemcpyDeviceToHost, st);
+  cudaMemcpyAsync(out_me_new, d_b, n * sizeof(double), cudaMemcpyDeviceToHost, st);
+  cudaMemcpyAsync(out_w_new, d_o, n * sizeof(double), cudaMemcpyDeviceToHost, st);
+  e = cudaStreamSynchronize(st);
+  if (e != cudaSuccess) { set_err("rwgt_run_host: %s", cudaGetErrorString(e)); return (int)e; }
+  return 0;
+}
+
+int rwgt_destroy(rwgt_handle* h) {
+  if (!h) return -1;
+  if (h->bg) rwgt::bg_destroy(h->bg);
+  if (h->scratch) cudaFree(h->scratch);
+  delete h;
+  return 0;
+}
+
+int rwgt_colour_matrix(int n_gluons, double* out) {
+  if (n_gluons < 2 || n_gluons > 5 || !out) return -1;
+  std::vector<double> C = rwgt::colour_matrix_fierz(n_gluons);
+  std::memcpy(out, C.data(), C.size() * sizeof(double));
+  int f = 1; for (int i = 2; i <= n_gluons; i++) f *= i;
+  return f;
+}
+
+}  // extern "C"

@@ -1,0 +1,148 @@
+// rwgt_math.cuh — device arithmetic of the helicity-amplitude evaluation (§3.1),
+// hand-specialised for the CHIRAL representation with two-component blocks.
+// Conventions: DESIGN.md "Readings".  Metric (+,-,-,-).
+//   gamma^0 = [[0,1],[1,0]], gamma^i = [[0,s^i],[-s^i,0]];  spinor = (psi0,psi1 | psi2,psi3)
+//   a-slash = [[0, a0 - s.a],[a0 + s.a, 0]]
+// Shares nothing with oracle/ (which uses generic 4x4 Dirac-representation matrices).
+#pragma once
+#include <cuda_runtime.h>
+
+namespace rwgt {
+
+template <typename T> struct cx { T re, im; };
+template <typename T> __device__ __forceinline__ cx<T> mk(T a, T b) { cx<T> r; r.re = a; r.im = b; return r; }
+template <typename T> __device__ __forceinline__ cx<T> operator+(cx<T> a, cx<T> b) { return mk<T>(a.re + b.re, a.im + b.im); }
+template <typename T> __device__ __forceinline__ cx<T> operator-(cx<T> a, cx<T> b) { return mk<T>(a.re - b.re, a.im - b.im); }
+template <typename T> __device__ __forceinline__ cx<T> operator-(cx<T> a) { return mk<T>(-a.re, -a.im); }
+template <typename T> __device__ __forceinline__ cx<T> operator*(cx<T> a, cx<T> b) { return mk<T>(a.re * b.re - a.im * b.im, a.re * b.im + a.im * b.re); }
+template <typename T> __device__ __forceinline__ cx<T> operator*(T s, cx<T> a) { return mk<T>(s * a.re, s * a.im); }
+template <typename T> __device__ __forceinline__ cx<T> conj(cx<T> a) { return mk<T>(a.re, -a.im); }
+template <typename T> __device__ __forceinline__ T norm2(cx<T> a) { return a.re * a.re + a.im * a.im; }
+// acc += a*b  (4 FMA)
+template <typename T> __device__ __forceinline__ void cfma(cx<T>& acc, cx<T> a, cx<T> b) {
+  acc.re = fma(a.re, b.re, acc.re); acc.re = fma(-a.im, b.im, acc.re);
+  acc.im = fma(a.re, b.im, acc.im); acc.im = fma(a.im, b.re, acc.im);
+}
+// acc += s*a  (2 FMA), s real
+template <typename T> __device__ __forceinline__ void rfma(cx<T>& acc, T s, cx<T> a) { acc.re = fma(s, a.re, acc.re); acc.im = fma(s, a.im, acc.im); }
+
+template <typename T> struct vec4 { cx<T> c[4]; };   // complex Lorentz vector, contravariant (t,x,y,z)
+template <typename T> struct spn { cx<T> c[4]; };    // Dirac spinor, chiral representation
+
+template <typename T> __device__ __forceinline__ T mdot_rr(const T* a, const T* b) { return a[0] * b[0] - a[1] * b[1] - a[2] * b[2] - a[3] * b[3]; }
+template <typename T> __device__ __forceinline__ cx<T> mdot_rc(const T* a, const vec4<T>& b) {
+  cx<T> r = a[0] * b.c[0]; rfma(r, -a[1], b.c[1]); rfma(r, -a[2], b.c[2]); rfma(r, -a[3], b.c[3]); return r;
+}
+template <typename T> __device__ __forceinline__ cx<T> mdot_cc(const vec4<T>& a, const vec4<T>& b) {
+  cx<T> r = a.c[0] * b.c[0]; cfma(r, -a.c[1], b.c[1]); cfma(r, -a.c[2], b.c[2]); cfma(r, -a.c[3], b.c[3]); return r;
+}
+
+// a-slash * psi, a complex
+template <typename T> __device__ __forceinline__ spn<T> slash_c(const vec4<T>& a, const spn<T>& s) {
+  cx<T> ap = a.c[0] + a.c[3], am = a.c[0] - a.c[3];
+  cx<T> ar = mk<T>(a.c[1].re + a.c[2].im, a.c[1].im - a.c[2].re);   // a1 - i a2
+  cx<T> al = mk<T>(a.c[1].re - a.c[2].im, a.c[1].im + a.c[2].re);   // a1 + i a2
+  spn<T> r;
+  r.c[0] = am * s.c[2]; cfma(r.c[0], -ar, s.c[3]);
+  r.c[1] = ap * s.c[3]; cfma(r.c[1], -al, s.c[2]);
+  r.c[2] = ap * s.c[0]; cfma(r.c[2], ar, s.c[1]);
+  r.c[3] = am * s.c[1]; cfma(r.c[3], al, s.c[0]);
+  return r;
+}
+// (q-slash + m) * psi, q real
+template <typename T> __device__ __forceinline__ spn<T> slash_r_plus_m(const T* q, T m, const spn<T>& s) {
+  T qp = q[0] + q[3], qm = q[0] - q[3];
+  cx<T> qr = mk<T>(q[1], -q[2]), ql = mk<T>(q[1], q[2]);
+  spn<T> r;
+  r.c[0] = m * s.c[0]; rfma(r.c[0], qm, s.c[2]); cfma(r.c[0], -qr, s.c[3]);
+  r.c[1] = m * s.c[1]; rfma(r.c[1], qp, s.c[3]); cfma(r.c[1], -ql, s.c[2]);
+  r.c[2] = m * s.c[2]; rfma(r.c[2], qp, s.c[0]); cfma(r.c[2], qr, s.c[1]);
+  r.c[3] = m * s.c[3]; rfma(r.c[3], qm, s.c[1]); cfma(r.c[3], ql, s.c[0]);
+  return r;
+}
+// row * (a-slash), a complex: psibar-type rows
+template <typename T> __device__ __forceinline__ spn<T> row_slash_c(const spn<T>& w, const vec4<T>& a) {
+  cx<T> ap = a.c[0] + a.c[3], am = a.c[0] - a.c[3];
+  cx<T> ar = mk<T>(a.c[1].re + a.c[2].im, a.c[1].im - a.c[2].re);
+  cx<T> al = mk<T>(a.c[1].re - a.c[2].im, a.c[1].im + a.c[2].re);
+  spn<T> r;   // r_j = sum_i w_i A_ij ; A = [[0,0,am,-ar],[0,0,-al,ap],[ap,ar,0,0],[al,am,0,0]]
+  r.c[0] = w.c[2] * ap; cfma(r.c[0], w.c[3], al);
+  r.c[1] = w.c[2] * ar; cfma(r.c[1], w.c[3], am);
+  r.c[2] = w.c[0] * am; cfma(r.c[2], -w.c[1], al);
+  r.c[3] = w.c[1] * ap; cfma(r.c[3], -w.c[0], ar);
+  return r;
+}
+// row * (q-slash + m), q real
+template <typename T> __device__ __forceinline__ spn<T> row_slash_r_plus_m(const spn<T>& w, const T* q, T m) {
+  T qp = q[0] + q[3], qm = q[0] - q[3];
+  cx<T> qr = mk<T>(q[1], -q[2]), ql = mk<T>(q[1], q[2]);
+  spn<T> r;
+  r.c[0] = m * w.c[0]; rfma(r.c[0], qp, w.c[2]); cfma(r.c[0], w.c[3], ql);
+  r.c[1] = m * w.c[1]; rfma(r.c[1], qm, w.c[3]); cfma(r.c[1], w.c[2], qr);
+  r.c[2] = m * w.c[2]; rfma(r.c[2], qm, w.c[0]); cfma(r.c[2], -w.c[1], ql);
+  r.c[3] = m * w.c[3]; rfma(r.c[3], qp, w.c[1]); cfma(r.c[3], -w.c[0], qr);
+  return r;
+}
+template <typename T> __device__ __forceinline__ cx<T> rowcol(const spn<T>& w, const spn<T>& s) {
+  cx<T> r = w.c[0] * s.c[0]; cfma(r, w.c[1], s.c[1]); cfma(r, w.c[2], s.c[2]); cfma(r, w.c[3], s.c[3]); return r;
+}
+
+// ---- external wavefunctions -------------------------------------------------------
+// two-component helicity eigenspinors chi_+, chi_- of direction p_vec; exact on the beam axis.
+template <typename T> struct chi_pair { cx<T> p[2], m[2]; T pabs; };
+template <typename T> __device__ __forceinline__ chi_pair<T> make_chi(T px, T py, T pz) {
+  chi_pair<T> r; T pt2 = px * px + py * py; T pabs = sqrt(pt2 + pz * pz); r.pabs = pabs;
+  if (pabs == T(0)) { r.p[0] = mk<T>(1, 0); r.p[1] = mk<T>(0, 0); r.m[0] = mk<T>(0, 0); r.m[1] = mk<T>(1, 0); return r; }
+  if (pt2 == T(0) && pz < T(0)) { r.p[0] = mk<T>(0, 0); r.p[1] = mk<T>(1, 0); r.m[0] = mk<T>(-1, 0); r.m[1] = mk<T>(0, 0); return r; }
+  T ppz = (pz >= T(0)) ? pabs + pz : pt2 / (pabs - pz);     // |p|+pz, cancellation-free
+  T N = T(1) / sqrt(T(2) * pabs * ppz);
+  r.p[0] = mk<T>(N * ppz, 0); r.p[1] = mk<T>(N * px, N * py);
+  r.m[0] = mk<T>(-N * px, N * py); r.m[1] = mk<T>(N * ppz, 0);
+  return r;
+}
+// u(p,lam) = ( sqrt(E-lam|p|) chi_lam , sqrt(E+lam|p|) chi_lam )
+template <typename T> __device__ __forceinline__ spn<T> spinor_u(const chi_pair<T>& x, T E, T m, int lam) {
+  T sp = sqrt(E + x.pabs), sm = (m == T(0)) ? T(0) : m / sp;
+  const cx<T>* c = lam > 0 ? x.p : x.m; T a = lam > 0 ? sm : sp, b = lam > 0 ? sp : sm;
+  spn<T> r; r.c[0] = a * c[0]; r.c[1] = a * c[1]; r.c[2] = b * c[0]; r.c[3] = b * c[1]; return r;
+}
+// v(p,lam) = ( -lam sqrt(E+lam|p|) chi_{-lam} , lam sqrt(E-lam|p|) chi_{-lam} )
+template <typename T> __device__ __forceinline__ spn<T> spinor_v(const chi_pair<T>& x, T E, T m, int lam) {
+  T sp = sqrt(E + x.pabs), sm = (m == T(0)) ? T(0) : m / sp;
+  const cx<T>* c = lam > 0 ? x.m : x.p; T a = lam > 0 ? -sp : sm, b = lam > 0 ? sm : -sp;
+  spn<T> r; r.c[0] = a * c[0]; r.c[1] = a * c[1]; r.c[2] = b * c[0]; r.c[3] = b * c[1]; return r;
+}
+// psibar = psi^dagger gamma^0 as a row
+template <typename T> __device__ __forceinline__ spn<T> bar(const spn<T>& s) {
+  spn<T> r; r.c[0] = conj(s.c[2]); r.c[1] = conj(s.c[3]); r.c[2] = conj(s.c[0]); r.c[3] = conj(s.c[1]); return r;
+}
+// eps(p,lam) = (0, (-lam e1 - i e2)/sqrt2), spatial-transverse in the given frame (binding, reading Q1)
+template <typename T> __device__ __forceinline__ vec4<T> polvec(T px, T py, T pz, int lam) {
+  T pt2 = px * px + py * py, pt = sqrt(pt2), pabs = sqrt(pt2 + pz * pz);
+  T e1x, e1y, e1z, e2x, e2y;
+  if (pt == T(0)) { e1x = pz >= T(0) ? T(1) : T(-1); e1y = 0; e1z = 0; e2x = 0; e2y = 1; }
+  else { T inv = T(1) / (pabs * pt); e1x = px * pz * inv; e1y = py * pz * inv; e1z = -pt2 * inv; T ip = T(1) / pt; e2x = -py * ip; e2y = px * ip; }
+  const T s = T(0.70710678118654752440); T l = T(lam);
+  vec4<T> r; r.c[0] = mk<T>(0, 0); r.c[1] = mk<T>(-l * s * e1x, -s * e2x); r.c[2] = mk<T>(-l * s * e1y, -s * e2y); r.c[3] = mk<T>(-l * s * e1z, 0);
+  return r;
+}
+template <typename T> __device__ __forceinline__ vec4<T> conj4(const vec4<T>& a) { vec4<T> r; for (int i = 0; i < 4; i++) r.c[i] = conj(a.c[i]); return r; }
+
+// ---- gluon self-interaction Lorentz structures --------------------------------------
+// L3(A,B) = (JA.JB)(KA-KB) + JB ((KA+2KB).JA) - JA ((2KA+KB).JB)
+template <typename T> __device__ __forceinline__ void L3_acc(vec4<T>& acc, T sgn, const vec4<T>& JA, const T* KA, const vec4<T>& JB, const T* KB) {
+  T d[4], u[4], w[4];
+#pragma unroll
+  for (int i = 0; i < 4; i++) { d[i] = KA[i] - KB[i]; u[i] = KA[i] + T(2) * KB[i]; w[i] = T(2) * KA[i] + KB[i]; }
+  cx<T> ab = sgn * mdot_cc(JA, JB), c1 = sgn * mdot_rc(u, JA), c2 = (-sgn) * mdot_rc(w, JB);
+#pragma unroll
+  for (int i = 0; i < 4; i++) { rfma(acc.c[i], d[i], ab); cfma(acc.c[i], c1, JB.c[i]); cfma(acc.c[i], c2, JA.c[i]); }
+}
+// colour-ordered quartic structure V4(X,Y,Z) = 2 (X.Z) Y - (Y.Z) X - (X.Y) Z
+template <typename T> __device__ __forceinline__ void V4_acc(vec4<T>& acc, T sgn, const vec4<T>& X, const vec4<T>& Y, const vec4<T>& Z) {
+  cx<T> xz = (T(2) * sgn) * mdot_cc(X, Z), yz = (-sgn) * mdot_cc(Y, Z), xy = (-sgn) * mdot_cc(X, Y);
+#pragma unroll
+  for (int i = 0; i < 4; i++) { cfma(acc.c[i], xz, Y.c[i]); cfma(acc.c[i], yz, X.c[i]); cfma(acc.c[i], xy, Z.c[i]); }
+}
+
+}  // namespace rwgt
