@@ -237,6 +237,7 @@ template <typename T> struct Smem {
   T* dR; T* dL;   // [nslot][32] 1/(q^2-m^2)
   T* A;           // [nslot][nperm][ncol][2]
   double* acc;    // [nslot][2]
+  double* red;    // [nslot][8] per-warp partial sums of the colour form
 };
 
 template <typename T> __device__ __forceinline__ vec4<T> ld4(const T* tab, int stride, int e) {
@@ -293,6 +294,7 @@ template <typename T> __device__ __forceinline__ void carve(Smem<T>& s, unsigned
   size_t off = 0; int ns = D.nslot;
   s.pm = (double*)(base + off); off += sizeof(double) * ns * (D.n + 2) * 4;
   s.acc = (double*)(base + off); off += sizeof(double) * ns * 2;
+  s.red = (double*)(base + off); off += sizeof(double) * ns * 8;
   s.G = (T*)(base + off); off += sizeof(T) * ns * 8 * D.nG;
   s.R = (T*)(base + off); off += sizeof(T) * ns * 8 * D.nR;
   s.L = (T*)(base + off); off += sizeof(T) * ns * 8 * D.nL;
@@ -305,7 +307,7 @@ template <typename T> __device__ __forceinline__ void carve(Smem<T>& s, unsigned
 }
 static size_t smem_bytes(const BgSched& S, int nslot, size_t sz) {
   size_t off = 0;
-  off += sizeof(double) * nslot * (S.n + 2) * 4 + sizeof(double) * nslot * 2;
+  off += sizeof(double) * nslot * (S.n + 2) * 4 + sizeof(double) * nslot * 10;
   off += sz * nslot * 8 * (size_t)(S.nG + S.nR + S.nL);
   off += sz * nslot * 32 * 7;
   off = (off + 15) & ~(size_t)15;
@@ -493,7 +495,7 @@ __global__ void __launch_bounds__(256, 1) bg_kernel(const double* __restrict__ m
           for (int t = tid; t < ns * percf; t += nth) {
             int sl = t / percf, o = t % percf; int chunk = o / ncol, col = o % ncol;
             const T* A = s.A + (size_t)sl * nperm * ncol * 2;
-            int r0 = chunk * RB, nr = min(RB, nperm - r0);
+            int r0 = chunk * RB, nr = max(0, min(RB, nperm - r0));
             double part = 0.0;
             if (sizeof(T) == 8) {
               const double* C = D.C64;
@@ -528,8 +530,14 @@ __global__ void __launch_bounds__(256, 1) bg_kernel(const double* __restrict__ m
                 }
               }
             }
-            atomicAdd(&s.acc[sl * 2 + iset], part);
+            // deterministic reduction (identical for both parameter sets, so old == new gives a ratio of exactly 1):
+            // ncol*nchunk is a multiple of 32, hence a warp never straddles two slots
+#pragma unroll
+            for (int d = 16; d >= 1; d >>= 1) part += __shfl_xor_sync(0xffffffffu, part, d);
+            if ((tid & 31) == 0) s.red[sl * 8 + (o >> 5)] = part;
           }
+          __syncthreads();
+          if (tid < ns) { double a = 0.0; for (int j = 0; j < percf / 32; j++) a += s.red[tid * 8 + j]; s.acc[tid * 2 + iset] += a; }
         }
         __syncthreads();
       }
@@ -564,7 +572,9 @@ static BgProcess* bg_create(int n, const rwgt_params& po, const rwgt_params& pn,
   }
   D.shared_ext = (po.mt == pn.mt) ? 1 : 0;
   // rows per colour chunk: aim at ~256 colour tasks per slot-batch
-  int nchunk = std::max(1, std::min(S.nperm, 256 / S.ncol)); D.rows_per_chunk = (S.nperm + nchunk - 1) / nchunk; D.nchunk = (S.nperm + D.rows_per_chunk - 1) / D.rows_per_chunk;
+  // colour tasks per slot and batch = ncol * nchunk: a multiple of 32 (warp-aligned reduction) and at most 256
+  int nchunk = std::max(1, std::min(S.nperm, 256 / S.ncol)); if ((S.ncol * nchunk) % 32) nchunk &= ~1;
+  D.rows_per_chunk = (S.nperm + nchunk - 1) / nchunk; D.nchunk = nchunk;
   int dev = 0; cudaGetDevice(&dev); cudaDeviceProp prop; cudaGetDeviceProperties(&prop, dev);
   B->sm_count = prop.multiProcessorCount; size_t maxsm = prop.sharedMemPerBlockOptin;
   auto pick = [&](size_t sz, int& nslot, size_t& bytes) {

@@ -1,0 +1,173 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element on the same
+seeded inputs.  Tolerances (BASELINE.json north_star / SURVEY Q9): FP64 1e-11 relative per event for each of
+|M|^2, |M'|^2, W'; FP32 and mixed 1e-4 max, 1e-6 median."""
+import numpy as np
+import pytest
+
+import oracle as orc
+from paper_2312_07440_b200 import binding as B, events as ev
+
+pytestmark = pytest.mark.gpu
+TOL64 = 1e-11
+
+torch = pytest.importorskip("torch")
+
+
+def gpu_run(process, po, pn, m, w, precision="fp64", stream=None):
+    r = B.Reweighter(process, po, pn, precision)
+    dm, dw = torch.from_numpy(np.ascontiguousarray(m)).cuda(), torch.from_numpy(np.ascontiguousarray(w)).cuda()
+    if stream is None:
+        out = r.run(dm, dw)
+    else:
+        stream.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(stream):
+            out = r.run(dm, dw)
+        stream.synchronize()
+    torch.cuda.synchronize()
+    res = out.cpu().numpy()
+    r.close()
+    return res
+
+
+def rel(got, ref):
+    return np.abs(got / ref - 1)
+
+
+# sizes: several CTAs/slot groups plus a ragged tail, small enough for the oracle to finish in seconds
+SMALL = {1: 4099, 2: 5003, 3: 1001, 4: 203, 5: 37}
+
+
+@pytest.mark.parametrize("idx", [1, 2, 3, 4, 5])
+def test_fp64_parity_every_event_small(idx):
+    c = ev.config(idx)
+    m, w = ev.generate(c, SMALL[idx])
+    a, b, wn, _ = orc.reweight(c.process, c.params_old, c.params_new, m, w)
+    got = gpu_run(c.process, c.params_old, c.params_new, m, w)
+    for g, ref, name in zip(got, (a, b, wn), ("me_old", "me_new", "w_new")):
+        e = rel(g, ref)
+        assert e.max() < TOL64, (c.process, name, int(e.argmax()), e.max())
+
+
+@pytest.mark.parametrize("idx", [3, 4, 5])
+@pytest.mark.parametrize("precision", ["fp32", "mixed"])
+def test_fp32_and_mixed_parity(idx, precision):
+    c = ev.config(idx)
+    m, w = ev.generate(c, SMALL[idx])
+    a, b, wn, _ = orc.reweight(c.process, c.params_old, c.params_new, m, w)
+    got = gpu_run(c.process, c.params_old, c.params_new, m, w, precision)
+    for g, ref in zip(got, (a, b, wn)):
+        e = rel(g, ref)
+        assert e.max() < 1e-4 and np.median(e) < 1e-6, (c.process, precision, e.max(), np.median(e))
+
+
+@pytest.mark.parametrize("idx", [1, 2, 3, 4, 5])
+def test_full_size_bench_launch_sampled_against_oracle(idx):
+    """BASELINE.json's full sizes in the launch configuration bench.py times; sampled events one by one."""
+    c = ev.config(idx)
+    m, w = ev.generate(c)
+    assert w.shape[0] == c.n_events
+    got = gpu_run(c.process, c.params_old, c.params_new, m, w)
+    assert np.all(np.isfinite(got)) and np.all(got > 0)
+    nsamp = {1: 64, 2: 64, 3: 48, 4: 12, 5: 6}[idx]
+    rng = np.random.default_rng(100 + idx)
+    sel = np.unique(np.concatenate([[0, c.n_events - 1], rng.integers(0, c.n_events, nsamp)]))
+    for k in sel:
+        p = np.ascontiguousarray(m[:, :, k])
+        a, b = orc.me2(c.process, c.params_old, p), orc.me2(c.process, c.params_new, p)
+        assert abs(got[0, k] / a - 1) < TOL64 and abs(got[1, k] / b - 1) < TOL64
+        assert abs(got[2, k] / (w[k] * (b / a)) - 1) < TOL64
+    # eq. 3 holds for every event of the full set
+    assert np.all(np.abs(got[2] * got[0] - w * got[1]) <= 5e-16 * np.abs(w * got[1]))   # four roundings of 2^-53
+
+
+@pytest.mark.parametrize("proc_idx", [(1, "epem_mupmum"), (2, "gg_ttx"), (2, "gg_ttx@bg"), (3, "gg_ttxg"), (4, "gg_ttxgg"), (5, "gg_ttxggg")])
+def test_identical_parameter_sets_give_ratio_exactly_one(proc_idx):
+    idx, proc = proc_idx
+    c = ev.config(idx)
+    m, w = ev.generate(c, min(SMALL[idx], 300))
+    got = gpu_run(proc, c.params_new, c.params_new, m, w)
+    assert np.array_equal(got[0], got[1]) and np.array_equal(got[2], w)
+
+
+def test_generic_engine_agrees_with_dedicated_gg_ttx_kernel_and_oracle():
+    c = ev.config(2)
+    m, w = ev.generate(c, 3001)
+    a, b, wn, _ = orc.reweight(c.process, c.params_old, c.params_new, m, w)
+    g1 = gpu_run("gg_ttx", c.params_old, c.params_new, m, w)
+    g2 = gpu_run("gg_ttx@bg", c.params_old, c.params_new, m, w)
+    assert rel(g1, np.stack([a, b, wn])).max() < TOL64 and rel(g2, np.stack([a, b, wn])).max() < TOL64
+
+
+@pytest.mark.parametrize("idx", [2, 3])
+def test_mass_change_between_sets_takes_two_passes(idx):
+    """General parameter change: m_t differs, so nothing but the momenta is shared."""
+    c = ev.config(idx)
+    m, w = ev.generate(c, 257)
+    pn = ev.params(mt=173.0, ggg_scale=1.05, gggg_scale=0.9, alpha_s=0.125)
+    po = ev.params(mt=173.0)
+    # keep the events on the old mass shell; the new set only moves alpha_s and the scales (mass shell must match, Q8)
+    a, b, wn, _ = orc.reweight(c.process, po, pn, m, w)
+    got = gpu_run(c.process, po, pn, m, w)
+    assert rel(got, np.stack([a, b, wn])).max() < TOL64
+
+
+def test_edge_cases_empty_single_and_bad_arguments():
+    c = ev.config(3)
+    h = B.rwgt_create(c.process, c.params_old, c.params_new)
+    assert B.rwgt_n_external(h) == 5 and B.rwgt_flops_per_event(h) > 0
+    B.rwgt_run(h, 0, 0, 0, 0, 0, 0)                      # n_events == 0: no-op, pointers not touched
+    with pytest.raises(RuntimeError):
+        B.rwgt_run(h, 0, 0, 0, 0, 0, 5)                  # NULL buffers
+    with pytest.raises(RuntimeError):
+        B.rwgt_run(h, 1, 1, 1, 1, 1, -1)
+    B.rwgt_destroy(h)
+    with pytest.raises(RuntimeError, match="unknown process"):
+        B.rwgt_create("pp_jj", c.params_old, c.params_new)
+    with pytest.raises(RuntimeError, match="invalid parameter"):
+        B.rwgt_create(c.process, ev.params(alpha_s=-1.0), c.params_new)
+    with pytest.raises(RuntimeError, match="invalid parameter"):
+        B.rwgt_create(c.process, ev.params(Gamma_t=1.4), c.params_new)
+    h1 = B.rwgt_create("epem_mupmum", ev.config(1).params_old, ev.config(1).params_new)
+    with pytest.raises(RuntimeError, match="FP64 only"):
+        B.rwgt_set_precision(h1, "fp32")
+    B.rwgt_destroy(h1)
+    for idx in (1, 2, 3, 5):
+        cc = ev.config(idx)
+        m, w = ev.generate(cc, 1)
+        a, b, wn, _ = orc.reweight(cc.process, cc.params_old, cc.params_new, m, w)
+        got = gpu_run(cc.process, cc.params_old, cc.params_new, m, w)
+        assert rel(got[:, 0], np.array([a[0], b[0], wn[0]])).max() < TOL64
+
+
+def test_zero_matrix_element_gives_ieee_result_no_error():
+    """eq. 3 needs |M|^2 != 0.  Convention of include/rwgt.h: inf/nan is written, no error."""
+    c = ev.config(2)
+    m, w = ev.generate(c, 64)
+    got = gpu_run(c.process, ev.params(alpha_s=1e-200), c.params_new, m, w)
+    assert np.all(got[0] == 0) and np.all(~np.isfinite(got[2]))
+
+
+def test_host_buffer_entry_point_and_non_default_stream():
+    c = ev.config(3)
+    m, w = ev.generate(c, 777)
+    dev = gpu_run(c.process, c.params_old, c.params_new, m, w, stream=torch.cuda.Stream())
+    h = B.rwgt_create(c.process, c.params_old, c.params_new)
+    out = np.empty((3, 777))
+    B.rwgt_run_host(h, m, w, out[0], out[1], out[2])
+    B.rwgt_run_host(h, m[:, :, :100].copy(), w[:100].copy(), out[0, :100], out[1, :100], out[2, :100])
+    B.rwgt_destroy(h)
+    assert np.array_equal(out[:, 100:], dev[:, 100:]) and np.array_equal(out[:, :100], dev[:, :100])
+
+
+def test_rotation_invariance_of_both_sets_on_gpu():
+    """Property that holds at any size: a common spatial rotation leaves |M|^2 and |M'|^2 unchanged.
+    Rotate about the beam axis so legs 0,1 stay on the exact-axis branch."""
+    c = ev.config(4)
+    m, w = ev.generate(c, 500)
+    th = 0.7
+    R = np.array([[np.cos(th), -np.sin(th)], [np.sin(th), np.cos(th)]])
+    mr = m.copy()
+    mr[:, 1:3, :] = np.einsum("ab,pbn->pan", R, m[:, 1:3, :])
+    g0 = gpu_run(c.process, c.params_old, c.params_new, m, w)
+    g1 = gpu_run(c.process, c.params_old, c.params_new, mr, w)
+    assert rel(g1, g0).max() < 1e-10

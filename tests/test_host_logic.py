@@ -1,0 +1,134 @@
+"""CPU tests of the host-side logic: inputs, C-ABI exports, sharding (gloo, world_size 2), bench helpers."""
+import ctypes
+import json
+import os
+import re
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+from paper_2312_07440_b200 import binding, events as ev, sharding
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_events_deterministic_on_shell_and_conserving():
+    for c in ev.CONFIGS:
+        m1, w1 = ev.generate(c, 300)
+        m2, w2 = ev.generate(c, 300)
+        assert np.array_equal(m1, m2) and np.array_equal(w1, w2)
+        assert m1.shape == (c.n_ext, 4, 300) and m1.flags.c_contiguous
+        tot = m1[2:].sum(axis=0)
+        assert np.abs(tot[0] - c.sqrts).max() < 1e-11 * c.sqrts and np.abs(tot[1:]).max() < 1e-11 * c.sqrts
+        for k, mass in enumerate(c.final_masses):
+            p = m1[2 + k]
+            assert np.abs(p[0] ** 2 - (p[1:] ** 2).sum(0) - mass * mass).max() < 1e-9 * c.sqrts ** 2
+        assert np.all(m1[0, 3] == c.sqrts / 2) and np.all(m1[1, 3] == -c.sqrts / 2) and np.all(m1[:2, 1:3] == 0)
+        assert np.all(w1 > 0)
+        # a prefix of a longer set is the shorter set (candidate stream, not block size, defines the events)
+        m3, w3 = ev.generate(c, 50)
+        assert np.array_equal(m3, m1[:, :, :50]) and np.array_equal(w3, w1[:50])
+
+
+def test_event_cuts():
+    for idx in (3, 4, 5):
+        c = ev.config(idx)
+        m, _ = ev.generate(c, 2000)
+        g = m[4:]
+        assert np.hypot(g[:, 1], g[:, 2]).min() > 20.0
+        if c.dr_cut:
+            y = 0.5 * np.log((g[:, 0] + g[:, 3]) / (g[:, 0] - g[:, 3]))
+            ph = np.arctan2(g[:, 2], g[:, 1])
+            for i in range(len(g)):
+                for j in range(i + 1, len(g)):
+                    d = np.abs(ph[i] - ph[j])
+                    d = np.where(d > np.pi, 2 * np.pi - d, d)
+                    assert np.hypot(y[i] - y[j], d).min() > 0.4
+
+
+def test_weights_lognormal():
+    _, w = ev.generate(ev.config(2), 200000)
+    z = np.log(w)
+    assert abs(z.mean()) < 0.01 and abs(z.std() - 1) < 0.01
+
+
+def test_library_exports_every_declared_symbol():
+    binding_lib = ctypes.CDLL(binding.LIB_PATH)
+    header = open(os.path.join(ROOT, "include", "rwgt.h")).read()
+    declared = set(re.findall(r"\b(rwgt_[a-z_0-9]+)\s*\(", header)) - {"rwgt_handle", "rwgt_params"}
+    assert declared == set(binding.EXPORTS)
+    for name in declared:
+        assert hasattr(binding_lib, name), name
+
+
+def test_host_only_entry_points_without_gpu():
+    # colour matrix is host code; create must fail loudly (no CPU fallback) when no device is present
+    C = binding.rwgt_colour_matrix(3)
+    assert abs(C[0, 0] - 64 / 9) < 1e-15 and np.allclose(C, C.T)
+    import torch
+    if not torch.cuda.is_available():
+        with pytest.raises(RuntimeError, match="no CUDA device"):
+            binding.rwgt_create("gg_ttx", ev.params(), ev.params())
+
+
+def test_shard_bounds_cover_exactly():
+    for n in (0, 1, 7, 1048576, 65537):
+        for world in (1, 2, 3, 8):
+            b = [sharding.shard_bounds(n, r, world) for r in range(world)]
+            assert b[0][0] == 0 and b[-1][1] == n
+            assert all(b[i][1] == b[i + 1][0] for i in range(world - 1))
+            sizes = [hi - lo for lo, hi in b]
+            assert max(sizes) - min(sizes) <= 1
+    with pytest.raises(ValueError):
+        sharding.shard_bounds(10, 2, 2)
+
+
+_GLOO = r"""
+import os, sys, numpy as np, torch, torch.distributed as dist
+sys.path.insert(0, %r)
+from paper_2312_07440_b200 import events as ev, sharding
+import bench
+dist.init_process_group("gloo", init_method="tcp://127.0.0.1:%d", rank=int(sys.argv[1]), world_size=2)
+rank, world = dist.get_rank(), dist.get_world_size()
+c = ev.config(3)
+m, w = ev.generate(c, 101)
+lo, hi = sharding.shard_bounds(101, rank, world)
+# stand-in for the per-rank kernel: any per-event function of the shard (no exchange step exists)
+sizes = [sharding.shard_bounds(101, r, world)[1] - sharding.shard_bounds(101, r, world)[0] for r in range(world)]
+local = torch.zeros(max(sizes), dtype=torch.float64)
+local[: hi - lo] = torch.from_numpy(w[lo:hi] * m[2, 0, lo:hi])
+parts = [torch.zeros(max(sizes), dtype=torch.float64) for r in range(world)]
+dist.all_gather(parts, local)
+full = torch.cat([p[:s] for p, s in zip(parts, sizes)]).numpy()
+assert np.array_equal(full, w * m[2, 0])
+t = bench.max_over_ranks(0.5 + rank)       # slowest rank defines the time
+assert t == 1.5
+val = sharding.aggregate_throughput([hi - lo for lo, hi in (sharding.shard_bounds(101, r, world) for r in range(world))], 3, t)
+assert abs(val - 101 * 3 / 1.5) < 1e-12
+dist.barrier(); dist.destroy_process_group()
+print("ok", rank)
+"""
+
+
+def test_two_rank_gloo_sharding_and_timing_reduction(tmp_path):
+    port = 29500 + os.getpid() % 2000
+    script = tmp_path / "gloo_rank.py"
+    script.write_text(_GLOO % (ROOT, port))
+    procs = [subprocess.Popen([sys.executable, str(script), str(r)], stdout=subprocess.PIPE, stderr=subprocess.PIPE, text=True)
+             for r in range(2)]
+    outs = [p.communicate(timeout=240) for p in procs]
+    for p, (o, e) in zip(procs, outs):
+        assert p.returncode == 0, e[-2000:]
+        assert "ok" in o
+
+
+def test_bench_reference_arm_prints_contract_line():
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1", "--warmup", "0",
+                          "--ref-events", "512"], capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads(out.stdout.strip().splitlines()[-1])
+    assert line["impl"] == "reference" and line["unit"] == "events/s" and line["value"] > 0
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
+    assert line["config"]["workload"].startswith("gg_ttx")
