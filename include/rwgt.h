@@ -103,6 +103,11 @@ const char* rwgt_last_error(void);
  * the SU(3) Fierz identity in exact integer arithmetic.  Returns n! or -1. */
 int rwgt_colour_matrix(int n_gluons, double* out);
 
+/* Measurement aid for the roofline: runs a register-resident FMA chain on the current
+ * device and writes the sustained rate in TFLOP/s (2 flop per FMA) to *out_tflops (HOST pointer).
+ * kind 0: FP64 FMA, 1: FP32 FMA, 2: FP64 tensor (mma m8n8k4).  Synchronises the device.  0 or -1. */
+int rwgt_measure_peak(int kind, double* out_tflops);
+
 #ifdef __cplusplus
 }
 #endif

@@ -16,7 +16,7 @@ RWGT_FP64, RWGT_FP32, RWGT_MIXED = 0, 1, 2
 PRECISIONS = {"fp64": RWGT_FP64, "fp32": RWGT_FP32, "mixed": RWGT_MIXED}
 
 EXPORTS = ("rwgt_create", "rwgt_set_precision", "rwgt_n_external", "rwgt_flops_per_event", "rwgt_run",
-           "rwgt_run_host", "rwgt_destroy", "rwgt_last_error", "rwgt_colour_matrix")
+           "rwgt_run_host", "rwgt_destroy", "rwgt_last_error", "rwgt_colour_matrix", "rwgt_measure_peak")
 
 
 class rwgt_params(C.Structure):
@@ -47,6 +47,7 @@ def lib():
         L.rwgt_destroy.argtypes = [vp]
         L.rwgt_last_error.restype = C.c_char_p
         L.rwgt_colour_matrix.argtypes = [C.c_int, dp]
+        L.rwgt_measure_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
@@ -114,6 +115,13 @@ def rwgt_colour_matrix(n_gluons: int) -> np.ndarray:
     if lib().rwgt_colour_matrix(n_gluons, out.ctypes.data) != f:
         raise RuntimeError("rwgt_colour_matrix: bad n_gluons")
     return out
+
+
+def rwgt_measure_peak(kind: int) -> float:
+    out = C.c_double()
+    if lib().rwgt_measure_peak(int(kind), C.byref(out)) != 0:
+        raise RuntimeError("rwgt_measure_peak failed")
+    return out.value
 
 
 class Reweighter:

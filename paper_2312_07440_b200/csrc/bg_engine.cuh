@@ -95,15 +95,12 @@ static inline uint32_t mkref(int base, int m, int shift, bool rev, bool neg, int
 struct BgSched {
   int n, c, lmax, rmax, nperm, npair;
   int nG, nR, nL;                   // table entries per slot
-  int fixbits;                      // number of gluon labels (0..fixbits-1) whose helicity is fixed per batch
-  int nbatch, nfree, ncol;          // batches, free gluon configs per batch, columns of the amplitude buffer
-  int ntG[6], offG[6], strideG[6];  // gluon levels m = 2..n-1: tuples, offset into words, words per task
-  int ntR[6], offR[6], strideR[6];  // right levels m = 1..rmax
-  int ntL[6], offL[6], strideL[6];  // left  levels m = 1..lmax
-  int offF, strideF, ntermF;        // finals: one task descriptor per sigma pair
+  int offG[6], strideG[6];          // gluon levels m = 2..n-1: offset into words, words per task
+  int offR[6], strideR[6];          // right levels m = 1..rmax
+  int offL[6], strideL[6];          // left  levels m = 1..lmax
+  int offF, strideF;                // finals: one task descriptor per sigma pair
   std::vector<uint32_t> words;
-  // instruction counts (FP-pipe instructions per event, one parameter set, all helicities)
-  double fp_per_set, fp_shared;
+  std::vector<double> lfrag;        // Cholesky factor L^T of the colour matrix in mma-fragment order
 };
 
 struct TupleTables {
@@ -127,26 +124,36 @@ static uint32_t qref(const std::map<std::vector<int>, int>& base, const std::vec
   std::vector<int> used(seq.begin() + lo, seq.begin() + hi); if (desc) std::reverse(used.begin(), used.end());
   return mkref(base.at(used), hi - lo, lo, desc, false, mask_of(used));
 }
-
 static void all_tuples(int n, int m, std::vector<std::vector<int>>& out) {
-  std::vector<int> idx(m); out.clear();
-  // ordered tuples of distinct labels, lexicographic
-  std::vector<int> cur; std::vector<bool> usedl(n, false);
+  out.clear(); std::vector<int> cur; std::vector<bool> usedl(n, false);
   struct Rec { static void go(int n, int m, std::vector<int>& cur, std::vector<bool>& u, std::vector<std::vector<int>>& out) {
     if ((int)cur.size() == m) { out.push_back(cur); return; }
     for (int i = 0; i < n; i++) if (!u[i]) { u[i] = true; cur.push_back(i); go(n, m, cur, u, out); cur.pop_back(); u[i] = false; } } };
   Rec::go(n, m, cur, usedl, out);
 }
 
-// per-operation FP-pipe instruction counts of rwgt_math.cuh (FMA, MUL, ADD each 1); see DESIGN.md "Flop counts"
-static const double OP_L3 = 90, OP_V4 = 102, OP_SLASH = 40, OP_PROP = 43, OP_ROWCOL = 16, OP_GSTORE = 24;
+// compile-time geometry of the schedule for N gluons (mirrored by build_schedule and checked in bg_create)
+__host__ __device__ constexpr int cfact(int n) { return n <= 1 ? 1 : n * cfact(n - 1); }
+__host__ __device__ constexpr int ctuples(int n, int m) { return cfact(n) / cfact(n - m); }     // ordered m-tuples of n labels
+template <int N> struct Geo {
+  static constexpr int C = (N + 1) / 2, LMAX = C - 1, RMAX = N - C, NJ = N - C + 1;            // N=2: C=1; 3: 2; 4: 2; 5: 3
+  static constexpr int NPERM = cfact(N), NPAIR = NPERM / 2, NPERM_P = (NPERM + 7) / 8 * 8;
+  static constexpr int NB = (N == 5) ? 1 : 0, NBATCH = 1 << NB;          // helicity batches (amplitude buffer size)
+  static constexpr int NFREE = 1 << (N - 1 - NB), NCOL = NFREE * 4;      // gluon 0 has helicity + only (parity), x4 quark helicities
+  static constexpr int ASTR = 2 * NCOL + 4;                              // row stride (doubles) of the amplitude buffer, bank-conflict-free
+  static constexpr int MT = NPERM_P / 8, KT = NPERM_P / 4, U = (MT + 1) / 2;
+  static constexpr int NT_ALL = 2 * NCOL / 8, NTG = (N == 4) ? 2 : 1, NT = NT_ALL / NTG;
+  static constexpr int NMASK = 1 << N;
+  static constexpr int NPHASE = (N - 1 > (RMAX > LMAX ? RMAX : LMAX) + 1) ? N - 1 : (RMAX > LMAX ? RMAX : LMAX) + 1;
+  static constexpr int NL3 = N - 1, NV4 = (N - 1) * (N - 2) / 2;
+  static constexpr int WOFF_TERMS = 4 + 2 * NL3 + 3 * NV4, WPER = C + NJ + NJ * C;
+  static constexpr int STRIDEF = WOFF_TERMS + 2 * WPER;
+};
 
 static BgSched build_schedule(int n) {
   BgSched S; S.n = n;
-  for (int m = 0; m < 6; m++) { S.ntG[m] = S.offG[m] = S.strideG[m] = S.ntR[m] = S.offR[m] = S.strideR[m] = S.ntL[m] = S.offL[m] = S.strideL[m] = 0; }
-  S.c = (n + 1) / 2; S.lmax = S.c - 1; S.rmax = n - S.c;          // n=2: c=1; 3: 2; 4: 2; 5: 3
-  S.fixbits = (n == 5) ? 2 : 0;
-  S.nbatch = 1 << S.fixbits; S.nfree = 1 << (n - S.fixbits); S.ncol = S.nfree * 4;
+  for (int m = 0; m < 6; m++) { S.offG[m] = S.strideG[m] = S.offR[m] = S.strideR[m] = S.offL[m] = S.strideL[m] = 0; }
+  S.c = (n + 1) / 2; S.lmax = S.c - 1; S.rmax = n - S.c;
   TupleTables T; std::vector<std::vector<int>> tl;
   int nG = 0, nR = 0, nL = 0;
   for (int m = 1; m <= n - 1; m++) { all_tuples(n, m, tl); for (auto& t : tl) if (is_canon(t)) { T.gbase[t] = nG; nG += 1 << m; } }
@@ -154,91 +161,108 @@ static BgSched build_schedule(int n) {
   for (int m = 1; m <= S.rmax; m++) { all_tuples(n, m, tl); for (auto& t : tl) { T.rbase[t] = nR; nR += 2 << m; } }
   for (int m = 1; m <= S.lmax; m++) { all_tuples(n, m, tl); for (auto& t : tl) { T.lbase[t] = nL; nL += 2 << m; } }
   S.nG = nG; S.nR = nR; S.nL = nL;
-  double fp = 0;
-  // gluon levels
   for (int m = 2; m <= n - 1; m++) {
-    all_tuples(n, m, tl); S.offG[m] = (int)S.words.size(); S.strideG[m] = 2 + 2 * (m - 1) + 3 * (m - 1) * (m - 2) / 2; int cnt = 0;
+    all_tuples(n, m, tl); S.offG[m] = (int)S.words.size(); S.strideG[m] = 2 + 2 * (m - 1) + 3 * (m - 1) * (m - 2) / 2;
     for (auto& t : tl) if (is_canon(t)) {
-      cnt++; S.words.push_back(T.gbase[t]); S.words.push_back(mask_of(t));
+      S.words.push_back(T.gbase[t]); S.words.push_back(mask_of(t));
       for (int k = 1; k < m; k++) { S.words.push_back(gref(T, t, 0, k, false)); S.words.push_back(gref(T, t, k, m, false)); }
       for (int j = 1; j < m; j++) for (int k = j + 1; k < m; k++) { S.words.push_back(gref(T, t, 0, j, false)); S.words.push_back(gref(T, t, j, k, false)); S.words.push_back(gref(T, t, k, m, false)); }
     }
-    S.ntG[m] = cnt;
-    fp += (double)cnt * (1 << m) * ((m - 1) * OP_L3 + (m - 1) * (m - 2) / 2 * OP_V4 + OP_GSTORE);
   }
   for (int m = 1; m <= S.rmax; m++) {
-    all_tuples(n, m, tl); S.offR[m] = (int)S.words.size(); S.strideR[m] = 2 + 2 * m; S.ntR[m] = (int)tl.size();
+    all_tuples(n, m, tl); S.offR[m] = (int)S.words.size(); S.strideR[m] = 2 + 2 * m;
     for (auto& t : tl) {
       S.words.push_back(T.rbase[t]); S.words.push_back(mask_of(t));
       for (int k = 1; k <= m; k++) { S.words.push_back(gref(T, t, 0, k, false)); S.words.push_back(qref(T.rbase, t, k, m, false)); }
     }
-    fp += (double)tl.size() * (2 << m) * (m * (OP_SLASH + 8) + OP_PROP);
   }
   for (int m = 1; m <= S.lmax; m++) {
-    all_tuples(n, m, tl); S.offL[m] = (int)S.words.size(); S.strideL[m] = 2 + 2 * m; S.ntL[m] = (int)tl.size();
+    all_tuples(n, m, tl); S.offL[m] = (int)S.words.size(); S.strideL[m] = 2 + 2 * m;
     for (auto& t : tl) {
       S.words.push_back(T.lbase[t]); S.words.push_back(mask_of(t));
       for (int k = 1; k <= m; k++) { S.words.push_back(qref(T.lbase, t, 0, m - k, false)); S.words.push_back(gref(T, t, m - k, m, false)); }
     }
-    fp += (double)tl.size() * (2 << m) * (m * (OP_SLASH + 8) + OP_PROP);
   }
   // finals: one descriptor per pair (sigma, sigma reversed), sigma_1 < sigma_n
   std::vector<std::vector<int>> perms; { std::vector<int> p(n); for (int i = 0; i < n; i++) p[i] = i; do perms.push_back(p); while (std::next_permutation(p.begin(), p.end())); }
   S.nperm = (int)perms.size(); std::map<std::vector<int>, int> rank; for (int i = 0; i < S.nperm; i++) rank[perms[i]] = i;
-  S.ntermF = S.c * (n - S.c + 1) - 1;
-  S.offF = (int)S.words.size(); S.strideF = 4 + 2 * (n - 1) + 3 * (n - 1) * (n - 2) / 2 + 2 * 3 * S.ntermF; S.npair = 0;
-  for (auto& s : perms) if (n == 1 || s.front() < s.back()) {
+  const int C = S.c, NJ = n - C + 1;
+  S.offF = (int)S.words.size(); S.strideF = 4 + 2 * (n - 1) + 3 * (n - 1) * (n - 2) / 2 + 2 * (C + NJ + NJ * C); S.npair = 0;
+  for (auto& s : perms) if (s.front() < s.back()) {
     S.npair++;
     std::vector<int> sr(s.rbegin(), s.rend());
     uint32_t packed = 0; for (int j = 0; j < n; j++) packed |= (uint32_t)s[j] << (3 * j);
     S.words.push_back(rank[s]); S.words.push_back(rank[sr]); S.words.push_back(packed); S.words.push_back(n % 2 == 0 ? 1u : 0u);   // J_n(rev) = (-1)^{n+1} J_n
     for (int k = 1; k < n; k++) { S.words.push_back(gref(T, s, 0, k, false)); S.words.push_back(gref(T, s, k, n, false)); }
     for (int j = 1; j < n; j++) for (int k = j + 1; k < n; k++) { S.words.push_back(gref(T, s, 0, j, false)); S.words.push_back(gref(T, s, j, k, false)); S.words.push_back(gref(T, s, k, n, false)); }
-    // terms of sigma: blocks [i,j) in sigma's ascending positions
-    for (int i = 0; i < S.c; i++) for (int j = S.c; j <= n; j++) { if (i == 0 && j == n) continue;
-      S.words.push_back(qref(T.lbase, s, 0, i, false)); S.words.push_back(gref(T, s, i, j, false)); S.words.push_back(qref(T.rbase, s, j, n, false)); }
-    // terms of sigma reversed: its positions [i,j) are sigma positions [n-j, n-i) read descending
-    for (int i = 0; i < S.c; i++) for (int j = S.c; j <= n; j++) { if (i == 0 && j == n) continue;
-      S.words.push_back(qref(T.lbase, s, n - i, n, true)); S.words.push_back(gref(T, s, n - j, n - i, true)); S.words.push_back(qref(T.rbase, s, 0, n - j, true)); }
+    for (int which = 0; which < 2; which++) {
+      // sigma: block [i,j) in ascending positions.  sigma reversed: its positions [i,j) are sigma's [n-j,n-i) read descending
+      for (int i = 0; i < C; i++) S.words.push_back(which == 0 ? qref(T.lbase, s, 0, i, false) : qref(T.lbase, s, n - i, n, true));
+      for (int j = C; j <= n; j++) S.words.push_back(which == 0 ? qref(T.rbase, s, j, n, false) : qref(T.rbase, s, 0, n - j, true));
+      for (int j = C; j <= n; j++) for (int i = 0; i < C; i++) {
+        if (i == 0 && j == n) { S.words.push_back(0u); continue; }
+        S.words.push_back(which == 0 ? gref(T, s, i, j, false) : gref(T, s, n - j, n - i, true));
+      }
+    }
   }
-  double per_final = (n - 1) * OP_L3 + (n - 1) * (n - 2) / 2 * OP_V4 + OP_GSTORE + 2 * OP_SLASH + 4 * OP_ROWCOL + 2 * S.ntermF * (2 * OP_SLASH + 4 * OP_ROWCOL);
-  fp += (double)S.npair * (1 << n) * per_final;
-  // colour form: per helicity column nperm^2 complex-by-real FMAs (2 each) + nperm * 2 for the row products
-  fp += (double)(4 << n) * (2.0 * S.nperm * S.nperm + 2.0 * S.nperm);
-  S.fp_per_set = fp;
-  // externals: polarisation vectors, spinors, 2^n momentum sums and denominators (rough, small)
-  S.fp_shared = n * 2 * 30.0 + 4 * 40.0 + (1 << n) * 40.0;
+  // Cholesky C = L L^T (C is positive definite); J^dagger C J = |L^T J|^2.  L^T in mma.m8n8k4 A-fragment order:
+  // for m-tile mt, k-steps kt = 2 mt .. KT-1 (upper triangle), element (lane>>2, lane&3) of the 8x4 tile.
+  {
+    int np = S.nperm, npp = (np + 7) / 8 * 8, MT = npp / 8, KT = npp / 4;
+    std::vector<double> Cm = colour_matrix_fierz(n), L((size_t)np * np, 0.0);
+    for (int j = 0; j < np; j++) {
+      double d = Cm[(size_t)j * np + j]; for (int k = 0; k < j; k++) d -= L[(size_t)j * np + k] * L[(size_t)j * np + k];
+      d = std::sqrt(d); L[(size_t)j * np + j] = d;
+      for (int i = j + 1; i < np; i++) { double x = Cm[(size_t)i * np + j]; for (int k = 0; k < j; k++) x -= L[(size_t)i * np + k] * L[(size_t)j * np + k]; L[(size_t)i * np + j] = x / d; }
+    }
+    for (int mt = 0; mt < MT; mt++) for (int kt = 2 * mt; kt < KT; kt++) for (int lane = 0; lane < 32; lane++) {
+      int row = 8 * mt + (lane >> 2), col = 4 * kt + (lane & 3);
+      S.lfrag.push_back((row < np && col < np && col >= row) ? L[(size_t)col * np + row] : 0.0);      // L^T[row][col] = L[col][row]
+    }
+  }
   return S;
 }
 
 // ------------------------------------------------------------------------------------------------ device side
-struct BgSet { double gq, g3, g4, mt, fac; };        // fac = gq^2 / D  (common factor |i gq|^2 and averaging)
+struct BgSet { double gq, g3, g4, mt, fac; };        // fac = 2 gq^2 / D  (|i gq|^2, parity factor 2, averaging)
 struct BgDev {
-  int n, c, nperm, npair, nG, nR, nL, fixbits, nbatch, nfree, ncol, ntermF;
-  int ntG[6], offG[6], strideG[6], ntR[6], offR[6], strideR[6], ntL[6], offL[6], strideL[6];
-  int offF, strideF, lmax, rmax;
-  int nslot, rows_per_chunk, nchunk;
-  int shared_ext;                    // 1: both sets share masses -> externals computed once
-  const uint32_t* words;
-  const double* C64; const float* C32;
+  int nG, nR, nL, nwords, nslot, shared_ext;
+  int offG[6], strideG[6], offR[6], strideR[6], offL[6], strideL[6], offF;
+  const uint32_t* words; const double* lfrag;
   BgSet set[2];
 };
 
 struct BgProcess {
-  BgSched S; BgDev D; uint32_t* d_words; double* d_C64; float* d_C32; int sm_count; size_t smem64, smem32; int nslot64, nslot32;
+  BgSched S; BgDev D; uint32_t* d_words; double* d_lfrag; int sm_count; size_t smem64, smem32; int nslot64, nslot32;
 };
 
 template <typename T> struct Smem {
-  // pointers into the dynamic shared memory of one CTA
+  uint32_t* W;    // schedule words (whole CTA)
   double* pm;     // [nslot][n_ext][4] momenta (always double)
-  T* G; T* R; T* L;  // [nslot][8][nX]
-  T* K;           // [nslot][32][4] momentum sums of gluon subsets
-  T* iK2;         // [nslot][32]
-  T* dR; T* dL;   // [nslot][32] 1/(q^2-m^2)
-  T* A;           // [nslot][nperm][ncol][2]
   double* acc;    // [nslot][2]
   double* red;    // [nslot][8] per-warp partial sums of the colour form
+  T* G; T* R; T* L;  // [nslot][8][nX]   SoA planes: conflict-free for consecutive helicity variants
+  T* K;           // [nslot][NMASK][4] momentum sums of gluon subsets
+  T* iK2;         // [nslot][NMASK]
+  T* dR; T* dL;   // [nslot][NMASK] 1/(q^2-m^2)
+  double* A;      // [nslot][NPERM_P][ASTR] colour-flow amplitudes (re,im interleaved along the row), always double
 };
+template <int N, typename T> __host__ __device__ inline size_t carve(Smem<T>& s, unsigned char* base, int ns, int nG, int nR, int nL, int nwords) {
+  typedef Geo<N> Ge; size_t off = 0;
+  s.A = (double*)(base + off); off += sizeof(double) * (size_t)ns * Ge::NPERM_P * Ge::ASTR;
+  s.pm = (double*)(base + off); off += sizeof(double) * ns * (N + 2) * 4;
+  s.acc = (double*)(base + off); off += sizeof(double) * ns * 2;
+  s.red = (double*)(base + off); off += sizeof(double) * ns * 8;
+  s.G = (T*)(base + off); off += sizeof(T) * (size_t)ns * 8 * nG;
+  s.R = (T*)(base + off); off += sizeof(T) * (size_t)ns * 8 * nR;
+  s.L = (T*)(base + off); off += sizeof(T) * (size_t)ns * 8 * nL;
+  s.K = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK * 4;
+  s.iK2 = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK;
+  s.dR = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK;
+  s.dL = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK;
+  s.W = (uint32_t*)(base + off); off += sizeof(uint32_t) * nwords;
+  return off;
+}
 
 template <typename T> __device__ __forceinline__ vec4<T> ld4(const T* tab, int stride, int e) {
   vec4<T> r;
@@ -266,278 +290,281 @@ __device__ __forceinline__ int ref_m(uint32_t r) { return (int)((r >> 16) & 7u);
 __device__ __forceinline__ int ref_mask(uint32_t r) { return (int)((r >> 24) & 31u); }
 template <typename T> __device__ __forceinline__ T ref_sign(uint32_t r) { return (r & REF_NEG) ? T(-1) : T(1); }
 
-// gluon current of one ordered tuple/variant from lower currents; returns the unscaled sums
-template <typename T> __device__ __forceinline__ vec4<T> gluon_sum(const uint32_t* __restrict__ w, int m, uint32_t v, const T* G, int nG,
-                                                                  const T* K, T g3, T g4) {
+// gluon current of one ordered M-tuple / helicity variant from shorter currents (unscaled by the propagator)
+template <int M, typename T> __device__ __forceinline__ vec4<T> gluon_sum(const uint32_t* w, uint32_t v, const T* G, int nG, const T* K, T g3, T g4) {
   vec4<T> a3, a4;
 #pragma unroll
   for (int i = 0; i < 4; i++) { a3.c[i] = mk<T>(0, 0); a4.c[i] = mk<T>(0, 0); }
-  for (int k = 0; k < m - 1; k++) {
-    uint32_t ra = __ldg(w + 2 * k), rb = __ldg(w + 2 * k + 1);
+#pragma unroll
+  for (int k = 0; k < M - 1; k++) {
+    uint32_t ra = w[2 * k], rb = w[2 * k + 1];
     vec4<T> A = ld4(G, nG, ref_entry(ra, v)), B = ld4(G, nG, ref_entry(rb, v));
     L3_acc(a3, ref_sign<T>(ra) * ref_sign<T>(rb), A, K + 4 * ref_mask(ra), B, K + 4 * ref_mask(rb));
   }
-  const uint32_t* w4 = w + 2 * (m - 1);
-  int n4 = (m - 1) * (m - 2) / 2;
-  for (int t = 0; t < n4; t++) {
-    uint32_t rx = __ldg(w4 + 3 * t), ry = __ldg(w4 + 3 * t + 1), rz = __ldg(w4 + 3 * t + 2);
+  const uint32_t* w4 = w + 2 * (M - 1);
+#pragma unroll
+  for (int t = 0; t < (M - 1) * (M - 2) / 2; t++) {
+    uint32_t rx = w4[3 * t], ry = w4[3 * t + 1], rz = w4[3 * t + 2];
     vec4<T> X = ld4(G, nG, ref_entry(rx, v)), Y = ld4(G, nG, ref_entry(ry, v)), Z = ld4(G, nG, ref_entry(rz, v));
     V4_acc(a4, ref_sign<T>(rx) * ref_sign<T>(ry) * ref_sign<T>(rz), X, Y, Z);
   }
   vec4<T> r;
 #pragma unroll
-  for (int i = 0; i < 4; i++) { r.c[i] = (-g3) * a3.c[i]; rfma(r.c[i], g4, a4.c[i]); }
+  for (int i = 0; i < 4; i++) { r.c[i] = (-g3) * a3.c[i]; if (M > 2) rfma(r.c[i], g4, a4.c[i]); }
   return r;
 }
 
-template <typename T> __device__ __forceinline__ void carve(Smem<T>& s, unsigned char* base, const BgDev& D) {
-  size_t off = 0; int ns = D.nslot;
-  s.pm = (double*)(base + off); off += sizeof(double) * ns * (D.n + 2) * 4;
-  s.acc = (double*)(base + off); off += sizeof(double) * ns * 2;
-  s.red = (double*)(base + off); off += sizeof(double) * ns * 8;
-  s.G = (T*)(base + off); off += sizeof(T) * ns * 8 * D.nG;
-  s.R = (T*)(base + off); off += sizeof(T) * ns * 8 * D.nR;
-  s.L = (T*)(base + off); off += sizeof(T) * ns * 8 * D.nL;
-  s.K = (T*)(base + off); off += sizeof(T) * ns * 32 * 4;
-  s.iK2 = (T*)(base + off); off += sizeof(T) * ns * 32;
-  s.dR = (T*)(base + off); off += sizeof(T) * ns * 32;
-  s.dL = (T*)(base + off); off += sizeof(T) * ns * 32;
-  off = (off + 15) & ~(size_t)15;
-  s.A = (T*)(base + off);
-}
-static size_t smem_bytes(const BgSched& S, int nslot, size_t sz) {
-  size_t off = 0;
-  off += sizeof(double) * nslot * (S.n + 2) * 4 + sizeof(double) * nslot * 10;
-  off += sz * nslot * 8 * (size_t)(S.nG + S.nR + S.nL);
-  off += sz * nslot * 32 * 7;
-  off = (off + 15) & ~(size_t)15;
-  off += sz * nslot * (size_t)S.nperm * S.ncol * 2;
-  return off;
+template <typename T> struct Ctx {
+  Smem<T> s; int tid, ns, nG, nR, nL; T g3, g4, gq, mt; const BgDev* D;
+};
+
+// phase M: gluon currents of length M, right/left quark currents of length M-1 (all helicity variants)
+template <int N, int M, typename T, int NTH> __device__ __forceinline__ void level_phase(const Ctx<T>& c) {
+  typedef Geo<N> Ge;
+  constexpr bool HASG = (M <= N - 1), HASR = (M - 1 >= 1 && M - 1 <= Ge::RMAX), HASL = (M - 1 >= 1 && M - 1 <= Ge::LMAX);
+  constexpr int MM = M - 1;
+  constexpr int tg = HASG ? (ctuples(N, M) / 2) << M : 0, tr = HASR ? ctuples(N, MM) << M : 0, tl = HASL ? ctuples(N, MM) << M : 0, per = tg + tr + tl;
+  const Smem<T>& s = c.s; const int nG = c.nG, nR = c.nR, nL = c.nL, next = N + 2;
+  for (int t = c.tid; t < c.ns * per; t += NTH) {
+    int sl = t / per, o = t % per;
+    T* G = s.G + (size_t)sl * 8 * nG; T* R = s.R + (size_t)sl * 8 * nR; T* L = s.L + (size_t)sl * 8 * nL;
+    const T* K = s.K + (size_t)sl * Ge::NMASK * 4;
+    if (HASG && o < tg) {
+      int tup = o >> M; uint32_t v = o & ((1 << M) - 1);
+      const uint32_t* w = s.W + c.D->offG[M] + tup * (2 + 2 * (M - 1) + 3 * (M - 1) * (M - 2) / 2);
+      int ob = w[0], mask = w[1];
+      vec4<T> r = gluon_sum<M, T>(w + 2, v, G, nG, K, c.g3, c.g4);
+      T sc = s.iK2[sl * Ge::NMASK + mask];
+#pragma unroll
+      for (int i = 0; i < 4; i++) r.c[i] = sc * r.c[i];
+      st4(G, nG, ob + v, r);
+    } else if (HASR && o < tg + tr) {
+      int oo = o - tg; int tup = oo >> M; uint32_t vv = oo & ((1 << M) - 1); uint32_t v = vv & ((1 << MM) - 1); int hb = vv >> MM;
+      const uint32_t* w = s.W + c.D->offR[MM] + tup * (2 + 2 * MM);
+      int ob = w[0], mask = w[1];
+      spn<T> acc;
+#pragma unroll
+      for (int i = 0; i < 4; i++) acc.c[i] = mk<T>(0, 0);
+#pragma unroll
+      for (int k = 0; k < MM; k++) {
+        uint32_t rj = w[2 + 2 * k], rr = w[3 + 2 * k];
+        vec4<T> J = ld4(G, nG, ref_entry(rj, v));
+        spn<T> Rr = lds4(R, nR, ref_entry(rr, v) + (hb << ref_m(rr)));
+        spn<T> x = slash_c(J, Rr); T sg = ref_sign<T>(rj);
+#pragma unroll
+        for (int i = 0; i < 4; i++) rfma(acc.c[i], sg, x.c[i]);
+      }
+      T q[4];
+#pragma unroll
+      for (int mu = 0; mu < 4; mu++) q[mu] = K[4 * mask + mu] - (T)s.pm[sl * next * 4 + 12 + mu];
+      spn<T> r = slash_r_plus_m(q, c.mt, acc); T sc = -c.gq * s.dR[sl * Ge::NMASK + mask];
+#pragma unroll
+      for (int i = 0; i < 4; i++) r.c[i] = sc * r.c[i];
+      st4(R, nR, ob + v + (hb << MM), r);
+    } else if (HASL) {
+      int oo = o - tg - tr; int tup = oo >> M; uint32_t vv = oo & ((1 << M) - 1); uint32_t v = vv & ((1 << MM) - 1); int hb = vv >> MM;
+      const uint32_t* w = s.W + c.D->offL[MM] + tup * (2 + 2 * MM);
+      int ob = w[0], mask = w[1];
+      spn<T> acc;
+#pragma unroll
+      for (int i = 0; i < 4; i++) acc.c[i] = mk<T>(0, 0);
+#pragma unroll
+      for (int k = 0; k < MM; k++) {
+        uint32_t rl = w[2 + 2 * k], rj = w[3 + 2 * k];
+        spn<T> Ll = lds4(L, nL, ref_entry(rl, v) + (hb << ref_m(rl)));
+        vec4<T> J = ld4(G, nG, ref_entry(rj, v));
+        spn<T> x = row_slash_c(Ll, J); T sg = ref_sign<T>(rj);
+#pragma unroll
+        for (int i = 0; i < 4; i++) rfma(acc.c[i], sg, x.c[i]);
+      }
+      T q[4];
+#pragma unroll
+      for (int mu = 0; mu < 4; mu++) q[mu] = (T)s.pm[sl * next * 4 + 8 + mu] - K[4 * mask + mu];
+      spn<T> r = row_slash_r_plus_m(acc, q, c.mt); T sc = -c.gq * s.dL[sl * Ge::NMASK + mask];
+#pragma unroll
+      for (int i = 0; i < 4; i++) r.c[i] = sc * r.c[i];
+      st4(L, nL, ob + v + (hb << MM), r);
+    }
+  }
+  __syncthreads();
 }
 
-// MIXED: T = float but momentum sums / denominators are formed in double before rounding to T.
-template <typename T, bool MIXED>
-__global__ void __launch_bounds__(256, 1) bg_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
+__device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+// MIXED: T = float but momentum sums / propagator denominators are formed in double before rounding to T.
+// The colour form and the helicity sum are accumulated in double in every mode (FP64 tensor-core mma).
+template <int N, typename T, bool MIXED, int NTH>
+__global__ void __launch_bounds__(NTH, 1) bg_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
                                                     double* __restrict__ me_old, double* __restrict__ me_new,
                                                     double* __restrict__ w_new, long long nev, BgDev D) {
+  typedef Geo<N> Ge;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  Smem<T> s; carve<T>(s, smem_raw, D);
-  typedef typename std::conditional<MIXED, double, T>::type TK;      // type used to form momentum sums and denominators
-  const int tid = threadIdx.x, nth = blockDim.x, n = D.n, next = n + 2, ns = D.nslot;
-  const int nG = D.nG, nR = D.nR, nL = D.nL;
+  Ctx<T> c; c.D = &D; c.tid = threadIdx.x; c.ns = D.nslot; c.nG = D.nG; c.nR = D.nR; c.nL = D.nL;
+  carve<N, T>(c.s, smem_raw, D.nslot, D.nG, D.nR, D.nL, D.nwords);
+  const Smem<T>& s = c.s;
+  typedef typename std::conditional<MIXED, double, T>::type TK;
+  const int tid = threadIdx.x, next = N + 2, ns = D.nslot, nG = D.nG, nR = D.nR, nL = D.nL;
+  // once per CTA: schedule words into shared memory, zero the padding rows of the amplitude buffer
+  for (int t = tid; t < D.nwords; t += NTH) s.W[t] = __ldg(D.words + t);
+  for (int t = tid; t < ns * Ge::NPERM_P * Ge::ASTR; t += NTH) s.A[t] = 0.0;
   const long long ngroups = (nev + ns - 1) / ns;
   for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
     const long long ev0 = grp * ns;
-    __syncthreads();   // previous group's outputs were read
-    // ---- a1: load momenta (coalesced over events within the group) ----
-    for (int t = tid; t < ns * next * 4; t += nth) {
+    __syncthreads();   // previous group's outputs were read; words are visible
+    // ---- a1: load momenta (coalesced over the events of the group) ----
+    for (int t = tid; t < ns * next * 4; t += NTH) {
       int sl = t % ns, comp = t / ns; long long ev = ev0 + sl; if (ev >= nev) ev = nev - 1;
       s.pm[(sl * next * 4) + comp] = __ldg(mom + (size_t)comp * nev + ev);
     }
     if (tid < ns * 2) s.acc[tid] = 0.0;
     __syncthreads();
+#pragma unroll 1
     for (int iset = 0; iset < 2; iset++) {
       const BgSet& P = D.set[iset];
-      const T g3 = (T)P.g3, g4 = (T)P.g4, gq = (T)P.gq, mt = (T)P.mt;
+      c.g3 = (T)P.g3; c.g4 = (T)P.g4; c.gq = (T)P.gq; c.mt = (T)P.mt;
       if (iset == 0 || !D.shared_ext) {
         // ---- a2: external wavefunctions, momentum sums, propagator denominators ----
-        int nobj = 2 * n + 4 + 32;
-        for (int t = tid; t < ns * nobj; t += nth) {
+        constexpr int nobj = 2 * N + 4 + Ge::NMASK;
+        for (int t = tid; t < ns * nobj; t += NTH) {
           int sl = t / nobj, o = t % nobj; const double* pm = s.pm + sl * next * 4;
-          if (o < 2 * n) {                         // gluon i, helicity bit hb (0: +1, 1: -1); entry = 2*i + hb
+          if (o < 2 * N) {                         // gluon i, helicity bit hb (0: +1, 1: -1); entry = 2*i + hb
             int i = o >> 1, hb = o & 1, leg = i < 2 ? i : i + 2; const double* p = pm + 4 * leg;
             vec4<T> e = polvec<T>((T)p[1], (T)p[2], (T)p[3], hb ? -1 : +1);
             if (i >= 2) e = conj4(e);              // outgoing gluon carries eps*
             st4(s.G + (size_t)sl * 8 * nG, nG, 2 * i + hb, e);
-          } else if (o < 2 * n + 2) {              // v(p_tbar, lam), R() entries 0,1
-            int hb = o - 2 * n; const double* p = pm + 12;
+          } else if (o < 2 * N + 2) {              // v(p_tbar, lam), R() entries 0,1
+            int hb = o - 2 * N; const double* p = pm + 12;
             chi_pair<T> x = make_chi<T>((T)p[1], (T)p[2], (T)p[3]);
-            st4(s.R + (size_t)sl * 8 * nR, nR, hb, spinor_v<T>(x, (T)p[0], mt, hb ? -1 : +1));
-          } else if (o < 2 * n + 4) {              // ubar(p_t, lam), L() entries 0,1
-            int hb = o - 2 * n - 2; const double* p = pm + 8;
+            st4(s.R + (size_t)sl * 8 * nR, nR, hb, spinor_v<T>(x, (T)p[0], c.mt, hb ? -1 : +1));
+          } else if (o < 2 * N + 4) {              // ubar(p_t, lam), L() entries 0,1
+            int hb = o - 2 * N - 2; const double* p = pm + 8;
             chi_pair<T> x = make_chi<T>((T)p[1], (T)p[2], (T)p[3]);
-            st4(s.L + (size_t)sl * 8 * nL, nL, hb, bar(spinor_u<T>(x, (T)p[0], mt, hb ? -1 : +1)));
-          } else {                                 // subset mask
-            int mask = o - 2 * n - 4;
-            if (mask < (1 << n)) {
-              TK k[4] = {0, 0, 0, 0};
-              for (int i = 0; i < n; i++) if (mask >> i & 1) { int leg = i < 2 ? i : i + 2; TK sg = i < 2 ? TK(1) : TK(-1);
-                for (int mu = 0; mu < 4; mu++) k[mu] += sg * (TK)pm[4 * leg + mu]; }
-              TK k2 = mdot_rr<TK>(k, k);
-              TK qr[4], ql[4]; for (int mu = 0; mu < 4; mu++) { qr[mu] = k[mu] - (TK)pm[12 + mu]; ql[mu] = (TK)pm[8 + mu] - k[mu]; }
-              TK m2 = (TK)P.mt * (TK)P.mt;
-              T* K = s.K + (size_t)sl * 128 + 4 * mask; for (int mu = 0; mu < 4; mu++) K[mu] = (T)k[mu];
-              s.iK2[sl * 32 + mask] = (__popc(mask) >= 2) ? (T)(TK(1) / k2) : T(0);
-              s.dR[sl * 32 + mask] = (T)(TK(1) / (mdot_rr<TK>(qr, qr) - m2));
-              s.dL[sl * 32 + mask] = (T)(TK(1) / (mdot_rr<TK>(ql, ql) - m2));
-            }
-          }
-        }
-        __syncthreads();
-      }
-      // ---- a3: current levels.  phase m: gluon level m, right level m-1, left level m-1 ----
-      int nphase = max(n - 1, max(D.rmax, D.lmax) + 1);
-      for (int m = 2; m <= nphase; m++) {
-        int tg = (m <= n - 1) ? (D.ntG[m] << m) : 0;
-        int tr = (m - 1 >= 1 && m - 1 <= D.rmax) ? (D.ntR[m - 1] << m) : 0;      // 2^(m-1) variants x 2 quark helicities
-        int tl = (m - 1 >= 1 && m - 1 <= D.lmax) ? (D.ntL[m - 1] << m) : 0;
-        int per = tg + tr + tl;
-        for (int t = tid; t < ns * per; t += nth) {
-          int sl = t / per, o = t % per;
-          T* G = s.G + (size_t)sl * 8 * nG; T* R = s.R + (size_t)sl * 8 * nR; T* L = s.L + (size_t)sl * 8 * nL;
-          const T* K = s.K + (size_t)sl * 128;
-          if (o < tg) {
-            int tup = o >> m; uint32_t v = o & ((1 << m) - 1);
-            const uint32_t* w = D.words + D.offG[m] + tup * D.strideG[m];
-            int ob = __ldg(w), mask = __ldg(w + 1);
-            vec4<T> r = gluon_sum<T>(w + 2, m, v, G, nG, K, g3, g4);
-            T sc = s.iK2[sl * 32 + mask];
+            st4(s.L + (size_t)sl * 8 * nL, nL, hb, bar(spinor_u<T>(x, (T)p[0], c.mt, hb ? -1 : +1)));
+          } else {                                 // gluon subset `mask`
+            int mask = o - 2 * N - 4;
+            TK k[4] = {0, 0, 0, 0};
 #pragma unroll
-            for (int i = 0; i < 4; i++) r.c[i] = sc * r.c[i];
-            st4(G, nG, ob + v, r);
-          } else if (o < tg + tr) {
-            int mm = m - 1, oo = o - tg; int tup = oo >> m; uint32_t vv = oo & ((1 << m) - 1); uint32_t v = vv & ((1 << mm) - 1); int hb = vv >> mm;
-            const uint32_t* w = D.words + D.offR[mm] + tup * D.strideR[mm];
-            int ob = __ldg(w), mask = __ldg(w + 1);
-            spn<T> acc; for (int i = 0; i < 4; i++) acc.c[i] = mk<T>(0, 0);
-            for (int k = 0; k < mm; k++) {
-              uint32_t rj = __ldg(w + 2 + 2 * k), rr = __ldg(w + 3 + 2 * k);
-              vec4<T> J = ld4(G, nG, ref_entry(rj, v));
-              spn<T> Rr = lds4(R, nR, ref_entry(rr, v) + (hb << ref_m(rr)));
-              spn<T> x = slash_c(J, Rr); T sg = ref_sign<T>(rj);
-              for (int i = 0; i < 4; i++) rfma(acc.c[i], sg, x.c[i]);
-            }
-            T q[4]; for (int mu = 0; mu < 4; mu++) q[mu] = K[4 * mask + mu] - (T)s.pm[sl * next * 4 + 12 + mu];
-            spn<T> r = slash_r_plus_m(q, mt, acc); T sc = -gq * s.dR[sl * 32 + mask];
-            for (int i = 0; i < 4; i++) r.c[i] = sc * r.c[i];
-            st4(R, nR, ob + v + (hb << mm), r);
-          } else {
-            int mm = m - 1, oo = o - tg - tr; int tup = oo >> m; uint32_t vv = oo & ((1 << m) - 1); uint32_t v = vv & ((1 << mm) - 1); int hb = vv >> mm;
-            const uint32_t* w = D.words + D.offL[mm] + tup * D.strideL[mm];
-            int ob = __ldg(w), mask = __ldg(w + 1);
-            spn<T> acc; for (int i = 0; i < 4; i++) acc.c[i] = mk<T>(0, 0);
-            for (int k = 0; k < mm; k++) {
-              uint32_t rl = __ldg(w + 2 + 2 * k), rj = __ldg(w + 3 + 2 * k);
-              spn<T> Ll = lds4(L, nL, ref_entry(rl, v) + (hb << ref_m(rl)));
-              vec4<T> J = ld4(G, nG, ref_entry(rj, v));
-              spn<T> x = row_slash_c(Ll, J); T sg = ref_sign<T>(rj);
-              for (int i = 0; i < 4; i++) rfma(acc.c[i], sg, x.c[i]);
-            }
-            T q[4]; for (int mu = 0; mu < 4; mu++) q[mu] = (T)s.pm[sl * next * 4 + 8 + mu] - K[4 * mask + mu];
-            spn<T> r = row_slash_r_plus_m(acc, q, mt); T sc = -gq * s.dL[sl * 32 + mask];
-            for (int i = 0; i < 4; i++) r.c[i] = sc * r.c[i];
-            st4(L, nL, ob + v + (hb << mm), r);
+            for (int i = 0; i < N; i++) if (mask >> i & 1) { int leg = i < 2 ? i : i + 2; TK sg = i < 2 ? TK(1) : TK(-1);
+              for (int mu = 0; mu < 4; mu++) k[mu] += sg * (TK)pm[4 * leg + mu]; }
+            TK k2 = mdot_rr<TK>(k, k);
+            TK qr[4], ql[4]; for (int mu = 0; mu < 4; mu++) { qr[mu] = k[mu] - (TK)pm[12 + mu]; ql[mu] = (TK)pm[8 + mu] - k[mu]; }
+            TK m2 = (TK)P.mt * (TK)P.mt;
+            T* K = s.K + ((size_t)sl * Ge::NMASK + mask) * 4; for (int mu = 0; mu < 4; mu++) K[mu] = (T)k[mu];
+            s.iK2[sl * Ge::NMASK + mask] = (__popc(mask) >= 2) ? (T)(TK(1) / k2) : T(0);
+            s.dR[sl * Ge::NMASK + mask] = (T)(TK(1) / (mdot_rr<TK>(qr, qr) - m2));
+            s.dL[sl * Ge::NMASK + mask] = (T)(TK(1) / (mdot_rr<TK>(ql, ql) - m2));
           }
         }
         __syncthreads();
       }
-      // ---- a3/a4: colour-flow amplitudes per helicity batch; a5/a6: colour form and helicity sum ----
-      const int ncol = D.ncol, nperm = D.nperm;
-      for (int batch = 0; batch < D.nbatch; batch++) {
-        int per = D.npair * D.nfree;
-        for (int t = tid; t < ns * per; t += nth) {
-          int sl = t / per, o = t % per; int pair = o / D.nfree, f = o % D.nfree;
+      // ---- a3: current levels ----
+      level_phase<N, 2, T, NTH>(c);
+      if constexpr (Ge::NPHASE >= 3) level_phase<N, 3, T, NTH>(c);
+      if constexpr (Ge::NPHASE >= 4) level_phase<N, 4, T, NTH>(c);
+      // ---- a3/a4: colour-flow amplitudes of a helicity batch; a5/a6: colour form |L^T J|^2 and helicity sum ----
+#pragma unroll 1
+      for (int batch = 0; batch < Ge::NBATCH; batch++) {
+        constexpr int per = Ge::NPAIR * Ge::NFREE;
+        for (int t = tid; t < ns * per; t += NTH) {
+          int sl = t / per, o = t % per; int pair = o / Ge::NFREE, f = o % Ge::NFREE;
           const T* G = s.G + (size_t)sl * 8 * nG; const T* R = s.R + (size_t)sl * 8 * nR; const T* L = s.L + (size_t)sl * 8 * nL;
-          const T* K = s.K + (size_t)sl * 128;
-          const uint32_t* w = D.words + D.offF + pair * D.strideF;
-          uint32_t rk = __ldg(w), rkr = __ldg(w + 1), packed = __ldg(w + 2), negr = __ldg(w + 3);
-          uint32_t g = (uint32_t)batch | ((uint32_t)f << D.fixbits);        // helicity bits by gluon label
-          uint32_t v = 0; for (int j = 0; j < n; j++) v |= ((g >> ((packed >> (3 * j)) & 7u)) & 1u) << j;   // by position in sigma
-          vec4<T> Jn = gluon_sum<T>(w + 4, n, v, G, nG, K, g3, g4);
-          T sc = s.iK2[sl * 32 + ((1 << n) - 1)];
+          const T* K = s.K + (size_t)sl * Ge::NMASK * 4;
+          const uint32_t* w = s.W + D.offF + pair * Ge::STRIDEF;
+          uint32_t rk = w[0], rkr = w[1], packed = w[2], negr = w[3];
+          uint32_t g = ((uint32_t)batch << 1) | ((uint32_t)f << (1 + Ge::NB));   // helicity bits by gluon label; gluon 0: + (parity)
+          uint32_t v = 0;
+#pragma unroll
+          for (int j = 0; j < N; j++) v |= ((g >> ((packed >> (3 * j)) & 7u)) & 1u) << j;   // by position in sigma
+          vec4<T> Jn = gluon_sum<N, T>(w + 4, v, G, nG, K, c.g3, c.g4);
+          T sc = s.iK2[sl * Ge::NMASK + Ge::NMASK - 1];
 #pragma unroll
           for (int i = 0; i < 4; i++) Jn.c[i] = sc * Jn.c[i];
-          cx<T> As[2][2], Ar[2][2];
-          {
-            spn<T> u0 = lds4(L, nL, 0), u1 = lds4(L, nL, 1);
+          const spn<T> u0 = lds4(L, nL, 0), u1 = lds4(L, nL, 1);
+          double* A = s.A + (size_t)sl * Ge::NPERM_P * Ge::ASTR;
+          const uint32_t* wt = w + Ge::WOFF_TERMS;
 #pragma unroll
-            for (int hb = 0; hb < 2; hb++) {
-              spn<T> x = slash_c(Jn, lds4(R, nR, hb));
-              As[0][hb] = rowcol(u0, x); As[1][hb] = rowcol(u1, x);
+          for (int which = 0; which < 2; which++) {
+            cx<T> Acc[2][2];
+#pragma unroll
+            for (int a = 0; a < 2; a++)
+#pragma unroll
+              for (int b = 0; b < 2; b++) Acc[a][b] = mk<T>(0, 0);
+            T sfull = (which && negr) ? T(-1) : T(1);
+#pragma unroll
+            for (int jj = 0; jj < Ge::NJ; jj++) {
+              spn<T> X0, X1;
+#pragma unroll
+              for (int i = 0; i < 4; i++) { X0.c[i] = mk<T>(0, 0); X1.c[i] = mk<T>(0, 0); }
+#pragma unroll
+              for (int i = 0; i < Ge::C; i++) {
+                spn<T> y0, y1; T sg;
+                if (i == 0 && jj == Ge::NJ - 1) { y0 = row_slash_c(u0, Jn); y1 = row_slash_c(u1, Jn); sg = sfull; }
+                else {
+                  uint32_t rl = wt[i], rj = wt[Ge::C + Ge::NJ + jj * Ge::C + i];
+                  vec4<T> J = ld4(G, nG, ref_entry(rj, v)); sg = ref_sign<T>(rj);
+                  int el = ref_entry(rl, v), ml = ref_m(rl);
+                  y0 = row_slash_c(lds4(L, nL, el), J); y1 = row_slash_c(lds4(L, nL, el + (1 << ml)), J);
+                }
+#pragma unroll
+                for (int q = 0; q < 4; q++) { rfma(X0.c[q], sg, y0.c[q]); rfma(X1.c[q], sg, y1.c[q]); }
+              }
+              uint32_t rr = wt[Ge::C + jj]; int er = ref_entry(rr, v), mr = ref_m(rr);
+#pragma unroll
+              for (int hb = 0; hb < 2; hb++) {
+                spn<T> Rr = lds4(R, nR, er + (hb << mr));
+                cx<T> a0 = rowcol(X0, Rr), a1 = rowcol(X1, Rr);
+                Acc[0][hb] = Acc[0][hb] + a0; Acc[1][hb] = Acc[1][hb] + a1;
+              }
             }
-            T sr = negr ? T(-1) : T(1);
+            uint32_t row = which ? rkr : rk;
 #pragma unroll
             for (int ht = 0; ht < 2; ht++)
 #pragma unroll
-              for (int hb = 0; hb < 2; hb++) Ar[ht][hb] = sr * As[ht][hb];
-          }
-          const uint32_t* wt = w + 4 + 2 * (n - 1) + 3 * (n - 1) * (n - 2) / 2;
-          for (int which = 0; which < 2; which++) {
-            cx<T>(*Acc)[2] = which ? Ar : As;
-            for (int term = 0; term < D.ntermF; term++) {
-              uint32_t rl = __ldg(wt + 3 * term), rj = __ldg(wt + 3 * term + 1), rr = __ldg(wt + 3 * term + 2);
-              vec4<T> J = ld4(G, nG, ref_entry(rj, v)); T sg = ref_sign<T>(rj);
-              int el = ref_entry(rl, v), er = ref_entry(rr, v), ml = ref_m(rl), mr = ref_m(rr);
-              spn<T> l0 = lds4(L, nL, el), l1 = lds4(L, nL, el + (1 << ml));
-#pragma unroll
               for (int hb = 0; hb < 2; hb++) {
-                spn<T> x = slash_c(J, lds4(R, nR, er + (hb << mr)));
-                cx<T> a0 = rowcol(l0, x), a1 = rowcol(l1, x);
-                rfma(Acc[0][hb], sg, a0); rfma(Acc[1][hb], sg, a1);
+                int col = f * 4 + ht * 2 + hb;
+                *reinterpret_cast<double2*>(A + (size_t)row * Ge::ASTR + 2 * col) = make_double2((double)Acc[ht][hb].re, (double)Acc[ht][hb].im);
               }
-            }
-            wt += 3 * D.ntermF;
+            wt += Ge::WPER;
           }
-          T* A = s.A + (size_t)sl * nperm * ncol * 2;
-#pragma unroll
-          for (int ht = 0; ht < 2; ht++)
-#pragma unroll
-            for (int hb = 0; hb < 2; hb++) {
-              int col = f * 4 + ht * 2 + hb;
-              A[((size_t)rk * ncol + col) * 2] = As[ht][hb].re; A[((size_t)rk * ncol + col) * 2 + 1] = As[ht][hb].im;
-              A[((size_t)rkr * ncol + col) * 2] = Ar[ht][hb].re; A[((size_t)rkr * ncol + col) * 2 + 1] = Ar[ht][hb].im;
-            }
         }
         __syncthreads();
-        // colour form: thread = (slot, chunk of rows, column)
+        // colour form: Z = L^T A with FP64 tensor-core mma (upper-triangular tiles only), sum of squares of Z
         {
-          const int RB = D.rows_per_chunk, nchunk = D.nchunk; int percf = ncol * nchunk;
-          for (int t = tid; t < ns * percf; t += nth) {
-            int sl = t / percf, o = t % percf; int chunk = o / ncol, col = o % ncol;
-            const T* A = s.A + (size_t)sl * nperm * ncol * 2;
-            int r0 = chunk * RB, nr = max(0, min(RB, nperm - r0));
+          const int warp = tid >> 5, lane = tid & 31;
+          constexpr int UN = Ge::U * Ge::NTG;
+          for (int u = warp; u < ns * UN; u += NTH / 32) {
+            int sl = u / UN, rem = u % UN, unit = rem / Ge::NTG, grp = rem % Ge::NTG;
+            const double* A = s.A + (size_t)sl * Ge::NPERM_P * Ge::ASTR + grp * Ge::NT * 8 + (lane & 3) * Ge::ASTR + (lane >> 2);
             double part = 0.0;
-            if (sizeof(T) == 8) {
-              const double* C = D.C64;
-              for (int rb = 0; rb < nr; rb += 5) {            // register block of 5 rows
-                double yr[5] = {0, 0, 0, 0, 0}, yi[5] = {0, 0, 0, 0, 0}; int nb = min(5, nr - rb);
-                for (int sp = 0; sp < nperm; sp++) {
-                  double ar = (double)A[((size_t)sp * ncol + col) * 2], ai = (double)A[((size_t)sp * ncol + col) * 2 + 1];
-                  const double* Cr = C + (size_t)sp * nperm + r0 + rb;       // C symmetric: column sp == row sp
+#pragma unroll 1
+            for (int half = 0; half < 2; half++) {
+              int mt = half ? Ge::MT - 1 - unit : unit;
+              if (half && mt == unit) break;
+              double acc[Ge::NT][2];
 #pragma unroll
-                  for (int r = 0; r < 5; r++) if (r < nb) { double c = __ldg(Cr + r); yr[r] = fma(c, ar, yr[r]); yi[r] = fma(c, ai, yi[r]); }
-                }
+              for (int nt = 0; nt < Ge::NT; nt++) { acc[nt][0] = 0.0; acc[nt][1] = 0.0; }
+              const double* F = D.lfrag + (size_t)(mt * Ge::KT - mt * (mt - 1)) * 32 + lane;
+              int nk = Ge::KT - 2 * mt;
+              double a = __ldg(F);
+              for (int kk = 0; kk < nk; kk++) {
+                double an = (kk + 1 < nk) ? __ldg(F + (kk + 1) * 32) : 0.0;
+                const double* Br = A + (size_t)(4 * (2 * mt + kk)) * Ge::ASTR;
 #pragma unroll
-                for (int r = 0; r < 5; r++) if (r < nb) {
-                  double ar = (double)A[((size_t)(r0 + rb + r) * ncol + col) * 2], ai = (double)A[((size_t)(r0 + rb + r) * ncol + col) * 2 + 1];
-                  part = fma(ar, yr[r], part); part = fma(ai, yi[r], part);
-                }
+                for (int nt = 0; nt < Ge::NT; nt++) dmma884(acc[nt][0], acc[nt][1], a, Br[8 * nt]);
+                a = an;
               }
-            } else {
-              const float* C = D.C32;
-              for (int rb = 0; rb < nr; rb += 5) {
-                float yr[5] = {0, 0, 0, 0, 0}, yi[5] = {0, 0, 0, 0, 0}; int nb = min(5, nr - rb);
-                for (int sp = 0; sp < nperm; sp++) {
-                  float ar = (float)A[((size_t)sp * ncol + col) * 2], ai = (float)A[((size_t)sp * ncol + col) * 2 + 1];
-                  const float* Cr = C + (size_t)sp * nperm + r0 + rb;
 #pragma unroll
-                  for (int r = 0; r < 5; r++) if (r < nb) { float c = __ldg(Cr + r); yr[r] = fmaf(c, ar, yr[r]); yi[r] = fmaf(c, ai, yi[r]); }
-                }
-#pragma unroll
-                for (int r = 0; r < 5; r++) if (r < nb) {
-                  float ar = (float)A[((size_t)(r0 + rb + r) * ncol + col) * 2], ai = (float)A[((size_t)(r0 + rb + r) * ncol + col) * 2 + 1];
-                  part += (double)(ar * yr[r] + ai * yi[r]);
-                }
-              }
+              for (int nt = 0; nt < Ge::NT; nt++) { part = fma(acc[nt][0], acc[nt][0], part); part = fma(acc[nt][1], acc[nt][1], part); }
             }
-            // deterministic reduction (identical for both parameter sets, so old == new gives a ratio of exactly 1):
-            // ncol*nchunk is a multiple of 32, hence a warp never straddles two slots
+            // deterministic reduction (same order for both parameter sets => old == new gives a ratio of exactly 1)
 #pragma unroll
             for (int d = 16; d >= 1; d >>= 1) part += __shfl_xor_sync(0xffffffffu, part, d);
-            if ((tid & 31) == 0) s.red[sl * 8 + (o >> 5)] = part;
+            if (lane == 0) s.red[sl * 8 + rem] = part;
           }
           __syncthreads();
-          if (tid < ns) { double a = 0.0; for (int j = 0; j < percf / 32; j++) a += s.red[tid * 8 + j]; s.acc[tid * 2 + iset] += a; }
+          if (tid < ns) { double a = 0.0; for (int j = 0; j < UN; j++) a += s.red[tid * 8 + j]; s.acc[tid * 2 + iset] += a; }
         }
         __syncthreads();
       }
@@ -554,61 +581,91 @@ __global__ void __launch_bounds__(256, 1) bg_kernel(const double* __restrict__ m
 }
 
 // ------------------------------------------------------------------------------------------------ host API of the engine
+template <int N> static size_t smem_need(const BgSched& S, int nslot, bool dbl) {
+  if (dbl) { Smem<double> s; return carve<N, double>(s, nullptr, nslot, S.nG, S.nR, S.nL, (int)S.words.size()); }
+  Smem<float> s; return carve<N, float>(s, nullptr, nslot, S.nG, S.nR, S.nL, (int)S.words.size());
+}
+static size_t smem_need_n(int n, const BgSched& S, int nslot, bool dbl) {
+  switch (n) { case 2: return smem_need<2>(S, nslot, dbl); case 3: return smem_need<3>(S, nslot, dbl); case 4: return smem_need<4>(S, nslot, dbl); default: return smem_need<5>(S, nslot, dbl); }
+}
+// 16K registers per SM sub-partition: 3 warps x 168 registers (FP64) or 4 warps x 128 registers (FP32) per sub-partition
+static const int BG_THREADS64 = 384, BG_THREADS32 = 512;
+
+template <int N> static cudaError_t bg_set_attr(size_t s64, size_t s32) {
+  cudaError_t e = cudaFuncSetAttribute(bg_kernel<N, double, false, BG_THREADS64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s64);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, false, BG_THREADS32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, true, BG_THREADS32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
+  return e;
+}
+template <int N> static void bg_launch(int precision, int grid, size_t s64, size_t s32, cudaStream_t st, const double* mom, const double* w,
+                                       double* a, double* b, double* o, long long nev, const BgDev& D) {
+  if (precision == RWGT_FP64) bg_kernel<N, double, false, BG_THREADS64><<<grid, BG_THREADS64, s64, st>>>(mom, w, a, b, o, nev, D);
+  else if (precision == RWGT_FP32) bg_kernel<N, float, false, BG_THREADS32><<<grid, BG_THREADS32, s32, st>>>(mom, w, a, b, o, nev, D);
+  else bg_kernel<N, float, true, BG_THREADS32><<<grid, BG_THREADS32, s32, st>>>(mom, w, a, b, o, nev, D);
+}
+
 static BgProcess* bg_create(int n, const rwgt_params& po, const rwgt_params& pn, std::string& err) {
   BgProcess* B = new BgProcess();
   B->S = build_schedule(n);
   const BgSched& S = B->S;
   BgDev& D = B->D;
-  D.n = n; D.c = S.c; D.nperm = S.nperm; D.npair = S.npair; D.nG = S.nG; D.nR = S.nR; D.nL = S.nL; D.fixbits = S.fixbits; D.nbatch = S.nbatch;
-  D.nfree = S.nfree; D.ncol = S.ncol; D.ntermF = S.ntermF; D.offF = S.offF; D.strideF = S.strideF; D.lmax = S.lmax; D.rmax = S.rmax;
-  for (int m = 0; m < 6; m++) { D.ntG[m] = S.ntG[m]; D.offG[m] = S.offG[m]; D.strideG[m] = S.strideG[m]; D.ntR[m] = S.ntR[m]; D.offR[m] = S.offR[m];
-    D.strideR[m] = S.strideR[m]; D.ntL[m] = S.ntL[m]; D.offL[m] = S.offL[m]; D.strideL[m] = S.strideL[m]; }
+  D.nG = S.nG; D.nR = S.nR; D.nL = S.nL; D.nwords = (int)S.words.size(); D.offF = S.offF;
+  for (int m = 0; m < 6; m++) { D.offG[m] = S.offG[m]; D.strideG[m] = S.strideG[m]; D.offR[m] = S.offR[m]; D.strideR[m] = S.strideR[m]; D.offL[m] = S.offL[m]; D.strideL[m] = S.strideL[m]; }
   const rwgt_params* ps[2] = {&po, &pn};
   double fact = 1; for (int i = 2; i <= n - 2; i++) fact *= i;
   for (int k = 0; k < 2; k++) {
     double gs = std::sqrt(4.0 * 3.14159265358979323846 * ps[k]->alpha_s);
     D.set[k].gq = gs; D.set[k].g3 = gs * ps[k]->ggg_scale; D.set[k].g4 = gs * gs * ps[k]->gggg_scale; D.set[k].mt = ps[k]->mt;
-    D.set[k].fac = gs * gs / (256.0 * fact);
+    D.set[k].fac = 2.0 * gs * gs / (256.0 * fact);
   }
   D.shared_ext = (po.mt == pn.mt) ? 1 : 0;
-  // rows per colour chunk: aim at ~256 colour tasks per slot-batch
-  // colour tasks per slot and batch = ncol * nchunk: a multiple of 32 (warp-aligned reduction) and at most 256
-  int nchunk = std::max(1, std::min(S.nperm, 256 / S.ncol)); if ((S.ncol * nchunk) % 32) nchunk &= ~1;
-  D.rows_per_chunk = (S.nperm + nchunk - 1) / nchunk; D.nchunk = nchunk;
   int dev = 0; cudaGetDevice(&dev); cudaDeviceProp prop; cudaGetDeviceProperties(&prop, dev);
   B->sm_count = prop.multiProcessorCount; size_t maxsm = prop.sharedMemPerBlockOptin;
-  auto pick = [&](size_t sz, int& nslot, size_t& bytes) {
+  auto pick = [&](bool dbl, int& nslot, size_t& bytes) {
     int cap = (n == 2) ? 64 : (n == 3) ? 32 : (n == 4) ? 8 : 1; nslot = 0;
-    for (int e = cap; e >= 1; e--) if (smem_bytes(S, e, sz) <= maxsm) { nslot = e; break; }
-    bytes = nslot ? smem_bytes(S, nslot, sz) : 0;
+    for (int e = cap; e >= 1; e--) if (smem_need_n(n, S, e, dbl) <= maxsm) { nslot = e; break; }
+    bytes = nslot ? smem_need_n(n, S, nslot, dbl) : 0;
   };
-  pick(8, B->nslot64, B->smem64); pick(4, B->nslot32, B->smem32);
+  pick(true, B->nslot64, B->smem64); pick(false, B->nslot32, B->smem32);
   if (!B->nslot64 || !B->nslot32) { err = "not enough shared memory per block on this device"; delete B; return nullptr; }
-  std::vector<double> C = colour_matrix_fierz(n); std::vector<float> Cf(C.begin(), C.end());
   cudaError_t e = cudaMalloc((void**)&B->d_words, S.words.size() * sizeof(uint32_t));
-  if (e == cudaSuccess) e = cudaMalloc((void**)&B->d_C64, C.size() * sizeof(double));
-  if (e == cudaSuccess) e = cudaMalloc((void**)&B->d_C32, Cf.size() * sizeof(float));
+  if (e == cudaSuccess) e = cudaMalloc((void**)&B->d_lfrag, S.lfrag.size() * sizeof(double));
   if (e == cudaSuccess) e = cudaMemcpy(B->d_words, S.words.data(), S.words.size() * sizeof(uint32_t), cudaMemcpyHostToDevice);
-  if (e == cudaSuccess) e = cudaMemcpy(B->d_C64, C.data(), C.size() * sizeof(double), cudaMemcpyHostToDevice);
-  if (e == cudaSuccess) e = cudaMemcpy(B->d_C32, Cf.data(), Cf.size() * sizeof(float), cudaMemcpyHostToDevice);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<double, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)B->smem64);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<float, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)B->smem32);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<float, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)B->smem32);
+  if (e == cudaSuccess) e = cudaMemcpy(B->d_lfrag, S.lfrag.data(), S.lfrag.size() * sizeof(double), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) switch (n) { case 2: e = bg_set_attr<2>(B->smem64, B->smem32); break; case 3: e = bg_set_attr<3>(B->smem64, B->smem32); break;
+                                     case 4: e = bg_set_attr<4>(B->smem64, B->smem32); break; default: e = bg_set_attr<5>(B->smem64, B->smem32); }
   if (e != cudaSuccess) { err = std::string("CUDA: ") + cudaGetErrorString(e); delete B; return nullptr; }
-  D.words = B->d_words; D.C64 = B->d_C64; D.C32 = B->d_C32;
+  D.words = B->d_words; D.lfrag = B->d_lfrag;
   return B;
 }
-static void bg_destroy(BgProcess* B) { if (!B) return; cudaFree(B->d_words); cudaFree(B->d_C64); cudaFree(B->d_C32); delete B; }
-static double bg_flops_per_event(const BgProcess* B, int /*precision*/) { return 2.0 * (2.0 * B->S.fp_per_set + B->S.fp_shared); }
+static void bg_destroy(BgProcess* B) { if (!B) return; cudaFree(B->d_words); cudaFree(B->d_lfrag); delete B; }
+
+// FP-pipe instruction model (FMA, MUL, ADD each 1 instruction) of the schedule, both parameter sets; see DESIGN.md "Flop counts".
+static double bg_fp_instr_per_event(const BgProcess* B) {
+  const int n = B->S.n, C = B->S.c, NJ = n - C + 1; const double L3 = 90, V4 = 102, SL = 40, PROP = 43, RC = 16, GST = 24;
+  auto tup = [](int n, int m) { double r = 1; for (int i = 0; i < m; i++) r *= (n - i); return r; };
+  double fp = 0;
+  for (int m = 2; m <= n - 1; m++) fp += tup(n, m) / 2 * (1 << m) * ((m - 1) * L3 + (m - 1) * (m - 2) / 2 * V4 + GST);
+  for (int m = 1; m <= B->S.rmax; m++) fp += tup(n, m) * (2 << m) * (m * (SL + 8) + PROP);
+  for (int m = 1; m <= B->S.lmax; m++) fp += tup(n, m) * (2 << m) * (m * (SL + 8) + PROP);
+  double per_final = (n - 1) * L3 + (n - 1) * (n - 2) / 2 * V4 + GST + 2 * (NJ * C * 2 * (SL + 8) + NJ * 4 * RC);
+  fp += B->S.npair * (double)(1 << (n - 1)) * per_final;
+  // colour: upper-triangular mma tiles, 256 FMA each, over 2*ncol real columns
+  int npp = (B->S.nperm + 7) / 8 * 8, MT = npp / 8, KT = npp / 4; double ksteps = 0; for (int mt = 0; mt < MT; mt++) ksteps += KT - 2 * mt;
+  fp += ksteps * ((double)(4 << (n - 1)) * 2 / 8) * 256.0;
+  return 2.0 * fp + n * 2 * 30.0 + 4 * 40.0 + (1 << n) * 40.0;
+}
+static double bg_flops_per_event(const BgProcess* B, int /*precision*/) { return 2.0 * bg_fp_instr_per_event(B); }
+
 static int bg_run(BgProcess* B, int precision, const double* mom, const double* w, double* a, double* b, double* o, long long nev, cudaStream_t st) {
-  BgDev D = B->D;
-  if (precision == RWGT_FP64) {
-    D.nslot = B->nslot64; long long ngroups = (nev + D.nslot - 1) / D.nslot; int grid = (int)std::min<long long>(ngroups, B->sm_count);
-    bg_kernel<double, false><<<grid, 256, B->smem64, st>>>(mom, w, a, b, o, nev, D);
-  } else {
-    D.nslot = B->nslot32; long long ngroups = (nev + D.nslot - 1) / D.nslot; int grid = (int)std::min<long long>(ngroups, B->sm_count);
-    if (precision == RWGT_FP32) bg_kernel<float, false><<<grid, 256, B->smem32, st>>>(mom, w, a, b, o, nev, D);
-    else bg_kernel<float, true><<<grid, 256, B->smem32, st>>>(mom, w, a, b, o, nev, D);
+  BgDev D = B->D; const bool dbl = (precision == RWGT_FP64);
+  D.nslot = dbl ? B->nslot64 : B->nslot32;
+  long long ngroups = (nev + D.nslot - 1) / D.nslot; int grid = (int)std::min<long long>(ngroups, B->sm_count);
+  switch (B->S.n) {
+    case 2: bg_launch<2>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, D); break;
+    case 3: bg_launch<3>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, D); break;
+    case 4: bg_launch<4>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, D); break;
+    default: bg_launch<5>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, D);
   }
   return 0;
 }

@@ -10,6 +10,7 @@
 #include "../../include/rwgt.h"
 #include "kernels_small.cuh"
 #include "bg_engine.cuh"
+#include "microbench.cuh"
 
 namespace {
 
@@ -174,6 +175,11 @@ int rwgt_destroy(rwgt_handle* h) {
   if (h->scratch) cudaFree(h->scratch);
   delete h;
   return 0;
+}
+
+int rwgt_measure_peak(int kind, double* out_tflops) {
+  if (kind < 0 || kind > 2 || !out_tflops) return -1;
+  return rwgt::measure_peak(kind, out_tflops);
 }
 
 int rwgt_colour_matrix(int n_gluons, double* out) {
