@@ -135,19 +135,25 @@ static void all_tuples(int n, int m, std::vector<std::vector<int>>& out) {
 // compile-time geometry of the schedule for N gluons (mirrored by build_schedule and checked in bg_create)
 __host__ __device__ constexpr int cfact(int n) { return n <= 1 ? 1 : n * cfact(n - 1); }
 __host__ __device__ constexpr int ctuples(int n, int m) { return cfact(n) / cfact(n - m); }     // ordered m-tuples of n labels
+__host__ __device__ constexpr int c_nG(int n) { int r = 0; for (int m = 1; m <= n - 1; m++) r += (m == 1 ? n : ctuples(n, m) / 2) << m; return r; }
+__host__ __device__ constexpr int c_nQ(int n, int mmax) { int r = 2; for (int m = 1; m <= mmax; m++) r += ctuples(n, m) * (2 << m); return r; }
 template <int N> struct Geo {
   static constexpr int C = (N + 1) / 2, LMAX = C - 1, RMAX = N - C, NJ = N - C + 1;            // N=2: C=1; 3: 2; 4: 2; 5: 3
   static constexpr int NPERM = cfact(N), NPAIR = NPERM / 2, NPERM_P = (NPERM + 7) / 8 * 8;
-  static constexpr int NB = (N == 5) ? 1 : 0, NBATCH = 1 << NB;          // helicity batches (amplitude buffer size)
-  static constexpr int NFREE = 1 << (N - 1 - NB), NCOL = NFREE * 4;      // gluon 0 has helicity + only (parity), x4 quark helicities
+  // helicity batches: gluon 0 has helicity + only (parity); NB more gluon helicities are fixed per batch so that a
+  // batch is 16 amplitude columns (4 free gluon configurations x 4 quark helicities) for N >= 3
+  static constexpr int NB = (N == 5) ? 2 : (N == 4) ? 1 : 0, NBATCH = 1 << NB;
+  static constexpr int NFREE = 1 << (N - 1 - NB), NCOL = NFREE * 4;
   static constexpr int ASTR = 2 * NCOL + 4;                              // row stride (doubles) of the amplitude buffer, bank-conflict-free
   static constexpr int MT = NPERM_P / 8, KT = NPERM_P / 4, U = (MT + 1) / 2;
-  static constexpr int NT_ALL = 2 * NCOL / 8, NTG = (N == 4) ? 2 : 1, NT = NT_ALL / NTG;
+  static constexpr int NT = 2 * NCOL / 8;                                // mma n-tiles per batch
   static constexpr int NMASK = 1 << N;
   static constexpr int NPHASE = (N - 1 > (RMAX > LMAX ? RMAX : LMAX) + 1) ? N - 1 : (RMAX > LMAX ? RMAX : LMAX) + 1;
   static constexpr int NL3 = N - 1, NV4 = (N - 1) * (N - 2) / 2;
   static constexpr int WOFF_TERMS = 4 + 2 * NL3 + 3 * NV4, WPER = C + NJ + NJ * C;
   static constexpr int STRIDEF = WOFF_TERMS + 2 * WPER;
+  static constexpr size_t ABUF = (size_t)NPERM_P * ASTR;                 // doubles per slot per buffer
+  static constexpr int NG = c_nG(N), NR = c_nQ(N, RMAX), NL = c_nQ(N, LMAX);   // entries of the current tables (checked against the schedule)
 };
 
 static BgSched build_schedule(int n) {
@@ -227,7 +233,7 @@ static BgSched build_schedule(int n) {
 struct BgSet { double gq, g3, g4, mt, fac; };        // fac = 2 gq^2 / D  (|i gq|^2, parity factor 2, averaging)
 struct BgDev {
   int nG, nR, nL, nwords, nslot, shared_ext;
-  int offG[6], strideG[6], offR[6], strideR[6], offL[6], strideL[6], offF;
+  int offG[6], offR[6], offL[6], offF;
   const uint32_t* words; const double* lfrag;
   BgSet set[2];
 };
@@ -239,17 +245,17 @@ struct BgProcess {
 template <typename T> struct Smem {
   uint32_t* W;    // schedule words (whole CTA)
   double* pm;     // [nslot][n_ext][4] momenta (always double)
-  double* acc;    // [nslot][2]
-  double* red;    // [nslot][8] per-warp partial sums of the colour form
+  double* acc;    // [nslot][2]   helicity-summed colour forms (owned by the colour warps)
+  double* red;    // [nslot][8]   per-warp partial sums of the colour form
   T* G; T* R; T* L;  // [nslot][8][nX]   SoA planes: conflict-free for consecutive helicity variants
   T* K;           // [nslot][NMASK][4] momentum sums of gluon subsets
   T* iK2;         // [nslot][NMASK]
   T* dR; T* dL;   // [nslot][NMASK] 1/(q^2-m^2)
-  double* A;      // [nslot][NPERM_P][ASTR] colour-flow amplitudes (re,im interleaved along the row), always double
+  double* A;      // [2][nslot][NPERM_P][ASTR] double-buffered colour-flow amplitudes (re,im interleaved), always double
 };
-template <int N, typename T> __host__ __device__ inline size_t carve(Smem<T>& s, unsigned char* base, int ns, int nG, int nR, int nL, int nwords) {
-  typedef Geo<N> Ge; size_t off = 0;
-  s.A = (double*)(base + off); off += sizeof(double) * (size_t)ns * Ge::NPERM_P * Ge::ASTR;
+template <int N, typename T> __host__ __device__ inline size_t carve(Smem<T>& s, unsigned char* base, int ns, int nwords) {
+  typedef Geo<N> Ge; size_t off = 0; constexpr int nG = Ge::NG, nR = Ge::NR, nL = Ge::NL;
+  s.A = (double*)(base + off); off += sizeof(double) * 2 * (size_t)ns * Ge::ABUF;
   s.pm = (double*)(base + off); off += sizeof(double) * ns * (N + 2) * 4;
   s.acc = (double*)(base + off); off += sizeof(double) * ns * 2;
   s.red = (double*)(base + off); off += sizeof(double) * ns * 8;
@@ -288,25 +294,32 @@ __device__ __forceinline__ int ref_entry(uint32_t r, uint32_t v) {
 }
 __device__ __forceinline__ int ref_m(uint32_t r) { return (int)((r >> 16) & 7u); }
 __device__ __forceinline__ int ref_mask(uint32_t r) { return (int)((r >> 24) & 31u); }
-template <typename T> __device__ __forceinline__ T ref_sign(uint32_t r) { return (r & REF_NEG) ? T(-1) : T(1); }
+__device__ __forceinline__ bool ref_neg(uint32_t r) { return (r & REF_NEG) != 0; }
+
+// named barriers (ids 1..6; id 0 is __syncthreads): workers among themselves, colour warps among themselves,
+// and the full/empty handshake of the two amplitude buffers
+enum { BAR_WORK = 1, BAR_FULL0 = 2, BAR_EMPTY0 = 4, BAR_COLOUR = 6 };
+__device__ __forceinline__ void bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+__device__ __forceinline__ void bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 
 // gluon current of one ordered M-tuple / helicity variant from shorter currents (unscaled by the propagator)
-template <int M, typename T> __device__ __forceinline__ vec4<T> gluon_sum(const uint32_t* w, uint32_t v, const T* G, int nG, const T* K, T g3, T g4) {
+template <int M, int nG, typename T> __device__ __forceinline__ vec4<T> gluon_sum(const uint32_t* w, uint32_t v, const T* G, const T* K, T g3, T g4) {
   vec4<T> a3, a4;
 #pragma unroll
   for (int i = 0; i < 4; i++) { a3.c[i] = mk<T>(0, 0); a4.c[i] = mk<T>(0, 0); }
 #pragma unroll
   for (int k = 0; k < M - 1; k++) {
     uint32_t ra = w[2 * k], rb = w[2 * k + 1];
-    vec4<T> A = ld4(G, nG, ref_entry(ra, v)), B = ld4(G, nG, ref_entry(rb, v));
-    L3_acc(a3, ref_sign<T>(ra) * ref_sign<T>(rb), A, K + 4 * ref_mask(ra), B, K + 4 * ref_mask(rb));
+    vec4<T> A = cond_neg(ld4(G, nG, ref_entry(ra, v)), ref_neg(ra) != ref_neg(rb)), B = ld4(G, nG, ref_entry(rb, v));
+    L3_acc(a3, A, K + 4 * ref_mask(ra), B, K + 4 * ref_mask(rb));
   }
   const uint32_t* w4 = w + 2 * (M - 1);
 #pragma unroll
   for (int t = 0; t < (M - 1) * (M - 2) / 2; t++) {
     uint32_t rx = w4[3 * t], ry = w4[3 * t + 1], rz = w4[3 * t + 2];
-    vec4<T> X = ld4(G, nG, ref_entry(rx, v)), Y = ld4(G, nG, ref_entry(ry, v)), Z = ld4(G, nG, ref_entry(rz, v));
-    V4_acc(a4, ref_sign<T>(rx) * ref_sign<T>(ry) * ref_sign<T>(rz), X, Y, Z);
+    vec4<T> X = cond_neg(ld4(G, nG, ref_entry(rx, v)), (ref_neg(rx) != ref_neg(ry)) != ref_neg(rz));
+    vec4<T> Y = ld4(G, nG, ref_entry(ry, v)), Z = ld4(G, nG, ref_entry(rz, v));
+    V4_acc(a4, X, Y, Z);
   }
   vec4<T> r;
 #pragma unroll
@@ -315,17 +328,17 @@ template <int M, typename T> __device__ __forceinline__ vec4<T> gluon_sum(const 
 }
 
 template <typename T> struct Ctx {
-  Smem<T> s; int tid, ns, nG, nR, nL; T g3, g4, gq, mt; const BgDev* D;
+  Smem<T> s; int tid, ns; T g3, g4, gq, mt; const BgDev* D;
 };
 
-// phase M: gluon currents of length M, right/left quark currents of length M-1 (all helicity variants)
-template <int N, int M, typename T, int NTH> __device__ __forceinline__ void level_phase(const Ctx<T>& c) {
+// phase M (worker warps): gluon currents of length M, right/left quark currents of length M-1 (all helicity variants)
+template <int N, int M, typename T, int NWT> __device__ __forceinline__ void level_phase(const Ctx<T>& c) {
   typedef Geo<N> Ge;
   constexpr bool HASG = (M <= N - 1), HASR = (M - 1 >= 1 && M - 1 <= Ge::RMAX), HASL = (M - 1 >= 1 && M - 1 <= Ge::LMAX);
   constexpr int MM = M - 1;
   constexpr int tg = HASG ? (ctuples(N, M) / 2) << M : 0, tr = HASR ? ctuples(N, MM) << M : 0, tl = HASL ? ctuples(N, MM) << M : 0, per = tg + tr + tl;
-  const Smem<T>& s = c.s; const int nG = c.nG, nR = c.nR, nL = c.nL, next = N + 2;
-  for (int t = c.tid; t < c.ns * per; t += NTH) {
+  const Smem<T>& s = c.s; constexpr int nG = Ge::NG, nR = Ge::NR, nL = Ge::NL, next = N + 2;
+  for (int t = c.tid; t < c.ns * per; t += NWT) {
     int sl = t / per, o = t % per;
     T* G = s.G + (size_t)sl * 8 * nG; T* R = s.R + (size_t)sl * 8 * nR; T* L = s.L + (size_t)sl * 8 * nL;
     const T* K = s.K + (size_t)sl * Ge::NMASK * 4;
@@ -333,7 +346,7 @@ template <int N, int M, typename T, int NTH> __device__ __forceinline__ void lev
       int tup = o >> M; uint32_t v = o & ((1 << M) - 1);
       const uint32_t* w = s.W + c.D->offG[M] + tup * (2 + 2 * (M - 1) + 3 * (M - 1) * (M - 2) / 2);
       int ob = w[0], mask = w[1];
-      vec4<T> r = gluon_sum<M, T>(w + 2, v, G, nG, K, c.g3, c.g4);
+      vec4<T> r = gluon_sum<M, nG, T>(w + 2, v, G, K, c.g3, c.g4);
       T sc = s.iK2[sl * Ge::NMASK + mask];
 #pragma unroll
       for (int i = 0; i < 4; i++) r.c[i] = sc * r.c[i];
@@ -348,11 +361,8 @@ template <int N, int M, typename T, int NTH> __device__ __forceinline__ void lev
 #pragma unroll
       for (int k = 0; k < MM; k++) {
         uint32_t rj = w[2 + 2 * k], rr = w[3 + 2 * k];
-        vec4<T> J = ld4(G, nG, ref_entry(rj, v));
-        spn<T> Rr = lds4(R, nR, ref_entry(rr, v) + (hb << ref_m(rr)));
-        spn<T> x = slash_c(J, Rr); T sg = ref_sign<T>(rj);
-#pragma unroll
-        for (int i = 0; i < 4; i++) rfma(acc.c[i], sg, x.c[i]);
+        lcv<T> J = lightcone(cond_neg(ld4(G, nG, ref_entry(rj, v)), ref_neg(rj)));
+        slash_acc(acc, J, lds4(R, nR, ref_entry(rr, v) + (hb << ref_m(rr))));
       }
       T q[4];
 #pragma unroll
@@ -371,11 +381,8 @@ template <int N, int M, typename T, int NTH> __device__ __forceinline__ void lev
 #pragma unroll
       for (int k = 0; k < MM; k++) {
         uint32_t rl = w[2 + 2 * k], rj = w[3 + 2 * k];
-        spn<T> Ll = lds4(L, nL, ref_entry(rl, v) + (hb << ref_m(rl)));
-        vec4<T> J = ld4(G, nG, ref_entry(rj, v));
-        spn<T> x = row_slash_c(Ll, J); T sg = ref_sign<T>(rj);
-#pragma unroll
-        for (int i = 0; i < 4; i++) rfma(acc.c[i], sg, x.c[i]);
+        lcv<T> J = lightcone(cond_neg(ld4(G, nG, ref_entry(rj, v)), ref_neg(rj)));
+        row_slash_acc(acc, lds4(L, nL, ref_entry(rl, v) + (hb << ref_m(rl))), J);
       }
       T q[4];
 #pragma unroll
@@ -386,157 +393,181 @@ template <int N, int M, typename T, int NTH> __device__ __forceinline__ void lev
       st4(L, nL, ob + v + (hb << MM), r);
     }
   }
-  __syncthreads();
+  bar_sync(BAR_WORK, NWT);
 }
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-// MIXED: T = float but momentum sums / propagator denominators are formed in double before rounding to T.
-// The colour form and the helicity sum are accumulated in double in every mode (FP64 tensor-core mma).
-template <int N, typename T, bool MIXED, int NTH>
-__global__ void __launch_bounds__(NTH, 1) bg_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
-                                                    double* __restrict__ me_old, double* __restrict__ me_new,
-                                                    double* __restrict__ w_new, long long nev, BgDev D) {
+// One persistent CTA per SM.  Warps 0..NW-1 ("workers") build the currents and the colour-flow amplitudes of one helicity
+// batch after the other on the FP64 pipe; the last NCW warps ("colour") turn finished batches into |L^T J|^2 on the FP64
+// tensor pipe (a separate pipe, so the two overlap) and write the outputs.  The two amplitude buffers are handed over with
+// named barriers.  MIXED: T = float but momentum sums / propagator denominators are formed in double before rounding to T.
+template <int N, typename T, bool MIXED, int NW, int NCW>
+__global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
+                                                               double* __restrict__ me_old, double* __restrict__ me_new,
+                                                               double* __restrict__ w_new, long long nev, BgDev D) {
   typedef Geo<N> Ge;
+  constexpr int NTH = (NW + NCW) * 32, NWT = NW * 32, NCT = NCW * 32;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  Ctx<T> c; c.D = &D; c.tid = threadIdx.x; c.ns = D.nslot; c.nG = D.nG; c.nR = D.nR; c.nL = D.nL;
-  carve<N, T>(c.s, smem_raw, D.nslot, D.nG, D.nR, D.nL, D.nwords);
+  Ctx<T> c; c.D = &D; c.ns = D.nslot;
+  carve<N, T>(c.s, smem_raw, D.nslot, D.nwords);
   const Smem<T>& s = c.s;
   typedef typename std::conditional<MIXED, double, T>::type TK;
-  const int tid = threadIdx.x, next = N + 2, ns = D.nslot, nG = D.nG, nR = D.nR, nL = D.nL;
-  // once per CTA: schedule words into shared memory, zero the padding rows of the amplitude buffer
-  for (int t = tid; t < D.nwords; t += NTH) s.W[t] = __ldg(D.words + t);
-  for (int t = tid; t < ns * Ge::NPERM_P * Ge::ASTR; t += NTH) s.A[t] = 0.0;
+  constexpr int next = N + 2, nG = Ge::NG, nR = Ge::NR, nL = Ge::NL; const int ns = D.nslot;
   const long long ngroups = (nev + ns - 1) / ns;
-  for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
-    const long long ev0 = grp * ns;
-    __syncthreads();   // previous group's outputs were read; words are visible
-    // ---- a1: load momenta (coalesced over the events of the group) ----
-    for (int t = tid; t < ns * next * 4; t += NTH) {
-      int sl = t % ns, comp = t / ns; long long ev = ev0 + sl; if (ev >= nev) ev = nev - 1;
-      s.pm[(sl * next * 4) + comp] = __ldg(mom + (size_t)comp * nev + ev);
-    }
-    if (tid < ns * 2) s.acc[tid] = 0.0;
-    __syncthreads();
-#pragma unroll 1
-    for (int iset = 0; iset < 2; iset++) {
-      const BgSet& P = D.set[iset];
-      c.g3 = (T)P.g3; c.g4 = (T)P.g4; c.gq = (T)P.gq; c.mt = (T)P.mt;
-      if (iset == 0 || !D.shared_ext) {
-        // ---- a2: external wavefunctions, momentum sums, propagator denominators ----
-        constexpr int nobj = 2 * N + 4 + Ge::NMASK;
-        for (int t = tid; t < ns * nobj; t += NTH) {
-          int sl = t / nobj, o = t % nobj; const double* pm = s.pm + sl * next * 4;
-          if (o < 2 * N) {                         // gluon i, helicity bit hb (0: +1, 1: -1); entry = 2*i + hb
-            int i = o >> 1, hb = o & 1, leg = i < 2 ? i : i + 2; const double* p = pm + 4 * leg;
-            vec4<T> e = polvec<T>((T)p[1], (T)p[2], (T)p[3], hb ? -1 : +1);
-            if (i >= 2) e = conj4(e);              // outgoing gluon carries eps*
-            st4(s.G + (size_t)sl * 8 * nG, nG, 2 * i + hb, e);
-          } else if (o < 2 * N + 2) {              // v(p_tbar, lam), R() entries 0,1
-            int hb = o - 2 * N; const double* p = pm + 12;
-            chi_pair<T> x = make_chi<T>((T)p[1], (T)p[2], (T)p[3]);
-            st4(s.R + (size_t)sl * 8 * nR, nR, hb, spinor_v<T>(x, (T)p[0], c.mt, hb ? -1 : +1));
-          } else if (o < 2 * N + 4) {              // ubar(p_t, lam), L() entries 0,1
-            int hb = o - 2 * N - 2; const double* p = pm + 8;
-            chi_pair<T> x = make_chi<T>((T)p[1], (T)p[2], (T)p[3]);
-            st4(s.L + (size_t)sl * 8 * nL, nL, hb, bar(spinor_u<T>(x, (T)p[0], c.mt, hb ? -1 : +1)));
-          } else {                                 // gluon subset `mask`
-            int mask = o - 2 * N - 4;
-            TK k[4] = {0, 0, 0, 0};
-#pragma unroll
-            for (int i = 0; i < N; i++) if (mask >> i & 1) { int leg = i < 2 ? i : i + 2; TK sg = i < 2 ? TK(1) : TK(-1);
-              for (int mu = 0; mu < 4; mu++) k[mu] += sg * (TK)pm[4 * leg + mu]; }
-            TK k2 = mdot_rr<TK>(k, k);
-            TK qr[4], ql[4]; for (int mu = 0; mu < 4; mu++) { qr[mu] = k[mu] - (TK)pm[12 + mu]; ql[mu] = (TK)pm[8 + mu] - k[mu]; }
-            TK m2 = (TK)P.mt * (TK)P.mt;
-            T* K = s.K + ((size_t)sl * Ge::NMASK + mask) * 4; for (int mu = 0; mu < 4; mu++) K[mu] = (T)k[mu];
-            s.iK2[sl * Ge::NMASK + mask] = (__popc(mask) >= 2) ? (T)(TK(1) / k2) : T(0);
-            s.dR[sl * Ge::NMASK + mask] = (T)(TK(1) / (mdot_rr<TK>(qr, qr) - m2));
-            s.dL[sl * Ge::NMASK + mask] = (T)(TK(1) / (mdot_rr<TK>(ql, ql) - m2));
-          }
-        }
-        __syncthreads();
+  // once per CTA: zero both amplitude buffers (their padding rows are never written again)
+  for (int t = threadIdx.x; t < 2 * ns * (int)Ge::ABUF; t += NTH) s.A[t] = 0.0;
+  __syncthreads();
+  if (threadIdx.x < NWT) {
+    // =========================================================================================== worker warps
+    const int tid = threadIdx.x; c.tid = tid;
+    for (int t = tid; t < D.nwords; t += NWT) s.W[t] = __ldg(D.words + t);
+    unsigned step = 0;
+    for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+      const long long ev0 = grp * ns;
+      bar_sync(BAR_WORK, NWT);
+      // ---- a1: load momenta (coalesced over the events of the group) ----
+      for (int t = tid; t < ns * next * 4; t += NWT) {
+        int sl = t % ns, comp = t / ns; long long ev = ev0 + sl; if (ev >= nev) ev = nev - 1;
+        s.pm[(sl * next * 4) + comp] = __ldg(mom + (size_t)comp * nev + ev);
       }
-      // ---- a3: current levels ----
-      level_phase<N, 2, T, NTH>(c);
-      if constexpr (Ge::NPHASE >= 3) level_phase<N, 3, T, NTH>(c);
-      if constexpr (Ge::NPHASE >= 4) level_phase<N, 4, T, NTH>(c);
-      // ---- a3/a4: colour-flow amplitudes of a helicity batch; a5/a6: colour form |L^T J|^2 and helicity sum ----
+      bar_sync(BAR_WORK, NWT);
 #pragma unroll 1
-      for (int batch = 0; batch < Ge::NBATCH; batch++) {
-        constexpr int per = Ge::NPAIR * Ge::NFREE;
-        for (int t = tid; t < ns * per; t += NTH) {
-          int sl = t / per, o = t % per; int pair = o / Ge::NFREE, f = o % Ge::NFREE;
-          const T* G = s.G + (size_t)sl * 8 * nG; const T* R = s.R + (size_t)sl * 8 * nR; const T* L = s.L + (size_t)sl * 8 * nL;
-          const T* K = s.K + (size_t)sl * Ge::NMASK * 4;
-          const uint32_t* w = s.W + D.offF + pair * Ge::STRIDEF;
-          uint32_t rk = w[0], rkr = w[1], packed = w[2], negr = w[3];
-          uint32_t g = ((uint32_t)batch << 1) | ((uint32_t)f << (1 + Ge::NB));   // helicity bits by gluon label; gluon 0: + (parity)
-          uint32_t v = 0;
+      for (int iset = 0; iset < 2; iset++) {
+        const BgSet& P = D.set[iset];
+        c.g3 = (T)P.g3; c.g4 = (T)P.g4; c.gq = (T)P.gq; c.mt = (T)P.mt;
+        if (iset == 0 || !D.shared_ext) {
+          // ---- a2: external wavefunctions, momentum sums, propagator denominators ----
+          constexpr int nobj = 2 * N + 4 + Ge::NMASK;
+          for (int t = tid; t < ns * nobj; t += NWT) {
+            int sl = t / nobj, o = t % nobj; const double* pm = s.pm + sl * next * 4;
+            if (o < 2 * N) {                         // gluon i, helicity bit hb (0: +1, 1: -1); entry = 2*i + hb
+              int i = o >> 1, hb = o & 1, leg = i < 2 ? i : i + 2; const double* p = pm + 4 * leg;
+              vec4<T> e = polvec<T>((T)p[1], (T)p[2], (T)p[3], hb ? -1 : +1);
+              if (i >= 2) e = conj4(e);              // outgoing gluon carries eps*
+              st4(s.G + (size_t)sl * 8 * nG, nG, 2 * i + hb, e);
+            } else if (o < 2 * N + 2) {              // v(p_tbar, lam), R() entries 0,1
+              int hb = o - 2 * N; const double* p = pm + 12;
+              chi_pair<T> x = make_chi<T>((T)p[1], (T)p[2], (T)p[3]);
+              st4(s.R + (size_t)sl * 8 * nR, nR, hb, spinor_v<T>(x, (T)p[0], c.mt, hb ? -1 : +1));
+            } else if (o < 2 * N + 4) {              // ubar(p_t, lam), L() entries 0,1
+              int hb = o - 2 * N - 2; const double* p = pm + 8;
+              chi_pair<T> x = make_chi<T>((T)p[1], (T)p[2], (T)p[3]);
+              st4(s.L + (size_t)sl * 8 * nL, nL, hb, bar(spinor_u<T>(x, (T)p[0], c.mt, hb ? -1 : +1)));
+            } else {                                 // gluon subset `mask`
+              int mask = o - 2 * N - 4;
+              TK k[4] = {0, 0, 0, 0};
 #pragma unroll
-          for (int j = 0; j < N; j++) v |= ((g >> ((packed >> (3 * j)) & 7u)) & 1u) << j;   // by position in sigma
-          vec4<T> Jn = gluon_sum<N, T>(w + 4, v, G, nG, K, c.g3, c.g4);
-          T sc = s.iK2[sl * Ge::NMASK + Ge::NMASK - 1];
-#pragma unroll
-          for (int i = 0; i < 4; i++) Jn.c[i] = sc * Jn.c[i];
-          const spn<T> u0 = lds4(L, nL, 0), u1 = lds4(L, nL, 1);
-          double* A = s.A + (size_t)sl * Ge::NPERM_P * Ge::ASTR;
-          const uint32_t* wt = w + Ge::WOFF_TERMS;
-#pragma unroll
-          for (int which = 0; which < 2; which++) {
-            cx<T> Acc[2][2];
-#pragma unroll
-            for (int a = 0; a < 2; a++)
-#pragma unroll
-              for (int b = 0; b < 2; b++) Acc[a][b] = mk<T>(0, 0);
-            T sfull = (which && negr) ? T(-1) : T(1);
-#pragma unroll
-            for (int jj = 0; jj < Ge::NJ; jj++) {
-              spn<T> X0, X1;
-#pragma unroll
-              for (int i = 0; i < 4; i++) { X0.c[i] = mk<T>(0, 0); X1.c[i] = mk<T>(0, 0); }
-#pragma unroll
-              for (int i = 0; i < Ge::C; i++) {
-                spn<T> y0, y1; T sg;
-                if (i == 0 && jj == Ge::NJ - 1) { y0 = row_slash_c(u0, Jn); y1 = row_slash_c(u1, Jn); sg = sfull; }
-                else {
-                  uint32_t rl = wt[i], rj = wt[Ge::C + Ge::NJ + jj * Ge::C + i];
-                  vec4<T> J = ld4(G, nG, ref_entry(rj, v)); sg = ref_sign<T>(rj);
-                  int el = ref_entry(rl, v), ml = ref_m(rl);
-                  y0 = row_slash_c(lds4(L, nL, el), J); y1 = row_slash_c(lds4(L, nL, el + (1 << ml)), J);
-                }
-#pragma unroll
-                for (int q = 0; q < 4; q++) { rfma(X0.c[q], sg, y0.c[q]); rfma(X1.c[q], sg, y1.c[q]); }
-              }
-              uint32_t rr = wt[Ge::C + jj]; int er = ref_entry(rr, v), mr = ref_m(rr);
-#pragma unroll
-              for (int hb = 0; hb < 2; hb++) {
-                spn<T> Rr = lds4(R, nR, er + (hb << mr));
-                cx<T> a0 = rowcol(X0, Rr), a1 = rowcol(X1, Rr);
-                Acc[0][hb] = Acc[0][hb] + a0; Acc[1][hb] = Acc[1][hb] + a1;
-              }
+              for (int i = 0; i < N; i++) if (mask >> i & 1) { int leg = i < 2 ? i : i + 2; TK sg = i < 2 ? TK(1) : TK(-1);
+                for (int mu = 0; mu < 4; mu++) k[mu] += sg * (TK)pm[4 * leg + mu]; }
+              TK k2 = mdot_rr<TK>(k, k);
+              TK qr[4], ql[4]; for (int mu = 0; mu < 4; mu++) { qr[mu] = k[mu] - (TK)pm[12 + mu]; ql[mu] = (TK)pm[8 + mu] - k[mu]; }
+              TK m2 = (TK)P.mt * (TK)P.mt;
+              T* K = s.K + ((size_t)sl * Ge::NMASK + mask) * 4; for (int mu = 0; mu < 4; mu++) K[mu] = (T)k[mu];
+              s.iK2[sl * Ge::NMASK + mask] = (__popc(mask) >= 2) ? (T)(TK(1) / k2) : T(0);
+              s.dR[sl * Ge::NMASK + mask] = (T)(TK(1) / (mdot_rr<TK>(qr, qr) - m2));
+              s.dL[sl * Ge::NMASK + mask] = (T)(TK(1) / (mdot_rr<TK>(ql, ql) - m2));
             }
-            uint32_t row = which ? rkr : rk;
-#pragma unroll
-            for (int ht = 0; ht < 2; ht++)
-#pragma unroll
-              for (int hb = 0; hb < 2; hb++) {
-                int col = f * 4 + ht * 2 + hb;
-                *reinterpret_cast<double2*>(A + (size_t)row * Ge::ASTR + 2 * col) = make_double2((double)Acc[ht][hb].re, (double)Acc[ht][hb].im);
-              }
-            wt += Ge::WPER;
           }
+          bar_sync(BAR_WORK, NWT);
         }
-        __syncthreads();
-        // colour form: Z = L^T A with FP64 tensor-core mma (upper-triangular tiles only), sum of squares of Z
-        {
-          const int warp = tid >> 5, lane = tid & 31;
-          constexpr int UN = Ge::U * Ge::NTG;
-          for (int u = warp; u < ns * UN; u += NTH / 32) {
-            int sl = u / UN, rem = u % UN, unit = rem / Ge::NTG, grp = rem % Ge::NTG;
-            const double* A = s.A + (size_t)sl * Ge::NPERM_P * Ge::ASTR + grp * Ge::NT * 8 + (lane & 3) * Ge::ASTR + (lane >> 2);
+        // ---- a3: current levels ----
+        level_phase<N, 2, T, NWT>(c);
+        if constexpr (Ge::NPHASE >= 3) level_phase<N, 3, T, NWT>(c);
+        if constexpr (Ge::NPHASE >= 4) level_phase<N, 4, T, NWT>(c);
+        // ---- a3/a4: colour-flow amplitudes, one helicity batch per buffer hand-over ----
+#pragma unroll 1
+        for (int batch = 0; batch < Ge::NBATCH; batch++, step++) {
+          const int buf = step & 1;
+          if (step >= 2) bar_sync(BAR_EMPTY0 + buf, NTH);      // colour warps have finished reading this buffer
+          double* Abuf = s.A + (size_t)buf * ns * Ge::ABUF;
+          constexpr int per = Ge::NPAIR * Ge::NFREE;
+          for (int t = tid; t < ns * per; t += NWT) {
+            int sl = t / per, o = t % per; int pair = o / Ge::NFREE, f = o % Ge::NFREE;
+            const T* G = s.G + (size_t)sl * 8 * nG; const T* R = s.R + (size_t)sl * 8 * nR; const T* L = s.L + (size_t)sl * 8 * nL;
+            const T* K = s.K + (size_t)sl * Ge::NMASK * 4;
+            const uint32_t* w = s.W + D.offF + pair * Ge::STRIDEF;
+            uint32_t rk = w[0], rkr = w[1], packed = w[2], negr = w[3];
+            uint32_t g = ((uint32_t)batch << 1) | ((uint32_t)f << (1 + Ge::NB));   // helicity bits by gluon label; gluon 0: + (parity)
+            uint32_t v = 0;
+#pragma unroll
+            for (int j = 0; j < N; j++) v |= ((g >> ((packed >> (3 * j)) & 7u)) & 1u) << j;   // by position in sigma
+            vec4<T> Jn = gluon_sum<N, nG, T>(w + 4, v, G, K, c.g3, c.g4);
+            T sc = s.iK2[sl * Ge::NMASK + Ge::NMASK - 1];
+#pragma unroll
+            for (int i = 0; i < 4; i++) Jn.c[i] = sc * Jn.c[i];
+            double* A = Abuf + (size_t)sl * Ge::ABUF;
+            const uint32_t* wt = w + Ge::WOFF_TERMS;
+#pragma unroll 1
+            for (int which = 0; which < 2; which++) {
+              cx<T> Acc[2][2];
+#pragma unroll
+              for (int a = 0; a < 2; a++)
+#pragma unroll
+                for (int b = 0; b < 2; b++) Acc[a][b] = mk<T>(0, 0);
+#pragma unroll
+              for (int jj = 0; jj < Ge::NJ; jj++) {
+                spn<T> X0, X1;
+#pragma unroll
+                for (int i = 0; i < 4; i++) { X0.c[i] = mk<T>(0, 0); X1.c[i] = mk<T>(0, 0); }
+#pragma unroll
+                for (int i = 0; i < Ge::C; i++) {
+                  if (i == 0 && jj == Ge::NJ - 1) {                 // the full-length gluon current between ubar and v
+                    lcv<T> J = lightcone(cond_neg(Jn, which && negr));
+                    row_slash_acc(X0, lds4(L, nL, 0), J); row_slash_acc(X1, lds4(L, nL, 1), J);
+                  } else {
+                    uint32_t rl = wt[i], rj = wt[Ge::C + Ge::NJ + jj * Ge::C + i];
+                    lcv<T> J = lightcone(cond_neg(ld4(G, nG, ref_entry(rj, v)), ref_neg(rj)));
+                    int el = ref_entry(rl, v), ml = ref_m(rl);
+                    row_slash_acc(X0, lds4(L, nL, el), J); row_slash_acc(X1, lds4(L, nL, el + (1 << ml)), J);
+                  }
+                }
+                uint32_t rr = wt[Ge::C + jj]; int er = ref_entry(rr, v), mr = ref_m(rr);
+#pragma unroll
+                for (int hb = 0; hb < 2; hb++) {
+                  spn<T> Rr = lds4(R, nR, er + (hb << mr));
+                  rowcol_acc(Acc[0][hb], X0, Rr); rowcol_acc(Acc[1][hb], X1, Rr);
+                }
+              }
+              uint32_t row = which ? rkr : rk;
+#pragma unroll
+              for (int ht = 0; ht < 2; ht++)
+#pragma unroll
+                for (int hb = 0; hb < 2; hb++) {
+                  int col = f * 4 + ht * 2 + hb;
+                  *reinterpret_cast<double2*>(A + (size_t)row * Ge::ASTR + 2 * col) = make_double2((double)Acc[ht][hb].re, (double)Acc[ht][hb].im);
+                }
+              wt += Ge::WPER;
+            }
+          }
+          __threadfence_block();
+          bar_arrive(BAR_FULL0 + buf, NTH);                    // hand the batch to the colour warps
+        }
+        bar_sync(BAR_WORK, NWT);                               // the current tables are rewritten for the next parameter set / group
+      }
+    }
+  } else {
+    // =========================================================================================== colour warps
+    const int ctid = threadIdx.x - NWT, cwarp = ctid >> 5, lane = ctid & 31;
+    unsigned step = 0;
+    for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+      const long long ev0 = grp * ns;
+      if (ctid < ns * 2) s.acc[ctid] = 0.0;
+      for (int t = ctid + NCT; t < ns * 2; t += NCT) s.acc[t] = 0.0;
+      bar_sync(BAR_COLOUR, NCT);
+#pragma unroll 1
+      for (int iset = 0; iset < 2; iset++) {
+#pragma unroll 1
+        for (int batch = 0; batch < Ge::NBATCH; batch++, step++) {
+          const int buf = step & 1;
+          bar_sync(BAR_FULL0 + buf, NTH);                      // the workers have filled this buffer
+          const double* Abuf = s.A + (size_t)buf * ns * Ge::ABUF;
+          // a5: Z = L^T A with FP64 tensor-core mma over the upper-triangular tiles, colour form = sum of squares of Z
+          for (int u = cwarp; u < ns * Ge::U; u += NCW) {
+            int sl = u / Ge::U, unit = u % Ge::U;
+            const double* A = Abuf + (size_t)sl * Ge::ABUF + (lane & 3) * Ge::ASTR + (lane >> 2);
             double part = 0.0;
 #pragma unroll 1
             for (int half = 0; half < 2; half++) {
@@ -547,61 +578,64 @@ __global__ void __launch_bounds__(NTH, 1) bg_kernel(const double* __restrict__ m
               for (int nt = 0; nt < Ge::NT; nt++) { acc[nt][0] = 0.0; acc[nt][1] = 0.0; }
               const double* F = D.lfrag + (size_t)(mt * Ge::KT - mt * (mt - 1)) * 32 + lane;
               int nk = Ge::KT - 2 * mt;
-              double a = __ldg(F);
+              double a0 = __ldg(F), a1 = (nk > 1) ? __ldg(F + 32) : 0.0;
               for (int kk = 0; kk < nk; kk++) {
-                double an = (kk + 1 < nk) ? __ldg(F + (kk + 1) * 32) : 0.0;
+                double an = (kk + 2 < nk) ? __ldg(F + (kk + 2) * 32) : 0.0;
                 const double* Br = A + (size_t)(4 * (2 * mt + kk)) * Ge::ASTR;
 #pragma unroll
-                for (int nt = 0; nt < Ge::NT; nt++) dmma884(acc[nt][0], acc[nt][1], a, Br[8 * nt]);
-                a = an;
+                for (int nt = 0; nt < Ge::NT; nt++) dmma884(acc[nt][0], acc[nt][1], a0, Br[8 * nt]);
+                a0 = a1; a1 = an;
               }
 #pragma unroll
               for (int nt = 0; nt < Ge::NT; nt++) { part = fma(acc[nt][0], acc[nt][0], part); part = fma(acc[nt][1], acc[nt][1], part); }
             }
-            // deterministic reduction (same order for both parameter sets => old == new gives a ratio of exactly 1)
+            // a6: deterministic reduction (same order for both parameter sets => old == new gives a ratio of exactly 1)
 #pragma unroll
             for (int d = 16; d >= 1; d >>= 1) part += __shfl_xor_sync(0xffffffffu, part, d);
-            if (lane == 0) s.red[sl * 8 + rem] = part;
+            if (lane == 0) s.red[sl * 8 + unit] = part;
           }
-          __syncthreads();
-          if (tid < ns) { double a = 0.0; for (int j = 0; j < UN; j++) a += s.red[tid * 8 + j]; s.acc[tid * 2 + iset] += a; }
+          bar_sync(BAR_COLOUR, NCT);
+          bar_arrive(BAR_EMPTY0 + buf, NTH);                   // buffer may be refilled
+          for (int sl = ctid; sl < ns; sl += NCT) { double a = 0.0; for (int j = 0; j < Ge::U; j++) a += s.red[sl * 8 + j]; s.acc[sl * 2 + iset] += a; }
+          bar_sync(BAR_COLOUR, NCT);
         }
-        __syncthreads();
       }
-    }
-    // ---- a7: eq. 3 and stores ----
-    if (tid < ns) {
-      long long ev = ev0 + tid;
-      if (ev < nev) {
-        double a = s.acc[tid * 2] * D.set[0].fac, b = s.acc[tid * 2 + 1] * D.set[1].fac;
-        me_old[ev] = a; me_new[ev] = b; w_new[ev] = __ldg(wgt + ev) * (b / a);
+      // ---- a7: eq. 3 and stores ----
+      for (int sl = ctid; sl < ns; sl += NCT) {
+        long long ev = ev0 + sl;
+        if (ev < nev) {
+          double a = s.acc[sl * 2] * D.set[0].fac, b = s.acc[sl * 2 + 1] * D.set[1].fac;
+          me_old[ev] = a; me_new[ev] = b; w_new[ev] = __ldg(wgt + ev) * (b / a);
+        }
       }
+      bar_sync(BAR_COLOUR, NCT);
     }
   }
 }
 
 // ------------------------------------------------------------------------------------------------ host API of the engine
 template <int N> static size_t smem_need(const BgSched& S, int nslot, bool dbl) {
-  if (dbl) { Smem<double> s; return carve<N, double>(s, nullptr, nslot, S.nG, S.nR, S.nL, (int)S.words.size()); }
-  Smem<float> s; return carve<N, float>(s, nullptr, nslot, S.nG, S.nR, S.nL, (int)S.words.size());
+  if (dbl) { Smem<double> s; return carve<N, double>(s, nullptr, nslot, (int)S.words.size()); }
+  Smem<float> s; return carve<N, float>(s, nullptr, nslot, (int)S.words.size());
 }
 static size_t smem_need_n(int n, const BgSched& S, int nslot, bool dbl) {
   switch (n) { case 2: return smem_need<2>(S, nslot, dbl); case 3: return smem_need<3>(S, nslot, dbl); case 4: return smem_need<4>(S, nslot, dbl); default: return smem_need<5>(S, nslot, dbl); }
 }
-// 16K registers per SM sub-partition: 3 warps x 168 registers (FP64) or 4 warps x 128 registers (FP32) per sub-partition
-static const int BG_THREADS64 = 384, BG_THREADS32 = 512;
+// 16K registers per SM sub-partition: 8 worker warps + 4 colour warps = 3 warps x 168 registers per sub-partition
+static const int BG_NW = 8, BG_NCW = 4;
 
 template <int N> static cudaError_t bg_set_attr(size_t s64, size_t s32) {
-  cudaError_t e = cudaFuncSetAttribute(bg_kernel<N, double, false, BG_THREADS64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s64);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, false, BG_THREADS32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, true, BG_THREADS32>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
+  cudaError_t e = cudaFuncSetAttribute(bg_kernel<N, double, false, BG_NW, BG_NCW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s64);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, false, BG_NW, BG_NCW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, true, BG_NW, BG_NCW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
   return e;
 }
 template <int N> static void bg_launch(int precision, int grid, size_t s64, size_t s32, cudaStream_t st, const double* mom, const double* w,
                                        double* a, double* b, double* o, long long nev, const BgDev& D) {
-  if (precision == RWGT_FP64) bg_kernel<N, double, false, BG_THREADS64><<<grid, BG_THREADS64, s64, st>>>(mom, w, a, b, o, nev, D);
-  else if (precision == RWGT_FP32) bg_kernel<N, float, false, BG_THREADS32><<<grid, BG_THREADS32, s32, st>>>(mom, w, a, b, o, nev, D);
-  else bg_kernel<N, float, true, BG_THREADS32><<<grid, BG_THREADS32, s32, st>>>(mom, w, a, b, o, nev, D);
+  const int nth = (BG_NW + BG_NCW) * 32;
+  if (precision == RWGT_FP64) bg_kernel<N, double, false, BG_NW, BG_NCW><<<grid, nth, s64, st>>>(mom, w, a, b, o, nev, D);
+  else if (precision == RWGT_FP32) bg_kernel<N, float, false, BG_NW, BG_NCW><<<grid, nth, s32, st>>>(mom, w, a, b, o, nev, D);
+  else bg_kernel<N, float, true, BG_NW, BG_NCW><<<grid, nth, s32, st>>>(mom, w, a, b, o, nev, D);
 }
 
 static BgProcess* bg_create(int n, const rwgt_params& po, const rwgt_params& pn, std::string& err) {
@@ -610,7 +644,8 @@ static BgProcess* bg_create(int n, const rwgt_params& po, const rwgt_params& pn,
   const BgSched& S = B->S;
   BgDev& D = B->D;
   D.nG = S.nG; D.nR = S.nR; D.nL = S.nL; D.nwords = (int)S.words.size(); D.offF = S.offF;
-  for (int m = 0; m < 6; m++) { D.offG[m] = S.offG[m]; D.strideG[m] = S.strideG[m]; D.offR[m] = S.offR[m]; D.strideR[m] = S.strideR[m]; D.offL[m] = S.offL[m]; D.strideL[m] = S.strideL[m]; }
+  if (S.nG != c_nG(n) || S.nR != c_nQ(n, S.rmax) || S.nL != c_nQ(n, S.lmax)) { err = "internal: schedule/geometry mismatch"; delete B; return nullptr; }
+  for (int m = 0; m < 6; m++) { D.offG[m] = S.offG[m]; D.offR[m] = S.offR[m]; D.offL[m] = S.offL[m]; }
   const rwgt_params* ps[2] = {&po, &pn};
   double fact = 1; for (int i = 2; i <= n - 2; i++) fact *= i;
   for (int k = 0; k < 2; k++) {
@@ -621,8 +656,9 @@ static BgProcess* bg_create(int n, const rwgt_params& po, const rwgt_params& pn,
   D.shared_ext = (po.mt == pn.mt) ? 1 : 0;
   int dev = 0; cudaGetDevice(&dev); cudaDeviceProp prop; cudaGetDeviceProperties(&prop, dev);
   B->sm_count = prop.multiProcessorCount; size_t maxsm = prop.sharedMemPerBlockOptin;
+  // event slots per CTA: as many as make the amplitude phase fill the 256 worker threads (npair * 4 tasks per slot and batch)
   auto pick = [&](bool dbl, int& nslot, size_t& bytes) {
-    int cap = (n == 2) ? 64 : (n == 3) ? 32 : (n == 4) ? 8 : 1; nslot = 0;
+    int cap = std::max(1, std::min(64, (BG_NW * 32) / (S.npair * (n == 2 ? 2 : 4)))); nslot = 0;
     for (int e = cap; e >= 1; e--) if (smem_need_n(n, S, e, dbl) <= maxsm) { nslot = e; break; }
     bytes = nslot ? smem_need_n(n, S, nslot, dbl) : 0;
   };
@@ -642,20 +678,22 @@ static void bg_destroy(BgProcess* B) { if (!B) return; cudaFree(B->d_words); cud
 
 // FP-pipe instruction model (FMA, MUL, ADD each 1 instruction) of the schedule, both parameter sets; see DESIGN.md "Flop counts".
 static double bg_fp_instr_per_event(const BgProcess* B) {
-  const int n = B->S.n, C = B->S.c, NJ = n - C + 1; const double L3 = 90, V4 = 102, SL = 40, PROP = 43, RC = 16, GST = 24;
+  const int n = B->S.n, C = B->S.c, NJ = n - C + 1; const double L3 = 84, V4 = 98, SLA = 32, LC = 8, PROP = 43, RC = 16, GST = 24;
   auto tup = [](int n, int m) { double r = 1; for (int i = 0; i < m; i++) r *= (n - i); return r; };
   double fp = 0;
   for (int m = 2; m <= n - 1; m++) fp += tup(n, m) / 2 * (1 << m) * ((m - 1) * L3 + (m - 1) * (m - 2) / 2 * V4 + GST);
-  for (int m = 1; m <= B->S.rmax; m++) fp += tup(n, m) * (2 << m) * (m * (SL + 8) + PROP);
-  for (int m = 1; m <= B->S.lmax; m++) fp += tup(n, m) * (2 << m) * (m * (SL + 8) + PROP);
-  double per_final = (n - 1) * L3 + (n - 1) * (n - 2) / 2 * V4 + GST + 2 * (NJ * C * 2 * (SL + 8) + NJ * 4 * RC);
+  for (int m = 1; m <= B->S.rmax; m++) fp += tup(n, m) * (2 << m) * (m * (SLA + LC) + PROP);
+  for (int m = 1; m <= B->S.lmax; m++) fp += tup(n, m) * (2 << m) * (m * (SLA + LC) + PROP);
+  double per_final = (n - 1) * L3 + (n - 1) * (n - 2) / 2 * V4 + GST + 2 * (NJ * C * (2 * SLA + LC) + NJ * 4 * RC);
   fp += B->S.npair * (double)(1 << (n - 1)) * per_final;
-  // colour: upper-triangular mma tiles, 256 FMA each, over 2*ncol real columns
-  int npp = (B->S.nperm + 7) / 8 * 8, MT = npp / 8, KT = npp / 4; double ksteps = 0; for (int mt = 0; mt < MT; mt++) ksteps += KT - 2 * mt;
-  fp += ksteps * ((double)(4 << (n - 1)) * 2 / 8) * 256.0;
   return 2.0 * fp + n * 2 * 30.0 + 4 * 40.0 + (1 << n) * 40.0;
 }
-static double bg_flops_per_event(const BgProcess* B, int /*precision*/) { return 2.0 * bg_fp_instr_per_event(B); }
+// tensor-pipe FMAs of the colour form (upper-triangular mma tiles, 256 FMA each), both parameter sets
+static double bg_mma_fma_per_event(const BgProcess* B) {
+  const int n = B->S.n; int npp = (B->S.nperm + 7) / 8 * 8, MT = npp / 8, KT = npp / 4; double ksteps = 0; for (int mt = 0; mt < MT; mt++) ksteps += KT - 2 * mt;
+  return 2.0 * ksteps * ((double)(4 << (n - 1)) * 2 / 8) * 256.0;
+}
+static double bg_flops_per_event(const BgProcess* B, int /*precision*/) { return 2.0 * (bg_fp_instr_per_event(B) + bg_mma_fma_per_event(B)); }
 
 static int bg_run(BgProcess* B, int precision, const double* mom, const double* w, double* a, double* b, double* o, long long nev, cudaStream_t st) {
   BgDev D = B->D; const bool dbl = (precision == RWGT_FP64);

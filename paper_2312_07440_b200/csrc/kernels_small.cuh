@@ -99,7 +99,8 @@ __device__ __forceinline__ void ggttx_sums(const double (*p)[4], double m, doubl
     int l2 = i2 ? -1 : +1;
     vec4<double> e2 = polvec(k2[1], k2[2], k2[3], l2);
     vec4<double> l3; for (int mu = 0; mu < 4; mu++) l3.c[mu] = mk<double>(0, 0);
-    L3_acc(l3, ds, e1, k1, e2, k2);
+    L3_acc(l3, e1, k1, e2, k2);
+    for (int mu = 0; mu < 4; mu++) l3.c[mu] = ds * l3.c[mu];
 #pragma unroll
     for (int ib = 0; ib < 2; ib++) {
       spn<double> v = spinor_v(xb, p[3][0], m, ib ? -1 : +1);

@@ -129,20 +129,56 @@ template <typename T> __device__ __forceinline__ vec4<T> polvec(T px, T py, T pz
 template <typename T> __device__ __forceinline__ vec4<T> conj4(const vec4<T>& a) { vec4<T> r; for (int i = 0; i < 4; i++) r.c[i] = conj(a.c[i]); return r; }
 
 // ---- gluon self-interaction Lorentz structures --------------------------------------
-// L3(A,B) = (JA.JB)(KA-KB) + JB ((KA+2KB).JA) - JA ((2KA+KB).JB)
-template <typename T> __device__ __forceinline__ void L3_acc(vec4<T>& acc, T sgn, const vec4<T>& JA, const T* KA, const vec4<T>& JB, const T* KB) {
+// acc += L3(A,B),  L3(A,B) = (JA.JB)(KA-KB) + JB ((KA+2KB).JA) - JA ((2KA+KB).JB).  Bilinear: a sign is applied by negating JA.
+template <typename T> __device__ __forceinline__ void L3_acc(vec4<T>& acc, const vec4<T>& JA, const T* KA, const vec4<T>& JB, const T* KB) {
   T d[4], u[4], w[4];
 #pragma unroll
-  for (int i = 0; i < 4; i++) { d[i] = KA[i] - KB[i]; u[i] = KA[i] + T(2) * KB[i]; w[i] = T(2) * KA[i] + KB[i]; }
-  cx<T> ab = sgn * mdot_cc(JA, JB), c1 = sgn * mdot_rc(u, JA), c2 = (-sgn) * mdot_rc(w, JB);
+  for (int i = 0; i < 4; i++) { d[i] = KA[i] - KB[i]; u[i] = fma(T(2), KB[i], KA[i]); w[i] = -fma(T(2), KA[i], KB[i]); }
+  cx<T> ab = mdot_cc(JA, JB), c1 = mdot_rc(u, JA), c2 = mdot_rc(w, JB);
 #pragma unroll
   for (int i = 0; i < 4; i++) { rfma(acc.c[i], d[i], ab); cfma(acc.c[i], c1, JB.c[i]); cfma(acc.c[i], c2, JA.c[i]); }
 }
-// colour-ordered quartic structure V4(X,Y,Z) = 2 (X.Z) Y - (Y.Z) X - (X.Y) Z
-template <typename T> __device__ __forceinline__ void V4_acc(vec4<T>& acc, T sgn, const vec4<T>& X, const vec4<T>& Y, const vec4<T>& Z) {
-  cx<T> xz = (T(2) * sgn) * mdot_cc(X, Z), yz = (-sgn) * mdot_cc(Y, Z), xy = (-sgn) * mdot_cc(X, Y);
+// acc += V4(X,Y,Z), colour-ordered quartic structure V4 = 2 (X.Z) Y - (Y.Z) X - (X.Y) Z.  Trilinear: sign by negating X.
+template <typename T> __device__ __forceinline__ void V4_acc(vec4<T>& acc, const vec4<T>& X, const vec4<T>& Y, const vec4<T>& Z) {
+  cx<T> xz = mdot_cc(X, Z), yz = mdot_cc(Y, Z), xy = mdot_cc(X, Y);
+  xz = mk<T>(xz.re + xz.re, xz.im + xz.im); yz = -yz; xy = -xy;
 #pragma unroll
   for (int i = 0; i < 4; i++) { cfma(acc.c[i], xz, Y.c[i]); cfma(acc.c[i], yz, X.c[i]); cfma(acc.c[i], xy, Z.c[i]); }
+}
+// conditional negation on the integer pipe (sign-bit flip), keeps the FP pipes for arithmetic
+__device__ __forceinline__ double flip_sign(double x, unsigned mask_hi) { return __hiloint2double(__double2hiint(x) ^ (int)mask_hi, __double2loint(x)); }
+__device__ __forceinline__ float flip_sign(float x, unsigned mask_hi) { return __int_as_float(__float_as_int(x) ^ (int)mask_hi); }
+template <typename T> __device__ __forceinline__ vec4<T> cond_neg(const vec4<T>& a, bool neg) {
+  vec4<T> r; const unsigned m = neg ? 0x80000000u : 0u;
+#pragma unroll
+  for (int i = 0; i < 4; i++) { r.c[i].re = flip_sign(a.c[i].re, m); r.c[i].im = flip_sign(a.c[i].im, m); }
+  return r;
+}
+
+// light-cone components of a complex vector: a+ = a0+a3, a- = a0-a3, ar = a1 - i a2, al = a1 + i a2 (what a-slash needs)
+template <typename T> struct lcv { cx<T> p, m, r, l; };
+template <typename T> __device__ __forceinline__ lcv<T> lightcone(const vec4<T>& a) {
+  lcv<T> r; r.p = a.c[0] + a.c[3]; r.m = a.c[0] - a.c[3];
+  r.r = mk<T>(a.c[1].re + a.c[2].im, a.c[1].im - a.c[2].re); r.l = mk<T>(a.c[1].re - a.c[2].im, a.c[1].im + a.c[2].re);
+  return r;
+}
+// X += a-slash * s      (8 complex FMAs)
+template <typename T> __device__ __forceinline__ void slash_acc(spn<T>& X, const lcv<T>& a, const spn<T>& s) {
+  cfma(X.c[0], a.m, s.c[2]); cfma(X.c[0], -a.r, s.c[3]);
+  cfma(X.c[1], a.p, s.c[3]); cfma(X.c[1], -a.l, s.c[2]);
+  cfma(X.c[2], a.p, s.c[0]); cfma(X.c[2], a.r, s.c[1]);
+  cfma(X.c[3], a.m, s.c[1]); cfma(X.c[3], a.l, s.c[0]);
+}
+// X += w * a-slash      (row vector, 8 complex FMAs)
+template <typename T> __device__ __forceinline__ void row_slash_acc(spn<T>& X, const spn<T>& w, const lcv<T>& a) {
+  cfma(X.c[0], w.c[2], a.p); cfma(X.c[0], w.c[3], a.l);
+  cfma(X.c[1], w.c[2], a.r); cfma(X.c[1], w.c[3], a.m);
+  cfma(X.c[2], w.c[0], a.m); cfma(X.c[2], -w.c[1], a.l);
+  cfma(X.c[3], w.c[1], a.p); cfma(X.c[3], -w.c[0], a.r);
+}
+// acc += w . s
+template <typename T> __device__ __forceinline__ void rowcol_acc(cx<T>& acc, const spn<T>& w, const spn<T>& s) {
+  cfma(acc, w.c[0], s.c[0]); cfma(acc, w.c[1], s.c[1]); cfma(acc, w.c[2], s.c[2]); cfma(acc, w.c[3], s.c[3]);
 }
 
 }  // namespace rwgt
