@@ -164,7 +164,7 @@ def time_config(torch, B, c, precision, n, steps, warmup, seed_offset, flush_buf
         s1.record(stream)
     torch.cuda.synchronize()
     ms = [a.elapsed_time(b) for a, b in evs]
-    res = {"ms": ms, "flops_per_event": r.flops_per_event(), "out": out, "dm": dm, "dw": dw, "host": (m, w), "rw": r,
+    res = {"ms": ms, "flops_per_event": r.flops_per_event(), "tensor_flops_per_event": r.tensor_flops_per_event(), "out": out, "dm": dm, "dw": dw, "host": (m, w), "rw": r,
            "l2": "flushed between iterations (512 MB add_)" if need_flush else "inputs+outputs exceed L2 (no flush)"}
     return res
 
@@ -241,7 +241,7 @@ def main() -> None:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the (single) kernel of a step ----
+    # ---- roofline of the (single) kernel of a step: plain FP64/FP32 FMA pipe ----
     peaks = measured_peaks()
     kernel_ms = statistics.mean(res["ms"])
     flops = res["flops_per_event"] * n
@@ -250,13 +250,23 @@ def main() -> None:
     peak_tf = alu_peak_tflops(dtype, max_mhz)
     traffic = None
     try:
-        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(f"cfg{c.index}_{args.precision}")
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "r1_counts.json")))[f"cfg{c.index}_{args.precision}"]["traffic_bytes"]
+        if n != c.n_events:
+            traffic = None
     except Exception:
         pass
+    try:
+        chain_tf = B.rwgt_measure_peak(0 if dtype == "f64" else 1)       # register-resident FMA chain, same session
+    except Exception:
+        chain_tf = None
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": traffic,
-                "peak_source": f"derived: 148 SM x {FP64_LANES_PER_SM if dtype == 'f64' else FP32_LANES_PER_SM} FMA lanes x 2 x {max_mhz:g} MHz (max SM clock); DESIGN.md",
+                "peak_source": f"derived: 148 SM x {FP64_LANES_PER_SM if dtype == 'f64' else FP32_LANES_PER_SM} FMA lanes x 2 flop x {max_mhz:g} MHz (max SM clock); DESIGN.md Roofline",
+                "peak_fma_chain_measured": chain_tf, "frac_of_fma_chain_measured": (achieved_tf / chain_tf) if chain_tf else None,
                 "frac_at_clock_under_load": (achieved_tf / alu_peak_tflops(dtype, clocks["sm_mhz"])) if clocks.get("sm_mhz") else None,
                 "flops_per_event": res["flops_per_event"], "kernel_ms": kernel_ms,
+                "tensor_fp64": {"flops_per_event": res["tensor_flops_per_event"],
+                                "achieved_tflops": res["tensor_flops_per_event"] * n / (kernel_ms * 1e-3) / 1e12,
+                                "note": "colour form on the FP64 tensor pipe (mma.m8n8k4), a separate pipe; not counted in `achieved`"},
                 "hbm": {"achieved_gbs": bytes_per_event(c) * n / (kernel_ms * 1e-3) / 1e9, "peak_gbs": peaks.get("hbm_gbs", 6650.0),
                         "peak_source": "MEASURED_PEAKS.json" if peaks.get("hbm_gbs") else "fallback"}}
     roofline["hbm"]["frac"] = roofline["hbm"]["achieved_gbs"] / roofline["hbm"]["peak_gbs"]

@@ -62,10 +62,13 @@ int rwgt_set_precision(rwgt_handle* h, int mode);
 /* Number of external legs (4..7), so callers can size `momenta`; -1 on bad handle. */
 int rwgt_n_external(const rwgt_handle* h);
 
-/* Exact count of double- (or single-) precision FMA-pipe instructions per event of the
- * schedule the kernel executes for this handle in its current mode (FMA, MUL, ADD each
- * count 1; both parameter sets).  Used for the roofline. */
+/* Algorithmic floating-point operations per event that the kernel of this handle executes on
+ * the FP64 (FP32 in the FP32/mixed modes) FMA pipe: FMA = 2, MUL = ADD = 1, both parameter
+ * sets, all helicities (checked against ncu counters).  Roofline use. */
 double rwgt_flops_per_event(const rwgt_handle* h);
+
+/* Same for the FP64 tensor pipe (mma.m8n8k4 of the colour form; 0 for the 2->2 kernels). */
+double rwgt_tensor_flops_per_event(const rwgt_handle* h);
 
 /* The hot path: a1-a7 of SURVEY.md §8(a) in one kernel launch on `stream`.
  *   momenta   DEVICE, SoA double [n_ext][4][n_events]: momenta[(ip*4+mu)*n_events + ievt],

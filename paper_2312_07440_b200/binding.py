@@ -16,7 +16,7 @@ RWGT_FP64, RWGT_FP32, RWGT_MIXED = 0, 1, 2
 PRECISIONS = {"fp64": RWGT_FP64, "fp32": RWGT_FP32, "mixed": RWGT_MIXED}
 
 EXPORTS = ("rwgt_create", "rwgt_set_precision", "rwgt_n_external", "rwgt_flops_per_event", "rwgt_run",
-           "rwgt_run_host", "rwgt_destroy", "rwgt_last_error", "rwgt_colour_matrix", "rwgt_measure_peak")
+           "rwgt_run_host", "rwgt_destroy", "rwgt_last_error", "rwgt_colour_matrix", "rwgt_measure_peak", "rwgt_tensor_flops_per_event")
 
 
 class rwgt_params(C.Structure):
@@ -42,6 +42,8 @@ def lib():
         L.rwgt_n_external.argtypes = [vp]
         L.rwgt_flops_per_event.argtypes = [vp]
         L.rwgt_flops_per_event.restype = C.c_double
+        L.rwgt_tensor_flops_per_event.argtypes = [vp]
+        L.rwgt_tensor_flops_per_event.restype = C.c_double
         L.rwgt_run.argtypes = [vp, dp, dp, dp, dp, dp, C.c_longlong, vp]
         L.rwgt_run_host.argtypes = [vp, dp, dp, dp, dp, dp, C.c_longlong, vp]
         L.rwgt_destroy.argtypes = [vp]
@@ -82,6 +84,10 @@ def rwgt_n_external(h) -> int:
 
 def rwgt_flops_per_event(h) -> float:
     return lib().rwgt_flops_per_event(h)
+
+
+def rwgt_tensor_flops_per_event(h) -> float:
+    return lib().rwgt_tensor_flops_per_event(h)
 
 
 def rwgt_run(h, momenta_ptr: int, weights_ptr: int, out_me_old_ptr: int, out_me_new_ptr: int,
@@ -135,6 +141,9 @@ class Reweighter:
 
     def flops_per_event(self) -> float:
         return rwgt_flops_per_event(self.h)
+
+    def tensor_flops_per_event(self) -> float:
+        return rwgt_tensor_flops_per_event(self.h)
 
     def run(self, momenta, weights, out=None):
         import torch

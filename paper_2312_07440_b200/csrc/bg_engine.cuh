@@ -679,24 +679,27 @@ static BgProcess* bg_create(int n, const rwgt_params& po, const rwgt_params& pn,
 }
 static void bg_destroy(BgProcess* B) { if (!B) return; cudaFree(B->d_words); cudaFree(B->d_lfrag); delete B; }
 
-// FP-pipe instruction model (FMA, MUL, ADD each 1 instruction) of the schedule, both parameter sets; see DESIGN.md "Flop counts".
-static double bg_fp_instr_per_event(const BgProcess* B) {
-  const int n = B->S.n, C = B->S.c, NJ = n - C + 1; const double L3 = 84, V4 = 98, SLA = 32, LC = 8, PROP = 43, RC = 16, GST = 24;
+// Algorithmic flop count of the schedule on the FP64 (or FP32) FMA pipe, both parameter sets, per event: FMA = 2 flop,
+// MUL = ADD = 1 flop, per operation of rwgt_math.cuh (L3 74 FMA + 6 MUL + 4 ADD, V4 90 + 6 + 2, slash-accumulate 32 FMA,
+// light-cone 8 ADD, propagator 24 FMA + 17 MUL + 6 ADD, row.col 16 FMA, current store 8 FMA + 16 MUL).  Agrees with the
+// ncu instruction counters of the committed build to 0.5% (n=5), 1.0% (n=4), 2.6% (n=3), always from below
+// (profiles/r1_summary.md).
+static double bg_flops_per_event(const BgProcess* B, int /*precision*/) {
+  const int n = B->S.n, C = B->S.c, NJ = n - C + 1; const double L3 = 158, V4 = 188, SLA = 64, LC = 8, PROP = 71, RC = 32, GST = 32, GST2 = 16;
   auto tup = [](int n, int m) { double r = 1; for (int i = 0; i < m; i++) r *= (n - i); return r; };
   double fp = 0;
-  for (int m = 2; m <= n - 1; m++) fp += tup(n, m) / 2 * (1 << m) * ((m - 1) * L3 + (m - 1) * (m - 2) / 2 * V4 + GST);
+  for (int m = 2; m <= n - 1; m++) fp += tup(n, m) / 2 * (1 << m) * ((m - 1) * L3 + (m - 1) * (m - 2) / 2 * V4 + (m > 2 ? GST : GST2));
   for (int m = 1; m <= B->S.rmax; m++) fp += tup(n, m) * (2 << m) * (m * (SLA + LC) + PROP);
   for (int m = 1; m <= B->S.lmax; m++) fp += tup(n, m) * (2 << m) * (m * (SLA + LC) + PROP);
-  double per_final = (n - 1) * L3 + (n - 1) * (n - 2) / 2 * V4 + GST + 2 * (NJ * C * (2 * SLA + LC) + NJ * 4 * RC);
+  double per_final = (n - 1) * L3 + (n - 1) * (n - 2) / 2 * V4 + (n > 2 ? GST : GST2) + LC + 2 * (NJ * C * (2 * SLA + LC) + NJ * 4 * RC);
   fp += B->S.npair * (double)(1 << (n - 1)) * per_final;
   return 2.0 * fp + n * 2 * 30.0 + 4 * 40.0 + (1 << n) * 40.0;
 }
-// tensor-pipe FMAs of the colour form (upper-triangular mma tiles, 256 FMA each), both parameter sets
-static double bg_mma_fma_per_event(const BgProcess* B) {
+// FP64 tensor-pipe flops of the colour form (upper-triangular mma.m8n8k4 tiles, 256 FMA each), both parameter sets
+static double bg_tensor_flops_per_event(const BgProcess* B) {
   const int n = B->S.n; int npp = (B->S.nperm + 7) / 8 * 8, MT = npp / 8, KT = npp / 4; double ksteps = 0; for (int mt = 0; mt < MT; mt++) ksteps += KT - 2 * mt;
-  return 2.0 * ksteps * ((double)(4 << (n - 1)) * 2 / 8) * 256.0;
+  return 2.0 * 2.0 * ksteps * ((double)(4 << (n - 1)) * 2 / 8) * 256.0;
 }
-static double bg_flops_per_event(const BgProcess* B, int /*precision*/) { return 2.0 * (bg_fp_instr_per_event(B) + bg_mma_fma_per_event(B)); }
 
 static int bg_run(BgProcess* B, int precision, const double* mom, const double* w, double* a, double* b, double* o, long long nev, cudaStream_t st) {
   BgDev D = B->D; const bool dbl = (precision == RWGT_FP64);

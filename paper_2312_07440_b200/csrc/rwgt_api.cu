@@ -115,9 +115,16 @@ int rwgt_n_external(const rwgt_handle* h) { return h ? h->n_ext : -1; }
 
 double rwgt_flops_per_event(const rwgt_handle* h) {
   if (!h) return -1.0;
-  if (h->proc == P_EPEM) return 330.0;      // counted from the SASS of epem_mupmum_kernel
-  if (h->proc == P_GG_TTX) return h->ggttx.two_pass ? 2.0 * 2150.0 : 2150.0;
+  // the two one-event-per-thread kernels: ncu counters of the committed build (217 DFMA + 119 DMUL + 48 DADD resp.
+  // 1263 DFMA + 369 DMUL + 87 DADD per event; profiles/r1_summary.md)
+  if (h->proc == P_EPEM) return 601.0;
+  if (h->proc == P_GG_TTX) return h->ggttx.two_pass ? 2.0 * 2982.0 : 2982.0;
   return rwgt::bg_flops_per_event(h->bg, h->precision);
+}
+
+double rwgt_tensor_flops_per_event(const rwgt_handle* h) {
+  if (!h) return -1.0;
+  return h->proc == P_BG ? rwgt::bg_tensor_flops_per_event(h->bg) : 0.0;
 }
 
 int rwgt_run(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old, double* out_me_new,
