@@ -412,6 +412,8 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
                                                                double* __restrict__ w_new, long long nev, BgDev D) {
   typedef Geo<N> Ge;
   constexpr int NTH = (NW + NCW) * 32, NWT = NW * 32, NCT = NCW * 32;
+  // register hand-over between the warpgroups: the colour warps need few registers, the workers get the rest
+  constexpr int REG_COL = 56, REG_WORK = ((65536 / 32 - NCW * REG_COL) / NW) / 8 * 8 > 232 ? 232 : ((65536 / 32 - NCW * REG_COL) / NW) / 8 * 8;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Ctx<T> c; c.D = &D; c.ns = D.nslot;
   carve<N, T>(c.s, smem_raw, D.nslot, D.nwords);
@@ -424,6 +426,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
   __syncthreads();
   if (threadIdx.x < NWT) {
     // =========================================================================================== worker warps
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REG_WORK));
     const int tid = threadIdx.x; c.tid = tid;
     for (int t = tid; t < D.nwords; t += NWT) s.W[t] = __ldg(D.words + t);
     unsigned step = 0;
@@ -552,6 +555,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
     }
   } else {
     // =========================================================================================== colour warps
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REG_COL));
     const int ctid = threadIdx.x - NWT, cwarp = ctid >> 5, lane = ctid & 31;
     unsigned step = 0;
     for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
