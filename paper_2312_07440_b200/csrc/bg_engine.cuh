@@ -88,43 +88,46 @@ static std::vector<double> colour_matrix_fierz(int n) {
 }
 
 // ------------------------------------------------------------------------------------------------ schedule
-// operand reference: entry = base + variant bits of the operand extracted from the task's variant word
-enum : uint32_t { REF_REV = 1u << 22, REF_NEG = 1u << 23 };
-static inline uint32_t mkref(int base, int m, int shift, bool rev, bool neg, int mask) {
-  return (uint32_t)base | ((uint32_t)m << 16) | ((uint32_t)shift << 19) | (rev && m >= 2 ? REF_REV : 0u) | (neg ? REF_NEG : 0u) | ((uint32_t)mask << 24);
-}
+// Storage conventions of the current tables (chosen so that the device never needs a run-time sign flip):
+//   * entry = base(tuple) + helicity-variant bits of the tuple's gluons in the tuple's own position order
+//     (+ the quark helicity bit on top for R/L);
+//   * gluon tuples of length 1: one entry set per gluon; length 2: BOTH orientations are stored (J(b,a) = -J(a,b));
+//     length 3: the orientation with t_1 < t_3 (J(rev) = +J, only the variant bits are reversed: REF_REV);
+//     length 4 (n = 5 only): the orientation that runs along the "forward" direction of the 5-necklace
+//     (t_1..t_4, missing label) -- every block of a forward permutation is then stored as used, every block of
+//     its reversal is stored reversed (static sign (-1)^{m+1} and static bit reversal on the device);
+//   * gluon 0 only has helicity + (parity, reading R5): variants with its bit set are neither computed nor read.
+enum : uint32_t { REF_REV = 0x8000u };
 
 struct BgSched {
   int n, c, lmax, rmax, nperm, npair;
-  int nG, nR, nL;                   // table entries per slot
-  int offG[6], strideG[6];          // gluon levels m = 2..n-1: offset into words, words per task
-  int offR[6], strideR[6];          // right levels m = 1..rmax
-  int offL[6], strideL[6];          // left  levels m = 1..lmax
-  int offF, strideF;                // finals: one task descriptor per sigma pair
+  int nG, nR, nL;                    // table entries per slot
+  int offD[3][6];                    // descriptor offsets  [0:G,1:R,2:L][level]
+  int offT[6], ntask[3][6];          // per phase M: task-list offset, number of G / R / L tasks
+  int offF, strideF;                 // finals: one descriptor per permutation pair
   std::vector<uint32_t> words;
-  std::vector<double> lfrag;        // Cholesky factor L^T of the colour matrix in mma-fragment order
+  std::vector<double> lfrag;         // Cholesky factor L^T of the colour matrix in mma-fragment order
+  double fp_ops[8];                  // operation counts per event and parameter set: L3, V4, slash, lightcone, prop, rowcol, gstore, gstore2
 };
 
-struct TupleTables {
-  std::map<std::vector<int>, int> gbase;   // canonical gluon tuples
-  std::map<std::vector<int>, int> rbase, lbase;
-};
 static int mask_of(const std::vector<int>& t) { int m = 0; for (int x : t) m |= 1 << x; return m; }
-static bool is_canon(const std::vector<int>& t) { return t.size() < 2 || t.front() < t.back(); }
-// reference to the gluon current of the tuple obtained by reading positions [lo,hi) of `seq` (ascending if !desc)
-static uint32_t gref(const TupleTables& T, const std::vector<int>& seq, int lo, int hi, bool desc) {
-  std::vector<int> asc(seq.begin() + lo, seq.begin() + hi), used = asc;
-  if (desc) std::reverse(used.begin(), used.end());
-  int m = hi - lo; bool canon_is_asc = is_canon(asc);
-  std::vector<int> canon = asc; if (!canon_is_asc) std::reverse(canon.begin(), canon.end());
-  bool used_is_canon = (used == canon);
-  bool neg = !used_is_canon && (m % 2 == 0);            // J(rev) = (-1)^{m+1} J
-  // variant bits are given in ascending position order of `seq`; the stored entry uses the canonical tuple's order
-  return mkref(T.gbase.at(canon), m, lo, !canon_is_asc, neg, mask_of(asc));
+static bool has0(const std::vector<int>& t) { for (int x : t) if (x == 0) return true; return false; }
+static int pos0(const std::vector<int>& t) { for (size_t i = 0; i < t.size(); i++) if (t[i] == 0) return (int)i; return -1; }
+static std::vector<int> reversed(std::vector<int> t) { std::reverse(t.begin(), t.end()); return t; }
+// forward direction of a cyclic arrangement: the rotations of the lexicographically smallest of its 2n dihedral images
+static bool necklace_forward(const std::vector<int>& s) {
+  int n = (int)s.size(); std::vector<int> best; bool best_fwd = true;
+  for (int dir = 0; dir < 2; dir++) { std::vector<int> t = dir ? reversed(s) : s;
+    for (int r = 0; r < n; r++) { std::vector<int> u(n); for (int i = 0; i < n; i++) u[i] = t[(i + r) % n];
+      if (best.empty() || u < best) { best = u; best_fwd = (dir == 0); } } }
+  return best_fwd;
 }
-static uint32_t qref(const std::map<std::vector<int>, int>& base, const std::vector<int>& seq, int lo, int hi, bool desc) {
-  std::vector<int> used(seq.begin() + lo, seq.begin() + hi); if (desc) std::reverse(used.begin(), used.end());
-  return mkref(base.at(used), hi - lo, lo, desc, false, mask_of(used));
+// is this ordered gluon tuple the stored orientation?
+static bool is_stored(int n, const std::vector<int>& t) {
+  int m = (int)t.size();
+  if (m <= 2) return true;
+  if (m == 4 && n == 5) { std::vector<int> s = t; for (int e = 0; e < 5; e++) if (!(mask_of(t) >> e & 1)) s.push_back(e); return necklace_forward(s); }
+  return t.front() < t.back();
 }
 static void all_tuples(int n, int m, std::vector<std::vector<int>>& out) {
   out.clear(); std::vector<int> cur; std::vector<bool> usedl(n, false);
@@ -136,9 +139,13 @@ static void all_tuples(int n, int m, std::vector<std::vector<int>>& out) {
 
 // compile-time geometry of the schedule for N gluons (mirrored by build_schedule and checked in bg_create)
 __host__ __device__ constexpr int cfact(int n) { return n <= 1 ? 1 : n * cfact(n - 1); }
-__host__ __device__ constexpr int ctuples(int n, int m) { return cfact(n) / cfact(n - m); }     // ordered m-tuples of n labels
-__host__ __device__ constexpr int c_nG(int n) { int r = 0; for (int m = 1; m <= n - 1; m++) r += (m == 1 ? n : ctuples(n, m) / 2) << m; return r; }
+__host__ __device__ constexpr int ctuples(int n, int m) { return m > n ? 0 : cfact(n) / cfact(n - m); }     // ordered m-tuples of n labels
+__host__ __device__ constexpr int c_nG(int n) { int r = 0; for (int m = 1; m <= n - 1; m++) r += (m <= 2 ? ctuples(n, m) : ctuples(n, m) / 2) << m; return r; }
 __host__ __device__ constexpr int c_nQ(int n, int mmax) { int r = 2; for (int m = 1; m <= mmax; m++) r += ctuples(n, m) * (2 << m); return r; }
+// tasks of one level after parity pruning (gluon 0 at helicity + only)
+__host__ __device__ constexpr int c_ntaskG(int n, int m) { int can = ctuples(n, m) / 2, c0 = m * ctuples(n - 1, m - 1) / 2; return ((can - c0) << m) + (c0 << (m - 1)); }
+__host__ __device__ constexpr int c_ntaskQ(int n, int m) { int all = ctuples(n, m), c0 = m * ctuples(n - 1, m - 1); return ((all - c0) << (m + 1)) + (c0 << m); }
+__host__ __device__ constexpr int pad4(int x) { return (x + 3) / 4 * 4; }
 template <int N> struct Geo {
   static constexpr int C = (N + 1) / 2, LMAX = C - 1, RMAX = N - C, NJ = N - C + 1;            // N=2: C=1; 3: 2; 4: 2; 5: 3
   static constexpr int NPERM = cfact(N), NPAIR = NPERM / 2, NPERM_P = (NPERM + 7) / 8 * 8;
@@ -152,66 +159,134 @@ template <int N> struct Geo {
   static constexpr int NMASK = 1 << N;
   static constexpr int NPHASE = (N - 1 > (RMAX > LMAX ? RMAX : LMAX) + 1) ? N - 1 : (RMAX > LMAX ? RMAX : LMAX) + 1;
   static constexpr int NL3 = N - 1, NV4 = (N - 1) * (N - 2) / 2;
-  static constexpr int WOFF_TERMS = 4 + 2 * NL3 + 3 * NV4, WPER = C + NJ + NJ * C;
-  static constexpr int STRIDEF = WOFF_TERMS + 2 * WPER;
+  static constexpr int JW = pad4(2 * NL3 + 3 * NV4);                     // words of the n-gluon current's references
+  static constexpr int QH = C + NJ + NJ * C, QW = pad4((QH + 1) / 2);    // halfwords / words of one quark-line reference block
+  static constexpr int STRIDEF = 4 + JW + 2 * QW;
   static constexpr size_t ABUF = (size_t)NPERM_P * ASTR;                 // doubles per slot per buffer
   static constexpr int NG = c_nG(N), NR = c_nQ(N, RMAX), NL = c_nQ(N, LMAX);   // entries of the current tables (checked against the schedule)
 };
+__host__ __device__ constexpr int gdesc_words(int m) { return pad4(2 + 2 * (m - 1) + 3 * (m - 1) * (m - 2) / 2); }
+__host__ __device__ constexpr int qdesc_words(int m) { return pad4(1 + m); }
 
-static BgSched build_schedule(int n) {
+struct TupleTables {
+  std::map<std::vector<int>, int> gbase, rbase, lbase;
+};
+// 16-bit reference to the gluon current of the ordered tuple `used`; `exact` reports whether it is stored as used
+static uint32_t gref16(int n, const TupleTables& T, const std::vector<int>& used, bool* exact = nullptr) {
+  bool st = is_stored(n, used);
+  if (exact) *exact = st;
+  int base = T.gbase.at(st ? used : reversed(used));
+  return (uint32_t)base | ((!st && used.size() == 3) ? REF_REV : 0u);      // length 4: reversal and sign are static on the device
+}
+static std::vector<int> sub(const std::vector<int>& s, int lo, int hi) { return std::vector<int>(s.begin() + lo, s.begin() + hi); }
+
+static BgSched build_schedule(int n, std::string& err) {
   BgSched S; S.n = n;
-  for (int m = 0; m < 6; m++) { S.offG[m] = S.strideG[m] = S.offR[m] = S.strideR[m] = S.offL[m] = S.strideL[m] = 0; }
+  for (int k = 0; k < 3; k++) for (int m = 0; m < 6; m++) { S.offD[k][m] = 0; S.ntask[k][m] = 0; }
+  for (int m = 0; m < 6; m++) S.offT[m] = 0;
+  for (int k = 0; k < 8; k++) S.fp_ops[k] = 0;
   S.c = (n + 1) / 2; S.lmax = S.c - 1; S.rmax = n - S.c;
   TupleTables T; std::vector<std::vector<int>> tl;
   int nG = 0, nR = 0, nL = 0;
-  for (int m = 1; m <= n - 1; m++) { all_tuples(n, m, tl); for (auto& t : tl) if (is_canon(t)) { T.gbase[t] = nG; nG += 1 << m; } }
+  for (int m = 1; m <= n - 1; m++) { all_tuples(n, m, tl); for (auto& t : tl) if (is_stored(n, t)) { T.gbase[t] = nG; nG += 1 << m; } }
   T.rbase[{}] = nR; nR += 2; T.lbase[{}] = nL; nL += 2;
   for (int m = 1; m <= S.rmax; m++) { all_tuples(n, m, tl); for (auto& t : tl) { T.rbase[t] = nR; nR += 2 << m; } }
   for (int m = 1; m <= S.lmax; m++) { all_tuples(n, m, tl); for (auto& t : tl) { T.lbase[t] = nL; nL += 2 << m; } }
   S.nG = nG; S.nR = nR; S.nL = nL;
+  auto pad = [&]() { while (S.words.size() % 4) S.words.push_back(0u); };
+  auto gref32 = [&](const std::vector<int>& t, int lo, int hi) {          // reference inside a gluon recursion: must be stored as used (or length 3)
+    std::vector<int> u = sub(t, lo, hi); bool ex; uint32_t r = gref16(n, T, u, &ex);
+    if (!ex && u.size() != 3) err = "internal: gluon block not stored in the orientation it is used in";
+    return r | ((uint32_t)(mask_of(u) * 4) << 16);                        // high half: element offset of the block's momentum sum
+  };
+  auto gluon_refs = [&](const std::vector<int>& t) {
+    int m = (int)t.size();
+    for (int k = 1; k < m; k++) { S.words.push_back(gref32(t, 0, k)); S.words.push_back(gref32(t, k, m)); }
+    for (int j = 1; j < m; j++) for (int k = j + 1; k < m; k++) { S.words.push_back(gref32(t, 0, j)); S.words.push_back(gref32(t, j, k)); S.words.push_back(gref32(t, k, m)); }
+  };
+  std::vector<std::vector<uint32_t>> tasks(6);
+  // descriptors + task lists of the gluon levels
+  std::vector<std::vector<uint32_t>> tG(6), tR(6), tL(6);
   for (int m = 2; m <= n - 1; m++) {
-    all_tuples(n, m, tl); S.offG[m] = (int)S.words.size(); S.strideG[m] = 2 + 2 * (m - 1) + 3 * (m - 1) * (m - 2) / 2;
-    for (auto& t : tl) if (is_canon(t)) {
-      S.words.push_back(T.gbase[t]); S.words.push_back(mask_of(t));
-      for (int k = 1; k < m; k++) { S.words.push_back(gref(T, t, 0, k, false)); S.words.push_back(gref(T, t, k, m, false)); }
-      for (int j = 1; j < m; j++) for (int k = j + 1; k < m; k++) { S.words.push_back(gref(T, t, 0, j, false)); S.words.push_back(gref(T, t, j, k, false)); S.words.push_back(gref(T, t, k, m, false)); }
-    }
-  }
-  for (int m = 1; m <= S.rmax; m++) {
-    all_tuples(n, m, tl); S.offR[m] = (int)S.words.size(); S.strideR[m] = 2 + 2 * m;
+    all_tuples(n, m, tl); pad(); S.offD[0][m] = (int)S.words.size(); int idx = 0;
     for (auto& t : tl) {
-      S.words.push_back(T.rbase[t]); S.words.push_back(mask_of(t));
-      for (int k = 1; k <= m; k++) { S.words.push_back(gref(T, t, 0, k, false)); S.words.push_back(qref(T.rbase, t, k, m, false)); }
+      if (m == 2 ? !(t[0] < t[1]) : !is_stored(n, t)) continue;          // length 2: one task fills both orientations
+      size_t d0 = S.words.size();
+      S.words.push_back((uint32_t)T.gbase[t] | ((uint32_t)(m == 2 ? T.gbase[reversed(t)] : 0) << 16)); S.words.push_back((uint32_t)mask_of(t));
+      gluon_refs(t); pad();
+      if ((int)(S.words.size() - d0) != gdesc_words(m)) err = "internal: gluon descriptor size";
+      int p0 = pos0(t);
+      for (uint32_t v = 0; v < (1u << m); v++) if (p0 < 0 || !(v >> p0 & 1)) tG[m].push_back((uint32_t)idx | (v << 16));
+      idx++;
+      S.fp_ops[0] += (double)(m - 1) * ((p0 < 0) ? (1 << m) : (1 << (m - 1))); S.fp_ops[1] += (double)((m - 1) * (m - 2) / 2) * ((p0 < 0) ? (1 << m) : (1 << (m - 1)));
+      S.fp_ops[m > 2 ? 6 : 7] += (p0 < 0) ? (1 << m) : (1 << (m - 1));
     }
   }
-  for (int m = 1; m <= S.lmax; m++) {
-    all_tuples(n, m, tl); S.offL[m] = (int)S.words.size(); S.strideL[m] = 2 + 2 * m;
-    for (auto& t : tl) {
-      S.words.push_back(T.lbase[t]); S.words.push_back(mask_of(t));
-      for (int k = 1; k <= m; k++) { S.words.push_back(qref(T.lbase, t, 0, m - k, false)); S.words.push_back(gref(T, t, m - k, m, false)); }
+  for (int side = 0; side < 2; side++) {
+    int mmax = side == 0 ? S.rmax : S.lmax; auto& base = side == 0 ? T.rbase : T.lbase;
+    for (int m = 1; m <= mmax; m++) {
+      all_tuples(n, m, tl); pad(); S.offD[1 + side][m] = (int)S.words.size(); int idx = 0;
+      for (auto& t : tl) {
+        size_t d0 = S.words.size();
+        S.words.push_back((uint32_t)base[t] | ((uint32_t)mask_of(t) << 16));
+        for (int k = 1; k <= m; k++) {
+          // right: Jslash(t_1..k) R(t_k+1..m);  left: L(t_1..m-k) Jslash(t_m-k+1..m)
+          std::vector<int> gj = side == 0 ? sub(t, 0, k) : sub(t, m - k, m), q = side == 0 ? sub(t, k, m) : sub(t, 0, m - k);
+          bool ex; uint32_t rj = gref16(n, T, gj, &ex); if (!ex && gj.size() != 3) err = "internal: quark-current gluon block orientation";
+          S.words.push_back(rj | ((uint32_t)base.at(q) << 16));
+        }
+        pad();
+        if ((int)(S.words.size() - d0) != qdesc_words(m)) err = "internal: quark descriptor size";
+        int p0 = pos0(t);
+        for (uint32_t v = 0; v < (2u << m); v++) if (p0 < 0 || !(v >> p0 & 1)) (side == 0 ? tR : tL)[m + 1].push_back((uint32_t)idx | (v << 16));
+        idx++;
+        double cnt = (p0 < 0) ? (2 << m) : (1 << m);
+        S.fp_ops[2] += m * cnt; S.fp_ops[3] += m * cnt; S.fp_ops[4] += cnt;
+      }
     }
   }
-  // finals: one descriptor per pair (sigma, sigma reversed), sigma_1 < sigma_n
+  for (int M = 2; M < 6; M++) {
+    pad(); S.offT[M] = (int)S.words.size();
+    S.ntask[0][M] = (int)tG[M].size(); S.ntask[1][M] = (int)tR[M].size(); S.ntask[2][M] = (int)tL[M].size();
+    for (auto w : tG[M]) S.words.push_back(w); for (auto w : tR[M]) S.words.push_back(w); for (auto w : tL[M]) S.words.push_back(w);
+  }
+  // finals: one descriptor per pair (sigma, sigma reversed); "which = 0" is the forward permutation (n = 5: along the necklace)
   std::vector<std::vector<int>> perms; { std::vector<int> p(n); for (int i = 0; i < n; i++) p[i] = i; do perms.push_back(p); while (std::next_permutation(p.begin(), p.end())); }
   S.nperm = (int)perms.size(); std::map<std::vector<int>, int> rank; for (int i = 0; i < S.nperm; i++) rank[perms[i]] = i;
   const int C = S.c, NJ = n - C + 1;
-  S.offF = (int)S.words.size(); S.strideF = 4 + 2 * (n - 1) + 3 * (n - 1) * (n - 2) / 2 + 2 * (C + NJ + NJ * C); S.npair = 0;
-  for (auto& s : perms) if (s.front() < s.back()) {
+  const int JW = pad4(2 * (n - 1) + 3 * (n - 1) * (n - 2) / 2), QH = C + NJ + NJ * C, QW = pad4((QH + 1) / 2);
+  pad(); S.offF = (int)S.words.size(); S.strideF = 4 + JW + 2 * QW; S.npair = 0;
+  for (auto& s0 : perms) {
+    bool fwd = (n == 5) ? necklace_forward(s0) : (s0.front() < s0.back());
+    if (!fwd) continue;
     S.npair++;
-    std::vector<int> sr(s.rbegin(), s.rend());
-    uint32_t packed = 0; for (int j = 0; j < n; j++) packed |= (uint32_t)s[j] << (3 * j);
-    S.words.push_back(rank[s]); S.words.push_back(rank[sr]); S.words.push_back(packed); S.words.push_back(n % 2 == 0 ? 1u : 0u);   // J_n(rev) = (-1)^{n+1} J_n
-    for (int k = 1; k < n; k++) { S.words.push_back(gref(T, s, 0, k, false)); S.words.push_back(gref(T, s, k, n, false)); }
-    for (int j = 1; j < n; j++) for (int k = j + 1; k < n; k++) { S.words.push_back(gref(T, s, 0, j, false)); S.words.push_back(gref(T, s, j, k, false)); S.words.push_back(gref(T, s, k, n, false)); }
+    size_t d0 = S.words.size();
+    std::vector<int> sr = reversed(s0);
+    uint32_t packed = 0; for (int j = 0; j < n; j++) packed |= (uint32_t)s0[j] << (3 * j);
+    S.words.push_back((uint32_t)rank[s0] | ((uint32_t)rank[sr] << 16)); S.words.push_back(packed); S.words.push_back(0u); S.words.push_back(0u);
+    gluon_refs(s0); pad();
     for (int which = 0; which < 2; which++) {
-      // sigma: block [i,j) in ascending positions.  sigma reversed: its positions [i,j) are sigma's [n-j,n-i) read descending
-      for (int i = 0; i < C; i++) S.words.push_back(which == 0 ? qref(T.lbase, s, 0, i, false) : qref(T.lbase, s, n - i, n, true));
-      for (int j = C; j <= n; j++) S.words.push_back(which == 0 ? qref(T.rbase, s, j, n, false) : qref(T.rbase, s, 0, n - j, true));
+      const std::vector<int>& s = which ? sr : s0;
+      std::vector<uint32_t> hw;
+      for (int i = 0; i < C; i++) hw.push_back((uint32_t)T.lbase.at(sub(s, 0, i)));
+      for (int j = C; j <= n; j++) hw.push_back((uint32_t)T.rbase.at(sub(s, j, n)));
       for (int j = C; j <= n; j++) for (int i = 0; i < C; i++) {
-        if (i == 0 && j == n) { S.words.push_back(0u); continue; }
-        S.words.push_back(which == 0 ? gref(T, s, i, j, false) : gref(T, s, n - j, n - i, true));
+        if (i == 0 && j == n) { hw.push_back(0u); continue; }
+        std::vector<int> u = sub(s, i, j); bool ex; uint32_t r = gref16(n, T, u, &ex);
+        // static rule of the device code: blocks of length 4 are stored as used for which = 0 and reversed for which = 1
+        if (u.size() == 4 && ex != (which == 0)) err = "internal: length-4 block orientation does not follow the necklace rule";
+        if (u.size() != 3 && u.size() != 4 && !ex) err = "internal: block orientation";
+        hw.push_back(r);
       }
+      while ((int)hw.size() < 2 * QW) hw.push_back(0u);
+      for (int k = 0; k < QW; k++) S.words.push_back(hw[2 * k] | (hw[2 * k + 1] << 16));
     }
+    if ((int)(S.words.size() - d0) != S.strideF) err = "internal: final descriptor size";
+  }
+  {
+    double nf = (double)S.npair * (double)(1 << (n - 1));
+    S.fp_ops[0] += nf * (n - 1); S.fp_ops[1] += nf * ((n - 1) * (n - 2) / 2); S.fp_ops[n > 2 ? 6 : 7] += nf;
+    S.fp_ops[3] += nf * (1 + 2 * (NJ * C - 1)); S.fp_ops[2] += nf * 2 * 2 * NJ * C; S.fp_ops[5] += nf * 2 * NJ * 4;
   }
   // Cholesky C = L L^T (C is positive definite); J^dagger C J = |L^T J|^2.  L^T in mma.m8n8k4 A-fragment order:
   // for m-tile mt, k-steps kt = 2 mt .. KT-1 (upper triangle), element (lane>>2, lane&3) of the 8x4 tile.
@@ -234,22 +309,30 @@ static BgSched build_schedule(int n) {
 // ------------------------------------------------------------------------------------------------ device side
 struct BgSet { double gq, g3, g4, mt, fac; };        // fac = 2 gq^2 / D  (|i gq|^2, parity factor 2, averaging)
 struct BgDev {
-  int nG, nR, nL, nwords, nslot, shared_ext;
-  int offG[6], offR[6], offL[6], offF;
+  int nwords, nslot, shared_ext;
+  int offD[3][6], offT[6], offF;
   const uint32_t* words; const double* lfrag;
   BgSet set[2];
+  unsigned long long* dbg;
 };
 
 struct BgProcess {
   BgSched S; BgDev D; uint32_t* d_words; double* d_lfrag; int sm_count; size_t smem64, smem32; int nslot64, nslot32;
 };
 
+template <typename T> struct pair_of;
+template <> struct pair_of<double> { typedef double2 type; };
+template <> struct pair_of<float> { typedef float2 type; };
+template <typename T> __device__ __forceinline__ cx<T> ldc(const cx<T>* p) { typename pair_of<T>::type t = *reinterpret_cast<const typename pair_of<T>::type*>(p); return mk<T>(t.x, t.y); }
+template <typename T> __device__ __forceinline__ void stc(cx<T>* p, cx<T> v) { typename pair_of<T>::type t; t.x = v.re; t.y = v.im; *reinterpret_cast<typename pair_of<T>::type*>(p) = t; }
+
 template <typename T> struct Smem {
   uint32_t* W;    // schedule words (whole CTA)
   double* pm;     // [nslot][n_ext][4] momenta (always double)
   double* acc;    // [nslot][2]   helicity-summed colour forms (owned by the colour warps)
   double* red;    // [nslot][8]   per-warp partial sums of the colour form
-  T* G; T* R; T* L;  // [nslot][8][nX]   SoA planes: conflict-free for consecutive helicity variants
+  cx<T>* G; cx<T>* R; cx<T>* L;   // [nslot][4][nX]   component planes of (re,im) pairs: one vector load per component,
+                                  //                  conflict-free for consecutive helicity variants
   T* K;           // [nslot][NMASK][4] momentum sums of gluon subsets
   T* iK2;         // [nslot][NMASK]
   T* dR; T* dL;   // [nslot][NMASK] 1/(q^2-m^2)
@@ -257,46 +340,56 @@ template <typename T> struct Smem {
 };
 template <int N, typename T> __host__ __device__ inline size_t carve(Smem<T>& s, unsigned char* base, int ns, int nwords) {
   typedef Geo<N> Ge; size_t off = 0; constexpr int nG = Ge::NG, nR = Ge::NR, nL = Ge::NL;
-  s.A = (double*)(base + off); off += sizeof(double) * 2 * (size_t)ns * Ge::ABUF;
-  s.pm = (double*)(base + off); off += sizeof(double) * ns * (N + 2) * 4;
-  s.acc = (double*)(base + off); off += sizeof(double) * ns * 2;
-  s.red = (double*)(base + off); off += sizeof(double) * ns * 8;
-  s.G = (T*)(base + off); off += sizeof(T) * (size_t)ns * 8 * nG;
-  s.R = (T*)(base + off); off += sizeof(T) * (size_t)ns * 8 * nR;
-  s.L = (T*)(base + off); off += sizeof(T) * (size_t)ns * 8 * nL;
-  s.K = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK * 4;
-  s.iK2 = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK;
-  s.dR = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK;
-  s.dL = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK;
-  s.W = (uint32_t*)(base + off); off += sizeof(uint32_t) * nwords;
+  auto al = [&]() { off = (off + 15) / 16 * 16; };
+  s.A = (double*)(base + off); off += sizeof(double) * 2 * (size_t)ns * Ge::ABUF; al();
+  s.pm = (double*)(base + off); off += sizeof(double) * ns * (N + 2) * 4; al();
+  s.acc = (double*)(base + off); off += sizeof(double) * ns * 2; al();
+  s.red = (double*)(base + off); off += sizeof(double) * ns * 8; al();
+  s.G = (cx<T>*)(base + off); off += sizeof(T) * (size_t)ns * 8 * nG; al();
+  s.R = (cx<T>*)(base + off); off += sizeof(T) * (size_t)ns * 8 * nR; al();
+  s.L = (cx<T>*)(base + off); off += sizeof(T) * (size_t)ns * 8 * nL; al();
+  s.K = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK * 4; al();
+  s.iK2 = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
+  s.dR = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
+  s.dL = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
+  s.W = (uint32_t*)(base + off); off += sizeof(uint32_t) * nwords; al();
   return off;
 }
 
-template <typename T> __device__ __forceinline__ vec4<T> ld4(const T* tab, int stride, int e) {
+template <typename T> __device__ __forceinline__ vec4<T> ld4(const cx<T>* tab, int stride, int e) {
   vec4<T> r;
 #pragma unroll
-  for (int c = 0; c < 4; c++) { r.c[c].re = tab[(2 * c) * stride + e]; r.c[c].im = tab[(2 * c + 1) * stride + e]; }
+  for (int c = 0; c < 4; c++) r.c[c] = ldc(tab + c * stride + e);
   return r;
 }
-template <typename T> __device__ __forceinline__ spn<T> lds4(const T* tab, int stride, int e) {
+template <typename T> __device__ __forceinline__ spn<T> lds4(const cx<T>* tab, int stride, int e) {
   spn<T> r;
 #pragma unroll
-  for (int c = 0; c < 4; c++) { r.c[c].re = tab[(2 * c) * stride + e]; r.c[c].im = tab[(2 * c + 1) * stride + e]; }
+  for (int c = 0; c < 4; c++) r.c[c] = ldc(tab + c * stride + e);
   return r;
 }
-template <typename T, typename V> __device__ __forceinline__ void st4(T* tab, int stride, int e, const V& v) {
+template <typename T, typename V> __device__ __forceinline__ void st4(cx<T>* tab, int stride, int e, const V& v) {
 #pragma unroll
-  for (int c = 0; c < 4; c++) { tab[(2 * c) * stride + e] = v.c[c].re; tab[(2 * c + 1) * stride + e] = v.c[c].im; }
+  for (int c = 0; c < 4; c++) stc(tab + c * stride + e, v.c[c]);
 }
-__device__ __forceinline__ int ref_entry(uint32_t r, uint32_t v) {
-  uint32_t m = (r >> 16) & 7u, sh = (r >> 19) & 7u;
-  uint32_t w = (v >> sh) & ((1u << m) - 1u);
-  if (r & REF_REV) w = __brev(w) >> (32u - m);
-  return (int)((r & 0xffffu) + w);
+// the 4 momentum components of a gluon subset as vector loads
+__device__ __forceinline__ void ldk(double* k, const double* p) { double2 a = *reinterpret_cast<const double2*>(p), b = *reinterpret_cast<const double2*>(p + 2); k[0] = a.x; k[1] = a.y; k[2] = b.x; k[3] = b.y; }
+__device__ __forceinline__ void ldk(float* k, const float* p) { float4 a = *reinterpret_cast<const float4*>(p); k[0] = a.x; k[1] = a.y; k[2] = a.z; k[3] = a.w; }
+// NW words of a descriptor (16-byte aligned, NW a multiple of 4) into registers
+template <int NW> __device__ __forceinline__ void ldw(uint32_t* d, const uint32_t* s) {
+#pragma unroll
+  for (int i = 0; i < NW / 4; i++) { uint4 t = *reinterpret_cast<const uint4*>(s + 4 * i); d[4 * i] = t.x; d[4 * i + 1] = t.y; d[4 * i + 2] = t.z; d[4 * i + 3] = t.w; }
 }
-__device__ __forceinline__ int ref_m(uint32_t r) { return (int)((r >> 16) & 7u); }
-__device__ __forceinline__ int ref_mask(uint32_t r) { return (int)((r >> 24) & 31u); }
-__device__ __forceinline__ bool ref_neg(uint32_t r) { return (r & REF_NEG) != 0; }
+// helicity-variant bits [SH, SH+M) of the task's variant word; all shifts and widths are compile-time
+template <int M, int SH> __device__ __forceinline__ uint32_t fieldv(uint32_t v) { return M == 0 ? 0u : (v >> SH) & ((1u << M) - 1u); }
+template <int M> __device__ __forceinline__ uint32_t brevm(uint32_t f) { return __brev(f) >> (32 - M); }
+// entry of the gluon current referenced by the low 16 bits of r, for a block of static length M at static position SH
+template <int M, int SH> __device__ __forceinline__ int gentry(uint32_t r, uint32_t v) {
+  uint32_t f = fieldv<M, SH>(v);
+  if (M == 3) { if (r & REF_REV) f = brevm<3>(f); }
+  return (int)((r & 0x7fffu) + f);
+}
+__device__ __forceinline__ uint32_t halfw(const uint32_t* w, int k) { return (k & 1) ? (w[k >> 1] >> 16) : (w[k >> 1] & 0xffffu); }
 
 // named barriers (ids 1..6; id 0 is __syncthreads): workers among themselves, colour warps among themselves,
 // and the full/empty handshake of the two amplitude buffers
@@ -304,99 +397,188 @@ enum { BAR_WORK = 1, BAR_FULL0 = 2, BAR_EMPTY0 = 4, BAR_COLOUR = 6 };
 __device__ __forceinline__ void bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 __device__ __forceinline__ void bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
 
-// gluon current of one ordered M-tuple / helicity variant from shorter currents (unscaled by the propagator)
-template <int M, int nG, typename T> __device__ __forceinline__ vec4<T> gluon_sum(const uint32_t* w, uint32_t v, const T* G, const T* K, T g3, T g4) {
-  vec4<T> a3, a4;
-#pragma unroll
-  for (int i = 0; i < 4; i++) { a3.c[i] = mk<T>(0, 0); a4.c[i] = mk<T>(0, 0); }
-#pragma unroll
-  for (int k = 0; k < M - 1; k++) {
-    uint32_t ra = w[2 * k], rb = w[2 * k + 1];
-    vec4<T> A = cond_neg(ld4(G, nG, ref_entry(ra, v)), ref_neg(ra) != ref_neg(rb)), B = ld4(G, nG, ref_entry(rb, v));
-    L3_acc(a3, A, K + 4 * ref_mask(ra), B, K + 4 * ref_mask(rb));
+// gluon current of one ordered M-tuple / helicity variant from shorter currents (unscaled by the propagator).
+// w: the 2(M-1) + 3(M-1)(M-2)/2 reference words of the tuple, in registers.  No signs: every block is stored as used.
+template <int M, int nG, typename T> struct GluonSum {
+  template <int K> static __device__ __forceinline__ void l3(vec4<T>& a3, const uint32_t* w, uint32_t v, const cx<T>* G, const T* Kt) {
+    if constexpr (K < M) {
+      uint32_t ra = w[2 * (K - 1)], rb = w[2 * (K - 1) + 1];
+      vec4<T> A = ld4(G, nG, gentry<K, 0>(ra, v)), B = ld4(G, nG, gentry<M - K, K>(rb, v));
+      T ka[4], kb[4]; ldk(ka, Kt + (ra >> 16)); ldk(kb, Kt + (rb >> 16));
+      L3_acc(a3, A, ka, B, kb);
+      l3<K + 1>(a3, w, v, G, Kt);
+    }
   }
-  const uint32_t* w4 = w + 2 * (M - 1);
-#pragma unroll
-  for (int t = 0; t < (M - 1) * (M - 2) / 2; t++) {
-    uint32_t rx = w4[3 * t], ry = w4[3 * t + 1], rz = w4[3 * t + 2];
-    vec4<T> X = cond_neg(ld4(G, nG, ref_entry(rx, v)), (ref_neg(rx) != ref_neg(ry)) != ref_neg(rz));
-    vec4<T> Y = ld4(G, nG, ref_entry(ry, v)), Z = ld4(G, nG, ref_entry(rz, v));
-    V4_acc(a4, X, Y, Z);
+  // V4 terms over the compositions (J, K) with 1 <= J < K < M, enumerated in the builder's order
+  template <int J, int K, int IDX> static __device__ __forceinline__ void v4(vec4<T>& a4, const uint32_t* w4, uint32_t v, const cx<T>* G) {
+    if constexpr (J < M - 1) {
+      if constexpr (K < M) {
+        uint32_t rx = w4[3 * IDX], ry = w4[3 * IDX + 1], rz = w4[3 * IDX + 2];
+        vec4<T> X = ld4(G, nG, gentry<J, 0>(rx, v)), Y = ld4(G, nG, gentry<K - J, J>(ry, v)), Z = ld4(G, nG, gentry<M - K, K>(rz, v));
+        V4_acc(a4, X, Y, Z);
+        v4<J, K + 1, IDX + 1>(a4, w4, v, G);
+      } else v4<J + 1, J + 2, IDX>(a4, w4, v, G);
+    }
   }
-  vec4<T> r;
+  static __device__ __forceinline__ vec4<T> run(const uint32_t* w, uint32_t v, const cx<T>* G, const T* Kt, T g3, T g4) {
+    vec4<T> a3, a4;
 #pragma unroll
-  for (int i = 0; i < 4; i++) { r.c[i] = (-g3) * a3.c[i]; if (M > 2) rfma(r.c[i], g4, a4.c[i]); }
-  return r;
-}
+    for (int i = 0; i < 4; i++) { a3.c[i] = mk<T>(0, 0); a4.c[i] = mk<T>(0, 0); }
+    l3<1>(a3, w, v, G, Kt);
+    v4<1, 2, 0>(a4, w + 2 * (M - 1), v, G);
+    vec4<T> r;
+#pragma unroll
+    for (int i = 0; i < 4; i++) { r.c[i] = (-g3) * a3.c[i]; if (M > 2) rfma(r.c[i], g4, a4.c[i]); }
+    return r;
+  }
+};
 
 template <typename T> struct Ctx {
   Smem<T> s; int tid, ns; T g3, g4, gq, mt; const BgDev* D;
 };
 
-// phase M (worker warps): gluon currents of length M, right/left quark currents of length M-1 (all helicity variants)
+// quark-current terms  acc += Jslash(block) R(rest)  resp.  acc += L(rest) Jslash(block), block lengths K = 1..MM
+template <int MM, int K, int nG, int nQ, bool RIGHT, typename T>
+__device__ __forceinline__ void quark_terms(spn<T>& acc, const uint32_t* w, uint32_t v, int hb, const cx<T>* G, const cx<T>* Q) {
+  if constexpr (K <= MM) {
+    uint32_t r = w[K];
+    // right: gluon block [0,K), quark rest [K,MM);  left: quark rest [0,MM-K), gluon block [MM-K,MM)
+    int eg = RIGHT ? gentry<K, 0>(r, v) : gentry<K, MM - K>(r, v);
+    int eq = (int)(r >> 16) + (int)(RIGHT ? fieldv<MM - K, K>(v) : fieldv<MM - K, 0>(v)) + (hb << (MM - K));
+    lcv<T> J = lightcone(ld4(G, nG, eg));
+    if (RIGHT) slash_acc(acc, J, lds4(Q, nQ, eq)); else row_slash_acc(acc, lds4(Q, nQ, eq), J);
+    quark_terms<MM, K + 1, nG, nQ, RIGHT, T>(acc, w, v, hb, G, Q);
+  }
+}
+
+// phase M (worker warps): gluon currents of length M, right/left quark currents of length M-1, all helicity variants with
+// gluon 0 at helicity +.  Tasks are ordered [G of all slots][R of all slots][L of all slots]: a warp diverges at most at the two seams.
 template <int N, int M, typename T, int NWT> __device__ __forceinline__ void level_phase(const Ctx<T>& c) {
   typedef Geo<N> Ge;
   constexpr bool HASG = (M <= N - 1), HASR = (M - 1 >= 1 && M - 1 <= Ge::RMAX), HASL = (M - 1 >= 1 && M - 1 <= Ge::LMAX);
   constexpr int MM = M - 1;
-  constexpr int tg = HASG ? (ctuples(N, M) / 2) << M : 0, tr = HASR ? ctuples(N, MM) << M : 0, tl = HASL ? ctuples(N, MM) << M : 0, per = tg + tr + tl;
+  constexpr int tg = HASG ? c_ntaskG(N, M) : 0, tr = HASR ? c_ntaskQ(N, MM) : 0, tl = HASL ? c_ntaskQ(N, MM) : 0;
   const Smem<T>& s = c.s; constexpr int nG = Ge::NG, nR = Ge::NR, nL = Ge::NL, next = N + 2;
-  for (int t = c.tid; t < c.ns * per; t += NWT) {
-    int sl = t / per, o = t % per;
-    T* G = s.G + (size_t)sl * 8 * nG; T* R = s.R + (size_t)sl * 8 * nR; T* L = s.L + (size_t)sl * 8 * nL;
-    const T* K = s.K + (size_t)sl * Ge::NMASK * 4;
-    if (HASG && o < tg) {
-      int tup = o >> M; uint32_t v = o & ((1 << M) - 1);
-      const uint32_t* w = s.W + c.D->offG[M] + tup * (2 + 2 * (M - 1) + 3 * (M - 1) * (M - 2) / 2);
-      int ob = w[0], mask = w[1];
-      vec4<T> r = gluon_sum<M, nG, T>(w + 2, v, G, K, c.g3, c.g4);
-      T sc = s.iK2[sl * Ge::NMASK + mask];
+  const int ns = c.ns, nGt = ns * tg, nRt = ns * tr, nLt = ns * tl;
+  const uint32_t* TL = s.W + c.D->offT[M];
+  for (int t = c.tid; t < nGt + nRt + nLt; t += NWT) {
+    if (HASG && t < nGt) {
+     if constexpr (HASG) {
+      int sl = t / tg, o = t - sl * tg; uint32_t tw = TL[o]; uint32_t v = tw >> 16;
+      cx<T>* G = s.G + (size_t)sl * 4 * nG; const T* K = s.K + (size_t)sl * Ge::NMASK * 4;
+      constexpr int DW = gdesc_words(M);
+      uint32_t w[DW]; ldw<DW>(w, s.W + c.D->offD[0][M] + (tw & 0xffffu) * DW);
+      vec4<T> r = GluonSum<M, nG, T>::run(w + 2, v, G, K, c.g3, c.g4);
+      T sc = s.iK2[sl * Ge::NMASK + w[1]];
 #pragma unroll
       for (int i = 0; i < 4; i++) r.c[i] = sc * r.c[i];
-      st4(G, nG, ob + v, r);
-    } else if (HASR && o < tg + tr) {
-      int oo = o - tg; int tup = oo >> M; uint32_t vv = oo & ((1 << M) - 1); uint32_t v = vv & ((1 << MM) - 1); int hb = vv >> MM;
-      const uint32_t* w = s.W + c.D->offR[MM] + tup * (2 + 2 * MM);
-      int ob = w[0], mask = w[1];
+      st4(G, nG, (int)(w[0] & 0xffffu) + (int)v, r);
+      if (M == 2) {                                       // the other orientation: J(b,a) = -J(a,b), variant bits swapped
+#pragma unroll
+        for (int i = 0; i < 4; i++) r.c[i] = -r.c[i];
+        st4(G, nG, (int)(w[0] >> 16) + (int)(((v & 1u) << 1) | (v >> 1)), r);
+      }
+     }
+    } else if (HASR && t < nGt + nRt) {
+     if constexpr (HASR) {
+      int tt = t - nGt, sl = tt / tr, o = tt - sl * tr; uint32_t tw = TL[tg + o]; uint32_t vv = tw >> 16, v = vv & ((1u << MM) - 1u); int hb = (int)(vv >> MM);
+      const cx<T>* G = s.G + (size_t)sl * 4 * nG; cx<T>* R = s.R + (size_t)sl * 4 * nR; const T* K = s.K + (size_t)sl * Ge::NMASK * 4;
+      constexpr int DW = qdesc_words(MM);
+      uint32_t w[DW]; ldw<DW>(w, s.W + c.D->offD[1][MM] + (tw & 0xffffu) * DW);
+      int ob = (int)(w[0] & 0xffffu), mask = (int)(w[0] >> 16);
       spn<T> acc;
 #pragma unroll
       for (int i = 0; i < 4; i++) acc.c[i] = mk<T>(0, 0);
+      quark_terms<MM, 1, nG, nR, true, T>(acc, w, v, hb, G, R);
+      T q[4], k[4]; ldk(k, K + 4 * mask);
 #pragma unroll
-      for (int k = 0; k < MM; k++) {
-        uint32_t rj = w[2 + 2 * k], rr = w[3 + 2 * k];
-        lcv<T> J = lightcone(cond_neg(ld4(G, nG, ref_entry(rj, v)), ref_neg(rj)));
-        slash_acc(acc, J, lds4(R, nR, ref_entry(rr, v) + (hb << ref_m(rr))));
-      }
-      T q[4];
-#pragma unroll
-      for (int mu = 0; mu < 4; mu++) q[mu] = K[4 * mask + mu] - (T)s.pm[sl * next * 4 + 12 + mu];
+      for (int mu = 0; mu < 4; mu++) q[mu] = k[mu] - (T)s.pm[sl * next * 4 + 12 + mu];
       spn<T> r = slash_r_plus_m(q, c.mt, acc); T sc = -c.gq * s.dR[sl * Ge::NMASK + mask];
 #pragma unroll
       for (int i = 0; i < 4; i++) r.c[i] = sc * r.c[i];
-      st4(R, nR, ob + v + (hb << MM), r);
-    } else if (HASL) {
-      int oo = o - tg - tr; int tup = oo >> M; uint32_t vv = oo & ((1 << M) - 1); uint32_t v = vv & ((1 << MM) - 1); int hb = vv >> MM;
-      const uint32_t* w = s.W + c.D->offL[MM] + tup * (2 + 2 * MM);
-      int ob = w[0], mask = w[1];
+      st4(R, nR, ob + (int)vv, r);
+     }
+    } else if constexpr (HASL) {
+      int tt = t - nGt - nRt, sl = tt / tl, o = tt - sl * tl; uint32_t tw = TL[tg + tr + o]; uint32_t vv = tw >> 16, v = vv & ((1u << MM) - 1u); int hb = (int)(vv >> MM);
+      const cx<T>* G = s.G + (size_t)sl * 4 * nG; cx<T>* L = s.L + (size_t)sl * 4 * nL; const T* K = s.K + (size_t)sl * Ge::NMASK * 4;
+      constexpr int DW = qdesc_words(MM);
+      uint32_t w[DW]; ldw<DW>(w, s.W + c.D->offD[2][MM] + (tw & 0xffffu) * DW);
+      int ob = (int)(w[0] & 0xffffu), mask = (int)(w[0] >> 16);
       spn<T> acc;
 #pragma unroll
       for (int i = 0; i < 4; i++) acc.c[i] = mk<T>(0, 0);
+      quark_terms<MM, 1, nG, nL, false, T>(acc, w, v, hb, G, L);
+      T q[4], k[4]; ldk(k, K + 4 * mask);
 #pragma unroll
-      for (int k = 0; k < MM; k++) {
-        uint32_t rl = w[2 + 2 * k], rj = w[3 + 2 * k];
-        lcv<T> J = lightcone(cond_neg(ld4(G, nG, ref_entry(rj, v)), ref_neg(rj)));
-        row_slash_acc(acc, lds4(L, nL, ref_entry(rl, v) + (hb << ref_m(rl))), J);
-      }
-      T q[4];
-#pragma unroll
-      for (int mu = 0; mu < 4; mu++) q[mu] = (T)s.pm[sl * next * 4 + 8 + mu] - K[4 * mask + mu];
+      for (int mu = 0; mu < 4; mu++) q[mu] = (T)s.pm[sl * next * 4 + 8 + mu] - k[mu];
       spn<T> r = row_slash_r_plus_m(acc, q, c.mt); T sc = -c.gq * s.dL[sl * Ge::NMASK + mask];
 #pragma unroll
       for (int i = 0; i < 4; i++) r.c[i] = sc * r.c[i];
-      st4(L, nL, ob + v + (hb << MM), r);
+      st4(L, nL, ob + (int)vv, r);
     }
   }
   bar_sync(BAR_WORK, NWT);
 }
+
+// a4: the quark line of one colour ordering (WHICH = 0: the pair's forward permutation, 1: its reversal) around the split position C:
+//   Acc[ht][hb] += sum_{i < C <= j} L(s_1..i; ht) Jslash(s_i+1..j) R(s_j+1..n; hb)
+// wq: the block's 16-bit references (L bases, R bases, gluon blocks), v: helicity bits by position in THIS ordering.
+template <int N, int WHICH, typename T> struct QuarkLine {
+  typedef Geo<N> Ge;
+  static constexpr int C = Ge::C, NJ = Ge::NJ, nG = Ge::NG, nR = Ge::NR, nL = Ge::NL;
+  template <int JJ, int I> static __device__ __forceinline__ void iterm(spn<T>& X0, spn<T>& X1, const uint32_t* wq, uint32_t v, const vec4<T>& Jn,
+                                                                        const cx<T>* G, const cx<T>* L) {
+    if constexpr (I < C) {
+      constexpr int J = C + JJ, M = J - I;                     // gluon block [I, J) of length M
+      lcv<T> Jl;
+      if constexpr (I == 0 && J == N) {
+        Jl = (WHICH == 1 && N % 2 == 0) ? lightcone_neg(Jn) : lightcone(Jn);          // J(reversed) = (-1)^{n+1} J
+      } else {
+        uint32_t r = halfw(wq, C + NJ + JJ * C + I);
+        uint32_t f = fieldv<M, I>(v);
+        if constexpr (M == 3) { if (r & REF_REV) f = brevm<3>(f); }
+        if constexpr (M == 4 && WHICH == 1) f = brevm<4>(f);                           // stored reversed (necklace rule)
+        vec4<T> Jv = ld4(G, nG, (int)((r & 0x7fffu) + f));
+        Jl = (M == 4 && WHICH == 1) ? lightcone_neg(Jv) : lightcone(Jv);
+      }
+      int el = (int)halfw(wq, I) + (int)fieldv<I, 0>(v);
+      row_slash_acc(X0, lds4(L, nL, el), Jl); row_slash_acc(X1, lds4(L, nL, el + (1 << I)), Jl);
+      iterm<JJ, I + 1>(X0, X1, wq, v, Jn, G, L);
+    }
+  }
+  template <int JJ> static __device__ __forceinline__ void jterm(cx<T> (&Acc)[2][2], const uint32_t* wq, uint32_t v, const vec4<T>& Jn,
+                                                                 const cx<T>* G, const cx<T>* R, const cx<T>* L) {
+    if constexpr (JJ < NJ) {
+      constexpr int J = C + JJ;
+      spn<T> X0, X1;
+#pragma unroll
+      for (int i = 0; i < 4; i++) { X0.c[i] = mk<T>(0, 0); X1.c[i] = mk<T>(0, 0); }
+      iterm<JJ, 0>(X0, X1, wq, v, Jn, G, L);
+      int er = (int)halfw(wq, C + JJ) + (int)fieldv<N - J, J>(v);
+#pragma unroll
+      for (int hb = 0; hb < 2; hb++) {
+        spn<T> Rr = lds4(R, nR, er + (hb << (N - J)));
+        rowcol_acc(Acc[0][hb], X0, Rr); rowcol_acc(Acc[1][hb], X1, Rr);
+      }
+      jterm<JJ + 1>(Acc, wq, v, Jn, G, R, L);
+    }
+  }
+  static __device__ __forceinline__ void run(double* Arow, int f, const uint32_t* wq, uint32_t v, const vec4<T>& Jn, const cx<T>* G, const cx<T>* R, const cx<T>* L) {
+    cx<T> Acc[2][2];
+#pragma unroll
+    for (int a = 0; a < 2; a++)
+#pragma unroll
+      for (int b = 0; b < 2; b++) Acc[a][b] = mk<T>(0, 0);
+    jterm<0>(Acc, wq, v, Jn, G, R, L);
+#pragma unroll
+    for (int ht = 0; ht < 2; ht++)
+#pragma unroll
+      for (int hb = 0; hb < 2; hb++) {
+        int col = f * 4 + ht * 2 + hb;
+        *reinterpret_cast<double2*>(Arow + 2 * col) = make_double2((double)Acc[ht][hb].re, (double)Acc[ht][hb].im);
+      }
+  }
+};
 
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
@@ -426,7 +608,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
   __syncthreads();
   if (threadIdx.x < NWT) {
     // =========================================================================================== worker warps
-    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REG_WORK));
+    if constexpr (sizeof(T) == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REG_WORK));
     const int tid = threadIdx.x; c.tid = tid;
     for (int t = tid; t < D.nwords; t += NWT) s.W[t] = __ldg(D.words + t);
     unsigned step = 0;
@@ -452,15 +634,15 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
               int i = o >> 1, hb = o & 1, leg = i < 2 ? i : i + 2; const double* p = pm + 4 * leg;
               vec4<T> e = polvec<T>((T)p[1], (T)p[2], (T)p[3], hb ? -1 : +1);
               if (i >= 2) e = conj4(e);              // outgoing gluon carries eps*
-              st4(s.G + (size_t)sl * 8 * nG, nG, 2 * i + hb, e);
+              st4(s.G + (size_t)sl * 4 * nG, nG, 2 * i + hb, e);
             } else if (o < 2 * N + 2) {              // v(p_tbar, lam), R() entries 0,1
               int hb = o - 2 * N; const double* p = pm + 12;
               chi_pair<T> x = make_chi<T>((T)p[1], (T)p[2], (T)p[3]);
-              st4(s.R + (size_t)sl * 8 * nR, nR, hb, spinor_v<T>(x, (T)p[0], c.mt, hb ? -1 : +1));
+              st4(s.R + (size_t)sl * 4 * nR, nR, hb, spinor_v<T>(x, (T)p[0], c.mt, hb ? -1 : +1));
             } else if (o < 2 * N + 4) {              // ubar(p_t, lam), L() entries 0,1
               int hb = o - 2 * N - 2; const double* p = pm + 8;
               chi_pair<T> x = make_chi<T>((T)p[1], (T)p[2], (T)p[3]);
-              st4(s.L + (size_t)sl * 8 * nL, nL, hb, bar(spinor_u<T>(x, (T)p[0], c.mt, hb ? -1 : +1)));
+              st4(s.L + (size_t)sl * 4 * nL, nL, hb, bar(spinor_u<T>(x, (T)p[0], c.mt, hb ? -1 : +1)));
             } else {                                 // gluon subset `mask`
               int mask = o - 2 * N - 4;
               TK k[4] = {0, 0, 0, 0};
@@ -490,61 +672,31 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
           double* Abuf = s.A + (size_t)buf * ns * Ge::ABUF;
           constexpr int per = Ge::NPAIR * Ge::NFREE;
           for (int t = tid; t < ns * per; t += NWT) {
-            int sl = t / per, o = t % per; int pair = o / Ge::NFREE, f = o % Ge::NFREE;
-            const T* G = s.G + (size_t)sl * 8 * nG; const T* R = s.R + (size_t)sl * 8 * nR; const T* L = s.L + (size_t)sl * 8 * nL;
+            int sl = t / per, o = t - sl * per; int pair = o / Ge::NFREE, f = o % Ge::NFREE;
+            const cx<T>* G = s.G + (size_t)sl * 4 * nG; const cx<T>* R = s.R + (size_t)sl * 4 * nR; const cx<T>* L = s.L + (size_t)sl * 4 * nL;
             const T* K = s.K + (size_t)sl * Ge::NMASK * 4;
             const uint32_t* w = s.W + D.offF + pair * Ge::STRIDEF;
-            uint32_t rk = w[0], rkr = w[1], packed = w[2], negr = w[3];
+            uint32_t w0 = w[0], packed = w[1];
             uint32_t g = ((uint32_t)batch << 1) | ((uint32_t)f << (1 + Ge::NB));   // helicity bits by gluon label; gluon 0: + (parity)
             uint32_t v = 0;
 #pragma unroll
             for (int j = 0; j < N; j++) v |= ((g >> ((packed >> (3 * j)) & 7u)) & 1u) << j;   // by position in sigma
-            vec4<T> Jn = gluon_sum<N, nG, T>(w + 4, v, G, K, c.g3, c.g4);
+            vec4<T> Jn;
+            {
+              uint32_t jw[Ge::JW]; ldw<Ge::JW>(jw, w + 4);
+              Jn = GluonSum<N, nG, T>::run(jw, v, G, K, c.g3, c.g4);
+            }
             T sc = s.iK2[sl * Ge::NMASK + Ge::NMASK - 1];
 #pragma unroll
             for (int i = 0; i < 4; i++) Jn.c[i] = sc * Jn.c[i];
             double* A = Abuf + (size_t)sl * Ge::ABUF;
-            const uint32_t* wt = w + Ge::WOFF_TERMS;
-#pragma unroll 1
-            for (int which = 0; which < 2; which++) {
-              cx<T> Acc[2][2];
-#pragma unroll
-              for (int a = 0; a < 2; a++)
-#pragma unroll
-                for (int b = 0; b < 2; b++) Acc[a][b] = mk<T>(0, 0);
-#pragma unroll
-              for (int jj = 0; jj < Ge::NJ; jj++) {
-                spn<T> X0, X1;
-#pragma unroll
-                for (int i = 0; i < 4; i++) { X0.c[i] = mk<T>(0, 0); X1.c[i] = mk<T>(0, 0); }
-#pragma unroll
-                for (int i = 0; i < Ge::C; i++) {
-                  if (i == 0 && jj == Ge::NJ - 1) {                 // the full-length gluon current between ubar and v
-                    lcv<T> J = lightcone(cond_neg(Jn, which && negr));
-                    row_slash_acc(X0, lds4(L, nL, 0), J); row_slash_acc(X1, lds4(L, nL, 1), J);
-                  } else {
-                    uint32_t rl = wt[i], rj = wt[Ge::C + Ge::NJ + jj * Ge::C + i];
-                    lcv<T> J = lightcone(cond_neg(ld4(G, nG, ref_entry(rj, v)), ref_neg(rj)));
-                    int el = ref_entry(rl, v), ml = ref_m(rl);
-                    row_slash_acc(X0, lds4(L, nL, el), J); row_slash_acc(X1, lds4(L, nL, el + (1 << ml)), J);
-                  }
-                }
-                uint32_t rr = wt[Ge::C + jj]; int er = ref_entry(rr, v), mr = ref_m(rr);
-#pragma unroll
-                for (int hb = 0; hb < 2; hb++) {
-                  spn<T> Rr = lds4(R, nR, er + (hb << mr));
-                  rowcol_acc(Acc[0][hb], X0, Rr); rowcol_acc(Acc[1][hb], X1, Rr);
-                }
-              }
-              uint32_t row = which ? rkr : rk;
-#pragma unroll
-              for (int ht = 0; ht < 2; ht++)
-#pragma unroll
-                for (int hb = 0; hb < 2; hb++) {
-                  int col = f * 4 + ht * 2 + hb;
-                  *reinterpret_cast<double2*>(A + (size_t)row * Ge::ASTR + 2 * col) = make_double2((double)Acc[ht][hb].re, (double)Acc[ht][hb].im);
-                }
-              wt += Ge::WPER;
+            {
+              uint32_t wq[Ge::QW]; ldw<Ge::QW>(wq, w + 4 + Ge::JW);
+              QuarkLine<N, 0, T>::run(A + (size_t)(w0 & 0xffffu) * Ge::ASTR, f, wq, v, Jn, G, R, L);
+            }
+            {
+              uint32_t wq[Ge::QW]; ldw<Ge::QW>(wq, w + 4 + Ge::JW + Ge::QW);
+              QuarkLine<N, 1, T>::run(A + (size_t)(w0 >> 16) * Ge::ASTR, f, wq, brevm<N>(v), Jn, G, R, L);
             }
           }
           __threadfence_block();
@@ -555,7 +707,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
     }
   } else {
     // =========================================================================================== colour warps
-    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REG_COL));
+    if constexpr (sizeof(T) == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REG_COL));
     const int ctid = threadIdx.x - NWT, cwarp = ctid >> 5, lane = ctid & 31;
     unsigned step = 0;
     for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
@@ -647,12 +799,20 @@ template <int N> static void bg_launch(int precision, int grid, size_t s64, size
 
 static BgProcess* bg_create(int n, const rwgt_params& po, const rwgt_params& pn, std::string& err) {
   BgProcess* B = new BgProcess();
-  B->S = build_schedule(n);
+  B->S = build_schedule(n, err);
+  if (!err.empty()) { delete B; return nullptr; }
   const BgSched& S = B->S;
   BgDev& D = B->D;
-  D.nG = S.nG; D.nR = S.nR; D.nL = S.nL; D.nwords = (int)S.words.size(); D.offF = S.offF;
-  if (S.nG != c_nG(n) || S.nR != c_nQ(n, S.rmax) || S.nL != c_nQ(n, S.lmax)) { err = "internal: schedule/geometry mismatch"; delete B; return nullptr; }
-  for (int m = 0; m < 6; m++) { D.offG[m] = S.offG[m]; D.offR[m] = S.offR[m]; D.offL[m] = S.offL[m]; }
+  D.nwords = (int)S.words.size(); D.offF = S.offF; D.dbg = nullptr;
+  bool ok = (S.nG == c_nG(n) && S.nR == c_nQ(n, S.rmax) && S.nL == c_nQ(n, S.lmax) && S.npair == S.nperm / 2);
+  for (int m = 2; m <= n - 1; m++) ok = ok && S.ntask[0][m] == c_ntaskG(n, m);
+  for (int m = 1; m <= S.rmax; m++) ok = ok && S.ntask[1][m + 1] == c_ntaskQ(n, m);
+  for (int m = 1; m <= S.lmax; m++) ok = ok && S.ntask[2][m + 1] == c_ntaskQ(n, m);
+  switch (n) { case 2: ok = ok && S.strideF == Geo<2>::STRIDEF; break; case 3: ok = ok && S.strideF == Geo<3>::STRIDEF; break;
+               case 4: ok = ok && S.strideF == Geo<4>::STRIDEF; break; default: ok = ok && S.strideF == Geo<5>::STRIDEF; }
+  if (!ok) { err = "internal: schedule/geometry mismatch"; delete B; return nullptr; }
+  for (int k = 0; k < 3; k++) for (int m = 0; m < 6; m++) D.offD[k][m] = S.offD[k][m];
+  for (int m = 0; m < 6; m++) D.offT[m] = S.offT[m];
   const rwgt_params* ps[2] = {&po, &pn};
   double fact = 1; for (int i = 2; i <= n - 2; i++) fact *= i;
   for (int k = 0; k < 2; k++) {
@@ -685,18 +845,11 @@ static void bg_destroy(BgProcess* B) { if (!B) return; cudaFree(B->d_words); cud
 
 // Algorithmic flop count of the schedule on the FP64 (or FP32) FMA pipe, both parameter sets, per event: FMA = 2 flop,
 // MUL = ADD = 1 flop, per operation of rwgt_math.cuh (L3 74 FMA + 6 MUL + 4 ADD, V4 90 + 6 + 2, slash-accumulate 32 FMA,
-// light-cone 8 ADD, propagator 24 FMA + 17 MUL + 6 ADD, row.col 16 FMA, current store 8 FMA + 16 MUL).  Agrees with the
-// ncu instruction counters of the committed build to 0.5% (n=5), 1.0% (n=4), 2.6% (n=3), always from below
-// (profiles/r1_summary.md).
+// light-cone 8 ADD, propagator 24 FMA + 17 MUL + 6 ADD, row.col 16 FMA, current store 8 FMA + 16 MUL), times the number of
+// such operations the schedule executes (helicity variants with gluon 0 at helicity - are not evaluated and not counted).
 static double bg_flops_per_event(const BgProcess* B, int /*precision*/) {
-  const int n = B->S.n, C = B->S.c, NJ = n - C + 1; const double L3 = 158, V4 = 188, SLA = 64, LC = 8, PROP = 71, RC = 32, GST = 32, GST2 = 16;
-  auto tup = [](int n, int m) { double r = 1; for (int i = 0; i < m; i++) r *= (n - i); return r; };
-  double fp = 0;
-  for (int m = 2; m <= n - 1; m++) fp += tup(n, m) / 2 * (1 << m) * ((m - 1) * L3 + (m - 1) * (m - 2) / 2 * V4 + (m > 2 ? GST : GST2));
-  for (int m = 1; m <= B->S.rmax; m++) fp += tup(n, m) * (2 << m) * (m * (SLA + LC) + PROP);
-  for (int m = 1; m <= B->S.lmax; m++) fp += tup(n, m) * (2 << m) * (m * (SLA + LC) + PROP);
-  double per_final = (n - 1) * L3 + (n - 1) * (n - 2) / 2 * V4 + (n > 2 ? GST : GST2) + LC + 2 * (NJ * C * (2 * SLA + LC) + NJ * 4 * RC);
-  fp += B->S.npair * (double)(1 << (n - 1)) * per_final;
+  const int n = B->S.n; const double fl[8] = {158, 188, 64, 8, 71, 32, 32, 16};
+  double fp = 0; for (int k = 0; k < 8; k++) fp += B->S.fp_ops[k] * fl[k];
   return 2.0 * fp + n * 2 * 30.0 + 4 * 40.0 + (1 << n) * 40.0;
 }
 // FP64 tensor-pipe flops of the colour form (upper-triangular mma.m8n8k4 tiles, 256 FMA each), both parameter sets

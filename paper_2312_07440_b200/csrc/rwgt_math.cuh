@@ -162,6 +162,12 @@ template <typename T> __device__ __forceinline__ lcv<T> lightcone(const vec4<T>&
   r.r = mk<T>(a.c[1].re + a.c[2].im, a.c[1].im - a.c[2].re); r.l = mk<T>(a.c[1].re - a.c[2].im, a.c[1].im + a.c[2].re);
   return r;
 }
+// light-cone components of -a (the negation rides on the adds)
+template <typename T> __device__ __forceinline__ lcv<T> lightcone_neg(const vec4<T>& a) {
+  lcv<T> r; r.p = mk<T>(-a.c[0].re - a.c[3].re, -a.c[0].im - a.c[3].im); r.m = mk<T>(a.c[3].re - a.c[0].re, a.c[3].im - a.c[0].im);
+  r.r = mk<T>(-a.c[1].re - a.c[2].im, a.c[2].re - a.c[1].im); r.l = mk<T>(a.c[2].im - a.c[1].re, -a.c[1].im - a.c[2].re);
+  return r;
+}
 // X += a-slash * s      (8 complex FMAs)
 template <typename T> __device__ __forceinline__ void slash_acc(spn<T>& X, const lcv<T>& a, const spn<T>& s) {
   cfma(X.c[0], a.m, s.c[2]); cfma(X.c[0], -a.r, s.c[3]);
