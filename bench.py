@@ -143,9 +143,14 @@ def run_reference(args) -> None:
 
 
 # ------------------------------------------------------------------------------------------------- our arm
-def time_config(torch, B, c, precision, n, steps, warmup, seed_offset, flush_buf, sampler_index=None):
+def time_config(torch, B, c, precision, n, steps, warmup, seed_offset, flush_buf, sampler_index=None, tile_from=0):
     """Device-resident timing of one config. Returns dict with per-step ms list etc."""
-    m, w = ev.generate(c, n, seed=c.seed + 1000 * seed_offset)
+    if tile_from and tile_from < n:
+        m0, w0 = ev.generate(c, tile_from, seed=c.seed + 1000 * seed_offset)
+        reps = (n + tile_from - 1) // tile_from
+        m, w = np.tile(m0, (1, 1, reps))[:, :, :n].copy(), np.tile(w0, reps)[:n].copy()
+    else:
+        m, w = ev.generate(c, n, seed=c.seed + 1000 * seed_offset)
     dm, dw = torch.from_numpy(m).cuda(), torch.from_numpy(w).cuda()
     out = torch.empty((3, n), dtype=torch.float64, device="cuda")
     r = B.Reweighter(c.process, c.params_old, c.params_new, precision)
@@ -241,10 +246,14 @@ def main() -> None:
             dist.destroy_process_group()
         return
 
-    # ---- roofline of the (single) kernel of a step: plain FP64/FP32 FMA pipe ----
+    # ---- roofline of the (single) kernel of a step: the FP64 (FP32) arithmetic pipe ----
+    # FP64 mode: DFMA and DMMA share one pipe on B200 (rwgt_measure_peak kind 7), so the numerator is the vector flops
+    # plus the algorithmic flops of the colour form (a5, run as mma.m8n8k4).  FP32/mixed: the vector flops against the
+    # FP32 pipe; the colour form stays on the FP64 pipe and is reported beside it.
     peaks = measured_peaks()
     kernel_ms = statistics.mean(res["ms"])
-    flops = res["flops_per_event"] * n
+    vec_flops, col_flops = res["flops_per_event"] * n, res["tensor_flops_per_event"] * n
+    flops = vec_flops + (col_flops if dtype == "f64" else 0.0)
     achieved_tf = flops / (kernel_ms * 1e-3) / 1e12
     max_mhz = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
     peak_tf = alu_peak_tflops(dtype, max_mhz)
@@ -255,18 +264,26 @@ def main() -> None:
             traffic = None
     except Exception:
         pass
-    try:
-        chain_tf = B.rwgt_measure_peak(0 if dtype == "f64" else 1)       # register-resident FMA chain, same session
-    except Exception:
-        chain_tf = None
+    micro = {}
+    kinds = ({"fma_chain": 0, "fma_3_distinct_sources": 3, "fma_1_reused_source": 4, "dmma_chain": 2, "dfma_and_dmma_concurrent": 7}
+             if dtype == "f64" else {"fma_chain": 1, "fma_3_distinct_sources": 5, "fma_1_reused_source": 6})
+    for name, kind in kinds.items():
+        try:
+            micro[name] = B.rwgt_measure_peak(kind)          # register-resident microbenchmarks, same session
+        except Exception:
+            micro[name] = None
+    chain_tf = micro.get("fma_chain")
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": traffic,
                 "peak_source": f"derived: 148 SM x {FP64_LANES_PER_SM if dtype == 'f64' else FP32_LANES_PER_SM} FMA lanes x 2 flop x {max_mhz:g} MHz (max SM clock); DESIGN.md Roofline",
                 "peak_fma_chain_measured": chain_tf, "frac_of_fma_chain_measured": (achieved_tf / chain_tf) if chain_tf else None,
+                "microbench_tflops": micro,
                 "frac_at_clock_under_load": (achieved_tf / alu_peak_tflops(dtype, clocks["sm_mhz"])) if clocks.get("sm_mhz") else None,
-                "flops_per_event": res["flops_per_event"], "kernel_ms": kernel_ms,
-                "tensor_fp64": {"flops_per_event": res["tensor_flops_per_event"],
-                                "achieved_tflops": res["tensor_flops_per_event"] * n / (kernel_ms * 1e-3) / 1e12,
-                                "note": "colour form on the FP64 tensor pipe (mma.m8n8k4), a separate pipe; not counted in `achieved`"},
+                "flops_per_event": res["flops_per_event"] + (res["tensor_flops_per_event"] if dtype == "f64" else 0.0),
+                "vector_flops_per_event": res["flops_per_event"], "colour_form_flops_per_event": res["tensor_flops_per_event"],
+                "kernel_ms": kernel_ms,
+                "colour_form_fp64": {"flops_per_event": res["tensor_flops_per_event"],
+                                     "achieved_tflops": col_flops / (kernel_ms * 1e-3) / 1e12,
+                                     "note": "mma.m8n8k4 on the FP64 pipe (shared with DFMA); included in `achieved` in FP64 mode only"},
                 "hbm": {"achieved_gbs": bytes_per_event(c) * n / (kernel_ms * 1e-3) / 1e9, "peak_gbs": peaks.get("hbm_gbs", 6650.0),
                         "peak_source": "MEASURED_PEAKS.json" if peaks.get("hbm_gbs") else "fallback"}}
     roofline["hbm"]["frac"] = roofline["hbm"]["achieved_gbs"] / roofline["hbm"]["peak_gbs"]
@@ -307,13 +324,28 @@ def main() -> None:
                     rr = time_config(torch, B, cc, prec, cc.n_events, 5, 3, 0, flush_buf)
                     kms = statistics.mean(rr["ms"])
                     dt_ = "f64" if prec == "fp64" else "f32"
-                    tf = rr["flops_per_event"] * cc.n_events / (kms * 1e-3) / 1e12
+                    fpe = rr["flops_per_event"] + (rr["tensor_flops_per_event"] if dt_ == "f64" else 0.0)
+                    tf = fpe * cc.n_events / (kms * 1e-3) / 1e12
                     extra.append({"workload": workload_name(cc, cc.n_events), "precision": prec, "events_per_s": cc.n_events / (kms * 1e-3),
                                   "kernel_ms": kms, "alu_tflops": tf, "alu_frac": tf / alu_peak_tflops(dt_, max_mhz),
-                                  "hbm_gbs": bytes_per_event(cc) * cc.n_events / (kms * 1e-3) / 1e9, "l2": rr["l2"]})
+                                  "hbm_gbs": bytes_per_event(cc) * cc.n_events / (kms * 1e-3) / 1e9,
+                                  "hbm_frac": bytes_per_event(cc) * cc.n_events / (kms * 1e-3) / 1e9 / roofline["hbm"]["peak_gbs"], "l2": rr["l2"]})
                     rr["rw"].close()
                 except Exception as ex:  # keep the headline line alive
                     extra.append({"workload": workload_name(cc, cc.n_events), "precision": prec, "error": str(ex)})
+        # cfg 1 is launch-latency-bound at its 16,384 events: the same distribution at n = 2^24 (buffers >> L2)
+        try:
+            c1 = ev.config(1)
+            rr = time_config(torch, B, c1, "fp64", 1 << 24, 5, 3, 0, flush_buf, tile_from=1 << 20)
+            kms = statistics.mean(rr["ms"]); n1 = 1 << 24
+            gbs = bytes_per_event(c1) * n1 / (kms * 1e-3) / 1e9
+            tf = rr["flops_per_event"] * n1 / (kms * 1e-3) / 1e12
+            extra.append({"workload": workload_name(c1, n1) + " (asymptotic: the seeded set of 2^20 events tiled 16x)", "precision": "fp64",
+                          "events_per_s": n1 / (kms * 1e-3), "kernel_ms": kms, "alu_tflops": tf, "alu_frac": tf / alu_peak_tflops("f64", max_mhz),
+                          "hbm_gbs": gbs, "hbm_frac": gbs / roofline["hbm"]["peak_gbs"], "l2": rr["l2"]})
+            rr["rw"].close()
+        except Exception as ex:
+            extra.append({"workload": "epem_mupmum n=2^24", "error": str(ex)})
         line["other_configs"] = extra
     print(json.dumps(line), flush=True)
     if world > 1:

@@ -67,7 +67,9 @@ int rwgt_n_external(const rwgt_handle* h);
  * sets, all helicities (checked against ncu counters).  Roofline use. */
 double rwgt_flops_per_event(const rwgt_handle* h);
 
-/* Same for the FP64 tensor pipe (mma.m8n8k4 of the colour form; 0 for the 2->2 kernels). */
+/* Algorithmic flops per event of the colour form |L^T J|^2 (step a5), which the engine evaluates with FP64 mma.m8n8k4
+ * in every precision mode (0 for the 2->2 kernels, whose colour form is part of rwgt_flops_per_event).  DFMA and DMMA
+ * share one pipe on B200, so in FP64 mode the roofline numerator is the sum of the two counts. */
 double rwgt_tensor_flops_per_event(const rwgt_handle* h);
 
 /* The hot path: a1-a7 of SURVEY.md §8(a) in one kernel launch on `stream`.
@@ -90,8 +92,10 @@ int rwgt_run(rwgt_handle* h, const double* momenta, const double* weights, doubl
 
 /* Same computation with HOST buffers (pageable or pinned): copies the inputs to device
  * scratch owned by the handle (grown on demand), runs the kernel, copies the three outputs
- * back and synchronises `stream`.  This is the end-to-end path of bench.py's `e2e` key
- * (host<->device transfer is part of what a user pays).  Same return codes. */
+ * back and synchronises `stream`.  The events are processed in up to 8 chunks so that the host->device copy of one
+ * chunk, the kernel of the previous one and the device->host copy of the one before overlap (two internal copy
+ * streams; the overlap needs pinned host buffers, pageable ones still work).  This is the end-to-end path of
+ * bench.py's `e2e` key (host<->device transfer is part of what a user pays).  Same return codes. */
 int rwgt_run_host(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old,
                   double* out_me_new, double* out_w_new, long long n_events, void* stream);
 
@@ -108,7 +112,11 @@ int rwgt_colour_matrix(int n_gluons, double* out);
 
 /* Measurement aid for the roofline: runs a register-resident FMA chain on the current
  * device and writes the sustained rate in TFLOP/s (2 flop per FMA) to *out_tflops (HOST pointer).
- * kind 0: FP64 FMA, 1: FP32 FMA, 2: FP64 tensor (mma m8n8k4).  Synchronises the device.  0 or -1. */
+ * kind 0: FP64 FMA chain x = fma(x,a,b), 1: FP32 FMA chain, 2: FP64 tensor (mma m8n8k4) chain,
+ * 3 / 4: FP64 FMA with three distinct register sources / with one source reused by consecutive FMAs (the operand
+ * pattern of real complex arithmetic; register-file read bandwidth makes these slower than kind 0),
+ * 5 / 6: the same two patterns in FP32, 7: FP64 FMA chains and DMMA chains concurrently on every SM, summed rate
+ * (DFMA and DMMA share one pipe on B200: kind 7 = kind 0 = kind 2).  Synchronises the device.  0 or -1. */
 int rwgt_measure_peak(int kind, double* out_tflops);
 
 #ifdef __cplusplus

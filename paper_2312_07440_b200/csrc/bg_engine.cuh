@@ -591,7 +591,7 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 template <int N, typename T, bool MIXED, int NW, int NCW>
 __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
                                                                double* __restrict__ me_old, double* __restrict__ me_new,
-                                                               double* __restrict__ w_new, long long nev, BgDev D) {
+                                                               double* __restrict__ w_new, long long nev, long long stride, BgDev D) {
   typedef Geo<N> Ge;
   constexpr int NTH = (NW + NCW) * 32, NWT = NW * 32, NCT = NCW * 32;
   // register hand-over between the warpgroups: the colour warps need few registers, the workers get the rest
@@ -618,7 +618,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
       // ---- a1: load momenta (coalesced over the events of the group) ----
       for (int t = tid; t < ns * next * 4; t += NWT) {
         int sl = t % ns, comp = t / ns; long long ev = ev0 + sl; if (ev >= nev) ev = nev - 1;
-        s.pm[(sl * next * 4) + comp] = __ldg(mom + (size_t)comp * nev + ev);
+        s.pm[(sl * next * 4) + comp] = __ldg(mom + (size_t)comp * stride + ev);
       }
       bar_sync(BAR_WORK, NWT);
 #pragma unroll 1
@@ -790,11 +790,11 @@ template <int N> static cudaError_t bg_set_attr(size_t s64, size_t s32) {
   return e;
 }
 template <int N> static void bg_launch(int precision, int grid, size_t s64, size_t s32, cudaStream_t st, const double* mom, const double* w,
-                                       double* a, double* b, double* o, long long nev, const BgDev& D) {
+                                       double* a, double* b, double* o, long long nev, long long stride, const BgDev& D) {
   const int nth = (BG_NW + BG_NCW) * 32;
-  if (precision == RWGT_FP64) bg_kernel<N, double, false, BG_NW, BG_NCW><<<grid, nth, s64, st>>>(mom, w, a, b, o, nev, D);
-  else if (precision == RWGT_FP32) bg_kernel<N, float, false, BG_NW, BG_NCW><<<grid, nth, s32, st>>>(mom, w, a, b, o, nev, D);
-  else bg_kernel<N, float, true, BG_NW, BG_NCW><<<grid, nth, s32, st>>>(mom, w, a, b, o, nev, D);
+  if (precision == RWGT_FP64) bg_kernel<N, double, false, BG_NW, BG_NCW><<<grid, nth, s64, st>>>(mom, w, a, b, o, nev, stride, D);
+  else if (precision == RWGT_FP32) bg_kernel<N, float, false, BG_NW, BG_NCW><<<grid, nth, s32, st>>>(mom, w, a, b, o, nev, stride, D);
+  else bg_kernel<N, float, true, BG_NW, BG_NCW><<<grid, nth, s32, st>>>(mom, w, a, b, o, nev, stride, D);
 }
 
 static BgProcess* bg_create(int n, const rwgt_params& po, const rwgt_params& pn, std::string& err) {
@@ -852,21 +852,23 @@ static double bg_flops_per_event(const BgProcess* B, int /*precision*/) {
   double fp = 0; for (int k = 0; k < 8; k++) fp += B->S.fp_ops[k] * fl[k];
   return 2.0 * fp + n * 2 * 30.0 + 4 * 40.0 + (1 << n) * 40.0;
 }
-// FP64 tensor-pipe flops of the colour form (upper-triangular mma.m8n8k4 tiles, 256 FMA each), both parameter sets
+// Algorithmic flops of the colour form |L^T J|^2 (a5), both parameter sets: per evaluated helicity (2^(n+1) after parity)
+// the triangular product costs ncol (ncol + 1) / 2 FMAs for the real and for the imaginary part, plus 2 ncol FMAs for the
+// sum of squares.  They run as mma.m8n8k4 (DMMA) on the FP64 pipe, which DFMA and DMMA share on B200 (rwgt_measure_peak 7).
 static double bg_tensor_flops_per_event(const BgProcess* B) {
-  const int n = B->S.n; int npp = (B->S.nperm + 7) / 8 * 8, MT = npp / 8, KT = npp / 4; double ksteps = 0; for (int mt = 0; mt < MT; mt++) ksteps += KT - 2 * mt;
-  return 2.0 * 2.0 * ksteps * ((double)(4 << (n - 1)) * 2 / 8) * 256.0;
+  const int n = B->S.n; const double ncol = B->S.nperm, nhel = (double)(1 << (n + 1));
+  return 2.0 * nhel * (2.0 * (ncol * (ncol + 1) / 2) + 2.0 * ncol) * 2.0;
 }
 
-static int bg_run(BgProcess* B, int precision, const double* mom, const double* w, double* a, double* b, double* o, long long nev, cudaStream_t st) {
+static int bg_run(BgProcess* B, int precision, const double* mom, const double* w, double* a, double* b, double* o, long long nev, long long stride, cudaStream_t st) {
   BgDev D = B->D; const bool dbl = (precision == RWGT_FP64);
   D.nslot = dbl ? B->nslot64 : B->nslot32;
   long long ngroups = (nev + D.nslot - 1) / D.nslot; int grid = (int)std::min<long long>(ngroups, B->sm_count);
   switch (B->S.n) {
-    case 2: bg_launch<2>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, D); break;
-    case 3: bg_launch<3>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, D); break;
-    case 4: bg_launch<4>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, D); break;
-    default: bg_launch<5>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, D);
+    case 2: bg_launch<2>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, D); break;
+    case 3: bg_launch<3>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, D); break;
+    case 4: bg_launch<4>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, D); break;
+    default: bg_launch<5>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, D);
   }
   return 0;
 }

@@ -33,14 +33,14 @@ __device__ __forceinline__ vec4<double> bilinear2(const cx<double>* a, const cx<
 // are non-zero (tests check the oracle's full 16-term sum against this, reading Q5).
 __global__ void __launch_bounds__(256) epem_mupmum_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
                                                           double* __restrict__ me_old, double* __restrict__ me_new,
-                                                          double* __restrict__ w_new, long long n, EpemParams P) {
+                                                          double* __restrict__ w_new, long long n, long long stride, EpemParams P) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   double p[4][4];
 #pragma unroll
   for (int ip = 0; ip < 4; ip++)
 #pragma unroll
-    for (int mu = 0; mu < 4; mu++) p[ip][mu] = __ldg(mom + (size_t)(ip * 4 + mu) * n + i);
+    for (int mu = 0; mu < 4; mu++) p[ip][mu] = __ldg(mom + (size_t)(ip * 4 + mu) * stride + i);
   double W = __ldg(wgt + i);
   double q[4] = {p[0][0] + p[1][0], p[0][1] + p[1][1], p[0][2] + p[1][2], p[0][3] + p[1][3]};
   double s = mdot_rr(q, q);
@@ -123,14 +123,14 @@ __device__ __forceinline__ void ggttx_sums(const double (*p)[4], double m, doubl
 
 __global__ void __launch_bounds__(128) gg_ttx_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
                                                      double* __restrict__ me_old, double* __restrict__ me_new,
-                                                     double* __restrict__ w_new, long long n, GGttxParams P) {
+                                                     double* __restrict__ w_new, long long n, long long stride, GGttxParams P) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   double p[4][4];
 #pragma unroll
   for (int ip = 0; ip < 4; ip++)
 #pragma unroll
-    for (int mu = 0; mu < 4; mu++) p[ip][mu] = __ldg(mom + (size_t)(ip * 4 + mu) * n + i);
+    for (int mu = 0; mu < 4; mu++) p[ip][mu] = __ldg(mom + (size_t)(ip * 4 + mu) * stride + i);
   double W = __ldg(wgt + i);
   double a, b;
   if (!P.two_pass) ggttx_sums(p, P.mt[0], P.s3[0], P.s3[1], a, b);

@@ -1,5 +1,6 @@
 // rwgt_api.cu — C ABI of include/rwgt.h: handle management, parameter preparation, kernel dispatch.
 #include <cuda_runtime.h>
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -22,6 +23,7 @@ const double PI = 3.14159265358979323846;
 
 }  // namespace
 
+#define RWGT_MAX_CHUNKS 8
 struct rwgt_handle {
   int proc;
   int n_ext;
@@ -35,6 +37,8 @@ struct rwgt_handle {
   // device scratch for rwgt_run_host
   double* scratch;
   size_t scratch_bytes;
+  cudaStream_t s_in, s_out;                           // copy streams of rwgt_run_host (created on first use)
+  cudaEvent_t ev_in[RWGT_MAX_CHUNKS + 1], ev_k[RWGT_MAX_CHUNKS + 1];
 };
 
 static bool valid_params(const rwgt_params* p) {
@@ -69,7 +73,7 @@ rwgt_handle* rwgt_create(const char* process, const rwgt_params* params_old, con
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); set_err("rwgt_create: no CUDA device (this library has no CPU path)"); return nullptr; }
   rwgt_handle* h = new (std::nothrow) rwgt_handle();
   if (!h) { set_err("rwgt_create: out of memory"); return nullptr; }
-  h->proc = -1; h->po = *params_old; h->pn = *params_new; h->precision = RWGT_FP64; h->bg = nullptr; h->scratch = nullptr; h->scratch_bytes = 0;
+  h->proc = -1; h->po = *params_old; h->pn = *params_new; h->precision = RWGT_FP64; h->bg = nullptr; h->scratch = nullptr; h->scratch_bytes = 0; h->s_in = nullptr; h->s_out = nullptr;
   cudaGetDevice(&h->device);
   std::string p(process);
   // "@bg" suffix routes gg_ttx through the generic ordered-current engine (used by the tests to cross-check it)
@@ -127,20 +131,17 @@ double rwgt_tensor_flops_per_event(const rwgt_handle* h) {
   return h->proc == P_BG ? rwgt::bg_tensor_flops_per_event(h->bg) : 0.0;
 }
 
-int rwgt_run(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old, double* out_me_new,
-             double* out_w_new, long long n_events, void* stream) {
-  if (!h || n_events < 0) { set_err("rwgt_run: bad handle or n_events < 0"); return -1; }
-  if (n_events == 0) return 0;
-  if (!momenta || !weights || !out_me_old || !out_me_new || !out_w_new) { set_err("rwgt_run: NULL buffer"); return -1; }
-  cudaStream_t st = (cudaStream_t)stream;
+// one kernel launch over events [0, n) of buffers whose momentum planes are `stride` events apart
+static int launch_events(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old, double* out_me_new,
+                         double* out_w_new, long long n, long long stride, cudaStream_t st) {
   if (h->proc == P_EPEM) {
-    int bs = 256; long long nb = (n_events + bs - 1) / bs;
-    rwgt::epem_mupmum_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n_events, h->epem);
+    int bs = 256; long long nb = (n + bs - 1) / bs;
+    rwgt::epem_mupmum_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, h->epem);
   } else if (h->proc == P_GG_TTX) {
-    int bs = 128; long long nb = (n_events + bs - 1) / bs;
-    rwgt::gg_ttx_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n_events, h->ggttx);
+    int bs = 128; long long nb = (n + bs - 1) / bs;
+    rwgt::gg_ttx_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, h->ggttx);
   } else {
-    int rc = rwgt::bg_run(h->bg, h->precision, momenta, weights, out_me_old, out_me_new, out_w_new, n_events, st);
+    int rc = rwgt::bg_run(h->bg, h->precision, momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, st);
     if (rc != 0) { set_err("rwgt_run: engine launch failed"); return rc; }
   }
   cudaError_t e = cudaGetLastError();
@@ -148,31 +149,68 @@ int rwgt_run(rwgt_handle* h, const double* momenta, const double* weights, doubl
   return 0;
 }
 
+int rwgt_run(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old, double* out_me_new,
+             double* out_w_new, long long n_events, void* stream) {
+  if (!h || n_events < 0) { set_err("rwgt_run: bad handle or n_events < 0"); return -1; }
+  if (n_events == 0) return 0;
+  if (!momenta || !weights || !out_me_old || !out_me_new || !out_w_new) { set_err("rwgt_run: NULL buffer"); return -1; }
+  return launch_events(h, momenta, weights, out_me_old, out_me_new, out_w_new, n_events, n_events, (cudaStream_t)stream);
+}
+
+// Host-buffer path (the transfers are part of what a user pays).  The events are cut into chunks; the
+// host->device copy of chunk c+1 (copy stream), the kernel of chunk c (caller's stream) and the device->host copy of
+// chunk c-1 (second copy stream) overlap, so on a full-duplex link the call costs about max(H2D, D2H, kernel).
 int rwgt_run_host(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old, double* out_me_new,
                   double* out_w_new, long long n_events, void* stream) {
   if (!h || n_events < 0) { set_err("rwgt_run_host: bad handle or n_events < 0"); return -1; }
   if (n_events == 0) return 0;
   if (!momenta || !weights || !out_me_old || !out_me_new || !out_w_new) { set_err("rwgt_run_host: NULL buffer"); return -1; }
   cudaStream_t st = (cudaStream_t)stream;
-  size_t n = (size_t)n_events, nin = (size_t)h->n_ext * 4 * n, need = (nin + 4 * n) * sizeof(double);
-  cudaError_t e;
+  const size_t n = (size_t)n_events, planes = (size_t)h->n_ext * 4, nin = planes * n, need = (nin + 4 * n) * sizeof(double);
+  cudaError_t e = cudaSuccess;
+#define RWGT_CK(call) do { e = (call); if (e != cudaSuccess) { set_err("rwgt_run_host: %s", cudaGetErrorString(e)); return (int)e; } } while (0)
   if (need > h->scratch_bytes) {
     if (h->scratch) cudaFree(h->scratch);
     h->scratch = nullptr; h->scratch_bytes = 0;
-    e = cudaMalloc((void**)&h->scratch, need);
-    if (e != cudaSuccess) { set_err("rwgt_run_host: %s", cudaGetErrorString(e)); return (int)e; }
+    RWGT_CK(cudaMalloc((void**)&h->scratch, need));
     h->scratch_bytes = need;
   }
+  if (!h->s_in) {
+    RWGT_CK(cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking));
+    RWGT_CK(cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking));
+    for (int c = 0; c <= RWGT_MAX_CHUNKS; c++) {
+      RWGT_CK(cudaEventCreateWithFlags(&h->ev_in[c], cudaEventDisableTiming));
+      RWGT_CK(cudaEventCreateWithFlags(&h->ev_k[c], cudaEventDisableTiming));
+    }
+  }
   double* d_mom = h->scratch; double* d_w = d_mom + nin; double* d_a = d_w + n; double* d_b = d_a + n; double* d_o = d_b + n;
-  cudaMemcpyAsync(d_mom, momenta, nin * sizeof(double), cudaMemcpyHostToDevice, st);
-  cudaMemcpyAsync(d_w, weights, n * sizeof(double), cudaMemcpyHostToDevice, st);
-  int rc = rwgt_run(h, d_mom, d_w, d_a, d_b, d_o, n_events, stream);
-  if (rc != 0) return rc;
-  cudaMemcpyAsync(out_me_old, d_a, n * sizeof(double), cudaMemcpyDeviceToHost, st);
-  cudaMemcpyAsync(out_me_new, d_b, n * sizeof(double), cudaMemcpyDeviceToHost, st);
-  cudaMemcpyAsync(out_w_new, d_o, n * sizeof(double), cudaMemcpyDeviceToHost, st);
-  e = cudaStreamSynchronize(st);
-  if (e != cudaSuccess) { set_err("rwgt_run_host: %s", cudaGetErrorString(e)); return (int)e; }
+  // chunks of >= 64 Ki events, at most RWGT_MAX_CHUNKS
+  long long nchunk = (long long)((n + 65535) / 65536); if (nchunk > RWGT_MAX_CHUNKS) nchunk = RWGT_MAX_CHUNKS; if (nchunk < 1) nchunk = 1;
+  long long per = ((long long)n + nchunk - 1) / nchunk;
+  // the scratch may still be in use by earlier work on the caller's stream
+  RWGT_CK(cudaEventRecord(h->ev_in[RWGT_MAX_CHUNKS], st));
+  RWGT_CK(cudaStreamWaitEvent(h->s_in, h->ev_in[RWGT_MAX_CHUNKS], 0));
+  for (long long c = 0; c < nchunk; c++) {
+    long long a0 = c * per, cnt = std::min<long long>(per, (long long)n - a0);
+    if (cnt <= 0) { nchunk = c; break; }
+    RWGT_CK(cudaMemcpy2DAsync(d_mom + a0, n * sizeof(double), momenta + a0, n * sizeof(double), (size_t)cnt * sizeof(double), planes,
+                              cudaMemcpyHostToDevice, h->s_in));
+    RWGT_CK(cudaMemcpyAsync(d_w + a0, weights + a0, (size_t)cnt * sizeof(double), cudaMemcpyHostToDevice, h->s_in));
+    RWGT_CK(cudaEventRecord(h->ev_in[c], h->s_in));
+    RWGT_CK(cudaStreamWaitEvent(st, h->ev_in[c], 0));
+    int rc = launch_events(h, d_mom + a0, d_w + a0, d_a + a0, d_b + a0, d_o + a0, cnt, (long long)n, st);
+    if (rc != 0) return rc;
+    RWGT_CK(cudaEventRecord(h->ev_k[c], st));
+    RWGT_CK(cudaStreamWaitEvent(h->s_out, h->ev_k[c], 0));
+    RWGT_CK(cudaMemcpyAsync(out_me_old + a0, d_a + a0, (size_t)cnt * sizeof(double), cudaMemcpyDeviceToHost, h->s_out));
+    RWGT_CK(cudaMemcpyAsync(out_me_new + a0, d_b + a0, (size_t)cnt * sizeof(double), cudaMemcpyDeviceToHost, h->s_out));
+    RWGT_CK(cudaMemcpyAsync(out_w_new + a0, d_o + a0, (size_t)cnt * sizeof(double), cudaMemcpyDeviceToHost, h->s_out));
+  }
+  // the caller's stream continues only after the results are on the host; then wait for it
+  RWGT_CK(cudaEventRecord(h->ev_k[RWGT_MAX_CHUNKS], h->s_out));
+  RWGT_CK(cudaStreamWaitEvent(st, h->ev_k[RWGT_MAX_CHUNKS], 0));
+  RWGT_CK(cudaStreamSynchronize(st));
+#undef RWGT_CK
   return 0;
 }
 
@@ -180,12 +218,16 @@ int rwgt_destroy(rwgt_handle* h) {
   if (!h) return -1;
   if (h->bg) rwgt::bg_destroy(h->bg);
   if (h->scratch) cudaFree(h->scratch);
+  if (h->s_in) {
+    cudaStreamDestroy(h->s_in); cudaStreamDestroy(h->s_out);
+    for (int c = 0; c <= RWGT_MAX_CHUNKS; c++) { cudaEventDestroy(h->ev_in[c]); cudaEventDestroy(h->ev_k[c]); }
+  }
   delete h;
   return 0;
 }
 
 int rwgt_measure_peak(int kind, double* out_tflops) {
-  if (kind < 0 || kind > 2 || !out_tflops) return -1;
+  if (kind < 0 || kind > 7 || !out_tflops) return -1;
   return rwgt::measure_peak(kind, out_tflops);
 }
 

@@ -159,6 +159,26 @@ def test_host_buffer_entry_point_and_non_default_stream():
     assert np.array_equal(out[:, 100:], dev[:, 100:]) and np.array_equal(out[:, :100], dev[:, :100])
 
 
+def test_host_path_is_chunked_and_matches_device_path_bitwise():
+    """rwgt_run_host cuts the events into overlapping copy/compute chunks (ragged last chunk, strided SoA planes):
+    results must be bit-identical to one device launch, for pinned and pageable buffers."""
+    for idx, n in ((1, 3 * 65536 + 123), (2, 2 * 65536 + 1), (3, 65536 + 77)):
+        c = ev.config(idx)
+        m0, w0 = ev.generate(c, 4096)
+        reps = (n + 4095) // 4096
+        m, w = np.tile(m0, (1, 1, reps))[:, :, :n].copy(), np.tile(w0, reps)[:n].copy()
+        dev = gpu_run(c.process, c.params_old, c.params_new, m, w)
+        h = B.rwgt_create(c.process, c.params_old, c.params_new)
+        out = np.empty((3, n))
+        B.rwgt_run_host(h, m, w, out[0], out[1], out[2])                       # pageable
+        assert np.array_equal(out, dev)
+        pm, pw, po = torch.from_numpy(m).pin_memory(), torch.from_numpy(w).pin_memory(), torch.empty((3, n), dtype=torch.float64).pin_memory()
+        o = po.numpy()
+        B.rwgt_run_host(h, pm.numpy(), pw.numpy(), o[0], o[1], o[2], torch.cuda.Stream().cuda_stream)
+        assert np.array_equal(o, dev)
+        B.rwgt_destroy(h)
+
+
 def test_rotation_invariance_of_both_sets_on_gpu():
     """Property that holds at any size: a common spatial rotation leaves |M|^2 and |M'|^2 unchanged.
     Rotate about the beam axis so legs 0,1 stay on the exact-axis branch."""
