@@ -143,7 +143,7 @@ def run_reference(args) -> None:
 
 
 # ------------------------------------------------------------------------------------------------- our arm
-def time_config(torch, B, c, precision, n, steps, warmup, seed_offset, flush_buf, sampler_index=None, tile_from=0):
+def time_config(torch, B, c, precision, n, steps, warmup, seed_offset, flush_buf, sampler_index=None, tile_from=0, new_sets=None):
     """Device-resident timing of one config. Returns dict with per-step ms list etc."""
     if tile_from and tile_from < n:
         m0, w0 = ev.generate(c, tile_from, seed=c.seed + 1000 * seed_offset)
@@ -152,8 +152,9 @@ def time_config(torch, B, c, precision, n, steps, warmup, seed_offset, flush_buf
     else:
         m, w = ev.generate(c, n, seed=c.seed + 1000 * seed_offset)
     dm, dw = torch.from_numpy(m).cuda(), torch.from_numpy(w).cuda()
-    out = torch.empty((3, n), dtype=torch.float64, device="cuda")
-    r = B.Reweighter(c.process, c.params_old, c.params_new, precision)
+    k_sets = len(new_sets) if new_sets else 1
+    out = torch.empty((1 + 2 * k_sets, n), dtype=torch.float64, device="cuda")
+    r = B.Reweighter(c.process, c.params_old, new_sets if new_sets else c.params_new, precision)
     stream = torch.cuda.current_stream()
     in_bytes = dm.numel() * 8 + dw.numel() * 8 + out.numel() * 8
     need_flush = in_bytes < 2 * 126e6
@@ -333,6 +334,21 @@ def main() -> None:
                     rr["rw"].close()
                 except Exception as ex:  # keep the headline line alive
                     extra.append({"workload": workload_name(cc, cc.n_events), "precision": prec, "error": str(ex)})
+        # K new parameter sets in one pass (PAPER.md:87 step 7, Fig. 3 axis): kappa = 0.1 k / K
+        for ci, K in ((2, 8), (4, 8), (5, 4)):
+            try:
+                cc = ev.config(ci)
+                sets = [ev.params(ggg_scale=1 + 0.1 * (k + 1) / K, gggg_scale=1 + 0.1 * (k + 1) / K) for k in range(K)]
+                rr = time_config(torch, B, cc, "fp64", cc.n_events, 5, 3, 0, flush_buf, new_sets=sets)
+                kms = statistics.mean(rr["ms"])
+                fpe = rr["flops_per_event"] + rr["tensor_flops_per_event"]
+                tf = fpe * cc.n_events / (kms * 1e-3) / 1e12
+                extra.append({"workload": workload_name(cc, cc.n_events) + f" with K={K} new parameter sets in one pass", "precision": "fp64",
+                              "events_per_s": cc.n_events / (kms * 1e-3), "new_weights_per_s": K * cc.n_events / (kms * 1e-3), "kernel_ms": kms,
+                              "alu_tflops": tf, "alu_frac": tf / alu_peak_tflops("f64", max_mhz), "l2": rr["l2"]})
+                rr["rw"].close()
+            except Exception as ex:
+                extra.append({"workload": f"cfg{ci} K={K}", "error": str(ex)})
         # cfg 1 is launch-latency-bound at its 16,384 events: the same distribution at n = 2^24 (buffers >> L2)
         try:
             c1 = ev.config(1)

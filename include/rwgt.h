@@ -55,6 +55,18 @@ typedef struct {
  * "that can be modified at runtime": old and new share the process. */
 rwgt_handle* rwgt_create(const char* process, const rwgt_params* params_old, const rwgt_params* params_new);
 
+/* Several new parameter sets for the same events in one pass (PAPER.md:87 step 7, "Repeat steps 4 - 6 for all parameter
+ * sets"; PAPER.md:91 and Fig. 3: run time against the number of parameter sets).  `params_new` points to n_new sets,
+ * 1 <= n_new <= RWGT_MAX_SETS.  The event is loaded and its external wavefunctions, momentum sums and propagator
+ * denominators are formed ONCE; each set then costs one more evaluation of the currents and one more colour form.
+ * Sets may differ in any field; a differing top mass makes the externals of that set be recomputed.
+ * rwgt_create(p, old, new) is rwgt_create_multi(p, old, new, 1).  Same error behaviour as rwgt_create. */
+#define RWGT_MAX_SETS 16
+rwgt_handle* rwgt_create_multi(const char* process, const rwgt_params* params_old, const rwgt_params* params_new, int n_new);
+
+/* Number K of new parameter sets of the handle (1 for rwgt_create); -1 on NULL. */
+int rwgt_n_sets(const rwgt_handle* h);
+
 /* 0 on success, -1 on bad handle/mode or a mode the process does not support
  * (epem_mupmum and gg_ttx are FP64 only). */
 int rwgt_set_precision(rwgt_handle* h, int mode);
@@ -90,6 +102,13 @@ double rwgt_tensor_flops_per_event(const rwgt_handle* h);
 int rwgt_run(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old,
              double* out_me_new, double* out_w_new, long long n_events, void* stream);
 
+/* The same launch for a handle with K = rwgt_n_sets(h) new parameter sets:
+ *   out_me_new, out_w_new  DEVICE double [K][n_events]: set k at offset k * n_events
+ * (out_me_old stays [n_events]).  rwgt_run is this call restricted to K == 1 (it returns -1 for K > 1, so that a
+ * caller who sized the outputs for one set cannot be overrun). */
+int rwgt_run_multi(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old,
+                   double* out_me_new, double* out_w_new, long long n_events, void* stream);
+
 /* Same computation with HOST buffers (pageable or pinned): copies the inputs to device
  * scratch owned by the handle (grown on demand), runs the kernel, copies the three outputs
  * back and synchronises `stream`.  The events are processed in up to 8 chunks so that the host->device copy of one
@@ -98,6 +117,10 @@ int rwgt_run(rwgt_handle* h, const double* momenta, const double* weights, doubl
  * bench.py's `e2e` key (host<->device transfer is part of what a user pays).  Same return codes. */
 int rwgt_run_host(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old,
                   double* out_me_new, double* out_w_new, long long n_events, void* stream);
+
+/* rwgt_run_host for K >= 1 new sets: out_me_new, out_w_new are HOST double [K][n_events]. */
+int rwgt_run_multi_host(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old,
+                        double* out_me_new, double* out_w_new, long long n_events, void* stream);
 
 /* Frees device tables and scratch. 0 on success, -1 on NULL. */
 int rwgt_destroy(rwgt_handle* h);

@@ -15,7 +15,8 @@ LIB_PATH = os.path.join(_HERE, "librwgt.so")
 RWGT_FP64, RWGT_FP32, RWGT_MIXED = 0, 1, 2
 PRECISIONS = {"fp64": RWGT_FP64, "fp32": RWGT_FP32, "mixed": RWGT_MIXED}
 
-EXPORTS = ("rwgt_create", "rwgt_set_precision", "rwgt_n_external", "rwgt_flops_per_event", "rwgt_run",
+RWGT_MAX_SETS = 16
+EXPORTS = ("rwgt_create", "rwgt_create_multi", "rwgt_n_sets", "rwgt_run_multi", "rwgt_run_multi_host", "rwgt_set_precision", "rwgt_n_external", "rwgt_flops_per_event", "rwgt_run",
            "rwgt_run_host", "rwgt_destroy", "rwgt_last_error", "rwgt_colour_matrix", "rwgt_measure_peak", "rwgt_tensor_flops_per_event")
 
 
@@ -38,6 +39,11 @@ def lib():
         vp, dp = C.c_void_p, C.c_void_p
         L.rwgt_create.argtypes = [C.c_char_p, C.POINTER(rwgt_params), C.POINTER(rwgt_params)]
         L.rwgt_create.restype = vp
+        L.rwgt_create_multi.argtypes = [C.c_char_p, C.POINTER(rwgt_params), C.POINTER(rwgt_params), C.c_int]
+        L.rwgt_create_multi.restype = vp
+        L.rwgt_n_sets.argtypes = [vp]
+        L.rwgt_run_multi.argtypes = [vp, dp, dp, dp, dp, dp, C.c_longlong, vp]
+        L.rwgt_run_multi_host.argtypes = [vp, dp, dp, dp, dp, dp, C.c_longlong, vp]
         L.rwgt_set_precision.argtypes = [vp, C.c_int]
         L.rwgt_n_external.argtypes = [vp]
         L.rwgt_flops_per_event.argtypes = [vp]
@@ -72,6 +78,20 @@ def rwgt_create(process: str, params_old, params_new):
     return h
 
 
+def rwgt_create_multi(process: str, params_old, params_new_list):
+    """K new parameter sets for the same events (PAPER.md:87 step 7)."""
+    po = _params(params_old)
+    arr = (rwgt_params * len(params_new_list))(*[_params(p) for p in params_new_list])
+    h = lib().rwgt_create_multi(process.encode(), C.byref(po), arr, len(params_new_list))
+    if not h:
+        raise RuntimeError(rwgt_last_error())
+    return h
+
+
+def rwgt_n_sets(h) -> int:
+    return lib().rwgt_n_sets(h)
+
+
 def rwgt_set_precision(h, mode) -> None:
     mode = PRECISIONS.get(mode, mode)
     if lib().rwgt_set_precision(h, int(mode)) != 0:
@@ -97,6 +117,28 @@ def rwgt_run(h, momenta_ptr: int, weights_ptr: int, out_me_old_ptr: int, out_me_
                         int(n_events), stream or None)
     if rc != 0:
         raise RuntimeError(f"rwgt_run rc={rc}: {rwgt_last_error()}")
+
+
+def rwgt_run_multi(h, momenta_ptr: int, weights_ptr: int, out_me_old_ptr: int, out_me_new_ptr: int,
+                   out_w_new_ptr: int, n_events: int, stream: int = 0) -> None:
+    """As rwgt_run for K = rwgt_n_sets(h) new sets: out_me_new / out_w_new are device [K][n_events]."""
+    rc = lib().rwgt_run_multi(h, momenta_ptr, weights_ptr, out_me_old_ptr, out_me_new_ptr, out_w_new_ptr,
+                              int(n_events), stream or None)
+    if rc != 0:
+        raise RuntimeError(f"rwgt_run_multi rc={rc}: {rwgt_last_error()}")
+
+
+def rwgt_run_multi_host(h, momenta: np.ndarray, weights: np.ndarray, out_me_old: np.ndarray,
+                        out_me_new: np.ndarray, out_w_new: np.ndarray, stream: int = 0) -> None:
+    """Host numpy buffers; out_me_new / out_w_new have shape (K, n)."""
+    n = weights.shape[0]
+    for a in (momenta, weights, out_me_old, out_me_new, out_w_new):
+        assert a.dtype == np.float64 and a.flags.c_contiguous
+    assert out_me_new.shape == (rwgt_n_sets(h), n) and out_w_new.shape == (rwgt_n_sets(h), n)
+    rc = lib().rwgt_run_multi_host(h, momenta.ctypes.data, weights.ctypes.data, out_me_old.ctypes.data,
+                                   out_me_new.ctypes.data, out_w_new.ctypes.data, int(n), stream or None)
+    if rc != 0:
+        raise RuntimeError(f"rwgt_run_multi_host rc={rc}: {rwgt_last_error()}")
 
 
 def rwgt_run_host(h, momenta: np.ndarray, weights: np.ndarray, out_me_old: np.ndarray,
@@ -134,7 +176,11 @@ class Reweighter:
     """Convenience wrapper: one handle, torch device tensors in, torch device tensors out."""
 
     def __init__(self, process: str, params_old, params_new, precision="fp64"):
-        self.h = rwgt_create(process, params_old, params_new)
+        """params_new: one parameter set, or a list of K sets (then run() returns 1 + 2K rows:
+        |M|^2, K rows |M'_k|^2, K rows W'_k)."""
+        multi = isinstance(params_new, list)
+        self.h = rwgt_create_multi(process, params_old, params_new) if multi else rwgt_create(process, params_old, params_new)
+        self.k = rwgt_n_sets(self.h)
         self.process = process
         self.n_ext = rwgt_n_external(self.h)
         rwgt_set_precision(self.h, precision)
@@ -150,11 +196,13 @@ class Reweighter:
         n = weights.shape[0]
         assert momenta.is_cuda and momenta.dtype == torch.float64 and momenta.is_contiguous()
         assert momenta.shape == (self.n_ext, 4, n) and weights.dtype == torch.float64
+        k = self.k
         if out is None:
-            out = torch.empty((3, n), dtype=torch.float64, device=momenta.device)
+            out = torch.empty((1 + 2 * k, n), dtype=torch.float64, device=momenta.device)
+        assert out.shape == (1 + 2 * k, n) and out.is_contiguous()
         st = torch.cuda.current_stream(momenta.device).cuda_stream
-        rwgt_run(self.h, momenta.data_ptr(), weights.data_ptr(), out[0].data_ptr(), out[1].data_ptr(),
-                 out[2].data_ptr(), n, st)
+        rwgt_run_multi(self.h, momenta.data_ptr(), weights.data_ptr(), out[0].data_ptr(), out[1].data_ptr(),
+                       out[1 + k].data_ptr(), n, st)
         return out
 
     def close(self):

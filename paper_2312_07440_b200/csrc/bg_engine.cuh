@@ -308,11 +308,12 @@ static BgSched build_schedule(int n, std::string& err) {
 
 // ------------------------------------------------------------------------------------------------ device side
 struct BgSet { double gq, g3, g4, mt, fac; };        // fac = 2 gq^2 / D  (|i gq|^2, parity factor 2, averaging)
+constexpr int BG_NSMAX = 1 + RWGT_MAX_SETS;      // the old set plus up to RWGT_MAX_SETS new ones
 struct BgDev {
-  int nwords, nslot, shared_ext;
+  int nwords, nslot, shared_ext, nsets;
   int offD[3][6], offT[6], offF;
   const uint32_t* words; const double* lfrag;
-  BgSet set[2];
+  BgSet set[BG_NSMAX];
   unsigned long long* dbg;
 };
 
@@ -329,7 +330,7 @@ template <typename T> __device__ __forceinline__ void stc(cx<T>* p, cx<T> v) { t
 template <typename T> struct Smem {
   uint32_t* W;    // schedule words (whole CTA)
   double* pm;     // [nslot][n_ext][4] momenta (always double)
-  double* acc;    // [nslot][2]   helicity-summed colour forms (owned by the colour warps)
+  double* acc;    // [nslot][BG_NSMAX]   helicity-summed colour forms per parameter set (owned by the colour warps)
   double* red;    // [nslot][8]   per-warp partial sums of the colour form
   cx<T>* G; cx<T>* R; cx<T>* L;   // [nslot][4][nX]   component planes of (re,im) pairs: one vector load per component,
                                   //                  conflict-free for consecutive helicity variants
@@ -343,7 +344,7 @@ template <int N, typename T> __host__ __device__ inline size_t carve(Smem<T>& s,
   auto al = [&]() { off = (off + 15) / 16 * 16; };
   s.A = (double*)(base + off); off += sizeof(double) * 2 * (size_t)ns * Ge::ABUF; al();
   s.pm = (double*)(base + off); off += sizeof(double) * ns * (N + 2) * 4; al();
-  s.acc = (double*)(base + off); off += sizeof(double) * ns * 2; al();
+  s.acc = (double*)(base + off); off += sizeof(double) * ns * BG_NSMAX; al();
   s.red = (double*)(base + off); off += sizeof(double) * ns * 8; al();
   s.G = (cx<T>*)(base + off); off += sizeof(T) * (size_t)ns * 8 * nG; al();
   s.R = (cx<T>*)(base + off); off += sizeof(T) * (size_t)ns * 8 * nR; al();
@@ -591,7 +592,7 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 template <int N, typename T, bool MIXED, int NW, int NCW>
 __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
                                                                double* __restrict__ me_old, double* __restrict__ me_new,
-                                                               double* __restrict__ w_new, long long nev, long long stride, BgDev D) {
+                                                               double* __restrict__ w_new, long long nev, long long stride, long long ostride, BgDev D) {
   typedef Geo<N> Ge;
   constexpr int NTH = (NW + NCW) * 32, NWT = NW * 32, NCT = NCW * 32;
   // register hand-over between the warpgroups: the colour warps need few registers, the workers get the rest
@@ -622,7 +623,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
       }
       bar_sync(BAR_WORK, NWT);
 #pragma unroll 1
-      for (int iset = 0; iset < 2; iset++) {
+      for (int iset = 0; iset < D.nsets; iset++) {
         const BgSet& P = D.set[iset];
         c.g3 = (T)P.g3; c.g4 = (T)P.g4; c.gq = (T)P.gq; c.mt = (T)P.mt;
         if (iset == 0 || !D.shared_ext) {
@@ -712,11 +713,10 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
     unsigned step = 0;
     for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
       const long long ev0 = grp * ns;
-      if (ctid < ns * 2) s.acc[ctid] = 0.0;
-      for (int t = ctid + NCT; t < ns * 2; t += NCT) s.acc[t] = 0.0;
+      for (int t = ctid; t < ns * BG_NSMAX; t += NCT) s.acc[t] = 0.0;
       bar_sync(BAR_COLOUR, NCT);
 #pragma unroll 1
-      for (int iset = 0; iset < 2; iset++) {
+      for (int iset = 0; iset < D.nsets; iset++) {
 #pragma unroll 1
         for (int batch = 0; batch < Ge::NBATCH; batch++, step++) {
           const int buf = step & 1;
@@ -754,7 +754,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
           }
           bar_sync(BAR_COLOUR, NCT);
           bar_arrive(BAR_EMPTY0 + buf, NTH);                   // buffer may be refilled
-          for (int sl = ctid; sl < ns; sl += NCT) { double a = 0.0; for (int j = 0; j < Ge::U; j++) a += s.red[sl * 8 + j]; s.acc[sl * 2 + iset] += a; }
+          for (int sl = ctid; sl < ns; sl += NCT) { double a = 0.0; for (int j = 0; j < Ge::U; j++) a += s.red[sl * 8 + j]; s.acc[sl * BG_NSMAX + iset] += a; }
           bar_sync(BAR_COLOUR, NCT);
         }
       }
@@ -762,8 +762,12 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
       for (int sl = ctid; sl < ns; sl += NCT) {
         long long ev = ev0 + sl;
         if (ev < nev) {
-          double a = s.acc[sl * 2] * D.set[0].fac, b = s.acc[sl * 2 + 1] * D.set[1].fac;
-          me_old[ev] = a; me_new[ev] = b; w_new[ev] = __ldg(wgt + ev) * (b / a);
+          const double a = s.acc[sl * BG_NSMAX] * D.set[0].fac, W = __ldg(wgt + ev);
+          me_old[ev] = a;
+          for (int k = 1; k < D.nsets; k++) {
+            const double b = s.acc[sl * BG_NSMAX + k] * D.set[k].fac;
+            me_new[(size_t)(k - 1) * ostride + ev] = b; w_new[(size_t)(k - 1) * ostride + ev] = W * (b / a);
+          }
         }
       }
       bar_sync(BAR_COLOUR, NCT);
@@ -790,14 +794,14 @@ template <int N> static cudaError_t bg_set_attr(size_t s64, size_t s32) {
   return e;
 }
 template <int N> static void bg_launch(int precision, int grid, size_t s64, size_t s32, cudaStream_t st, const double* mom, const double* w,
-                                       double* a, double* b, double* o, long long nev, long long stride, const BgDev& D) {
+                                       double* a, double* b, double* o, long long nev, long long stride, long long ostride, const BgDev& D) {
   const int nth = (BG_NW + BG_NCW) * 32;
-  if (precision == RWGT_FP64) bg_kernel<N, double, false, BG_NW, BG_NCW><<<grid, nth, s64, st>>>(mom, w, a, b, o, nev, stride, D);
-  else if (precision == RWGT_FP32) bg_kernel<N, float, false, BG_NW, BG_NCW><<<grid, nth, s32, st>>>(mom, w, a, b, o, nev, stride, D);
-  else bg_kernel<N, float, true, BG_NW, BG_NCW><<<grid, nth, s32, st>>>(mom, w, a, b, o, nev, stride, D);
+  if (precision == RWGT_FP64) bg_kernel<N, double, false, BG_NW, BG_NCW><<<grid, nth, s64, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
+  else if (precision == RWGT_FP32) bg_kernel<N, float, false, BG_NW, BG_NCW><<<grid, nth, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
+  else bg_kernel<N, float, true, BG_NW, BG_NCW><<<grid, nth, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
 }
 
-static BgProcess* bg_create(int n, const rwgt_params& po, const rwgt_params& pn, std::string& err) {
+static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::string& err) {
   BgProcess* B = new BgProcess();
   B->S = build_schedule(n, err);
   if (!err.empty()) { delete B; return nullptr; }
@@ -813,14 +817,14 @@ static BgProcess* bg_create(int n, const rwgt_params& po, const rwgt_params& pn,
   if (!ok) { err = "internal: schedule/geometry mismatch"; delete B; return nullptr; }
   for (int k = 0; k < 3; k++) for (int m = 0; m < 6; m++) D.offD[k][m] = S.offD[k][m];
   for (int m = 0; m < 6; m++) D.offT[m] = S.offT[m];
-  const rwgt_params* ps[2] = {&po, &pn};
   double fact = 1; for (int i = 2; i <= n - 2; i++) fact *= i;
-  for (int k = 0; k < 2; k++) {
-    double gs = std::sqrt(4.0 * 3.14159265358979323846 * ps[k]->alpha_s);
-    D.set[k].gq = gs; D.set[k].g3 = gs * ps[k]->ggg_scale; D.set[k].g4 = gs * gs * ps[k]->gggg_scale; D.set[k].mt = ps[k]->mt;
+  D.nsets = nsets; D.shared_ext = 1;
+  for (int k = 0; k < nsets; k++) {
+    double gs = std::sqrt(4.0 * 3.14159265358979323846 * sets[k].alpha_s);
+    D.set[k].gq = gs; D.set[k].g3 = gs * sets[k].ggg_scale; D.set[k].g4 = gs * gs * sets[k].gggg_scale; D.set[k].mt = sets[k].mt;
     D.set[k].fac = 2.0 * gs * gs / (256.0 * fact);
+    if (sets[k].mt != sets[0].mt) D.shared_ext = 0;     // externals, momentum sums and denominators are then redone per set
   }
-  D.shared_ext = (po.mt == pn.mt) ? 1 : 0;
   int dev = 0; cudaGetDevice(&dev); cudaDeviceProp prop; cudaGetDeviceProperties(&prop, dev);
   B->sm_count = prop.multiProcessorCount; size_t maxsm = prop.sharedMemPerBlockOptin;
   // event slots per CTA: as many as make the amplitude phase fill the 256 worker threads (npair * 4 tasks per slot and batch)
@@ -843,32 +847,32 @@ static BgProcess* bg_create(int n, const rwgt_params& po, const rwgt_params& pn,
 }
 static void bg_destroy(BgProcess* B) { if (!B) return; cudaFree(B->d_words); cudaFree(B->d_lfrag); delete B; }
 
-// Algorithmic flop count of the schedule on the FP64 (or FP32) FMA pipe, both parameter sets, per event: FMA = 2 flop,
+// Algorithmic flop count of the schedule on the FP64 (or FP32) FMA pipe, all parameter sets of the handle, per event: FMA = 2 flop,
 // MUL = ADD = 1 flop, per operation of rwgt_math.cuh (L3 74 FMA + 6 MUL + 4 ADD, V4 90 + 6 + 2, slash-accumulate 32 FMA,
 // light-cone 8 ADD, propagator 24 FMA + 17 MUL + 6 ADD, row.col 16 FMA, current store 8 FMA + 16 MUL), times the number of
 // such operations the schedule executes (helicity variants with gluon 0 at helicity - are not evaluated and not counted).
 static double bg_flops_per_event(const BgProcess* B, int /*precision*/) {
   const int n = B->S.n; const double fl[8] = {158, 188, 64, 8, 71, 32, 32, 16};
   double fp = 0; for (int k = 0; k < 8; k++) fp += B->S.fp_ops[k] * fl[k];
-  return 2.0 * fp + n * 2 * 30.0 + 4 * 40.0 + (1 << n) * 40.0;
+  return B->D.nsets * fp + (B->D.shared_ext ? 1 : B->D.nsets) * (n * 2 * 30.0 + 4 * 40.0 + (1 << n) * 40.0);
 }
 // Algorithmic flops of the colour form |L^T J|^2 (a5), both parameter sets: per evaluated helicity (2^(n+1) after parity)
 // the triangular product costs ncol (ncol + 1) / 2 FMAs for the real and for the imaginary part, plus 2 ncol FMAs for the
 // sum of squares.  They run as mma.m8n8k4 (DMMA) on the FP64 pipe, which DFMA and DMMA share on B200 (rwgt_measure_peak 7).
 static double bg_tensor_flops_per_event(const BgProcess* B) {
   const int n = B->S.n; const double ncol = B->S.nperm, nhel = (double)(1 << (n + 1));
-  return 2.0 * nhel * (2.0 * (ncol * (ncol + 1) / 2) + 2.0 * ncol) * 2.0;
+  return B->D.nsets * nhel * (2.0 * (ncol * (ncol + 1) / 2) + 2.0 * ncol) * 2.0;
 }
 
-static int bg_run(BgProcess* B, int precision, const double* mom, const double* w, double* a, double* b, double* o, long long nev, long long stride, cudaStream_t st) {
+static int bg_run(BgProcess* B, int precision, const double* mom, const double* w, double* a, double* b, double* o, long long nev, long long stride, long long ostride, cudaStream_t st) {
   BgDev D = B->D; const bool dbl = (precision == RWGT_FP64);
   D.nslot = dbl ? B->nslot64 : B->nslot32;
   long long ngroups = (nev + D.nslot - 1) / D.nslot; int grid = (int)std::min<long long>(ngroups, B->sm_count);
   switch (B->S.n) {
-    case 2: bg_launch<2>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, D); break;
-    case 3: bg_launch<3>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, D); break;
-    case 4: bg_launch<4>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, D); break;
-    default: bg_launch<5>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, D);
+    case 2: bg_launch<2>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, ostride, D); break;
+    case 3: bg_launch<3>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, ostride, D); break;
+    case 4: bg_launch<4>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, ostride, D); break;
+    default: bg_launch<5>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, ostride, D);
   }
   return 0;
 }

@@ -4,6 +4,7 @@
 // Steps a1-a7 of SURVEY §8(a) in one launch: coalesced SoA loads, external wavefunctions,
 // vertices, colour form, helicity sum, eq. 3, three coalesced stores.
 #pragma once
+#include "../../include/rwgt.h"
 #include "rwgt_math.cuh"
 
 namespace rwgt {
@@ -15,7 +16,8 @@ struct EpemSet {          // per parameter set, prepared on the host
   double gL, gR;          // -1/2 + sW^2, sW^2
   double mZ2, mZGZ;       // mZ^2, mZ*GammaZ
 };
-struct EpemParams { EpemSet set[2]; };
+constexpr int SMALL_NSMAX = 1 + RWGT_MAX_SETS;     // the old set plus up to RWGT_MAX_SETS new ones
+struct EpemParams { EpemSet set[SMALL_NSMAX]; int nsets; };
 
 // chi_a^dagger sigma^mu chi_b (bar=false) or chi_a^dagger sigmabar^mu chi_b (bar=true)
 __device__ __forceinline__ vec4<double> bilinear2(const cx<double>* a, const cx<double>* b, bool barred) {
@@ -33,7 +35,7 @@ __device__ __forceinline__ vec4<double> bilinear2(const cx<double>* a, const cx<
 // are non-zero (tests check the oracle's full 16-term sum against this, reading Q5).
 __global__ void __launch_bounds__(256) epem_mupmum_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
                                                           double* __restrict__ me_old, double* __restrict__ me_new,
-                                                          double* __restrict__ w_new, long long n, long long stride, EpemParams P) {
+                                                          double* __restrict__ w_new, long long n, long long stride, long long ostride, EpemParams P) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   double p[4][4];
@@ -55,9 +57,9 @@ __global__ void __launch_bounds__(256) epem_mupmum_kernel(const double* __restri
   double c2 = ce * cm; c2 *= c2;
   double dLL = norm2(mdot_cc(JeL, JmL)) * c2, dLR = norm2(mdot_cc(JeL, JmR)) * c2;
   double dRL = norm2(mdot_cc(JeR, JmL)) * c2, dRR = norm2(mdot_cc(JeR, JmR)) * c2;
-  double me[2];
-#pragma unroll
-  for (int k = 0; k < 2; k++) {
+  double me0 = 0;
+#pragma unroll 1
+  for (int k = 0; k < P.nsets; k++) {
     const EpemSet& S = P.set[k];
     // photon e^2/s (Q_e Q_mu = +1) plus Z g_Z^2 g_a g_b / (s - mZ^2 + i mZ GammaZ)
     double dr = s - S.mZ2, di = S.mZGZ, inv = 1.0 / (dr * dr + di * di);
@@ -65,17 +67,19 @@ __global__ void __launch_bounds__(256) epem_mupmum_kernel(const double* __restri
     double fLL = norm2(mk<double>(ph + S.gL * S.gL * zr, S.gL * S.gL * zi));
     double fLR = norm2(mk<double>(ph + S.gL * S.gR * zr, S.gL * S.gR * zi));
     double fRR = norm2(mk<double>(ph + S.gR * S.gR * zr, S.gR * S.gR * zi));
-    me[k] = 0.25 * (fLL * dLL + fLR * (dLR + dRL) + fRR * dRR);
+    const double me = 0.25 * (fLL * dLL + fLR * (dLR + dRL) + fRR * dRR);
+    if (k == 0) { me0 = me; me_old[i] = me; }
+    else { me_new[(size_t)(k - 1) * ostride + i] = me; w_new[(size_t)(k - 1) * ostride + i] = W * (me / me0); }
   }
-  me_old[i] = me[0]; me_new[i] = me[1]; w_new[i] = W * (me[1] / me[0]);
 }
 
 // ------------------------------------------------------------------------------------- cfg 2
 struct GGttxParams {
-  double mt[2];           // top mass per set
-  double fac[2];          // g_s^4 / 256 per set (averaging denominator D = 4*64)
-  double s3[2];           // ggg_scale per set
-  int two_pass;           // masses differ: evaluate each set with its own mass
+  double mt[SMALL_NSMAX];   // top mass per set
+  double fac[SMALL_NSMAX];  // g_s^4 / 256 per set (averaging denominator D = 4*64)
+  double s3[SMALL_NSMAX];   // ggg_scale per set
+  int nsets;                // 1 + number of new sets
+  int two_pass;             // masses differ: evaluate each set with its own mass
 };
 
 // Helicity-summed colour forms for ONE mass and two values of the ggg scale.
@@ -123,7 +127,7 @@ __device__ __forceinline__ void ggttx_sums(const double (*p)[4], double m, doubl
 
 __global__ void __launch_bounds__(128) gg_ttx_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
                                                      double* __restrict__ me_old, double* __restrict__ me_new,
-                                                     double* __restrict__ w_new, long long n, long long stride, GGttxParams P) {
+                                                     double* __restrict__ w_new, long long n, long long stride, long long /*ostride*/, GGttxParams P) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
   double p[4][4];
@@ -137,6 +141,78 @@ __global__ void __launch_bounds__(128) gg_ttx_kernel(const double* __restrict__ 
   else { double t; ggttx_sums(p, P.mt[0], P.s3[0], P.s3[0], a, t); ggttx_sums(p, P.mt[1], P.s3[1], P.s3[1], t, b); }
   a *= P.fac[0]; b *= P.fac[1];
   me_old[i] = a; me_new[i] = b; w_new[i] = W * (b / a);
+}
+
+// K > 1 new sets of equal top mass: the helicity amplitudes X12, X21, Y are formed once, every set is one more
+// pair of real FMAs and one more colour form (PAPER.md:87 step 7).  sums[k] for k < nsets.
+__device__ __forceinline__ void ggttx_sums_multi(const double (*p)[4], double m, const double* s3, int nsets, double* sums) {
+  const double* k1 = p[0]; const double* k2 = p[1];
+  double q1[4], q2[4], kk[4];
+#pragma unroll
+  for (int mu = 0; mu < 4; mu++) { q1[mu] = k1[mu] - p[3][mu]; q2[mu] = k2[mu] - p[3][mu]; kk[mu] = k1[mu] + k2[mu]; }
+  double m2 = m * m;
+  double d1 = -1.0 / (mdot_rr(q1, q1) - m2), d2 = -1.0 / (mdot_rr(q2, q2) - m2), ds = -1.0 / mdot_rr(kk, kk);
+  chi_pair<double> xt = make_chi(p[2][1], p[2][2], p[2][3]), xb = make_chi(p[3][1], p[3][2], p[3][3]);
+#pragma unroll
+  for (int k = 0; k < SMALL_NSMAX; k++) sums[k] = 0;
+  vec4<double> e1 = polvec(k1[1], k1[2], k1[3], +1);
+#pragma unroll 1
+  for (int i2 = 0; i2 < 2; i2++) {
+    vec4<double> e2 = polvec(k2[1], k2[2], k2[3], i2 ? -1 : +1);
+    vec4<double> l3; for (int mu = 0; mu < 4; mu++) l3.c[mu] = mk<double>(0, 0);
+    L3_acc(l3, e1, k1, e2, k2);
+    for (int mu = 0; mu < 4; mu++) l3.c[mu] = ds * l3.c[mu];
+#pragma unroll 1
+    for (int ib = 0; ib < 2; ib++) {
+      spn<double> v = spinor_v(xb, p[3][0], m, ib ? -1 : +1);
+      spn<double> psi1 = slash_r_plus_m(q1, m, slash_c(e1, v)), psi2 = slash_r_plus_m(q2, m, slash_c(e2, v));
+      spn<double> c12 = slash_c(e1, psi2), c21 = slash_c(e2, psi1), cy = slash_c(l3, v);
+#pragma unroll 1
+      for (int it = 0; it < 2; it++) {
+        spn<double> ub = bar(spinor_u(xt, p[2][0], m, it ? -1 : +1));
+        cx<double> X12 = d2 * rowcol(ub, c12), X21 = d1 * rowcol(ub, c21), Y = rowcol(ub, cy);
+#pragma unroll
+        for (int k = 0; k < SMALL_NSMAX; k++) if (k < nsets) {
+          cx<double> A1 = X12, A2 = X21; rfma(A1, s3[k], Y); rfma(A2, -s3[k], Y);
+          sums[k] += 16.0 * (norm2(A1) + norm2(A2)) - 4.0 * (A1.re * A2.re + A1.im * A2.im);
+        }
+      }
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < SMALL_NSMAX; k++) sums[k] *= 2.0 / 3.0;
+}
+
+__global__ void __launch_bounds__(128) gg_ttx_multi_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
+                                                           double* __restrict__ me_old, double* __restrict__ me_new,
+                                                           double* __restrict__ w_new, long long n, long long stride, long long ostride, GGttxParams P) {
+  long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  double p[4][4];
+#pragma unroll
+  for (int ip = 0; ip < 4; ip++)
+#pragma unroll
+    for (int mu = 0; mu < 4; mu++) p[ip][mu] = __ldg(mom + (size_t)(ip * 4 + mu) * stride + i);
+  const double W = __ldg(wgt + i);
+  if (!P.two_pass) {
+    double sums[SMALL_NSMAX];
+    ggttx_sums_multi(p, P.mt[0], P.s3, P.nsets, sums);
+    const double a = sums[0] * P.fac[0];
+    me_old[i] = a;
+#pragma unroll
+    for (int k = 1; k < SMALL_NSMAX; k++) if (k < P.nsets) {
+      const double b = sums[k] * P.fac[k];
+      me_new[(size_t)(k - 1) * ostride + i] = b; w_new[(size_t)(k - 1) * ostride + i] = W * (b / a);
+    }
+  } else {                               // masses differ: one full evaluation per set
+    double a = 0;
+#pragma unroll 1
+    for (int k = 0; k < P.nsets; k++) {
+      double x, t; ggttx_sums(p, P.mt[k], P.s3[k], P.s3[k], x, t); x *= P.fac[k];
+      if (k == 0) { a = x; me_old[i] = x; }
+      else { me_new[(size_t)(k - 1) * ostride + i] = x; w_new[(size_t)(k - 1) * ostride + i] = W * (x / a); }
+    }
+  }
 }
 
 }  // namespace rwgt

@@ -30,7 +30,8 @@ struct rwgt_handle {
   int n_gluons;
   int precision;
   int device;
-  rwgt_params po, pn;
+  int nsets;                  // 1 + K
+  rwgt_params sets[1 + RWGT_MAX_SETS];   // [0] = old, [1..K] = new
   rwgt::EpemParams epem;
   rwgt::GGttxParams ggttx;
   rwgt::BgProcess* bg;        // ordered-current engine (n_gluons >= 3, or gg_ttx when forced)
@@ -66,14 +67,19 @@ extern "C" {
 
 const char* rwgt_last_error(void) { return g_err; }
 
-rwgt_handle* rwgt_create(const char* process, const rwgt_params* params_old, const rwgt_params* params_new) {
+rwgt_handle* rwgt_create_multi(const char* process, const rwgt_params* params_old, const rwgt_params* params_new, int n_new) {
   if (!process || !params_old || !params_new) { set_err("rwgt_create: NULL argument"); return nullptr; }
-  if (!valid_params(params_old) || !valid_params(params_new)) { set_err("rwgt_create: invalid parameter set for %s", process); return nullptr; }
+  if (n_new < 1 || n_new > RWGT_MAX_SETS) { set_err("rwgt_create: number of new parameter sets must be in 1..RWGT_MAX_SETS"); return nullptr; }
+  bool okp = valid_params(params_old);
+  for (int k = 0; k < n_new; k++) okp = okp && valid_params(params_new + k);
+  if (!okp) { set_err("rwgt_create: invalid parameter set for %s", process); return nullptr; }
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); set_err("rwgt_create: no CUDA device (this library has no CPU path)"); return nullptr; }
   rwgt_handle* h = new (std::nothrow) rwgt_handle();
   if (!h) { set_err("rwgt_create: out of memory"); return nullptr; }
-  h->proc = -1; h->po = *params_old; h->pn = *params_new; h->precision = RWGT_FP64; h->bg = nullptr; h->scratch = nullptr; h->scratch_bytes = 0; h->s_in = nullptr; h->s_out = nullptr;
+  h->proc = -1; h->precision = RWGT_FP64; h->bg = nullptr; h->scratch = nullptr; h->scratch_bytes = 0; h->s_in = nullptr; h->s_out = nullptr;
+  h->nsets = 1 + n_new; h->sets[0] = *params_old;
+  for (int k = 0; k < n_new; k++) h->sets[1 + k] = params_new[k];
   cudaGetDevice(&h->device);
   std::string p(process);
   // "@bg" suffix routes gg_ttx through the generic ordered-current engine (used by the tests to cross-check it)
@@ -87,26 +93,33 @@ rwgt_handle* rwgt_create(const char* process, const rwgt_params* params_old, con
   else if (p == "gg_ttxggg") { ng = 5; }
   else { set_err("rwgt_create: unknown process '%s'", process); delete h; return nullptr; }
   if (h->proc == P_EPEM) {
-    h->epem.set[0] = make_epem(h->po); h->epem.set[1] = make_epem(h->pn);
+    h->epem.nsets = h->nsets;
+    for (int k = 0; k < h->nsets; k++) h->epem.set[k] = make_epem(h->sets[k]);
     return h;
   }
   h->n_gluons = ng; h->n_ext = ng + 2;
   if (ng == 2 && !force_bg) {
     h->proc = P_GG_TTX;
-    const rwgt_params* ps[2] = {&h->po, &h->pn};
-    for (int k = 0; k < 2; k++) {
-      double gs2 = 4.0 * PI * ps[k]->alpha_s;
-      h->ggttx.mt[k] = ps[k]->mt; h->ggttx.fac[k] = gs2 * gs2 / 256.0; h->ggttx.s3[k] = ps[k]->ggg_scale;
+    h->ggttx.nsets = h->nsets; h->ggttx.two_pass = 0;
+    for (int k = 0; k < h->nsets; k++) {
+      double gs2 = 4.0 * PI * h->sets[k].alpha_s;
+      h->ggttx.mt[k] = h->sets[k].mt; h->ggttx.fac[k] = gs2 * gs2 / 256.0; h->ggttx.s3[k] = h->sets[k].ggg_scale;
+      if (h->sets[k].mt != h->sets[0].mt) h->ggttx.two_pass = 1;
     }
-    h->ggttx.two_pass = (h->po.mt != h->pn.mt) ? 1 : 0;
     return h;
   }
   h->proc = P_BG;
   std::string err;
-  h->bg = rwgt::bg_create(ng, h->po, h->pn, err);
+  h->bg = rwgt::bg_create(ng, h->sets, h->nsets, err);
   if (!h->bg) { set_err("rwgt_create: %s", err.c_str()); delete h; return nullptr; }
   return h;
 }
+
+rwgt_handle* rwgt_create(const char* process, const rwgt_params* params_old, const rwgt_params* params_new) {
+  return rwgt_create_multi(process, params_old, params_new, 1);
+}
+
+int rwgt_n_sets(const rwgt_handle* h) { return h ? h->nsets - 1 : -1; }
 
 int rwgt_set_precision(rwgt_handle* h, int mode) {
   if (!h || mode < 0 || mode > 2) { set_err("rwgt_set_precision: bad argument"); return -1; }
@@ -121,8 +134,9 @@ double rwgt_flops_per_event(const rwgt_handle* h) {
   if (!h) return -1.0;
   // the two one-event-per-thread kernels: ncu counters of the committed build (217 DFMA + 119 DMUL + 48 DADD resp.
   // 1263 DFMA + 369 DMUL + 87 DADD per event; profiles/r1_summary.md)
-  if (h->proc == P_EPEM) return 601.0;
-  if (h->proc == P_GG_TTX) return h->ggttx.two_pass ? 2.0 * 2982.0 : 2982.0;
+  if (h->proc == P_EPEM) return 601.0 + (h->nsets - 2) * 45.0;
+  // gg_ttx: 2982 for two sets of equal mass; a further set of equal mass costs 8 helicities x (4 FMA + colour form 5 FMA + 4 MUL/ADD)
+  if (h->proc == P_GG_TTX) return h->ggttx.two_pass ? h->nsets * 2982.0 : 2982.0 + (h->nsets - 2) * 8 * 26.0;
   return rwgt::bg_flops_per_event(h->bg, h->precision);
 }
 
@@ -131,17 +145,19 @@ double rwgt_tensor_flops_per_event(const rwgt_handle* h) {
   return h->proc == P_BG ? rwgt::bg_tensor_flops_per_event(h->bg) : 0.0;
 }
 
-// one kernel launch over events [0, n) of buffers whose momentum planes are `stride` events apart
+// one kernel launch over events [0, n) of buffers whose momentum planes are `stride` events apart and whose per-set
+// output planes are `ostride` events apart
 static int launch_events(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old, double* out_me_new,
-                         double* out_w_new, long long n, long long stride, cudaStream_t st) {
+                         double* out_w_new, long long n, long long stride, long long ostride, cudaStream_t st) {
   if (h->proc == P_EPEM) {
     int bs = 256; long long nb = (n + bs - 1) / bs;
-    rwgt::epem_mupmum_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, h->epem);
+    rwgt::epem_mupmum_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->epem);
   } else if (h->proc == P_GG_TTX) {
     int bs = 128; long long nb = (n + bs - 1) / bs;
-    rwgt::gg_ttx_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, h->ggttx);
+    if (h->nsets == 2) rwgt::gg_ttx_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->ggttx);
+    else rwgt::gg_ttx_multi_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->ggttx);
   } else {
-    int rc = rwgt::bg_run(h->bg, h->precision, momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, st);
+    int rc = rwgt::bg_run(h->bg, h->precision, momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, st);
     if (rc != 0) { set_err("rwgt_run: engine launch failed"); return rc; }
   }
   cudaError_t e = cudaGetLastError();
@@ -149,24 +165,30 @@ static int launch_events(rwgt_handle* h, const double* momenta, const double* we
   return 0;
 }
 
-int rwgt_run(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old, double* out_me_new,
-             double* out_w_new, long long n_events, void* stream) {
+int rwgt_run_multi(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old, double* out_me_new,
+                   double* out_w_new, long long n_events, void* stream) {
   if (!h || n_events < 0) { set_err("rwgt_run: bad handle or n_events < 0"); return -1; }
   if (n_events == 0) return 0;
   if (!momenta || !weights || !out_me_old || !out_me_new || !out_w_new) { set_err("rwgt_run: NULL buffer"); return -1; }
-  return launch_events(h, momenta, weights, out_me_old, out_me_new, out_w_new, n_events, n_events, (cudaStream_t)stream);
+  return launch_events(h, momenta, weights, out_me_old, out_me_new, out_w_new, n_events, n_events, n_events, (cudaStream_t)stream);
+}
+
+int rwgt_run(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old, double* out_me_new,
+             double* out_w_new, long long n_events, void* stream) {
+  if (h && h->nsets != 2) { set_err("rwgt_run: handle has several new parameter sets, use rwgt_run_multi"); return -1; }
+  return rwgt_run_multi(h, momenta, weights, out_me_old, out_me_new, out_w_new, n_events, stream);
 }
 
 // Host-buffer path (the transfers are part of what a user pays).  The events are cut into chunks; the
 // host->device copy of chunk c+1 (copy stream), the kernel of chunk c (caller's stream) and the device->host copy of
 // chunk c-1 (second copy stream) overlap, so on a full-duplex link the call costs about max(H2D, D2H, kernel).
-int rwgt_run_host(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old, double* out_me_new,
-                  double* out_w_new, long long n_events, void* stream) {
+int rwgt_run_multi_host(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old, double* out_me_new,
+                        double* out_w_new, long long n_events, void* stream) {
   if (!h || n_events < 0) { set_err("rwgt_run_host: bad handle or n_events < 0"); return -1; }
   if (n_events == 0) return 0;
   if (!momenta || !weights || !out_me_old || !out_me_new || !out_w_new) { set_err("rwgt_run_host: NULL buffer"); return -1; }
   cudaStream_t st = (cudaStream_t)stream;
-  const size_t n = (size_t)n_events, planes = (size_t)h->n_ext * 4, nin = planes * n, need = (nin + 4 * n) * sizeof(double);
+  const size_t n = (size_t)n_events, planes = (size_t)h->n_ext * 4, nin = planes * n, K = (size_t)h->nsets - 1, need = (nin + (2 + 2 * K) * n) * sizeof(double);
   cudaError_t e = cudaSuccess;
 #define RWGT_CK(call) do { e = (call); if (e != cudaSuccess) { set_err("rwgt_run_host: %s", cudaGetErrorString(e)); return (int)e; } } while (0)
   if (need > h->scratch_bytes) {
@@ -183,7 +205,7 @@ int rwgt_run_host(rwgt_handle* h, const double* momenta, const double* weights, 
       RWGT_CK(cudaEventCreateWithFlags(&h->ev_k[c], cudaEventDisableTiming));
     }
   }
-  double* d_mom = h->scratch; double* d_w = d_mom + nin; double* d_a = d_w + n; double* d_b = d_a + n; double* d_o = d_b + n;
+  double* d_mom = h->scratch; double* d_w = d_mom + nin; double* d_a = d_w + n; double* d_b = d_a + n; double* d_o = d_b + K * n;
   // chunks of >= 64 Ki events, at most RWGT_MAX_CHUNKS
   long long nchunk = (long long)((n + 65535) / 65536); if (nchunk > RWGT_MAX_CHUNKS) nchunk = RWGT_MAX_CHUNKS; if (nchunk < 1) nchunk = 1;
   long long per = ((long long)n + nchunk - 1) / nchunk;
@@ -198,13 +220,13 @@ int rwgt_run_host(rwgt_handle* h, const double* momenta, const double* weights, 
     RWGT_CK(cudaMemcpyAsync(d_w + a0, weights + a0, (size_t)cnt * sizeof(double), cudaMemcpyHostToDevice, h->s_in));
     RWGT_CK(cudaEventRecord(h->ev_in[c], h->s_in));
     RWGT_CK(cudaStreamWaitEvent(st, h->ev_in[c], 0));
-    int rc = launch_events(h, d_mom + a0, d_w + a0, d_a + a0, d_b + a0, d_o + a0, cnt, (long long)n, st);
+    int rc = launch_events(h, d_mom + a0, d_w + a0, d_a + a0, d_b + a0, d_o + a0, cnt, (long long)n, (long long)n, st);
     if (rc != 0) return rc;
     RWGT_CK(cudaEventRecord(h->ev_k[c], st));
     RWGT_CK(cudaStreamWaitEvent(h->s_out, h->ev_k[c], 0));
     RWGT_CK(cudaMemcpyAsync(out_me_old + a0, d_a + a0, (size_t)cnt * sizeof(double), cudaMemcpyDeviceToHost, h->s_out));
-    RWGT_CK(cudaMemcpyAsync(out_me_new + a0, d_b + a0, (size_t)cnt * sizeof(double), cudaMemcpyDeviceToHost, h->s_out));
-    RWGT_CK(cudaMemcpyAsync(out_w_new + a0, d_o + a0, (size_t)cnt * sizeof(double), cudaMemcpyDeviceToHost, h->s_out));
+    RWGT_CK(cudaMemcpy2DAsync(out_me_new + a0, n * sizeof(double), d_b + a0, n * sizeof(double), (size_t)cnt * sizeof(double), K, cudaMemcpyDeviceToHost, h->s_out));
+    RWGT_CK(cudaMemcpy2DAsync(out_w_new + a0, n * sizeof(double), d_o + a0, n * sizeof(double), (size_t)cnt * sizeof(double), K, cudaMemcpyDeviceToHost, h->s_out));
   }
   // the caller's stream continues only after the results are on the host; then wait for it
   RWGT_CK(cudaEventRecord(h->ev_k[RWGT_MAX_CHUNKS], h->s_out));
@@ -212,6 +234,12 @@ int rwgt_run_host(rwgt_handle* h, const double* momenta, const double* weights, 
   RWGT_CK(cudaStreamSynchronize(st));
 #undef RWGT_CK
   return 0;
+}
+
+int rwgt_run_host(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old, double* out_me_new,
+                  double* out_w_new, long long n_events, void* stream) {
+  if (h && h->nsets != 2) { set_err("rwgt_run_host: handle has several new parameter sets, use rwgt_run_multi_host"); return -1; }
+  return rwgt_run_multi_host(h, momenta, weights, out_me_old, out_me_new, out_w_new, n_events, stream);
 }
 
 int rwgt_destroy(rwgt_handle* h) {

@@ -1,0 +1,120 @@
+"""GPU parity of the K-parameter-set pass (PAPER.md:87 step 7): rwgt_create_multi /
+rwgt_run_multi against the CPU oracle evaluated once per set, element by element."""
+import numpy as np
+import pytest
+
+import oracle as orc
+from paper_2312_07440_b200 import binding as B, events as ev
+
+pytestmark = pytest.mark.gpu
+TOL64 = 1e-11
+torch = pytest.importorskip("torch")
+
+
+def rel(got, ref):
+    return np.abs(got / ref - 1)
+
+
+def new_sets(idx):
+    c = ev.config(idx)
+    if idx == 1:
+        return [c.params_new, ev.params(GammaZ=2.3, sin2_thetaW=0.2250), ev.params(mZ=92.5, alpha_em=1 / 128.0), c.params_old.copy()]
+    return [c.params_new, ev.params(ggg_scale=0.9, gggg_scale=0.8), ev.params(ggg_scale=1.25, gggg_scale=1.1, alpha_s=0.13),
+            c.params_old.copy(), ev.params(ggg_scale=-1.0, gggg_scale=1.0)]
+
+
+def run_multi(c, sets, m, w, precision="fp64"):
+    r = B.Reweighter(c.process, c.params_old, sets, precision)
+    out = r.run(torch.from_numpy(m).cuda(), torch.from_numpy(w).cuda())
+    torch.cuda.synchronize()
+    res = out.cpu().numpy()
+    r.close()
+    return res
+
+
+@pytest.mark.parametrize("idx,n", [(1, 3001), (2, 2049), (3, 601), (4, 103), (5, 19)])
+def test_multi_set_fp64_parity_every_event(idx, n):
+    c = ev.config(idx)
+    sets = new_sets(idx)
+    K = len(sets)
+    m, w = ev.generate(c, n)
+    got = run_multi(c, sets, m, w)
+    assert got.shape == (1 + 2 * K, n)
+    for k, pn in enumerate(sets):
+        a, b, wn, _ = orc.reweight(c.process, c.params_old, pn, m, w)
+        for g, ref, name in ((got[0], a, "me_old"), (got[1 + k], b, "me_new"), (got[1 + K + k], wn, "w_new")):
+            e = rel(g, ref)
+            assert e.max() < TOL64, (c.process, k, name, int(e.argmax()), e.max())
+    # the set equal to the old one: ratio exactly 1 (north_star), bitwise
+    k_same = 3
+    assert np.array_equal(got[1 + k_same], got[0]) and np.array_equal(got[1 + K + k_same], w)
+
+
+@pytest.mark.parametrize("idx,n", [(2, 515), (3, 301)])
+def test_multi_set_with_different_top_masses(idx, n):
+    """A set with another top mass makes the library redo externals, momentum sums and denominators for that set
+    (reading R12).  The comparison with the oracle is only defined for momenta on the mass shell of the set's own m_t
+    (reading Q8: off shell, sqrt(E+-m) and sqrt(E+-|p|) spinor normalisations differ), so the masses here differ by
+    one ulp: the separate-externals code path runs, the numbers stay within tolerance of the on-shell oracle."""
+    c = ev.config(idx)
+    up, dn = float(np.nextafter(173.0, 200.0)), float(np.nextafter(173.0, 0.0))
+    sets = [ev.params(mt=up, ggg_scale=1.1, gggg_scale=1.1), c.params_new, ev.params(mt=dn, ggg_scale=0.7)]
+    m, w = ev.generate(c, n)
+    got = run_multi(c, sets, m, w)
+    K = len(sets)
+    for k, pn in enumerate(sets):
+        a, b, wn, _ = orc.reweight(c.process, c.params_old, pn, m, w)
+        assert rel(got[0], a).max() < TOL64 and rel(got[1 + k], b).max() < TOL64 and rel(got[1 + K + k], wn).max() < TOL64
+
+
+def test_multi_set_matches_single_set_calls_bitwise_and_max_sets():
+    """K sets in one pass give bit-identical numbers to K separate (old, new_k) handles; K = RWGT_MAX_SETS works,
+    K = RWGT_MAX_SETS + 1 is refused."""
+    c = ev.config(4)
+    kappas = np.linspace(-0.3, 0.45, B.RWGT_MAX_SETS)
+    sets = [ev.params(ggg_scale=1 + k, gggg_scale=1 + k) for k in kappas]
+    m, w = ev.generate(c, 57)
+    got = run_multi(c, sets, m, w)
+    K = len(sets)
+    dm, dw = torch.from_numpy(m).cuda(), torch.from_numpy(w).cuda()
+    for k in (0, 7, K - 1):
+        r = B.Reweighter(c.process, c.params_old, sets[k])
+        one = r.run(dm, dw).cpu().numpy()
+        r.close()
+        assert np.array_equal(one[0], got[0]) and np.array_equal(one[1], got[1 + k]) and np.array_equal(one[2], got[1 + K + k])
+    with pytest.raises(RuntimeError, match="RWGT_MAX_SETS"):
+        B.rwgt_create_multi(c.process, c.params_old, sets + [sets[0]])
+    h = B.rwgt_create_multi(c.process, c.params_old, sets[:3])
+    assert B.rwgt_n_sets(h) == 3
+    with pytest.raises(RuntimeError, match="rwgt_run_multi"):
+        B.rwgt_run(h, 1, 1, 1, 1, 1, 5)              # single-set entry point refuses a multi-set handle
+    B.rwgt_destroy(h)
+
+
+@pytest.mark.parametrize("precision", ["fp32", "mixed"])
+def test_multi_set_fp32_and_mixed(precision):
+    c = ev.config(4)
+    sets = new_sets(4)[:3]
+    m, w = ev.generate(c, 203)
+    got = run_multi(c, sets, m, w, precision)
+    K = len(sets)
+    for k, pn in enumerate(sets):
+        a, b, wn, _ = orc.reweight(c.process, c.params_old, pn, m, w)
+        for g, ref in ((got[0], a), (got[1 + k], b), (got[1 + K + k], wn)):
+            e = rel(g, ref)
+            assert e.max() < 1e-4 and np.median(e) < 1e-6, (precision, k, e.max(), np.median(e))
+
+
+def test_multi_set_host_path_chunked():
+    c = ev.config(2)
+    sets = new_sets(2)[:3]
+    n = 2 * 65536 + 11
+    m0, w0 = ev.generate(c, 2048)
+    reps = (n + 2047) // 2048
+    m, w = np.tile(m0, (1, 1, reps))[:, :, :n].copy(), np.tile(w0, reps)[:n].copy()
+    dev = run_multi(c, sets, m, w)
+    h = B.rwgt_create_multi(c.process, c.params_old, sets)
+    a, b, o = np.empty(n), np.empty((3, n)), np.empty((3, n))
+    B.rwgt_run_multi_host(h, m, w, a, b, o)
+    B.rwgt_destroy(h)
+    assert np.array_equal(a, dev[0]) and np.array_equal(b, dev[1:4]) and np.array_equal(o, dev[4:7])
