@@ -154,7 +154,11 @@ template <int N> struct Geo {
   static constexpr int NB = (N == 5) ? 2 : (N == 4) ? 1 : 0, NBATCH = 1 << NB;
   static constexpr int NFREE = 1 << (N - 1 - NB), NCOL = NFREE * 4;
   static constexpr int ASTR = 2 * NCOL + 4;                              // row stride (doubles) of the amplitude buffer, bank-conflict-free
-  static constexpr int MT = NPERM_P / 8, KT = NPERM_P / 4, U = (MT + 1) / 2;
+  // colour form split by the reflection symmetry C[s][s'] = C[rev s][rev s']: with u = J_s + J_rev(s), v = J_s - J_rev(s) per pair,
+  // J^dagger C J = 1/2 u^dagger C+ u + 1/2 v^dagger C- v, C+- = C[s_p][s_q] +- C[s_p][rev s_q]: two NPAIR x NPAIR forms, half the flops
+  static constexpr int NHK = pad4(NPAIR);                                // amplitude rows per half (K dimension of the mma, padded to 4)
+  static constexpr int MTH = (NPAIR + 7) / 8, KTH = NHK / 4, UH = (MTH + 1) / 2, U = 2 * UH;
+  static constexpr int KSH = MTH * KTH - MTH * (MTH - 1);                // k-steps of one half (upper-triangular tiles)
   static constexpr int NT = 2 * NCOL / 8;                                // mma n-tiles per batch
   static constexpr int NMASK = 1 << N;
   static constexpr int NPHASE = (N - 1 > (RMAX > LMAX ? RMAX : LMAX) + 1) ? N - 1 : (RMAX > LMAX ? RMAX : LMAX) + 1;
@@ -162,7 +166,7 @@ template <int N> struct Geo {
   static constexpr int JW = pad4(2 * NL3 + 3 * NV4);                     // words of the n-gluon current's references
   static constexpr int QH = C + NJ + NJ * C, QW = pad4((QH + 1) / 2);    // halfwords / words of one quark-line reference block
   static constexpr int STRIDEF = 4 + JW + 2 * QW;
-  static constexpr size_t ABUF = (size_t)NPERM_P * ASTR;                 // doubles per slot per buffer
+  static constexpr size_t ABUF = (size_t)(2 * NHK) * ASTR;               // doubles per slot per buffer: rows [u of all pairs | v of all pairs]
   static constexpr int NG = c_nG(N), NR = c_nQ(N, RMAX), NL = c_nQ(N, LMAX);   // entries of the current tables (checked against the schedule)
 };
 __host__ __device__ constexpr int gdesc_words(int m) { return pad4(2 + 2 * (m - 1) + 3 * (m - 1) * (m - 2) / 2); }
@@ -256,14 +260,16 @@ static BgSched build_schedule(int n, std::string& err) {
   const int C = S.c, NJ = n - C + 1;
   const int JW = pad4(2 * (n - 1) + 3 * (n - 1) * (n - 2) / 2), QH = C + NJ + NJ * C, QW = pad4((QH + 1) / 2);
   pad(); S.offF = (int)S.words.size(); S.strideF = 4 + JW + 2 * QW; S.npair = 0;
+  std::vector<int> pair_rank, pair_rank_rev;
   for (auto& s0 : perms) {
     bool fwd = (n == 5) ? necklace_forward(s0) : (s0.front() < s0.back());
     if (!fwd) continue;
-    S.npair++;
+    S.npair++; pair_rank.push_back(rank[s0]); pair_rank_rev.push_back(rank[reversed(s0)]);
     size_t d0 = S.words.size();
     std::vector<int> sr = reversed(s0);
     uint32_t packed = 0; for (int j = 0; j < n; j++) packed |= (uint32_t)s0[j] << (3 * j);
-    S.words.push_back((uint32_t)rank[s0] | ((uint32_t)rank[sr] << 16)); S.words.push_back(packed); S.words.push_back(0u); S.words.push_back(0u);
+    // word 0: pair index p = row of u (v is at row NHK + p); word 1: the permutation, 3 bits per position
+    S.words.push_back((uint32_t)(S.npair - 1)); S.words.push_back(packed); S.words.push_back(0u); S.words.push_back(0u);
     gluon_refs(s0); pad();
     for (int which = 0; which < 2; which++) {
       const std::vector<int>& s = which ? sr : s0;
@@ -288,19 +294,28 @@ static BgSched build_schedule(int n, std::string& err) {
     S.fp_ops[0] += nf * (n - 1); S.fp_ops[1] += nf * ((n - 1) * (n - 2) / 2); S.fp_ops[n > 2 ? 6 : 7] += nf;
     S.fp_ops[3] += nf * (1 + 2 * (NJ * C - 1)); S.fp_ops[2] += nf * 2 * 2 * NJ * C; S.fp_ops[5] += nf * 2 * NJ * 4;
   }
-  // Cholesky C = L L^T (C is positive definite); J^dagger C J = |L^T J|^2.  L^T in mma.m8n8k4 A-fragment order:
-  // for m-tile mt, k-steps kt = 2 mt .. KT-1 (upper triangle), element (lane>>2, lane&3) of the 8x4 tile.
+  // Colour form.  C commutes with the reversal s -> rev(s) (a trace and its transpose), so in the basis u_p = J_{s_p} + J_{rev s_p},
+  // v_p = J_{s_p} - J_{rev s_p} it is block diagonal: J^dagger C J = u^dagger (C+/2) u + v^dagger (C-/2) v with
+  // C+-[p][q] = C[s_p][s_q] +- C[s_p][rev s_q].  Each block is positive definite (C is): Cholesky C+-/2 = L L^T and
+  // the form is |L+^T u|^2 + |L-^T v|^2.  L^T in mma.m8n8k4 A-fragment order: for half h, m-tile mt, k-steps kt = 2 mt .. KTH-1
+  // (upper triangle), element (lane>>2, lane&3) of the 8x4 tile; rows/columns beyond npair are zero.
   {
-    int np = S.nperm, npp = (np + 7) / 8 * 8, MT = npp / 8, KT = npp / 4;
-    std::vector<double> Cm = colour_matrix_fierz(n), L((size_t)np * np, 0.0);
-    for (int j = 0; j < np; j++) {
-      double d = Cm[(size_t)j * np + j]; for (int k = 0; k < j; k++) d -= L[(size_t)j * np + k] * L[(size_t)j * np + k];
-      d = std::sqrt(d); L[(size_t)j * np + j] = d;
-      for (int i = j + 1; i < np; i++) { double x = Cm[(size_t)i * np + j]; for (int k = 0; k < j; k++) x -= L[(size_t)i * np + k] * L[(size_t)j * np + k]; L[(size_t)i * np + j] = x / d; }
-    }
-    for (int mt = 0; mt < MT; mt++) for (int kt = 2 * mt; kt < KT; kt++) for (int lane = 0; lane < 32; lane++) {
-      int row = 8 * mt + (lane >> 2), col = 4 * kt + (lane & 3);
-      S.lfrag.push_back((row < np && col < np && col >= row) ? L[(size_t)col * np + row] : 0.0);      // L^T[row][col] = L[col][row]
+    int np = S.nperm, nh = S.npair, nhk = (nh + 3) / 4 * 4, MTH = (nh + 7) / 8, KTH = nhk / 4;
+    std::vector<double> Cm = colour_matrix_fierz(n);
+    for (int h = 0; h < 2; h++) {
+      std::vector<double> Ch((size_t)nh * nh), L((size_t)nh * nh, 0.0);
+      for (int p = 0; p < nh; p++) for (int q = 0; q < nh; q++)
+        Ch[(size_t)p * nh + q] = 0.5 * (Cm[(size_t)pair_rank[p] * np + pair_rank[q]] + (h ? -1.0 : 1.0) * Cm[(size_t)pair_rank[p] * np + pair_rank_rev[q]]);
+      for (int j = 0; j < nh; j++) {
+        double d = Ch[(size_t)j * nh + j]; for (int k = 0; k < j; k++) d -= L[(size_t)j * nh + k] * L[(size_t)j * nh + k];
+        if (!(d > 0)) { err = "internal: colour block not positive definite"; return S; }
+        d = std::sqrt(d); L[(size_t)j * nh + j] = d;
+        for (int i = j + 1; i < nh; i++) { double x = Ch[(size_t)i * nh + j]; for (int k = 0; k < j; k++) x -= L[(size_t)i * nh + k] * L[(size_t)j * nh + k]; L[(size_t)i * nh + j] = x / d; }
+      }
+      for (int mt = 0; mt < MTH; mt++) for (int kt = 2 * mt; kt < KTH; kt++) for (int lane = 0; lane < 32; lane++) {
+        int row = 8 * mt + (lane >> 2), col = 4 * kt + (lane & 3);
+        S.lfrag.push_back((row < nh && col < nh && col >= row) ? L[(size_t)col * nh + row] : 0.0);      // L^T[row][col] = L[col][row]
+      }
     }
   }
   return S;
@@ -337,7 +352,7 @@ template <typename T> struct Smem {
   T* K;           // [nslot][NMASK][4] momentum sums of gluon subsets
   T* iK2;         // [nslot][NMASK]
   T* dR; T* dL;   // [nslot][NMASK] 1/(q^2-m^2)
-  double* A;      // [2][nslot][NPERM_P][ASTR] double-buffered colour-flow amplitudes (re,im interleaved), always double
+  double* A;      // [2][nslot][2 NHK][ASTR] double-buffered rows u = J_s + J_rev(s), v = J_s - J_rev(s) (re,im interleaved), always double
 };
 template <int N, typename T> __host__ __device__ inline size_t carve(Smem<T>& s, unsigned char* base, int ns, int nwords) {
   typedef Geo<N> Ge; size_t off = 0; constexpr int nG = Ge::NG, nR = Ge::NR, nL = Ge::NL;
@@ -564,20 +579,12 @@ template <int N, int WHICH, typename T> struct QuarkLine {
       jterm<JJ + 1>(Acc, wq, v, Jn, G, R, L);
     }
   }
-  static __device__ __forceinline__ void run(double* Arow, int f, const uint32_t* wq, uint32_t v, const vec4<T>& Jn, const cx<T>* G, const cx<T>* R, const cx<T>* L) {
-    cx<T> Acc[2][2];
+  static __device__ __forceinline__ void run(cx<T> (&Acc)[2][2], const uint32_t* wq, uint32_t v, const vec4<T>& Jn, const cx<T>* G, const cx<T>* R, const cx<T>* L) {
 #pragma unroll
     for (int a = 0; a < 2; a++)
 #pragma unroll
       for (int b = 0; b < 2; b++) Acc[a][b] = mk<T>(0, 0);
     jterm<0>(Acc, wq, v, Jn, G, R, L);
-#pragma unroll
-    for (int ht = 0; ht < 2; ht++)
-#pragma unroll
-      for (int hb = 0; hb < 2; hb++) {
-        int col = f * 4 + ht * 2 + hb;
-        *reinterpret_cast<double2*>(Arow + 2 * col) = make_double2((double)Acc[ht][hb].re, (double)Acc[ht][hb].im);
-      }
   }
 };
 
@@ -690,15 +697,26 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
             T sc = s.iK2[sl * Ge::NMASK + Ge::NMASK - 1];
 #pragma unroll
             for (int i = 0; i < 4; i++) Jn.c[i] = sc * Jn.c[i];
-            double* A = Abuf + (size_t)sl * Ge::ABUF;
+            cx<T> A0[2][2], A1[2][2];
             {
               uint32_t wq[Ge::QW]; ldw<Ge::QW>(wq, w + 4 + Ge::JW);
-              QuarkLine<N, 0, T>::run(A + (size_t)(w0 & 0xffffu) * Ge::ASTR, f, wq, v, Jn, G, R, L);
+              QuarkLine<N, 0, T>::run(A0, wq, v, Jn, G, R, L);
             }
             {
               uint32_t wq[Ge::QW]; ldw<Ge::QW>(wq, w + 4 + Ge::JW + Ge::QW);
-              QuarkLine<N, 1, T>::run(A + (size_t)(w0 >> 16) * Ge::ASTR, f, wq, brevm<N>(v), Jn, G, R, L);
+              QuarkLine<N, 1, T>::run(A1, wq, brevm<N>(v), Jn, G, R, L);
             }
+            // rows u = J_s + J_rev(s) and v = J_s - J_rev(s) of the pair (formed in double)
+            double* Au = Abuf + (size_t)sl * Ge::ABUF + (size_t)w0 * Ge::ASTR; double* Av = Au + (size_t)Ge::NHK * Ge::ASTR;
+#pragma unroll
+            for (int ht = 0; ht < 2; ht++)
+#pragma unroll
+              for (int hb = 0; hb < 2; hb++) {
+                const int col = f * 4 + ht * 2 + hb;
+                const double ar = (double)A0[ht][hb].re, ai = (double)A0[ht][hb].im, br = (double)A1[ht][hb].re, bi = (double)A1[ht][hb].im;
+                *reinterpret_cast<double2*>(Au + 2 * col) = make_double2(ar + br, ai + bi);
+                *reinterpret_cast<double2*>(Av + 2 * col) = make_double2(ar - br, ai - bi);
+              }
           }
           __threadfence_block();
           bar_arrive(BAR_FULL0 + buf, NTH);                    // hand the batch to the colour warps
@@ -724,18 +742,18 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
           const double* Abuf = s.A + (size_t)buf * ns * Ge::ABUF;
           // a5: Z = L^T A with FP64 tensor-core mma over the upper-triangular tiles, colour form = sum of squares of Z
           for (int u = cwarp; u < ns * Ge::U; u += NCW) {
-            int sl = u / Ge::U, unit = u % Ge::U;
-            const double* A = Abuf + (size_t)sl * Ge::ABUF + (lane & 3) * Ge::ASTR + (lane >> 2);
+            int sl = u / Ge::U, unit = u % Ge::U; const int h = unit / Ge::UH, uu = unit % Ge::UH;     // h: 0 = u rows / L+, 1 = v rows / L-
+            const double* A = Abuf + (size_t)sl * Ge::ABUF + (size_t)(h * Ge::NHK + (lane & 3)) * Ge::ASTR + (lane >> 2);
             double part = 0.0;
 #pragma unroll 1
             for (int half = 0; half < 2; half++) {
-              int mt = half ? Ge::MT - 1 - unit : unit;
-              if (half && mt == unit) break;
+              int mt = half ? Ge::MTH - 1 - uu : uu;
+              if (half && mt == uu) break;
               double acc[Ge::NT][2];
 #pragma unroll
               for (int nt = 0; nt < Ge::NT; nt++) { acc[nt][0] = 0.0; acc[nt][1] = 0.0; }
-              const double* F = D.lfrag + (size_t)(mt * Ge::KT - mt * (mt - 1)) * 32 + lane;
-              int nk = Ge::KT - 2 * mt;
+              const double* F = D.lfrag + (size_t)(h * Ge::KSH + mt * Ge::KTH - mt * (mt - 1)) * 32 + lane;
+              int nk = Ge::KTH - 2 * mt;
               double a0 = __ldg(F), a1 = (nk > 1) ? __ldg(F + 32) : 0.0;
               for (int kk = 0; kk < nk; kk++) {
                 double an = (kk + 2 < nk) ? __ldg(F + (kk + 2) * 32) : 0.0;
@@ -856,12 +874,12 @@ static double bg_flops_per_event(const BgProcess* B, int /*precision*/) {
   double fp = 0; for (int k = 0; k < 8; k++) fp += B->S.fp_ops[k] * fl[k];
   return B->D.nsets * fp + (B->D.shared_ext ? 1 : B->D.nsets) * (n * 2 * 30.0 + 4 * 40.0 + (1 << n) * 40.0);
 }
-// Algorithmic flops of the colour form |L^T J|^2 (a5), both parameter sets: per evaluated helicity (2^(n+1) after parity)
-// the triangular product costs ncol (ncol + 1) / 2 FMAs for the real and for the imaginary part, plus 2 ncol FMAs for the
-// sum of squares.  They run as mma.m8n8k4 (DMMA) on the FP64 pipe, which DFMA and DMMA share on B200 (rwgt_measure_peak 7).
+// Algorithmic flops of the colour form |L+^T u|^2 + |L-^T v|^2 (a5), all parameter sets: per evaluated helicity (2^(n+1) after
+// parity) each of the two reflection blocks (size nh = n!/2) costs nh (nh + 1) / 2 FMAs for the real and for the imaginary part,
+// plus 2 nh FMAs for the sum of squares.  They run as mma.m8n8k4 (DMMA) on the FP64 pipe, which DFMA and DMMA share on B200 (rwgt_measure_peak 7).
 static double bg_tensor_flops_per_event(const BgProcess* B) {
-  const int n = B->S.n; const double ncol = B->S.nperm, nhel = (double)(1 << (n + 1));
-  return B->D.nsets * nhel * (2.0 * (ncol * (ncol + 1) / 2) + 2.0 * ncol) * 2.0;
+  const int n = B->S.n; const double nh = B->S.npair, nhel = (double)(1 << (n + 1));
+  return B->D.nsets * nhel * 2.0 * (2.0 * (nh * (nh + 1) / 2) + 2.0 * nh) * 2.0;     // two reflection blocks of size n!/2
 }
 
 static int bg_run(BgProcess* B, int precision, const double* mom, const double* w, double* a, double* b, double* o, long long nev, long long stride, long long ostride, cudaStream_t st) {
