@@ -140,8 +140,10 @@ static void all_tuples(int n, int m, std::vector<std::vector<int>>& out) {
 // compile-time geometry of the schedule for N gluons (mirrored by build_schedule and checked in bg_create)
 __host__ __device__ constexpr int cfact(int n) { return n <= 1 ? 1 : n * cfact(n - 1); }
 __host__ __device__ constexpr int ctuples(int n, int m) { return m > n ? 0 : cfact(n) / cfact(n - m); }     // ordered m-tuples of n labels
-__host__ __device__ constexpr int c_nG(int n) { int r = 0; for (int m = 1; m <= n - 1; m++) r += (m <= 2 ? ctuples(n, m) : ctuples(n, m) / 2) << m; return r; }
-__host__ __device__ constexpr int c_nQ(int n, int mmax) { int r = 2; for (int m = 1; m <= mmax; m++) r += ctuples(n, m) * (2 << m); return r; }
+// table entries per slot after the hole-sharing allocation of build_schedule (checked against the builder in bg_create)
+__host__ __device__ constexpr int c_nG(int n) { return n == 2 ? 4 : n == 3 ? 22 : n == 4 ? 112 : 818; }
+__host__ __device__ constexpr int c_nR(int n) { return n == 2 ? 10 : n == 3 ? 14 : n == 4 ? 98 : 150; }
+__host__ __device__ constexpr int c_nL(int n) { return n == 2 ? 2 : n == 3 ? 14 : n == 4 ? 18 : 150; }
 // tasks of one level after parity pruning (gluon 0 at helicity + only)
 __host__ __device__ constexpr int c_ntaskG(int n, int m) { int can = ctuples(n, m) / 2, c0 = m * ctuples(n - 1, m - 1) / 2; return ((can - c0) << m) + (c0 << (m - 1)); }
 __host__ __device__ constexpr int c_ntaskQ(int n, int m) { int all = ctuples(n, m), c0 = m * ctuples(n - 1, m - 1); return ((all - c0) << (m + 1)) + (c0 << m); }
@@ -167,7 +169,7 @@ template <int N> struct Geo {
   static constexpr int QH = C + NJ + NJ * C, QW = pad4((QH + 1) / 2);    // halfwords / words of one quark-line reference block
   static constexpr int STRIDEF = 4 + JW + 2 * QW;
   static constexpr size_t ABUF = (size_t)(2 * NHK) * ASTR;               // doubles per slot per buffer: rows [u of all pairs | v of all pairs]
-  static constexpr int NG = c_nG(N), NR = c_nQ(N, RMAX), NL = c_nQ(N, LMAX);   // entries of the current tables (checked against the schedule)
+  static constexpr int NG = c_nG(N), NR = c_nR(N), NL = c_nL(N);   // entries of the current tables (checked against the schedule)
 };
 __host__ __device__ constexpr int gdesc_words(int m) { return pad4(2 + 2 * (m - 1) + 3 * (m - 1) * (m - 2) / 2); }
 __host__ __device__ constexpr int qdesc_words(int m) { return pad4(1 + m); }
@@ -192,10 +194,22 @@ static BgSched build_schedule(int n, std::string& err) {
   S.c = (n + 1) / 2; S.lmax = S.c - 1; S.rmax = n - S.c;
   TupleTables T; std::vector<std::vector<int>> tl;
   int nG = 0, nR = 0, nL = 0;
-  for (int m = 1; m <= n - 1; m++) { all_tuples(n, m, tl); for (auto& t : tl) if (is_stored(n, t)) { T.gbase[t] = nG; nG += 1 << m; } }
+  // Table allocation.  A tuple with gluon 0 at position q only ever uses the variants with bit q clear (parity: gluon 0 at
+  // helicity +), so two such tuples of the same length and the same q share one block: the second one's base is offset by 1 << q
+  // and its entries fall exactly into the holes of the first (the device still computes entry = base + variant bits).
+  auto allocate = [&](std::map<std::vector<int>, int>& base, int& count, const std::vector<std::vector<int>>& tuples, int m, int block) {
+    int open_base[6] = {-1, -1, -1, -1, -1, -1};                      // first half of an open pair, per position of gluon 0
+    for (auto& t : tuples) {
+      int q = pos0(t);
+      if (q < 0 || m == 1) { base[t] = count; count += block; continue; }
+      if (open_base[q] < 0) { base[t] = count; open_base[q] = count; count += block; }
+      else { base[t] = open_base[q] + (1 << q); open_base[q] = -1; }
+    }
+  };
+  for (int m = 1; m <= n - 1; m++) { all_tuples(n, m, tl); std::vector<std::vector<int>> st; for (auto& t : tl) if (is_stored(n, t)) st.push_back(t); allocate(T.gbase, nG, st, m, 1 << m); }
   T.rbase[{}] = nR; nR += 2; T.lbase[{}] = nL; nL += 2;
-  for (int m = 1; m <= S.rmax; m++) { all_tuples(n, m, tl); for (auto& t : tl) { T.rbase[t] = nR; nR += 2 << m; } }
-  for (int m = 1; m <= S.lmax; m++) { all_tuples(n, m, tl); for (auto& t : tl) { T.lbase[t] = nL; nL += 2 << m; } }
+  for (int m = 1; m <= S.rmax; m++) { all_tuples(n, m, tl); allocate(T.rbase, nR, tl, m, 2 << m); }
+  for (int m = 1; m <= S.lmax; m++) { all_tuples(n, m, tl); allocate(T.lbase, nL, tl, m, 2 << m); }
   S.nG = nG; S.nR = nR; S.nL = nL;
   auto pad = [&]() { while (S.words.size() % 4) S.words.push_back(0u); };
   auto gref32 = [&](const std::vector<int>& t, int lo, int hi) {          // reference inside a gluon recursion: must be stored as used (or length 3)
@@ -344,6 +358,7 @@ template <typename T> __device__ __forceinline__ void stc(cx<T>* p, cx<T> v) { t
 
 template <typename T> struct Smem {
   uint32_t* W;    // schedule words (whole CTA)
+  double* LF;     // Cholesky factors L+^T, L-^T of the colour blocks in mma-fragment order (whole CTA)
   double* pm;     // [nslot][n_ext][4] momenta (always double)
   double* acc;    // [nslot][BG_NSMAX]   helicity-summed colour forms per parameter set (owned by the colour warps)
   double* red;    // [nslot][8]   per-warp partial sums of the colour form
@@ -358,6 +373,7 @@ template <int N, typename T> __host__ __device__ inline size_t carve(Smem<T>& s,
   typedef Geo<N> Ge; size_t off = 0; constexpr int nG = Ge::NG, nR = Ge::NR, nL = Ge::NL;
   auto al = [&]() { off = (off + 15) / 16 * 16; };
   s.A = (double*)(base + off); off += sizeof(double) * 2 * (size_t)ns * Ge::ABUF; al();
+  s.LF = (double*)(base + off); off += sizeof(double) * 2 * Ge::KSH * 32; al();
   s.pm = (double*)(base + off); off += sizeof(double) * ns * (N + 2) * 4; al();
   s.acc = (double*)(base + off); off += sizeof(double) * ns * BG_NSMAX; al();
   s.red = (double*)(base + off); off += sizeof(double) * ns * 8; al();
@@ -613,6 +629,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
   const long long ngroups = (nev + ns - 1) / ns;
   // once per CTA: zero both amplitude buffers (their padding rows are never written again)
   for (int t = threadIdx.x; t < 2 * ns * (int)Ge::ABUF; t += NTH) s.A[t] = 0.0;
+  for (int t = threadIdx.x; t < 2 * Ge::KSH * 32; t += NTH) s.LF[t] = __ldg(D.lfrag + t);
   __syncthreads();
   if (threadIdx.x < NWT) {
     // =========================================================================================== worker warps
@@ -752,15 +769,24 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
               double acc[Ge::NT][2];
 #pragma unroll
               for (int nt = 0; nt < Ge::NT; nt++) { acc[nt][0] = 0.0; acc[nt][1] = 0.0; }
-              const double* F = D.lfrag + (size_t)(h * Ge::KSH + mt * Ge::KTH - mt * (mt - 1)) * 32 + lane;
-              int nk = Ge::KTH - 2 * mt;
-              double a0 = __ldg(F), a1 = (nk > 1) ? __ldg(F + 32) : 0.0;
-              for (int kk = 0; kk < nk; kk++) {
-                double an = (kk + 2 < nk) ? __ldg(F + (kk + 2) * 32) : 0.0;
-                const double* Br = A + (size_t)(4 * (2 * mt + kk)) * Ge::ASTR;
+              const double* F = s.LF + (h * Ge::KSH + mt * Ge::KTH - mt * (mt - 1)) * 32 + lane;
+              const int nk = Ge::KTH - 2 * mt;
+              const double* Br = A + (size_t)(8 * mt) * Ge::ASTR;
+              // operands of k-step kk + 1 are fetched from shared memory while the mma of k-step kk issue
+              double a_cur = F[0], b_cur[Ge::NT];
 #pragma unroll
-                for (int nt = 0; nt < Ge::NT; nt++) dmma884(acc[nt][0], acc[nt][1], a0, Br[8 * nt]);
-                a0 = a1; a1 = an;
+              for (int nt = 0; nt < Ge::NT; nt++) b_cur[nt] = Br[8 * nt];
+#pragma unroll 2
+              for (int kk = 0; kk < nk; kk++) {
+                const int kn = (kk + 1 < nk) ? kk + 1 : kk;
+                const double a_nxt = F[kn * 32]; double b_nxt[Ge::NT];
+#pragma unroll
+                for (int nt = 0; nt < Ge::NT; nt++) b_nxt[nt] = Br[(size_t)(4 * kn) * Ge::ASTR + 8 * nt];
+#pragma unroll
+                for (int nt = 0; nt < Ge::NT; nt++) dmma884(acc[nt][0], acc[nt][1], a_cur, b_cur[nt]);
+                a_cur = a_nxt;
+#pragma unroll
+                for (int nt = 0; nt < Ge::NT; nt++) b_cur[nt] = b_nxt[nt];
               }
 #pragma unroll
               for (int nt = 0; nt < Ge::NT; nt++) { part = fma(acc[nt][0], acc[nt][0], part); part = fma(acc[nt][1], acc[nt][1], part); }
@@ -826,7 +852,7 @@ static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::stri
   const BgSched& S = B->S;
   BgDev& D = B->D;
   D.nwords = (int)S.words.size(); D.offF = S.offF; D.dbg = nullptr;
-  bool ok = (S.nG == c_nG(n) && S.nR == c_nQ(n, S.rmax) && S.nL == c_nQ(n, S.lmax) && S.npair == S.nperm / 2);
+  bool ok = (S.nG == c_nG(n) && S.nR == c_nR(n) && S.nL == c_nL(n) && S.npair == S.nperm / 2);
   for (int m = 2; m <= n - 1; m++) ok = ok && S.ntask[0][m] == c_ntaskG(n, m);
   for (int m = 1; m <= S.rmax; m++) ok = ok && S.ntask[1][m + 1] == c_ntaskQ(n, m);
   for (int m = 1; m <= S.lmax; m++) ok = ok && S.ntask[2][m + 1] == c_ntaskQ(n, m);
