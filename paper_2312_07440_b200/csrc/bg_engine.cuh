@@ -35,6 +35,18 @@
 
 namespace rwgt {
 
+// Diagnostic build only (python -m paper_2312_07440_b200.experiments; never defined for librwgt.so): run-time switches that
+// REMOVE parts of the engine to time the rest.  Results are wrong by construction.  c_exp = {table-entry multiplier (0: every
+// table load reads entry 0, i.e. a conflict-free broadcast), skip colour mma, skip current levels, skip amplitude tasks}.
+#ifdef RWGT_EXPERIMENT
+__constant__ int c_exp[4] = {1, 0, 0, 0};
+#define RWGT_EXP_ENTRY(e) ((e) * c_exp[0])
+#define RWGT_EXP_SKIP(i) (c_exp[i] != 0)
+#else
+#define RWGT_EXP_ENTRY(e) (e)
+#define RWGT_EXP_SKIP(i) false
+#endif
+
 // ------------------------------------------------------------------------------------------------ host: colour matrix
 // C_{ss'} = sum_a Tr(T^{a_s1}..T^{a_sn} T^{a_s'n}..T^{a_s'1}) by repeated use of the SU(N) Fierz identity
 //   T^a_ij T^a_kl = 1/2 (d_il d_jk - 1/N d_ij d_kl), exact integers over (2N)^n.  (Independent of the oracle's
@@ -389,13 +401,13 @@ template <int N, typename T> __host__ __device__ inline size_t carve(Smem<T>& s,
 }
 
 template <typename T> __device__ __forceinline__ vec4<T> ld4(const cx<T>* tab, int stride, int e) {
-  vec4<T> r;
+  vec4<T> r; e = RWGT_EXP_ENTRY(e);
 #pragma unroll
   for (int c = 0; c < 4; c++) r.c[c] = ldc(tab + c * stride + e);
   return r;
 }
 template <typename T> __device__ __forceinline__ spn<T> lds4(const cx<T>* tab, int stride, int e) {
-  spn<T> r;
+  spn<T> r; e = RWGT_EXP_ENTRY(e);
 #pragma unroll
   for (int c = 0; c < 4; c++) r.c[c] = ldc(tab + c * stride + e);
   return r;
@@ -493,7 +505,7 @@ template <int N, int M, typename T, int NWT> __device__ __forceinline__ void lev
   const Smem<T>& s = c.s; constexpr int nG = Ge::NG, nR = Ge::NR, nL = Ge::NL, next = N + 2;
   const int ns = c.ns, nGt = ns * tg, nRt = ns * tr, nLt = ns * tl;
   const uint32_t* TL = s.W + c.D->offT[M];
-  for (int t = c.tid; t < nGt + nRt + nLt; t += NWT) {
+  for (int t = c.tid; t < nGt + nRt + nLt && !RWGT_EXP_SKIP(2); t += NWT) {
     if (HASG && t < nGt) {
      if constexpr (HASG) {
       int sl = t / tg, o = t - sl * tg; uint32_t tw = TL[o]; uint32_t v = tw >> 16;
@@ -696,7 +708,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
           if (step >= 2) bar_sync(BAR_EMPTY0 + buf, NTH);      // colour warps have finished reading this buffer
           double* Abuf = s.A + (size_t)buf * ns * Ge::ABUF;
           constexpr int per = Ge::NPAIR * Ge::NFREE;
-          for (int t = tid; t < ns * per; t += NWT) {
+          for (int t = tid; t < ns * per && !RWGT_EXP_SKIP(3); t += NWT) {
             int sl = t / per, o = t - sl * per; int pair = o / Ge::NFREE, f = o % Ge::NFREE;
             const cx<T>* G = s.G + (size_t)sl * 4 * nG; const cx<T>* R = s.R + (size_t)sl * 4 * nR; const cx<T>* L = s.L + (size_t)sl * 4 * nL;
             const T* K = s.K + (size_t)sl * Ge::NMASK * 4;
@@ -758,7 +770,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
           bar_sync(BAR_FULL0 + buf, NTH);                      // the workers have filled this buffer
           const double* Abuf = s.A + (size_t)buf * ns * Ge::ABUF;
           // a5: Z = L^T A with FP64 tensor-core mma over the upper-triangular tiles, colour form = sum of squares of Z
-          for (int u = cwarp; u < ns * Ge::U; u += NCW) {
+          for (int u = cwarp; u < ns * Ge::U && !RWGT_EXP_SKIP(1); u += NCW) {
             int sl = u / Ge::U, unit = u % Ge::U; const int h = unit / Ge::UH, uu = unit % Ge::UH;     // h: 0 = u rows / L+, 1 = v rows / L-
             const double* A = Abuf + (size_t)sl * Ge::ABUF + (size_t)(h * Ge::NHK + (lane & 3)) * Ge::ASTR + (lane >> 2);
             double part = 0.0;
@@ -910,6 +922,9 @@ static double bg_tensor_flops_per_event(const BgProcess* B) {
 
 static int bg_run(BgProcess* B, int precision, const double* mom, const double* w, double* a, double* b, double* o, long long nev, long long stride, long long ostride, cudaStream_t st) {
   BgDev D = B->D; const bool dbl = (precision == RWGT_FP64);
+#ifdef RWGT_EXPERIMENT
+  { const char* v = getenv("RWGT_EXP"); int f = v ? atoi(v) : 0; int h[4] = {(f & 1) ? 0 : 1, (f >> 1) & 1, (f >> 2) & 1, (f >> 3) & 1}; cudaMemcpyToSymbol(c_exp, h, sizeof(h)); }
+#endif
   D.nslot = dbl ? B->nslot64 : B->nslot32;
   long long ngroups = (nev + D.nslot - 1) / D.nslot; int grid = (int)std::min<long long>(ngroups, B->sm_count);
   switch (B->S.n) {

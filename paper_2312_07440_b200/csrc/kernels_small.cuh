@@ -33,7 +33,7 @@ __device__ __forceinline__ vec4<double> bilinear2(const cx<double>* a, const cx<
 
 // Massless leptons: only the 4 helicity combinations with opposite helicities on each fermion line
 // are non-zero (tests check the oracle's full 16-term sum against this, reading Q5).
-__global__ void __launch_bounds__(256) epem_mupmum_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
+__global__ void __launch_bounds__(256, 3) epem_mupmum_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
                                                           double* __restrict__ me_old, double* __restrict__ me_new,
                                                           double* __restrict__ w_new, long long n, long long stride, long long ostride, EpemParams P) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
