@@ -25,16 +25,51 @@ template <typename T> __device__ __forceinline__ void cfma(cx<T>& acc, cx<T> a, 
 }
 // acc += s*a  (2 FMA), s real
 template <typename T> __device__ __forceinline__ void rfma(cx<T>& acc, T s, cx<T> a) { acc.re = fma(s, a.re, acc.re); acc.im = fma(s, a.im, acc.im); }
+// acc -= a*b,  acc -= s*a   (the same instruction sequences as cfma(acc, -a, b), rfma(acc, -s, a))
+template <typename T> __device__ __forceinline__ void cfms(cx<T>& acc, cx<T> a, cx<T> b) { cfma(acc, -a, b); }
+template <typename T> __device__ __forceinline__ void rfms(cx<T>& acc, T s, cx<T> a) { rfma(acc, -s, a); }
+
+// ---- FP32: packed two-lane arithmetic (PTX fma/mul/add.rn.f32x2 = SASS FFMA2/FMUL2/FADD2 on sm_100a) -------------------
+// A complex float is an aligned (re, im) register pair.  A complex multiply-add is TWO FFMA2:
+//     acc += b * a.re ;  acc += (-b.im, b.re) * a.im
+// ptxas folds the lane swap, the per-lane negation and the scalar broadcast into operand modifiers of FFMA2
+// (R.F32x2.LO_HI.NP, R.F32) when the swapped/negated pair is the FIRST source and the broadcast the second, so no
+// packing instruction is issued (checked with cuobjdump -sass).  Measured on B200 with three distinct register sources:
+// FFMA 42 TFLOP/s, FFMA2 50-67 TFLOP/s, and half the issue slots.
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi) { f32x2 r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(lo), "f"(hi)); return r; }
+__device__ __forceinline__ cx<float> upk2(f32x2 v) { cx<float> r; asm("mov.b64 {%0,%1}, %2;" : "=f"(r.re), "=f"(r.im) : "l"(v)); return r; }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) { f32x2 d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b) { f32x2 d; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) { f32x2 d; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b)); return d; }
+__device__ __forceinline__ void cfma(cx<float>& acc, cx<float> a, cx<float> b) {
+  f32x2 A = pk2(acc.re, acc.im);
+  A = fma2(pk2(b.re, b.im), pk2(a.re, a.re), A); A = fma2(pk2(-b.im, b.re), pk2(a.im, a.im), A);
+  acc = upk2(A);
+}
+__device__ __forceinline__ void cfms(cx<float>& acc, cx<float> a, cx<float> b) {
+  f32x2 A = pk2(acc.re, acc.im);
+  A = fma2(pk2(-b.re, -b.im), pk2(a.re, a.re), A); A = fma2(pk2(b.im, -b.re), pk2(a.im, a.im), A);
+  acc = upk2(A);
+}
+__device__ __forceinline__ void rfma(cx<float>& acc, float s, cx<float> a) { acc = upk2(fma2(pk2(a.re, a.im), pk2(s, s), pk2(acc.re, acc.im))); }
+__device__ __forceinline__ void rfms(cx<float>& acc, float s, cx<float> a) { acc = upk2(fma2(pk2(-a.re, -a.im), pk2(s, s), pk2(acc.re, acc.im))); }
+__device__ __forceinline__ cx<float> operator*(cx<float> a, cx<float> b) {
+  f32x2 A = mul2(pk2(b.re, b.im), pk2(a.re, a.re)); return upk2(fma2(pk2(-b.im, b.re), pk2(a.im, a.im), A));
+}
+__device__ __forceinline__ cx<float> operator*(float s, cx<float> a) { return upk2(mul2(pk2(a.re, a.im), pk2(s, s))); }
+__device__ __forceinline__ cx<float> operator+(cx<float> a, cx<float> b) { return upk2(add2(pk2(a.re, a.im), pk2(b.re, b.im))); }
+__device__ __forceinline__ cx<float> operator-(cx<float> a, cx<float> b) { return upk2(add2(pk2(a.re, a.im), pk2(-b.re, -b.im))); }
 
 template <typename T> struct vec4 { cx<T> c[4]; };   // complex Lorentz vector, contravariant (t,x,y,z)
 template <typename T> struct spn { cx<T> c[4]; };    // Dirac spinor, chiral representation
 
 template <typename T> __device__ __forceinline__ T mdot_rr(const T* a, const T* b) { return a[0] * b[0] - a[1] * b[1] - a[2] * b[2] - a[3] * b[3]; }
 template <typename T> __device__ __forceinline__ cx<T> mdot_rc(const T* a, const vec4<T>& b) {
-  cx<T> r = a[0] * b.c[0]; rfma(r, -a[1], b.c[1]); rfma(r, -a[2], b.c[2]); rfma(r, -a[3], b.c[3]); return r;
+  cx<T> r = a[0] * b.c[0]; rfms(r, a[1], b.c[1]); rfms(r, a[2], b.c[2]); rfms(r, a[3], b.c[3]); return r;
 }
 template <typename T> __device__ __forceinline__ cx<T> mdot_cc(const vec4<T>& a, const vec4<T>& b) {
-  cx<T> r = a.c[0] * b.c[0]; cfma(r, -a.c[1], b.c[1]); cfma(r, -a.c[2], b.c[2]); cfma(r, -a.c[3], b.c[3]); return r;
+  cx<T> r = a.c[0] * b.c[0]; cfms(r, a.c[1], b.c[1]); cfms(r, a.c[2], b.c[2]); cfms(r, a.c[3], b.c[3]); return r;
 }
 
 // a-slash * psi, a complex
@@ -43,8 +78,8 @@ template <typename T> __device__ __forceinline__ spn<T> slash_c(const vec4<T>& a
   cx<T> ar = mk<T>(a.c[1].re + a.c[2].im, a.c[1].im - a.c[2].re);   // a1 - i a2
   cx<T> al = mk<T>(a.c[1].re - a.c[2].im, a.c[1].im + a.c[2].re);   // a1 + i a2
   spn<T> r;
-  r.c[0] = am * s.c[2]; cfma(r.c[0], -ar, s.c[3]);
-  r.c[1] = ap * s.c[3]; cfma(r.c[1], -al, s.c[2]);
+  r.c[0] = am * s.c[2]; cfms(r.c[0], ar, s.c[3]);
+  r.c[1] = ap * s.c[3]; cfms(r.c[1], al, s.c[2]);
   r.c[2] = ap * s.c[0]; cfma(r.c[2], ar, s.c[1]);
   r.c[3] = am * s.c[1]; cfma(r.c[3], al, s.c[0]);
   return r;
@@ -54,8 +89,8 @@ template <typename T> __device__ __forceinline__ spn<T> slash_r_plus_m(const T* 
   T qp = q[0] + q[3], qm = q[0] - q[3];
   cx<T> qr = mk<T>(q[1], -q[2]), ql = mk<T>(q[1], q[2]);
   spn<T> r;
-  r.c[0] = m * s.c[0]; rfma(r.c[0], qm, s.c[2]); cfma(r.c[0], -qr, s.c[3]);
-  r.c[1] = m * s.c[1]; rfma(r.c[1], qp, s.c[3]); cfma(r.c[1], -ql, s.c[2]);
+  r.c[0] = m * s.c[0]; rfma(r.c[0], qm, s.c[2]); cfms(r.c[0], qr, s.c[3]);
+  r.c[1] = m * s.c[1]; rfma(r.c[1], qp, s.c[3]); cfms(r.c[1], ql, s.c[2]);
   r.c[2] = m * s.c[2]; rfma(r.c[2], qp, s.c[0]); cfma(r.c[2], qr, s.c[1]);
   r.c[3] = m * s.c[3]; rfma(r.c[3], qm, s.c[1]); cfma(r.c[3], ql, s.c[0]);
   return r;
@@ -68,8 +103,8 @@ template <typename T> __device__ __forceinline__ spn<T> row_slash_c(const spn<T>
   spn<T> r;   // r_j = sum_i w_i A_ij ; A = [[0,0,am,-ar],[0,0,-al,ap],[ap,ar,0,0],[al,am,0,0]]
   r.c[0] = w.c[2] * ap; cfma(r.c[0], w.c[3], al);
   r.c[1] = w.c[2] * ar; cfma(r.c[1], w.c[3], am);
-  r.c[2] = w.c[0] * am; cfma(r.c[2], -w.c[1], al);
-  r.c[3] = w.c[1] * ap; cfma(r.c[3], -w.c[0], ar);
+  r.c[2] = w.c[0] * am; cfms(r.c[2], w.c[1], al);
+  r.c[3] = w.c[1] * ap; cfms(r.c[3], w.c[0], ar);
   return r;
 }
 // row * (q-slash + m), q real
@@ -79,8 +114,8 @@ template <typename T> __device__ __forceinline__ spn<T> row_slash_r_plus_m(const
   spn<T> r;
   r.c[0] = m * w.c[0]; rfma(r.c[0], qp, w.c[2]); cfma(r.c[0], w.c[3], ql);
   r.c[1] = m * w.c[1]; rfma(r.c[1], qm, w.c[3]); cfma(r.c[1], w.c[2], qr);
-  r.c[2] = m * w.c[2]; rfma(r.c[2], qm, w.c[0]); cfma(r.c[2], -w.c[1], ql);
-  r.c[3] = m * w.c[3]; rfma(r.c[3], qp, w.c[1]); cfma(r.c[3], -w.c[0], qr);
+  r.c[2] = m * w.c[2]; rfma(r.c[2], qm, w.c[0]); cfms(r.c[2], w.c[1], ql);
+  r.c[3] = m * w.c[3]; rfma(r.c[3], qp, w.c[1]); cfms(r.c[3], w.c[0], qr);
   return r;
 }
 template <typename T> __device__ __forceinline__ cx<T> rowcol(const spn<T>& w, const spn<T>& s) {
@@ -170,8 +205,8 @@ template <typename T> __device__ __forceinline__ lcv<T> lightcone_neg(const vec4
 }
 // X += a-slash * s      (8 complex FMAs)
 template <typename T> __device__ __forceinline__ void slash_acc(spn<T>& X, const lcv<T>& a, const spn<T>& s) {
-  cfma(X.c[0], a.m, s.c[2]); cfma(X.c[0], -a.r, s.c[3]);
-  cfma(X.c[1], a.p, s.c[3]); cfma(X.c[1], -a.l, s.c[2]);
+  cfma(X.c[0], a.m, s.c[2]); cfms(X.c[0], a.r, s.c[3]);
+  cfma(X.c[1], a.p, s.c[3]); cfms(X.c[1], a.l, s.c[2]);
   cfma(X.c[2], a.p, s.c[0]); cfma(X.c[2], a.r, s.c[1]);
   cfma(X.c[3], a.m, s.c[1]); cfma(X.c[3], a.l, s.c[0]);
 }
@@ -179,8 +214,8 @@ template <typename T> __device__ __forceinline__ void slash_acc(spn<T>& X, const
 template <typename T> __device__ __forceinline__ void row_slash_acc(spn<T>& X, const spn<T>& w, const lcv<T>& a) {
   cfma(X.c[0], w.c[2], a.p); cfma(X.c[0], w.c[3], a.l);
   cfma(X.c[1], w.c[2], a.r); cfma(X.c[1], w.c[3], a.m);
-  cfma(X.c[2], w.c[0], a.m); cfma(X.c[2], -w.c[1], a.l);
-  cfma(X.c[3], w.c[1], a.p); cfma(X.c[3], -w.c[0], a.r);
+  cfma(X.c[2], w.c[0], a.m); cfms(X.c[2], w.c[1], a.l);
+  cfma(X.c[3], w.c[1], a.p); cfms(X.c[3], w.c[0], a.r);
 }
 // acc += w . s
 template <typename T> __device__ __forceinline__ void rowcol_acc(cx<T>& acc, const spn<T>& w, const spn<T>& s) {
