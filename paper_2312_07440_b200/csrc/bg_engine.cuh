@@ -438,8 +438,20 @@ __device__ __forceinline__ uint32_t halfw(const uint32_t* w, int k) { return (k 
 // named barriers (ids 1..6; id 0 is __syncthreads): workers among themselves, colour warps among themselves,
 // and the full/empty handshake of the two amplitude buffers
 enum { BAR_WORK = 1, BAR_FULL0 = 2, BAR_EMPTY0 = 4, BAR_COLOUR = 6 };
-__device__ __forceinline__ void bar_sync(int id, int count) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(count) : "memory"); }
-__device__ __forceinline__ void bar_arrive(int id, int count) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(count) : "memory"); }
+// the barrier id is an immediate (a register id makes ptxas reserve all 16 barriers, which limits the CTAs per SM)
+__device__ __forceinline__ void bar_sync(int id, int count) {
+  switch (id) {
+    case 1: asm volatile("bar.sync 1, %0;" ::"r"(count) : "memory"); break; case 2: asm volatile("bar.sync 2, %0;" ::"r"(count) : "memory"); break;
+    case 3: asm volatile("bar.sync 3, %0;" ::"r"(count) : "memory"); break; case 4: asm volatile("bar.sync 4, %0;" ::"r"(count) : "memory"); break;
+    case 5: asm volatile("bar.sync 5, %0;" ::"r"(count) : "memory"); break; default: asm volatile("bar.sync 6, %0;" ::"r"(count) : "memory");
+  }
+}
+__device__ __forceinline__ void bar_arrive(int id, int count) {
+  switch (id) {
+    case 2: asm volatile("bar.arrive 2, %0;" ::"r"(count) : "memory"); break; case 3: asm volatile("bar.arrive 3, %0;" ::"r"(count) : "memory"); break;
+    case 4: asm volatile("bar.arrive 4, %0;" ::"r"(count) : "memory"); break; default: asm volatile("bar.arrive 5, %0;" ::"r"(count) : "memory");
+  }
+}
 
 // gluon current of one ordered M-tuple / helicity variant from shorter currents (unscaled by the propagator).
 // w: the 2(M-1) + 3(M-1)(M-2)/2 reference words of the tuple, in registers.  No signs: every block is stored as used.
@@ -624,14 +636,16 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 // batch after the other on the FP64 pipe; the last NCW warps ("colour") turn finished batches into |L^T J|^2 on the FP64
 // tensor pipe (a separate pipe, so the two overlap) and write the outputs.  The two amplitude buffers are handed over with
 // named barriers.  MIXED: T = float but momentum sums / propagator denominators are formed in double before rounding to T.
-template <int N, typename T, bool MIXED, int NW, int NCW>
-__global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
+template <int N, typename T, bool MIXED, int NW, int NCW, int CTAS>
+__global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
                                                                double* __restrict__ me_old, double* __restrict__ me_new,
                                                                double* __restrict__ w_new, long long nev, long long stride, long long ostride, BgDev D) {
   typedef Geo<N> Ge;
   constexpr int NTH = (NW + NCW) * 32, NWT = NW * 32, NCT = NCW * 32;
   // register hand-over between the warpgroups: the colour warps need few registers, the workers get the rest
-  constexpr int REG_COL = 56, REG_WORK = ((65536 / 32 - NCW * REG_COL) / NW) / 8 * 8 > 232 ? 232 : ((65536 / 32 - NCW * REG_COL) / NW) / 8 * 8;
+  // (setmaxnreg is a warpgroup instruction: both groups must be whole warpgroups of 4 warps)
+  constexpr bool HANDOVER = sizeof(T) == 8 && NW % 4 == 0 && NCW % 4 == 0;
+  constexpr int REG_COL = 56, REG_POOL = 65536 / 32 / CTAS, REG_WORK = ((REG_POOL - NCW * REG_COL) / NW) / 8 * 8 > 232 ? 232 : ((REG_POOL - NCW * REG_COL) / NW) / 8 * 8;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Ctx<T> c; c.D = &D; c.ns = D.nslot;
   carve<N, T>(c.s, smem_raw, D.nslot, D.nwords);
@@ -645,7 +659,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
   __syncthreads();
   if (threadIdx.x < NWT) {
     // =========================================================================================== worker warps
-    if constexpr (sizeof(T) == 8) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REG_WORK));
+    if constexpr (HANDOVER) asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REG_WORK));
     const int tid = threadIdx.x; c.tid = tid;
     for (int t = tid; t < D.nwords; t += NWT) s.W[t] = __ldg(D.words + t);
     unsigned step = 0;
@@ -755,7 +769,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, 1) bg_kernel(const double* __
     }
   } else {
     // =========================================================================================== colour warps
-    if constexpr (sizeof(T) == 8) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REG_COL));
+    if constexpr (HANDOVER) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REG_COL));
     const int ctid = threadIdx.x - NWT, cwarp = ctid >> 5, lane = ctid & 31;
     unsigned step = 0;
     for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
@@ -839,22 +853,27 @@ template <int N> static size_t smem_need(const BgSched& S, int nslot, bool dbl) 
 static size_t smem_need_n(int n, const BgSched& S, int nslot, bool dbl) {
   switch (n) { case 2: return smem_need<2>(S, nslot, dbl); case 3: return smem_need<3>(S, nslot, dbl); case 4: return smem_need<4>(S, nslot, dbl); default: return smem_need<5>(S, nslot, dbl); }
 }
-// Warp split: 8 worker warps (FP64 pipe) + 4 colour warps (FP64 tensor pipe) = 3 warps x 168 registers per SM sub-partition
-// (16K registers each).  Measured on B200 against 10+2, 6+2 and 12+4: best or within 4% of best for every process.
-static const int BG_NW = 8, BG_NCW = 4;
+// Warp split: one CTA per SM, 8 worker warps (FP64 / FP32 pipe) + 4 colour warps (DMMA) = 3 warps x 168 registers per SM
+// sub-partition.  Measured on B200 against 10+2, 6+2, 12+4 and (n = 3) two CTAs of 4+2 warps per SM: best or within 4 % of best
+// for every process.  (The kernel is parametrised on the split and on the CTAs per SM.)
+template <int N> struct BgCfg { static constexpr int NW = 8, NCW = 4, CTAS = 1; };
+static int bg_nw(int n) { return n <= 3 ? BgCfg<3>::NW : BgCfg<5>::NW; }
+static int bg_ctas(int n) { return n <= 3 ? BgCfg<3>::CTAS : BgCfg<5>::CTAS; }
 
 template <int N> static cudaError_t bg_set_attr(size_t s64, size_t s32) {
-  cudaError_t e = cudaFuncSetAttribute(bg_kernel<N, double, false, BG_NW, BG_NCW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s64);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, false, BG_NW, BG_NCW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, true, BG_NW, BG_NCW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
+  typedef BgCfg<N> Cf;
+  cudaError_t e = cudaFuncSetAttribute(bg_kernel<N, double, false, Cf::NW, Cf::NCW, Cf::CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s64);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, false, Cf::NW, Cf::NCW, Cf::CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, true, Cf::NW, Cf::NCW, Cf::CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
   return e;
 }
 template <int N> static void bg_launch(int precision, int grid, size_t s64, size_t s32, cudaStream_t st, const double* mom, const double* w,
                                        double* a, double* b, double* o, long long nev, long long stride, long long ostride, const BgDev& D) {
-  const int nth = (BG_NW + BG_NCW) * 32;
-  if (precision == RWGT_FP64) bg_kernel<N, double, false, BG_NW, BG_NCW><<<grid, nth, s64, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
-  else if (precision == RWGT_FP32) bg_kernel<N, float, false, BG_NW, BG_NCW><<<grid, nth, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
-  else bg_kernel<N, float, true, BG_NW, BG_NCW><<<grid, nth, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
+  typedef BgCfg<N> Cf;
+  const int nth = (Cf::NW + Cf::NCW) * 32;
+  if (precision == RWGT_FP64) bg_kernel<N, double, false, Cf::NW, Cf::NCW, Cf::CTAS><<<grid, nth, s64, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
+  else if (precision == RWGT_FP32) bg_kernel<N, float, false, Cf::NW, Cf::NCW, Cf::CTAS><<<grid, nth, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
+  else bg_kernel<N, float, true, Cf::NW, Cf::NCW, Cf::CTAS><<<grid, nth, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
 }
 
 static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::string& err) {
@@ -885,8 +904,10 @@ static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::stri
   B->sm_count = prop.multiProcessorCount; size_t maxsm = prop.sharedMemPerBlockOptin;
   // event slots per CTA: as many as make the amplitude phase fill the 256 worker threads (npair * 4 tasks per slot and batch)
   auto pick = [&](bool dbl, int& nslot, size_t& bytes) {
-    int cap = std::max(1, std::min(64, (BG_NW * 32) / (S.npair * (n == 2 ? 2 : 4)))); nslot = 0;
-    for (int e = cap; e >= 1; e--) if (smem_need_n(n, S, e, dbl) <= maxsm) { nslot = e; break; }
+    int cap = std::max(1, std::min(64, (bg_nw(n) * 32) / (S.npair * (n == 2 ? 2 : 4)))); nslot = 0;
+    // with k CTAs per SM each gets 1/k of the SM's shared memory (1 KB per CTA is reserved by the system)
+    size_t budget = std::min(maxsm, prop.sharedMemPerMultiprocessor / bg_ctas(n) - 1024);
+    for (int e = cap; e >= 1; e--) if (smem_need_n(n, S, e, dbl) <= budget) { nslot = e; break; }
     bytes = nslot ? smem_need_n(n, S, nslot, dbl) : 0;
   };
   pick(true, B->nslot64, B->smem64); pick(false, B->nslot32, B->smem32);
@@ -926,7 +947,7 @@ static int bg_run(BgProcess* B, int precision, const double* mom, const double* 
   { const char* v = getenv("RWGT_EXP"); int f = v ? atoi(v) : 0; int h[4] = {(f & 1) ? 0 : 1, (f >> 1) & 1, (f >> 2) & 1, (f >> 3) & 1}; cudaMemcpyToSymbol(c_exp, h, sizeof(h)); }
 #endif
   D.nslot = dbl ? B->nslot64 : B->nslot32;
-  long long ngroups = (nev + D.nslot - 1) / D.nslot; int grid = (int)std::min<long long>(ngroups, B->sm_count);
+  long long ngroups = (nev + D.nslot - 1) / D.nslot; int grid = (int)std::min<long long>(ngroups, (long long)B->sm_count * bg_ctas(B->S.n));
   switch (B->S.n) {
     case 2: bg_launch<2>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, ostride, D); break;
     case 3: bg_launch<3>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, ostride, D); break;
