@@ -29,6 +29,7 @@ def lib():
         L.orc_jamps.argtypes = [C.c_int, _dp, _dp, _ip, _dp, _dp]
         L.orc_me2_hel.argtypes = [C.c_int, _dp, _dp, _ip, C.c_int, _dp]
         L.orc_amp_epem.argtypes = [_dp, _dp, _ip, _dp]
+        L.orc_amp_epem_ng.argtypes = [C.c_int, _dp, _dp, _ip, _dp, _dp]
         L.orc_denominator.argtypes = [C.c_int]
         L.orc_denominator.restype = C.c_double
         _lib = L
@@ -143,3 +144,18 @@ def amp_epem(par, p, hel) -> complex:
 
 def denominator(n: int) -> float:
     return lib().orc_denominator(n)
+
+
+def amp_epem_ng(n: int, par, p, hel, eps_override=None) -> complex:
+    """Helicity amplitude iM of e+ e- -> n photons (PAPER.md:72-77 for n = 5); p[n+2,4], hel[n+2] = +-1."""
+    par, pp = _d(par)
+    p, ppp = _d(p)
+    hel, ph = _i(hel)
+    out = np.empty(2)
+    if eps_override is not None:
+        eo = np.ascontiguousarray(eps_override, dtype=np.complex128).reshape(n, 4)
+        peo = eo.view(np.float64).ctypes.data_as(_dp)
+    else:
+        peo = None
+    lib().orc_amp_epem_ng(n, pp, ppp, ph, peo, out.ctypes.data_as(_dp))
+    return complex(out[0], out[1])

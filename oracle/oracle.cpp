@@ -21,6 +21,10 @@
 // rotation invariance for the new set; route F == route E (explicit 8^n colour sum, uses
 // f^{abc} instead of colour strings) at n=2,3 (+ a few helicities at n=4); colour-matrix
 // table SURVEY C7; polynomial degree 2(n-1) in kappa; worked values SURVEY C10.
+// e+ e- -> n photons (n = 2..5; n = 5 is the paper's own measured process): pinned in
+// tests/test_oracle_pins_photons.py by the textbook closed forms at n = 2, 3, the soft-photon theorem linking n + 1 to n up to
+// n = 5, gauge invariance eps -> k of every helicity amplitude, boost/rotation invariance, helicity selection rules and the
+// exact (alpha'/alpha)^n scaling.
 // PARITY UNPINNED (stated in DESIGN.md): absolute normalisation 1/(n-2)! of cfgs 4,5 and
 // the explicit-colour check of all helicities at n=5 (too slow).
 //
@@ -453,6 +457,54 @@ static double me2_hel_E(const Kin& k) {
   return total;
 }
 
+
+// ---------------------------------------------------------------- e+(p1) e-(p2) -> n photons  (Table 1: the paper's own
+// measured process is e+ e- -> 5 gamma).  Plain definition: the sum of the n! Feynman diagrams, one per order in
+// which the photons leave the electron line (SM, massless electron: no other tree diagram exists):
+//   iM = sum_perm vbar(p1) (i e eps-slash*_{sn}) S(q_{n-1}) ... S(q_1) (i e eps-slash*_{s1}) u(p2),   q_j = p2 - k_{s1} - .. - k_{sj},
+// with the rules of SURVEY C3: lepton-photon vertex -i e Q gamma^mu (Q = -1), massless propagator S(q) = i q-slash / q^2,
+// outgoing photons carry eps* (SURVEY C2).  eps_override ([n][4] complex, used as given) serves the gauge test eps -> k.
+static cd amp_epem_ng(const Par& P, int n, const double* p /*[n+2][4]*/, const int* hel /*[n+2]*/, const cd* eps_override) {
+  const double e = std::sqrt(4.0 * PI * P.alpha_em), Q = -1.0;
+  Sp vb1 = bar(spinor_v(p, 0.0, hel[0])), u2 = spinor_u(p + 4, 0.0, hel[1]);
+  std::vector<M4> vert(n);
+  for (int i = 0; i < n; i++) {
+    V4 eps; if (eps_override) { for (int mu = 0; mu < 4; mu++) eps.c[mu] = eps_override[4 * i + mu]; } else eps = conjv(polvec(p + 4 * (i + 2), hel[i + 2]));
+    vert[i] = (-I_ * e * Q) * slash(eps);
+  }
+  std::vector<int> perm(n); for (int i = 0; i < n; i++) perm[i] = i;
+  cd tot = 0;
+  do {
+    Sp psi = u2; double q[4] = {p[4], p[5], p[6], p[7]};
+    for (int j = 0; j < n; j++) {
+      psi = vert[perm[j]] * psi;
+      if (j + 1 < n) {
+        const double* k = p + 4 * (perm[j] + 2); for (int mu = 0; mu < 4; mu++) q[mu] -= k[mu];
+        psi = (I_ / mink2(q)) * (slash(realv(q)) * psi);
+      }
+    }
+    tot += rowcol(vb1, psi);
+  } while (std::next_permutation(perm.begin(), perm.end()));
+  return tot;     // = iM
+}
+// averaged over the 2x2 initial helicities and divided by n! for the identical photons (reading Q3 applied to this process)
+static double me2_epem_ng(const Par& P, int n, const double* p) {
+  double sum = 0; int hel[8];
+  for (int h = 0; h < (1 << (n + 2)); h++) {          // full helicity sum
+    for (int i = 0; i < n + 2; i++) hel[i] = ((h >> i) & 1) ? 1 : -1;
+    sum += std::norm(amp_epem_ng(P, n, p, hel, nullptr));
+  }
+  double fact = 1; for (int i = 2; i <= n; i++) fact *= i;
+  return sum / (4.0 * fact);
+}
+static int process_n_photons(const char* proc) {
+  if (!std::strcmp(proc, "epem_aa")) return 2;
+  if (!std::strcmp(proc, "epem_aaa")) return 3;
+  if (!std::strcmp(proc, "epem_aaaa")) return 4;
+  if (!std::strcmp(proc, "epem_aaaaa")) return 5;
+  return -1;
+}
+
 // ---------------------------------------------------------------- process table
 static int process_n_gluons(const char* proc) {
   if (!std::strcmp(proc, "gg_ttx")) return 2;
@@ -461,9 +513,14 @@ static int process_n_gluons(const char* proc) {
   if (!std::strcmp(proc, "gg_ttxggg")) return 5;
   return -1;
 }
-static int process_n_ext(const char* proc) { if (!std::strcmp(proc, "epem_mupmum")) return 4; int n = process_n_gluons(proc); return n < 0 ? -1 : n + 2; }
+static int process_n_ext(const char* proc) {
+  if (!std::strcmp(proc, "epem_mupmum")) return 4;
+  int na = process_n_photons(proc); if (na > 0) return na + 2;
+  int n = process_n_gluons(proc); return n < 0 ? -1 : n + 2;
+}
 static double me2_any(const char* proc, const Par& P, const double* p) {
   if (!std::strcmp(proc, "epem_mupmum")) { double q[4][4]; std::memcpy(q, p, sizeof(q)); return me2_epem(P, q); }
+  int na = process_n_photons(proc); if (na > 0) return me2_epem_ng(P, na, p);
   return me2_qcd_F(process_n_gluons(proc), P, p);
 }
 
@@ -536,5 +593,11 @@ void orc_amp_epem(const double* par, const double* p, const int* hel, double* ou
   double q[4][4]; std::memcpy(q, p, sizeof(q)); cd a = amp_epem(par_from(par), q, hel); out2[0] = a.real(); out2[1] = a.imag();
 }
 double orc_denominator(int n) { return denom_qcd(n); }
+// helicity amplitude iM of e+ e- -> n photons for one helicity configuration; eps_override as in orc_jamps
+void orc_amp_epem_ng(int n, const double* par, const double* p, const int* hel, const double* eps_override, double* out2) {
+  std::vector<cd> ov;
+  if (eps_override) { ov.resize(4 * n); for (int i = 0; i < 4 * n; i++) ov[i] = cd(eps_override[2 * i], eps_override[2 * i + 1]); }
+  cd a = amp_epem_ng(par_from(par), n, p, hel, eps_override ? ov.data() : nullptr); out2[0] = a.real(); out2[1] = a.imag();
+}
 
 }  // extern "C"

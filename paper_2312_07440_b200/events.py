@@ -1,4 +1,4 @@
-"""Seeded synthetic event sets for the five BASELINE.json configs.
+"""Seeded synthetic event sets for the five BASELINE.json configs (+ the paper's own e+e- -> 5 gamma).
 
 This module is the ONLY code shared by the CPU oracle (tests / cpu_baseline) and
 the CUDA path.  It holds none of the method's arithmetic (no wavefunctions,
@@ -51,7 +51,7 @@ class Config:
     n_events: int
     sqrts: float
     final_masses: tuple   # masses of the final-state legs, in leg order
-    n_extra_gluons: int
+    n_extra_gluons: int   # number of trailing final-state legs the pT / Delta R cuts apply to
     dr_cut: bool
     seed: int
     params_old: np.ndarray
@@ -79,7 +79,21 @@ CONFIGS = (
     Config(5, "gg_ttxggg", 65536, 1500.0, (_MT, _MT, 0.0, 0.0, 0.0), 3, True, 20231207 + 5,
            params(), params(ggg_scale=1 + _KAPPA, gggg_scale=1 + _KAPPA),
            ("fp64", "fp32")),
+    # Not a BASELINE.json config: the process the paper itself measured (Table 1:
+    # e+ e- -> 5 gamma, SM, the electroweak coupling re-drawn per reweight iteration).
+    # 2^17 events stand in for the "10^5 events" of the paper's Fig. 3; sqrt(s) and the
+    # cuts are not stated in the paper: 500 GeV as cfg 1, every photon pT > 20 GeV and Delta R > 0.4.
+    Config(6, "epem_aaaaa", 131072, 500.0, (0.0,) * 5, 5, True, 20231207 + 6,
+           params(), params(alpha_em=1.0 / 128.0), ("fp64",)),
 )
+
+
+def photon_config(n_photons: int, n_events: int = 4096) -> Config:
+    """e+ e- -> n photons, n = 2..5 (n = 5 is config 6; the others are parity-test cases)."""
+    if n_photons == 5:
+        return dataclasses.replace(CONFIGS[5], n_events=n_events)
+    return Config(60 + n_photons, "epem_" + "a" * n_photons, n_events, 500.0, (0.0,) * n_photons,
+                  n_photons, True, 20231207 + 60 + n_photons, params(), params(alpha_em=1.0 / 128.0), ("fp64",))
 
 
 def config(index_or_process) -> Config:
