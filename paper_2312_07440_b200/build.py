@@ -8,7 +8,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "librwgt.so")
 LIB_EXP = os.path.join(HERE, "librwgt_exp.so")
 SOURCES = [os.path.join(CSRC, "rwgt_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("rwgt_math.cuh", "kernels_small.cuh", "bg_engine.cuh", "microbench.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, f) for f in ("rwgt_math.cuh", "kernels_small.cuh", "bg_engine.cuh", "photon_kernel.cuh", "microbench.cuh")] + [
     os.path.join(os.path.dirname(HERE), "include", "rwgt.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-shared", "--fmad=true"]

@@ -1,0 +1,200 @@
+// photon_kernel.cuh — e+(p1) e-(p2) -> NG photons, NG = 2..5, FP64 (NG = 5 is the process the paper itself measured:
+// PAPER.md:72-77, Table 1).  Steps a1-a7 of SURVEY 8(a) in one launch.
+//
+// What it evaluates: the sum of the NG! diagrams in which the photons leave the massless electron line in every order
+// (rules of SURVEY C3: vertex -i e Q gamma^mu, propagator i q-slash / q^2; outgoing photons carry eps*), squared, summed over
+// helicities, averaged (1/4 for the initial helicities, 1/NG! for the identical photons; reading R3), for every parameter set, and
+// eq. 3.  Only alpha_em enters, and only through the overall factor e^(2 NG): the currents are evaluated once with
+// unit coupling and each set multiplies the helicity sum by its own factor ("setting the electroweak coupling
+// constant to be a randomly determined non-zero value for each reweight iteration"; so |M'|^2/|M|^2 = (alpha'/alpha)^NG exactly).
+//
+// Algorithm (not the diagram sum): off-shell electron currents of photon SUBSETS with helicity recycling,
+//     psi_S = 1/q_S^2  q_S-slash  sum_{i in S} eps-slash*_i psi_{S \ i},   q_S = p2 - sum_{i in S} k_i,   psi_{} = u(p2, +),
+// one per subset S and helicity assignment of ITS photons (3^NG - 2^NG currents instead of NG! 2^NG diagram evaluations), then
+//     M(h) = vbar(p1, -) sum_i eps-slash*_i psi_{all \ i}.
+// Massless line in the chiral representation: u(p2,+) has lower components only, eps-slash maps lower -> upper with the 2x2 block
+// (eps0 - sigma.eps), q-slash maps upper -> lower with (q0 + sigma.q): every current is a TWO-component spinor.  The other electron
+// helicity follows from parity (|M_{-h}| = |M_h|, pinned on the oracle): x2.  Equal e+ and e- helicities give zero.
+//
+// B200 mapping: persistent CTAs; a CTA holds E events in shared memory (currents as two component planes of (re,im) pairs,
+// consecutive helicity variants in consecutive 16-byte words), a thread owns one (event, subset, helicity variant) task per level,
+// levels are separated by __syncthreads; the 2^NG final amplitudes of an event sit in consecutive lanes and are reduced by a fixed
+// shuffle tree (deterministic: equal parameter sets give W' = W bitwise).
+#pragma once
+#include <cuda_runtime.h>
+#include <cstdint>
+
+#include "../../include/rwgt.h"
+#include "rwgt_math.cuh"
+#include "kernels_small.cuh"
+#include "bg_engine.cuh"      // ldc / stc (vector loads of (re,im) pairs)
+
+namespace rwgt {
+
+struct PhotonParams { double fac[SMALL_NSMAX]; int nsets; };      // fac = 2 e^(2 NG) / (4 NG!)  per parameter set
+
+__host__ __device__ constexpr int ipow(int b, int e) { return e == 0 ? 1 : b * ipow(b, e - 1); }
+__host__ __device__ constexpr int binom(int n, int k) { return k == 0 ? 1 : binom(n - 1, k - 1) * n / k; }
+
+template <int NG> struct PhGeo {
+  static constexpr int NSUB = 1 << NG, NENT = ipow(3, NG) - NSUB;          // stored currents: every subset but the full one
+  static constexpr int NEXTOBJ = 2 * NG + 2 + NSUB;                        // external tasks per event
+  // doubles per event slot
+  static constexpr int O_PM = 0, O_EPS = O_PM + (NG + 2) * 4, O_Q = O_EPS + NG * 2 * 8, O_IQ2 = O_Q + NSUB * 4,
+                       O_W = O_IQ2 + NSUB, O_PSI = O_W + 4, SLOT = O_PSI + 4 * NENT;
+};
+
+template <int NG, int E, int NTH>
+__global__ void __launch_bounds__(NTH) epem_photons_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
+                                                           double* __restrict__ me_old, double* __restrict__ me_new,
+                                                           double* __restrict__ w_new, long long nev, long long stride, long long ostride,
+                                                           PhotonParams P) {
+  typedef PhGeo<NG> Ge;
+  constexpr int next = NG + 2, NSUB = Ge::NSUB, NENT = Ge::NENT;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  double* sm = reinterpret_cast<double*>(smem_raw);
+  __shared__ unsigned short s_off[NSUB];            // first entry of subset S
+  __shared__ unsigned char s_sub[NSUB];             // subsets ordered by (size, value)
+  __shared__ unsigned char s_lvl[NG + 2];           // s_sub index of the first subset of each size
+  const int tid = threadIdx.x;
+  if (tid == 0) {
+    int o = 0; for (int S = 0; S < NSUB; S++) { s_off[S] = (unsigned short)o; o += 1 << __popc(S); }
+    int j = 0; for (int k = 0; k <= NG; k++) { s_lvl[k] = (unsigned char)j; for (int S = 0; S < NSUB; S++) if (__popc(S) == k) s_sub[j++] = (unsigned char)S; }
+    s_lvl[NG + 1] = (unsigned char)j;
+  }
+  __syncthreads();
+  const long long ngroups = (nev + E - 1) / E;
+  for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+    const long long ev0 = grp * E;
+    // ---- a1: momenta (coalesced over the events of the group) ----
+    for (int t = tid; t < E * next * 4; t += NTH) {
+      int sl = t % E, comp = t / E; long long ev = ev0 + sl; if (ev >= nev) ev = nev - 1;
+      sm[sl * Ge::SLOT + Ge::O_PM + comp] = __ldg(mom + (size_t)comp * stride + ev);
+    }
+    __syncthreads();
+    // ---- a2: external wavefunctions, momenta and inverse virtualities of the electron line ----
+    for (int t = tid; t < E * Ge::NEXTOBJ; t += NTH) {
+      int sl = t / Ge::NEXTOBJ, o = t % Ge::NEXTOBJ; double* s = sm + sl * Ge::SLOT; const double* pm = s + Ge::O_PM;
+      if (o < 2 * NG) {                            // photon i, helicity bit hb (0: +1, 1: -1): the block (eps0 - sigma.eps*) = [[m, -r], [-l, p]]
+        int i = o >> 1, hb = o & 1; const double* k = pm + 4 * (i + 2);
+        lcv<double> a = lightcone(conj4(polvec<double>(k[1], k[2], k[3], hb ? -1 : +1)));
+        cx<double>* M = reinterpret_cast<cx<double>*>(s + Ge::O_EPS) + (i * 2 + hb) * 4;
+        M[0] = a.m; M[1] = -a.r; M[2] = -a.l; M[3] = a.p;
+      } else if (o == 2 * NG) {                    // psi_{} = lower components of u(p2, +)
+        const double* p = pm + 4; chi_pair<double> x = make_chi<double>(p[1], p[2], p[3]);
+        spn<double> u = spinor_u<double>(x, p[0], 0.0, +1);
+        cx<double>* T = reinterpret_cast<cx<double>*>(s + Ge::O_PSI); T[0] = u.c[2]; T[NENT] = u.c[3];
+      } else if (o == 2 * NG + 1) {                // row of vbar(p1, -) that meets upper components: (lower components of v)^*
+        const double* p = pm; chi_pair<double> x = make_chi<double>(p[1], p[2], p[3]);
+        spn<double> v = spinor_v<double>(x, p[0], 0.0, -1);
+        cx<double>* W = reinterpret_cast<cx<double>*>(s + Ge::O_W); W[0] = conj(v.c[2]); W[1] = conj(v.c[3]);
+      } else {                                     // q_S = p2 - K_S
+        int S = o - 2 * NG - 2; double q[4] = {pm[4], pm[5], pm[6], pm[7]};
+#pragma unroll
+        for (int i = 0; i < NG; i++) if (S >> i & 1) { for (int mu = 0; mu < 4; mu++) q[mu] -= pm[4 * (i + 2) + mu]; }
+        double* Q = s + Ge::O_Q + 4 * S; Q[0] = q[0]; Q[1] = q[1]; Q[2] = q[2]; Q[3] = q[3];
+        s[Ge::O_IQ2 + S] = (S != 0 && S != NSUB - 1) ? 1.0 / mdot_rr(q, q) : 0.0;
+      }
+    }
+    __syncthreads();
+    // ---- a3: current levels k = 1 .. NG-1 ----
+#pragma unroll 1
+    for (int k = 1; k < NG; k++) {
+      const int nsub = s_lvl[k + 1] - s_lvl[k], per = nsub << k;
+      for (int t = tid; t < E * per; t += NTH) {
+        int sl = t / per, o = t - sl * per; const int S = s_sub[s_lvl[k] + (o >> k)]; const unsigned v = o & ((1u << k) - 1u);
+        double* s = sm + sl * Ge::SLOT;
+        const cx<double>* M = reinterpret_cast<const cx<double>*>(s + Ge::O_EPS);
+        cx<double>* T = reinterpret_cast<cx<double>*>(s + Ge::O_PSI);
+        cx<double> a0 = mk<double>(0, 0), a1 = mk<double>(0, 0);
+        int r = 0;
+#pragma unroll
+        for (int i = 0; i < NG; i++) if (S >> i & 1) {
+          const unsigned hb = (v >> r) & 1u, vp = (v & ((1u << r) - 1u)) | ((v >> (r + 1)) << r);
+          const int e = s_off[S ^ (1 << i)] + (int)vp;
+          const cx<double> x0 = ldc(T + e), x1 = ldc(T + NENT + e); const cx<double>* m = M + (i * 2 + hb) * 4;
+          cfma(a0, m[0], x0); cfma(a0, m[1], x1); cfma(a1, m[2], x0); cfma(a1, m[3], x1);
+          r++;
+        }
+        const double* q = s + Ge::O_Q + 4 * S; const double sc = s[Ge::O_IQ2 + S];
+        const double qp = (q[0] + q[3]) * sc, qm = (q[0] - q[3]) * sc; const cx<double> qr = mk<double>(q[1] * sc, -q[2] * sc), ql = mk<double>(q[1] * sc, q[2] * sc);
+        cx<double> o0 = qp * a0; cfma(o0, qr, a1);           // (q0 + sigma.q) = [[q+, qr], [ql, q-]]
+        cx<double> o1 = qm * a1; cfma(o1, ql, a0);
+        const int eo = s_off[S] + (int)v;
+        stc(T + eo, o0); stc(T + NENT + eo, o1);
+      }
+      __syncthreads();
+    }
+    // ---- a4-a7: the 2^NG amplitudes of an event in consecutive lanes, helicity sum by a fixed shuffle tree, eq. 3 ----
+    for (int t = tid; t < (E << NG); t += NTH) {
+      const int sl = t >> NG; const unsigned v = t & (NSUB - 1);
+      const double* s = sm + sl * Ge::SLOT;
+      const cx<double>* M = reinterpret_cast<const cx<double>*>(s + Ge::O_EPS);
+      const cx<double>* T = reinterpret_cast<const cx<double>*>(s + Ge::O_PSI);
+      cx<double> a0 = mk<double>(0, 0), a1 = mk<double>(0, 0);
+#pragma unroll
+      for (int i = 0; i < NG; i++) {
+        const unsigned hb = (v >> i) & 1u, vp = (v & ((1u << i) - 1u)) | ((v >> (i + 1)) << i);
+        const int e = s_off[(NSUB - 1) ^ (1 << i)] + (int)vp;
+        const cx<double> x0 = ldc(T + e), x1 = ldc(T + NENT + e); const cx<double>* m = M + (i * 2 + hb) * 4;
+        cfma(a0, m[0], x0); cfma(a0, m[1], x1); cfma(a1, m[2], x0); cfma(a1, m[3], x1);
+      }
+      const cx<double>* W = reinterpret_cast<const cx<double>*>(s + Ge::O_W);
+      cx<double> amp = W[0] * a0; cfma(amp, W[1], a1);
+      double part = norm2(amp);
+#pragma unroll
+      for (int d = NSUB / 2; d >= 1; d >>= 1) part += __shfl_xor_sync(0xffffffffu, part, d);
+      const long long ev = ev0 + sl;
+      if (v == 0 && ev < nev) {
+        const double a = part * P.fac[0], Wt = __ldg(wgt + ev);
+        me_old[ev] = a;
+        for (int k = 1; k < P.nsets; k++) {
+          const double b = part * P.fac[k];
+          me_new[(size_t)(k - 1) * ostride + ev] = b; w_new[(size_t)(k - 1) * ostride + ev] = Wt * (b / a);
+        }
+      }
+    }
+    __syncthreads();
+  }
+}
+
+// Algorithmic flops per event (FMA = 2, MUL = ADD = 1): a level-k task is k 2x2 complex blocks (16 FMA each), the (q0 + sigma.q)
+// block with the propagator folded in (8 FMA + 4 MUL for the block, 6 MUL + 2 ADD for its scaled entries); a final amplitude is NG
+// blocks, the row contraction (6 FMA + 2 MUL) and the square (1 FMA + 1 MUL); externals ~60 per polarisation block, ~50 per
+// spinor, ~20 per subset momentum.
+static double photon_flops_per_event(int ng) {
+  double f = 0;
+  for (int k = 1; k < ng; k++) f += (double)binom(ng, k) * (1 << k) * (32.0 * k + 16 + 4 + 8);
+  f += (double)(1 << ng) * (32.0 * ng + 14 + 3 + ng /* shuffle adds */);
+  f += 2.0 * ng * 60 + 2 * 50 + (1 << ng) * 20.0;
+  return f;
+}
+
+// host side: E = 16 events per CTA, 512 threads (the 16 x 32 final amplitudes of n = 5 are one task per thread)
+constexpr int PH_E = 16, PH_NTH = 512;
+template <int NG> static cudaError_t photon_launch_n(int sm_count, cudaStream_t st, const double* mom, const double* w, double* a, double* b, double* o,
+                                                     long long nev, long long stride, long long ostride, const PhotonParams& P) {
+  static bool attr_set = false;
+  const size_t smem = sizeof(double) * PH_E * PhGeo<NG>::SLOT;
+  if (!attr_set) {
+    cudaError_t e = cudaFuncSetAttribute(epem_photons_kernel<NG, PH_E, PH_NTH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    attr_set = true;
+  }
+  const long long ngroups = (nev + PH_E - 1) / PH_E;
+  const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(2048 / PH_NTH, (size_t)(227 * 1024) / (smem + 2048)));
+  const int grid = (int)std::min<long long>(ngroups, (long long)sm_count * per_sm);
+  epem_photons_kernel<NG, PH_E, PH_NTH><<<grid, PH_NTH, smem, st>>>(mom, w, a, b, o, nev, stride, ostride, P);
+  return cudaSuccess;
+}
+static cudaError_t photon_launch(int ng, int sm_count, cudaStream_t st, const double* mom, const double* w, double* a, double* b, double* o,
+                                 long long nev, long long stride, long long ostride, const PhotonParams& P) {
+  switch (ng) {
+    case 2: return photon_launch_n<2>(sm_count, st, mom, w, a, b, o, nev, stride, ostride, P);
+    case 3: return photon_launch_n<3>(sm_count, st, mom, w, a, b, o, nev, stride, ostride, P);
+    case 4: return photon_launch_n<4>(sm_count, st, mom, w, a, b, o, nev, stride, ostride, P);
+    default: return photon_launch_n<5>(sm_count, st, mom, w, a, b, o, nev, stride, ostride, P);
+  }
+}
+
+}  // namespace rwgt

@@ -11,6 +11,7 @@
 #include "../../include/rwgt.h"
 #include "kernels_small.cuh"
 #include "bg_engine.cuh"
+#include "photon_kernel.cuh"
 #include "microbench.cuh"
 
 namespace {
@@ -18,7 +19,7 @@ namespace {
 thread_local char g_err[512] = "";
 void set_err(const char* fmt, const char* a = "") { std::snprintf(g_err, sizeof(g_err), fmt, a); }
 
-enum Proc { P_EPEM = 0, P_GG_TTX = 1, P_BG = 2 };
+enum Proc { P_EPEM = 0, P_GG_TTX = 1, P_BG = 2, P_PHOTONS = 3 };
 const double PI = 3.14159265358979323846;
 
 }  // namespace
@@ -34,6 +35,8 @@ struct rwgt_handle {
   rwgt_params sets[1 + RWGT_MAX_SETS];   // [0] = old, [1..K] = new
   rwgt::EpemParams epem;
   rwgt::GGttxParams ggttx;
+  rwgt::PhotonParams photons; // e+ e- -> n_photons gamma
+  int n_photons, sm_count;
   rwgt::BgProcess* bg;        // ordered-current engine (n_gluons >= 3, or gg_ttx when forced)
   // device scratch for rwgt_run_host
   double* scratch;
@@ -91,6 +94,15 @@ rwgt_handle* rwgt_create_multi(const char* process, const rwgt_params* params_ol
   else if (p == "gg_ttxg") { ng = 3; }
   else if (p == "gg_ttxgg") { ng = 4; }
   else if (p == "gg_ttxggg") { ng = 5; }
+  else if (p == "epem_aa" || p == "epem_aaa" || p == "epem_aaaa" || p == "epem_aaaaa") {
+    // e+ e- -> n photons (n = 5: the paper's measured process): only alpha_em enters, as e^(2n)
+    const int na = (int)p.size() - 5;
+    h->proc = P_PHOTONS; h->n_photons = na; h->n_ext = na + 2; h->n_gluons = 0; h->photons.nsets = h->nsets;
+    double fact = 1; for (int i = 2; i <= na; i++) fact *= i;
+    for (int k = 0; k < h->nsets; k++) h->photons.fac[k] = 2.0 * std::pow(4.0 * PI * h->sets[k].alpha_em, na) / (4.0 * fact);
+    cudaDeviceProp prop; cudaGetDeviceProperties(&prop, h->device); h->sm_count = prop.multiProcessorCount;
+    return h;
+  }
   else { set_err("rwgt_create: unknown process '%s'", process); delete h; return nullptr; }
   if (h->proc == P_EPEM) {
     h->epem.nsets = h->nsets;
@@ -135,6 +147,7 @@ double rwgt_flops_per_event(const rwgt_handle* h) {
   // the two one-event-per-thread kernels: ncu counters of the committed build (217 DFMA + 119 DMUL + 48 DADD resp.
   // 1263 DFMA + 369 DMUL + 87 DADD per event; profiles/r1_summary.md)
   if (h->proc == P_EPEM) return 601.0 + (h->nsets - 2) * 45.0;
+  if (h->proc == P_PHOTONS) return rwgt::photon_flops_per_event(h->n_photons);
   // gg_ttx: 2982 for two sets of equal mass; a further set of equal mass costs 8 helicities x (4 FMA + colour form 5 FMA + 4 MUL/ADD)
   if (h->proc == P_GG_TTX) return h->ggttx.two_pass ? h->nsets * 2982.0 : 2982.0 + (h->nsets - 2) * 8 * 26.0;
   return rwgt::bg_flops_per_event(h->bg, h->precision);
@@ -156,6 +169,9 @@ static int launch_events(rwgt_handle* h, const double* momenta, const double* we
     int bs = 128; long long nb = (n + bs - 1) / bs;
     if (h->nsets == 2) rwgt::gg_ttx_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->ggttx);
     else rwgt::gg_ttx_multi_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->ggttx);
+  } else if (h->proc == P_PHOTONS) {
+    cudaError_t e = rwgt::photon_launch(h->n_photons, h->sm_count, st, momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->photons);
+    if (e != cudaSuccess) { set_err("rwgt_run: %s", cudaGetErrorString(e)); return (int)e; }
   } else {
     int rc = rwgt::bg_run(h->bg, h->precision, momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, st);
     if (rc != 0) { set_err("rwgt_run: engine launch failed"); return rc; }
