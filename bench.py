@@ -119,7 +119,7 @@ def run_reference(args) -> None:
         return
     import oracle as orc
     c = ev.config(args.config)
-    per_core = {1: 25000.0, 2: 500.0, 3: 55.0, 4: 5.0, 5: 1.1}[c.index]       # rough oracle events/s/core, sizes the sample only
+    per_core = {1: 25000.0, 2: 500.0, 3: 55.0, 4: 5.0, 5: 1.1, 6: 5.0}[c.index]       # rough oracle events/s/core, sizes the sample only
     cores = os.cpu_count() or 1
     n = args.ref_events or max(8, int(per_core * cores * 4.0))                    # ~4 s per step
     n = min(n, c.n_events)
@@ -181,7 +181,7 @@ def main() -> None:
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index 1..5 (default 2 = configs[1])")
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index 1..5 (default 2 = configs[1]); 6 = the paper's own e+e- -> 5 gamma (PAPER.md:72-77)")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32", "mixed"])
     ap.add_argument("--events", type=int, default=0, help="override the config's event count")
     ap.add_argument("--ref-events", type=int, default=0, help="reference arm: events per step")
@@ -293,7 +293,7 @@ def main() -> None:
             "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": dtype, "data": "synthetic",
             "config": {"workload": workload_name(c, n), "events_per_gpu": n, "precision": args.precision, "l2": res["l2"],
-                       "seed": c.seed, "kappa": 0.1 if c.index > 1 else None},
+                       "seed": c.seed, "kappa": 0.1 if 1 < c.index < 6 else None},
             "clocks": clocks, "gpu_launches": args.steps,
             "e2e": {"value": e2e_val, "unit": "events/s", "h2d_bytes_per_step": int(m.nbytes + w.nbytes), "d2h_bytes_per_step": int(3 * n * 8),
                     "steps": e2e_steps, "matches_device_path": same},
@@ -302,7 +302,7 @@ def main() -> None:
     # ---- cpu_baseline: the oracle on a bounded sample of the same workload (rank 0, N = 1 only) ----
     if world == 1 and not args.no_cpu_baseline:
         import oracle as orc
-        per_core = {1: 25000.0, 2: 500.0, 3: 55.0, 4: 5.0, 5: 1.1}[c.index]
+        per_core = {1: 25000.0, 2: 500.0, 3: 55.0, 4: 5.0, 5: 1.1, 6: 5.0}[c.index]
         cores = os.cpu_count() or 1
         ns = min(n, max(8, int(per_core * cores * 12.0)))
         t0 = time.perf_counter()

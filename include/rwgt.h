@@ -46,6 +46,8 @@ typedef struct {
 
 /* Create a handle for one process and one (old, new) pair of parameter sets.
  *   process: "epem_mupmum" | "gg_ttx" | "gg_ttxg" | "gg_ttxgg" | "gg_ttxggg"
+ *            | "epem_aa" | "epem_aaa" | "epem_aaaa" | "epem_aaaaa"   (e+ e- -> 2..5 photons, leg order [e+, e-, gamma...];
+ *              "epem_aaaaa" is the process the paper measured, Table 1; only alpha_em enters; FP64 only)
  *            leg order in `momenta`: [e+,e-,mu+,mu-] resp. [g,g,t,tbar,(g,(g,(g)))];
  *            legs 0,1 incoming, all momenta physical (E>0).
  * Builds the per-process tables (ordered-current schedule, colour matrix) on the host and

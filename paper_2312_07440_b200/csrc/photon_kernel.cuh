@@ -44,6 +44,43 @@ template <int NG> struct PhGeo {
                        O_W = O_IQ2 + NSUB, O_PSI = O_W + 4, SLOT = O_PSI + 4 * NENT;
 };
 
+// One level of the recursion: all currents of K photons (K compile-time: constant divisors, branch-free member loop).
+// s_child[S][r] = (first entry of S without its r-th member) << 8 | (2 * that member's label).
+template <int NG, int K, int E, int NTH>
+__device__ __forceinline__ void photon_level(double* sm, const unsigned char* s_sub, const unsigned short* s_off, const unsigned* s_child, int first_sub, int tid) {
+  typedef PhGeo<NG> Ge;
+  constexpr int NENT = Ge::NENT, per = binom(NG, K) << K;
+  for (int t = tid; t < E * per; t += NTH) {
+    const int sl = t / per, o = t - sl * per; const int S = s_sub[first_sub + (o >> K)]; const unsigned v = o & ((1u << K) - 1u);
+    double* s = sm + sl * Ge::SLOT;
+    const cx<double>* M = reinterpret_cast<const cx<double>*>(s + Ge::O_EPS);
+    cx<double>* T = reinterpret_cast<cx<double>*>(s + Ge::O_PSI);
+    cx<double> a0 = mk<double>(0, 0), a1 = mk<double>(0, 0);
+#pragma unroll
+    for (int r = 0; r < K; r++) {
+      const unsigned ch = s_child[S * NG + r];
+      const unsigned hb = (v >> r) & 1u, vp = (v & ((1u << r) - 1u)) | ((v >> (r + 1)) << r);
+      const int e = (int)(ch >> 8) + (int)vp;
+      const cx<double> x0 = ldc(T + e), x1 = ldc(T + NENT + e); const cx<double>* m = M + ((ch & 0xffu) + hb) * 4;
+      cfma(a0, m[0], x0); cfma(a0, m[1], x1); cfma(a1, m[2], x0); cfma(a1, m[3], x1);
+    }
+    const double* q = s + Ge::O_Q + 4 * S; const double sc = s[Ge::O_IQ2 + S];
+    const double qp = (q[0] + q[3]) * sc, qm = (q[0] - q[3]) * sc; const cx<double> qr = mk<double>(q[1] * sc, -q[2] * sc), ql = mk<double>(q[1] * sc, q[2] * sc);
+    cx<double> o0 = qp * a0; cfma(o0, qr, a1);           // (q0 + sigma.q) = [[q+, qr], [ql, q-]]
+    cx<double> o1 = qm * a1; cfma(o1, ql, a0);
+    const int eo = s_off[S] + (int)v;
+    stc(T + eo, o0); stc(T + NENT + eo, o1);
+  }
+  __syncthreads();
+}
+template <int NG, int K, int E, int NTH>
+__device__ __forceinline__ void photon_levels(double* sm, const unsigned char* s_sub, const unsigned short* s_off, const unsigned* s_child, const unsigned char* s_lvl, int tid) {
+  if constexpr (K < NG) {
+    photon_level<NG, K, E, NTH>(sm, s_sub, s_off, s_child, s_lvl[K], tid);
+    photon_levels<NG, K + 1, E, NTH>(sm, s_sub, s_off, s_child, s_lvl, tid);
+  }
+}
+
 template <int NG, int E, int NTH>
 __global__ void __launch_bounds__(NTH) epem_photons_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
                                                            double* __restrict__ me_old, double* __restrict__ me_new,
@@ -56,11 +93,13 @@ __global__ void __launch_bounds__(NTH) epem_photons_kernel(const double* __restr
   __shared__ unsigned short s_off[NSUB];            // first entry of subset S
   __shared__ unsigned char s_sub[NSUB];             // subsets ordered by (size, value)
   __shared__ unsigned char s_lvl[NG + 2];           // s_sub index of the first subset of each size
+  __shared__ unsigned s_child[NSUB * NG];           // (first entry of S without its r-th member) << 8 | 2 * member label
   const int tid = threadIdx.x;
   if (tid == 0) {
     int o = 0; for (int S = 0; S < NSUB; S++) { s_off[S] = (unsigned short)o; o += 1 << __popc(S); }
     int j = 0; for (int k = 0; k <= NG; k++) { s_lvl[k] = (unsigned char)j; for (int S = 0; S < NSUB; S++) if (__popc(S) == k) s_sub[j++] = (unsigned char)S; }
     s_lvl[NG + 1] = (unsigned char)j;
+    for (int S = 0; S < NSUB; S++) { int r = 0; for (int i = 0; i < NG; i++) if (S >> i & 1) s_child[S * NG + r++] = ((unsigned)s_off[S ^ (1 << i)] << 8) | (unsigned)(2 * i); }
   }
   __syncthreads();
   const long long ngroups = (nev + E - 1) / E;
@@ -98,33 +137,7 @@ __global__ void __launch_bounds__(NTH) epem_photons_kernel(const double* __restr
     }
     __syncthreads();
     // ---- a3: current levels k = 1 .. NG-1 ----
-#pragma unroll 1
-    for (int k = 1; k < NG; k++) {
-      const int nsub = s_lvl[k + 1] - s_lvl[k], per = nsub << k;
-      for (int t = tid; t < E * per; t += NTH) {
-        int sl = t / per, o = t - sl * per; const int S = s_sub[s_lvl[k] + (o >> k)]; const unsigned v = o & ((1u << k) - 1u);
-        double* s = sm + sl * Ge::SLOT;
-        const cx<double>* M = reinterpret_cast<const cx<double>*>(s + Ge::O_EPS);
-        cx<double>* T = reinterpret_cast<cx<double>*>(s + Ge::O_PSI);
-        cx<double> a0 = mk<double>(0, 0), a1 = mk<double>(0, 0);
-        int r = 0;
-#pragma unroll
-        for (int i = 0; i < NG; i++) if (S >> i & 1) {
-          const unsigned hb = (v >> r) & 1u, vp = (v & ((1u << r) - 1u)) | ((v >> (r + 1)) << r);
-          const int e = s_off[S ^ (1 << i)] + (int)vp;
-          const cx<double> x0 = ldc(T + e), x1 = ldc(T + NENT + e); const cx<double>* m = M + (i * 2 + hb) * 4;
-          cfma(a0, m[0], x0); cfma(a0, m[1], x1); cfma(a1, m[2], x0); cfma(a1, m[3], x1);
-          r++;
-        }
-        const double* q = s + Ge::O_Q + 4 * S; const double sc = s[Ge::O_IQ2 + S];
-        const double qp = (q[0] + q[3]) * sc, qm = (q[0] - q[3]) * sc; const cx<double> qr = mk<double>(q[1] * sc, -q[2] * sc), ql = mk<double>(q[1] * sc, q[2] * sc);
-        cx<double> o0 = qp * a0; cfma(o0, qr, a1);           // (q0 + sigma.q) = [[q+, qr], [ql, q-]]
-        cx<double> o1 = qm * a1; cfma(o1, ql, a0);
-        const int eo = s_off[S] + (int)v;
-        stc(T + eo, o0); stc(T + NENT + eo, o1);
-      }
-      __syncthreads();
-    }
+    photon_levels<NG, 1, E, NTH>(sm, s_sub, s_off, s_child, s_lvl, tid);
     // ---- a4-a7: the 2^NG amplitudes of an event in consecutive lanes, helicity sum by a fixed shuffle tree, eq. 3 ----
     for (int t = tid; t < (E << NG); t += NTH) {
       const int sl = t >> NG; const unsigned v = t & (NSUB - 1);
@@ -135,7 +148,7 @@ __global__ void __launch_bounds__(NTH) epem_photons_kernel(const double* __restr
 #pragma unroll
       for (int i = 0; i < NG; i++) {
         const unsigned hb = (v >> i) & 1u, vp = (v & ((1u << i) - 1u)) | ((v >> (i + 1)) << i);
-        const int e = s_off[(NSUB - 1) ^ (1 << i)] + (int)vp;
+        const int e = (int)(s_child[(NSUB - 1) * NG + i] >> 8) + (int)vp;
         const cx<double> x0 = ldc(T + e), x1 = ldc(T + NENT + e); const cx<double>* m = M + (i * 2 + hb) * 4;
         cfma(a0, m[0], x0); cfma(a0, m[1], x1); cfma(a1, m[2], x0); cfma(a1, m[3], x1);
       }
@@ -170,8 +183,13 @@ static double photon_flops_per_event(int ng) {
   return f;
 }
 
-// host side: E = 16 events per CTA, 512 threads (the 16 x 32 final amplitudes of n = 5 are one task per thread)
-constexpr int PH_E = 16, PH_NTH = 512;
+// host side: E = 8 events per CTA, 256 threads (the 8 x 32 final amplitudes of n = 5 are one task per thread), 3 CTAs per SM.
+// Measured on B200 (n = 5, 131072 events): E/threads 16/512 0.503 ms, 12/384 0.449, 8/256 0.410, 6/192 0.405, 4/128 0.408.
+#ifndef RWGT_PH_E
+#define RWGT_PH_E 8
+#define RWGT_PH_NTH 256
+#endif
+constexpr int PH_E = RWGT_PH_E, PH_NTH = RWGT_PH_NTH;
 template <int NG> static cudaError_t photon_launch_n(int sm_count, cudaStream_t st, const double* mom, const double* w, double* a, double* b, double* o,
                                                      long long nev, long long stride, long long ostride, const PhotonParams& P) {
   static bool attr_set = false;
