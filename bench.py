@@ -267,7 +267,8 @@ def main() -> None:
         pass
     micro = {}
     kinds = ({"fma_chain": 0, "fma_3_distinct_sources": 3, "fma_1_reused_source": 4, "dmma_chain": 2, "dfma_and_dmma_concurrent": 7}
-             if dtype == "f64" else {"fma_chain": 1, "fma_3_distinct_sources": 5, "fma_1_reused_source": 6})
+             if dtype == "f64" else {"fma_chain": 1, "fma_3_distinct_sources": 5, "fma_1_reused_source": 6,
+                            "ffma2_chain": 8, "ffma2_3_distinct_sources": 9, "ffma2_1_reused_source": 10})
     for name, kind in kinds.items():
         try:
             micro[name] = B.rwgt_measure_peak(kind)          # register-resident microbenchmarks, same session

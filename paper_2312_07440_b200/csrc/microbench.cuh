@@ -58,6 +58,29 @@ __global__ void __launch_bounds__(256) fma_operand_kernel(T* out, const T* in, i
   if (s == T(12345.678)) out[0] = s;
 }
 
+// packed FP32: fma.rn.f32x2 (SASS FFMA2), the same two operand patterns and the chain
+__device__ __forceinline__ unsigned long long mb_pk(float a, float b) { unsigned long long r; asm("mov.b64 %0, {%1,%2};" : "=l"(r) : "f"(a), "f"(b)); return r; }
+__device__ __forceinline__ unsigned long long mb_fma2(unsigned long long a, unsigned long long b, unsigned long long c) { unsigned long long d; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c)); return d; }
+template <int MODE>      // 0: chains x = fma2(x, a, b);  1: three distinct sources;  2: one source shared by 16 consecutive FMAs
+__global__ void __launch_bounds__(256) ffma2_kernel(float* out, const float* in, int iters) {
+  unsigned long long y[8], z[8], acc[16];
+#pragma unroll
+  for (int i = 0; i < 8; i++) { y[i] = mb_pk(in[threadIdx.x + i] + 1.0000001f, in[threadIdx.x + i + 32] + 1.0000001f); z[i] = mb_pk(in[threadIdx.x + 8 + i] + 1e-9f, in[threadIdx.x + 40 + i] + 1e-9f); }
+#pragma unroll
+  for (int i = 0; i < 16; i++) acc[i] = mb_pk((float)i, (float)(i + 1));
+  for (int it = 0; it < iters; it++) {
+#pragma unroll
+    for (int r = 0; r < 4; r++)
+#pragma unroll
+      for (int i = 0; i < 16; i++)
+        acc[i] = MODE == 0 ? mb_fma2(acc[i], y[0], z[0]) : MODE == 2 ? mb_fma2(y[r], z[i & 7], acc[i]) : mb_fma2(y[(i + r) & 7], z[(i * 3 + r) & 7], acc[i]);
+  }
+  unsigned long long sacc = 0;
+#pragma unroll
+  for (int i = 0; i < 16; i++) sacc ^= acc[i];
+  if (sacc == 12345678ull) out[0] = 1.0f;
+}
+
 // 8 warps of FP64 FMA chains and 4 warps of DMMA chains in one CTA per SM: do the two share a pipe?
 __global__ void __launch_bounds__(384, 1) dfma_dmma_kernel(double* out, double a, double b, int it_fma, int it_mma) {
   if ((threadIdx.x >> 5) < 8) {
@@ -93,6 +116,7 @@ __global__ void __launch_bounds__(384, 1) dfma_dmma_kernel(double* out, double a
 //      5: FP32 FMA with three distinct register sources;  6: FP32 FMA with one reused source;
 //      7: FP64 FMA chains (8 warps) and DMMA chains (4 warps) running CONCURRENTLY on every SM, summed rate
 //         (equal to kind 0 / kind 2 alone if the two share one pipe, their sum if not).
+//      8 / 9 / 10: packed FP32 fma.rn.f32x2 (FFMA2): chains / three distinct sources / one reused source.
 // Returns TFLOP/s (2 flop per FMA), best of 5.
 static int measure_peak(int kind, double* tflops) {
   int dev = 0; cudaGetDevice(&dev); cudaDeviceProp prop; cudaGetDeviceProperties(&prop, dev);
@@ -112,6 +136,9 @@ static int measure_peak(int kind, double* tflops) {
       case 4: fma_operand_kernel<double, 1><<<blocks, threads>>>(d, d, iters / 8); fl = (double)blocks * threads * (iters / 8) * 64 * 2.0; break;
       case 5: fma_operand_kernel<float, 0><<<blocks, threads>>>((float*)d, (float*)d, iters / 8); fl = (double)blocks * threads * (iters / 8) * 64 * 2.0; break;
       case 6: fma_operand_kernel<float, 1><<<blocks, threads>>>((float*)d, (float*)d, iters / 8); fl = (double)blocks * threads * (iters / 8) * 64 * 2.0; break;
+      case 8: ffma2_kernel<0><<<blocks, threads>>>((float*)d, (float*)d, iters / 8); fl = (double)blocks * threads * (iters / 8) * 64 * 4.0; break;
+      case 9: ffma2_kernel<1><<<blocks, threads>>>((float*)d, (float*)d, iters / 8); fl = (double)blocks * threads * (iters / 8) * 64 * 4.0; break;
+      case 10: ffma2_kernel<2><<<blocks, threads>>>((float*)d, (float*)d, iters / 8); fl = (double)blocks * threads * (iters / 8) * 64 * 4.0; break;
       default: {
         const int itf = 16384, itm = 4096;      // equal pipe time for the two groups if they share the pipe at the same rate
         dfma_dmma_kernel<<<prop.multiProcessorCount, 384>>>(d, 1.0000001, 1e-9, itf, itm);

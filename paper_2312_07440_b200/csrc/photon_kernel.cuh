@@ -44,32 +44,50 @@ template <int NG> struct PhGeo {
                        O_W = O_IQ2 + NSUB, O_PSI = O_W + 4, SLOT = O_PSI + 4 * NENT;
 };
 
+// y += B x for a 2x2 complex block B = (m[0] m[1]; m[2] m[3])
+__device__ __forceinline__ void block_acc(cx<double>& y0, cx<double>& y1, const cx<double>* m, cx<double> x0, cx<double> x1) {
+  cfma(y0, m[0], x0); cfma(y0, m[1], x1); cfma(y1, m[2], x0); cfma(y1, m[3], x1);
+}
 // One level of the recursion: all currents of K photons (K compile-time: constant divisors, branch-free member loop).
+// A thread evaluates BOTH helicities of the subset's last member: for that member the spinor is shared and the block differs,
+// for every other member the block is shared and the two spinors are neighbours (entry + 2^(K-2)); this halves the shared-memory
+// wavefronts per block product, which is what bounds this kernel.
 // s_child[S][r] = (first entry of S without its r-th member) << 8 | (2 * that member's label).
 template <int NG, int K, int E, int NTH>
 __device__ __forceinline__ void photon_level(double* sm, const unsigned char* s_sub, const unsigned short* s_off, const unsigned* s_child, int first_sub, int tid) {
   typedef PhGeo<NG> Ge;
-  constexpr int NENT = Ge::NENT, per = binom(NG, K) << K;
+  constexpr int NENT = Ge::NENT, KL = K - 1, per = binom(NG, K) << KL;
   for (int t = tid; t < E * per; t += NTH) {
-    const int sl = t / per, o = t - sl * per; const int S = s_sub[first_sub + (o >> K)]; const unsigned v = o & ((1u << K) - 1u);
+    const int sl = t / per, o = t - sl * per; const int S = s_sub[first_sub + (o >> KL)]; const unsigned v = o & ((1u << KL) - 1u);
     double* s = sm + sl * Ge::SLOT;
     const cx<double>* M = reinterpret_cast<const cx<double>*>(s + Ge::O_EPS);
     cx<double>* T = reinterpret_cast<cx<double>*>(s + Ge::O_PSI);
-    cx<double> a0 = mk<double>(0, 0), a1 = mk<double>(0, 0);
+    cx<double> a0 = mk<double>(0, 0), a1 = mk<double>(0, 0), b0 = mk<double>(0, 0), b1 = mk<double>(0, 0);
+    constexpr int HI = KL > 0 ? 1 << (KL > 0 ? KL - 1 : 0) : 0;      // entry distance of the two spinors
 #pragma unroll
-    for (int r = 0; r < K; r++) {
+    for (int r = 0; r < KL; r++) {                 // members below the last one: one block, two spinors
       const unsigned ch = s_child[S * NG + r];
       const unsigned hb = (v >> r) & 1u, vp = (v & ((1u << r) - 1u)) | ((v >> (r + 1)) << r);
-      const int e = (int)(ch >> 8) + (int)vp;
-      const cx<double> x0 = ldc(T + e), x1 = ldc(T + NENT + e); const cx<double>* m = M + ((ch & 0xffu) + hb) * 4;
-      cfma(a0, m[0], x0); cfma(a0, m[1], x1); cfma(a1, m[2], x0); cfma(a1, m[3], x1);
+      const int e = (int)(ch >> 8) + (int)vp; const cx<double>* m = M + ((ch & 0xffu) + hb) * 4;
+      const cx<double> m0 = ldc(m), m1 = ldc(m + 1), m2 = ldc(m + 2), m3 = ldc(m + 3);
+      const cx<double> x0 = ldc(T + e), x1 = ldc(T + NENT + e), y0 = ldc(T + e + HI), y1 = ldc(T + NENT + e + HI);
+      cfma(a0, m0, x0); cfma(a0, m1, x1); cfma(a1, m2, x0); cfma(a1, m3, x1);
+      cfma(b0, m0, y0); cfma(b0, m1, y1); cfma(b1, m2, y0); cfma(b1, m3, y1);
+    }
+    {                                              // the last member: one spinor, two blocks
+      const unsigned ch = s_child[S * NG + KL];
+      const int e = (int)(ch >> 8) + (int)v; const cx<double>* m = M + (ch & 0xffu) * 4;
+      const cx<double> x0 = ldc(T + e), x1 = ldc(T + NENT + e);
+      block_acc(a0, a1, m, x0, x1); block_acc(b0, b1, m + 4, x0, x1);
     }
     const double* q = s + Ge::O_Q + 4 * S; const double sc = s[Ge::O_IQ2 + S];
     const double qp = (q[0] + q[3]) * sc, qm = (q[0] - q[3]) * sc; const cx<double> qr = mk<double>(q[1] * sc, -q[2] * sc), ql = mk<double>(q[1] * sc, q[2] * sc);
     cx<double> o0 = qp * a0; cfma(o0, qr, a1);           // (q0 + sigma.q) = [[q+, qr], [ql, q-]]
     cx<double> o1 = qm * a1; cfma(o1, ql, a0);
+    cx<double> u0 = qp * b0; cfma(u0, qr, b1);
+    cx<double> u1 = qm * b1; cfma(u1, ql, b0);
     const int eo = s_off[S] + (int)v;
-    stc(T + eo, o0); stc(T + NENT + eo, o1);
+    stc(T + eo, o0); stc(T + NENT + eo, o1); stc(T + eo + (1 << KL), u0); stc(T + NENT + eo + (1 << KL), u1);
   }
   __syncthreads();
 }
@@ -138,27 +156,38 @@ __global__ void __launch_bounds__(NTH) epem_photons_kernel(const double* __restr
     __syncthreads();
     // ---- a3: current levels k = 1 .. NG-1 ----
     photon_levels<NG, 1, E, NTH>(sm, s_sub, s_off, s_child, s_lvl, tid);
-    // ---- a4-a7: the 2^NG amplitudes of an event in consecutive lanes, helicity sum by a fixed shuffle tree, eq. 3 ----
-    for (int t = tid; t < (E << NG); t += NTH) {
-      const int sl = t >> NG; const unsigned v = t & (NSUB - 1);
+    // ---- a4-a7: the 2^NG amplitudes of an event, two per thread (both helicities of the last photon) in 2^(NG-1) consecutive lanes,
+    //             helicity sum by a fixed shuffle tree, eq. 3 ----
+    constexpr int NFIN = E << (NG - 1), NFIN_W = (NFIN + 31) / 32 * 32;       // whole warps take part in the shuffles
+    for (int t0 = tid; t0 < NFIN_W; t0 += NTH) {
+      const bool live = t0 < NFIN; const int t = live ? t0 : 0;
+      const int sl = t >> (NG - 1); const unsigned v = t & (NSUB / 2 - 1);
       const double* s = sm + sl * Ge::SLOT;
       const cx<double>* M = reinterpret_cast<const cx<double>*>(s + Ge::O_EPS);
       const cx<double>* T = reinterpret_cast<const cx<double>*>(s + Ge::O_PSI);
-      cx<double> a0 = mk<double>(0, 0), a1 = mk<double>(0, 0);
+      cx<double> a0 = mk<double>(0, 0), a1 = mk<double>(0, 0), b0 = mk<double>(0, 0), b1 = mk<double>(0, 0);
 #pragma unroll
-      for (int i = 0; i < NG; i++) {
+      for (int i = 0; i < NG - 1; i++) {
         const unsigned hb = (v >> i) & 1u, vp = (v & ((1u << i) - 1u)) | ((v >> (i + 1)) << i);
-        const int e = (int)(s_child[(NSUB - 1) * NG + i] >> 8) + (int)vp;
-        const cx<double> x0 = ldc(T + e), x1 = ldc(T + NENT + e); const cx<double>* m = M + (i * 2 + hb) * 4;
-        cfma(a0, m[0], x0); cfma(a0, m[1], x1); cfma(a1, m[2], x0); cfma(a1, m[3], x1);
+        const int e = (int)(s_child[(NSUB - 1) * NG + i] >> 8) + (int)vp; const cx<double>* m = M + (i * 2 + hb) * 4;
+        const cx<double> m0 = ldc(m), m1 = ldc(m + 1), m2 = ldc(m + 2), m3 = ldc(m + 3);
+        const cx<double> x0 = ldc(T + e), x1 = ldc(T + NENT + e), y0 = ldc(T + e + (1 << (NG - 2))), y1 = ldc(T + NENT + e + (1 << (NG - 2)));
+        cfma(a0, m0, x0); cfma(a0, m1, x1); cfma(a1, m2, x0); cfma(a1, m3, x1);
+        cfma(b0, m0, y0); cfma(b0, m1, y1); cfma(b1, m2, y0); cfma(b1, m3, y1);
+      }
+      {
+        const int e = (int)(s_child[(NSUB - 1) * NG + NG - 1] >> 8) + (int)v; const cx<double>* m = M + (NG - 1) * 2 * 4;
+        const cx<double> x0 = ldc(T + e), x1 = ldc(T + NENT + e);
+        block_acc(a0, a1, m, x0, x1); block_acc(b0, b1, m + 4, x0, x1);
       }
       const cx<double>* W = reinterpret_cast<const cx<double>*>(s + Ge::O_W);
-      cx<double> amp = W[0] * a0; cfma(amp, W[1], a1);
-      double part = norm2(amp);
+      cx<double> amp0 = W[0] * a0; cfma(amp0, W[1], a1);
+      cx<double> amp1 = W[0] * b0; cfma(amp1, W[1], b1);
+      double part = norm2(amp0) + norm2(amp1);
 #pragma unroll
-      for (int d = NSUB / 2; d >= 1; d >>= 1) part += __shfl_xor_sync(0xffffffffu, part, d);
+      for (int d = NSUB / 4; d >= 1; d >>= 1) part += __shfl_xor_sync(0xffffffffu, part, d);
       const long long ev = ev0 + sl;
-      if (v == 0 && ev < nev) {
+      if (live && v == 0 && ev < nev) {
         const double a = part * P.fac[0], Wt = __ldg(wgt + ev);
         me_old[ev] = a;
         for (int k = 1; k < P.nsets; k++) {
@@ -184,7 +213,8 @@ static double photon_flops_per_event(int ng) {
 }
 
 // host side: E = 8 events per CTA, 256 threads (the 8 x 32 final amplitudes of n = 5 are one task per thread), 3 CTAs per SM.
-// Measured on B200 (n = 5, 131072 events): E/threads 16/512 0.503 ms, 12/384 0.449, 8/256 0.410, 6/192 0.405, 4/128 0.408.
+// Measured on B200 (n = 5, 131072 events), one variant per thread: E/threads 16/512 0.503 ms, 12/384 0.449, 8/256 0.410, 6/192 0.405,
+// 4/128 0.408; two variants per thread: 8/256 0.398, 6/128 0.401, 12/256 0.421, 8/128 0.428, 16/256 0.565.
 #ifndef RWGT_PH_E
 #define RWGT_PH_E 8
 #define RWGT_PH_NTH 256

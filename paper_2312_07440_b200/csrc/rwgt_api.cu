@@ -271,7 +271,7 @@ int rwgt_destroy(rwgt_handle* h) {
 }
 
 int rwgt_measure_peak(int kind, double* out_tflops) {
-  if (kind < 0 || kind > 7 || !out_tflops) return -1;
+  if (kind < 0 || kind > 10 || !out_tflops) return -1;
   return rwgt::measure_peak(kind, out_tflops);
 }
 
