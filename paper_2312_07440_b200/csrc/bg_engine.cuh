@@ -379,6 +379,9 @@ template <typename T> struct Smem {
   T* K;           // [nslot][NMASK][4] momentum sums of gluon subsets
   T* iK2;         // [nslot][NMASK]
   T* dR; T* dL;   // [nslot][NMASK] 1/(q^2-m^2)
+  // staging copy of everything step a1/a2 produces for the NEXT event group (written by the colour warps while the workers run the
+  // current group): momenta, external wavefunctions (table entries 0..2N-1 of G, 0..1 of R and L), momentum sums, denominators
+  double* pmS; cx<T>* GS; cx<T>* RS; cx<T>* LS; T* KS; T* iK2S; T* dRS; T* dLS;
   double* A;      // [2][nslot][2 NHK][ASTR] double-buffered rows u = J_s + J_rev(s), v = J_s - J_rev(s) (re,im interleaved), always double
 };
 template <int N, typename T> __host__ __device__ inline size_t carve(Smem<T>& s, unsigned char* base, int ns, int nwords) {
@@ -396,6 +399,14 @@ template <int N, typename T> __host__ __device__ inline size_t carve(Smem<T>& s,
   s.iK2 = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
   s.dR = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
   s.dL = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
+  s.pmS = (double*)(base + off); off += sizeof(double) * ns * (N + 2) * 4; al();
+  s.GS = (cx<T>*)(base + off); off += sizeof(T) * (size_t)ns * 8 * (2 * N); al();
+  s.RS = (cx<T>*)(base + off); off += sizeof(T) * (size_t)ns * 8 * 2; al();
+  s.LS = (cx<T>*)(base + off); off += sizeof(T) * (size_t)ns * 8 * 2; al();
+  s.KS = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK * 4; al();
+  s.iK2S = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
+  s.dRS = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
+  s.dLS = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
   s.W = (uint32_t*)(base + off); off += sizeof(uint32_t) * nwords; al();
   return off;
 }
@@ -437,19 +448,21 @@ __device__ __forceinline__ uint32_t halfw(const uint32_t* w, int k) { return (k 
 
 // named barriers (ids 1..6; id 0 is __syncthreads): workers among themselves, colour warps among themselves,
 // and the full/empty handshake of the two amplitude buffers
-enum { BAR_WORK = 1, BAR_FULL0 = 2, BAR_EMPTY0 = 4, BAR_COLOUR = 6 };
+enum { BAR_WORK = 1, BAR_FULL0 = 2, BAR_EMPTY0 = 4, BAR_COLOUR = 6, BAR_STAGE_FULL = 7, BAR_STAGE_EMPTY = 8 };
 // the barrier id is an immediate (a register id makes ptxas reserve all 16 barriers, which limits the CTAs per SM)
 __device__ __forceinline__ void bar_sync(int id, int count) {
   switch (id) {
     case 1: asm volatile("bar.sync 1, %0;" ::"r"(count) : "memory"); break; case 2: asm volatile("bar.sync 2, %0;" ::"r"(count) : "memory"); break;
     case 3: asm volatile("bar.sync 3, %0;" ::"r"(count) : "memory"); break; case 4: asm volatile("bar.sync 4, %0;" ::"r"(count) : "memory"); break;
-    case 5: asm volatile("bar.sync 5, %0;" ::"r"(count) : "memory"); break; default: asm volatile("bar.sync 6, %0;" ::"r"(count) : "memory");
+    case 5: asm volatile("bar.sync 5, %0;" ::"r"(count) : "memory"); break; case 6: asm volatile("bar.sync 6, %0;" ::"r"(count) : "memory"); break;
+    case 7: asm volatile("bar.sync 7, %0;" ::"r"(count) : "memory"); break; default: asm volatile("bar.sync 8, %0;" ::"r"(count) : "memory");
   }
 }
 __device__ __forceinline__ void bar_arrive(int id, int count) {
   switch (id) {
     case 2: asm volatile("bar.arrive 2, %0;" ::"r"(count) : "memory"); break; case 3: asm volatile("bar.arrive 3, %0;" ::"r"(count) : "memory"); break;
-    case 4: asm volatile("bar.arrive 4, %0;" ::"r"(count) : "memory"); break; default: asm volatile("bar.arrive 5, %0;" ::"r"(count) : "memory");
+    case 4: asm volatile("bar.arrive 4, %0;" ::"r"(count) : "memory"); break; case 5: asm volatile("bar.arrive 5, %0;" ::"r"(count) : "memory"); break;
+    case 7: asm volatile("bar.arrive 7, %0;" ::"r"(count) : "memory"); break; default: asm volatile("bar.arrive 8, %0;" ::"r"(count) : "memory");
   }
 }
 
@@ -628,6 +641,55 @@ template <int N, int WHICH, typename T> struct QuarkLine {
   }
 };
 
+// Steps a1 + a2 for one event group, by `nth` threads (index t0): momenta (coalesced over the events of the group) into pm, then
+// external wavefunctions (gluon i, helicity bit hb -> entry 2 i + hb of G; v(p_tbar) -> entries 0,1 of R; ubar(p_t) -> 0,1 of L),
+// momentum sums of the gluon subsets and the inverse propagator denominators.  sG / sR / sL: entries per component plane of the
+// destination tables.  SYNC(): a barrier over the calling threads between the two steps.
+template <int N, typename T, typename TK, typename SYNC>
+__device__ __forceinline__ void group_externals(int t0, int nth, int ns, long long ev0, long long nev, long long stride, const double* __restrict__ mom,
+                                                double mtd, double* pmD, cx<T>* Gd, int sG, cx<T>* Rd, int sR, cx<T>* Ld, int sL, T* Kd, T* iK2d, T* dRd, T* dLd,
+                                                bool load, SYNC sync) {
+  typedef Geo<N> Ge; constexpr int next = N + 2; const T mt = (T)mtd;
+  if (load) {
+    for (int t = t0; t < ns * next * 4; t += nth) {
+      int sl = t % ns, comp = t / ns; long long ev = ev0 + sl; if (ev >= nev) ev = nev - 1;
+      pmD[(sl * next * 4) + comp] = __ldg(mom + (size_t)comp * stride + ev);
+    }
+    sync();
+  }
+  constexpr int nobj = 2 * N + 4 + Ge::NMASK;
+  for (int t = t0; t < ns * nobj; t += nth) {
+    int sl = t / nobj, o = t % nobj; const double* pm = pmD + sl * next * 4;
+    if (o < 2 * N) {                         // gluon i, helicity bit hb (0: +1, 1: -1); entry = 2*i + hb
+      int i = o >> 1, hb = o & 1, leg = i < 2 ? i : i + 2; const double* p = pm + 4 * leg;
+      vec4<T> e = polvec<T>((T)p[1], (T)p[2], (T)p[3], hb ? -1 : +1);
+      if (i >= 2) e = conj4(e);              // outgoing gluon carries eps*
+      st4(Gd + (size_t)sl * 4 * sG, sG, 2 * i + hb, e);
+    } else if (o < 2 * N + 2) {              // v(p_tbar, lam), R() entries 0,1
+      int hb = o - 2 * N; const double* p = pm + 12;
+      chi_pair<T> x = make_chi<T>((T)p[1], (T)p[2], (T)p[3]);
+      st4(Rd + (size_t)sl * 4 * sR, sR, hb, spinor_v<T>(x, (T)p[0], mt, hb ? -1 : +1));
+    } else if (o < 2 * N + 4) {              // ubar(p_t, lam), L() entries 0,1
+      int hb = o - 2 * N - 2; const double* p = pm + 8;
+      chi_pair<T> x = make_chi<T>((T)p[1], (T)p[2], (T)p[3]);
+      st4(Ld + (size_t)sl * 4 * sL, sL, hb, bar(spinor_u<T>(x, (T)p[0], mt, hb ? -1 : +1)));
+    } else {                                 // gluon subset `mask`
+      int mask = o - 2 * N - 4;
+      TK k[4] = {0, 0, 0, 0};
+#pragma unroll
+      for (int i = 0; i < N; i++) if (mask >> i & 1) { int leg = i < 2 ? i : i + 2; TK sg = i < 2 ? TK(1) : TK(-1);
+        for (int mu = 0; mu < 4; mu++) k[mu] += sg * (TK)pm[4 * leg + mu]; }
+      TK k2 = mdot_rr<TK>(k, k);
+      TK qr[4], ql[4]; for (int mu = 0; mu < 4; mu++) { qr[mu] = k[mu] - (TK)pm[12 + mu]; ql[mu] = (TK)pm[8 + mu] - k[mu]; }
+      TK m2 = (TK)mtd * (TK)mtd;
+      T* K = Kd + ((size_t)sl * Ge::NMASK + mask) * 4; for (int mu = 0; mu < 4; mu++) K[mu] = (T)k[mu];
+      iK2d[sl * Ge::NMASK + mask] = (__popc(mask) >= 2) ? (T)(TK(1) / k2) : T(0);
+      dRd[sl * Ge::NMASK + mask] = (T)(TK(1) / (mdot_rr<TK>(qr, qr) - m2));
+      dLd[sl * Ge::NMASK + mask] = (T)(TK(1) / (mdot_rr<TK>(ql, ql) - m2));
+    }
+  }
+}
+
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
@@ -644,8 +706,14 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
   constexpr int NTH = (NW + NCW) * 32, NWT = NW * 32, NCT = NCW * 32;
   // register hand-over between the warpgroups: the colour warps need few registers, the workers get the rest
   // (setmaxnreg is a warpgroup instruction: both groups must be whole warpgroups of 4 warps)
+  // a1/a2 of the next group on the colour warps: pays when the colour warps are mostly idle and the per-group fixed work is small
+  // next to the currents (n >= 4); for n <= 3 four colour warps are slower at it than eight workers (measured: 5.4 -> 5.9 ms)
+  constexpr bool STAGE = (N >= 4);
   constexpr bool HANDOVER = sizeof(T) == 8 && NW % 4 == 0 && NCW % 4 == 0;
-  constexpr int REG_COL = 56, REG_POOL = 65536 / 32 / CTAS, REG_WORK = ((REG_POOL - NCW * REG_COL) / NW) / 8 * 8 > 232 ? 232 : ((REG_POOL - NCW * REG_COL) / NW) / 8 * 8;
+  // the CTA's pool is what it was launched with: (registers per thread under the launch bounds) x warps; an inc beyond it never returns
+  constexpr int REG_LAUNCH = (65536 / CTAS / NTH) / 8 * 8 > 255 ? 248 : (65536 / CTAS / NTH) / 8 * 8, REG_POOL = REG_LAUNCH * (NW + NCW);
+  constexpr int REG_COL = 56, REG_WORK = ((REG_POOL - NCW * REG_COL) / NW) / 8 * 8 > 232 ? 232 : ((REG_POOL - NCW * REG_COL) / NW) / 8 * 8;
+  static_assert(NW * REG_WORK + NCW * REG_COL <= REG_POOL, "register hand-over exceeds the CTA's pool");
   extern __shared__ __align__(16) unsigned char smem_raw[];
   Ctx<T> c; c.D = &D; c.ns = D.nslot;
   carve<N, T>(c.s, smem_raw, D.nslot, D.nwords);
@@ -665,50 +733,34 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
     unsigned step = 0;
     for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
       const long long ev0 = grp * ns;
-      bar_sync(BAR_WORK, NWT);
-      // ---- a1: load momenta (coalesced over the events of the group) ----
-      for (int t = tid; t < ns * next * 4; t += NWT) {
-        int sl = t % ns, comp = t / ns; long long ev = ev0 + sl; if (ev >= nev) ev = nev - 1;
-        s.pm[(sl * next * 4) + comp] = __ldg(mom + (size_t)comp * stride + ev);
+      if constexpr (!STAGE) {
+        // ---- a1/a2 by the workers themselves ----
+        bar_sync(BAR_WORK, NWT);
+        group_externals<N, T, TK>(tid, NWT, ns, ev0, nev, stride, mom, D.set[0].mt, s.pm, s.G, nG, s.R, nR, s.L, nL, s.K, s.iK2, s.dR, s.dL, true,
+                                  [] { bar_sync(BAR_WORK, NWT); });
+      } else {
+      // ---- a1/a2 were done for this group by the colour warps (staging buffers): copy them into the tables ----
+      bar_sync(BAR_STAGE_FULL, NTH);
+      {
+        constexpr int n2 = 2 * N;
+        for (int t = tid; t < ns * next * 4; t += NWT) s.pm[t] = s.pmS[t];
+        for (int t = tid; t < ns * 4 * n2; t += NWT) { int sl = t / (4 * n2), r = t - sl * 4 * n2, cc = r / n2, e = r - cc * n2; s.G[(size_t)sl * 4 * nG + cc * nG + e] = s.GS[t]; }
+        for (int t = tid; t < ns * 8; t += NWT) { int sl = t >> 3, r = t & 7, cc = r >> 1, e = r & 1;
+          s.R[(size_t)sl * 4 * nR + cc * nR + e] = s.RS[t]; s.L[(size_t)sl * 4 * nL + cc * nL + e] = s.LS[t]; }
+        for (int t = tid; t < ns * Ge::NMASK * 4; t += NWT) s.K[t] = s.KS[t];
+        for (int t = tid; t < ns * Ge::NMASK; t += NWT) { s.iK2[t] = s.iK2S[t]; s.dR[t] = s.dRS[t]; s.dL[t] = s.dLS[t]; }
+      }
+      __threadfence_block();
+      bar_arrive(BAR_STAGE_EMPTY, NTH);                        // the colour warps may stage the next group
       }
       bar_sync(BAR_WORK, NWT);
 #pragma unroll 1
       for (int iset = 0; iset < D.nsets; iset++) {
         const BgSet& P = D.set[iset];
         c.g3 = (T)P.g3; c.g4 = (T)P.g4; c.gq = (T)P.gq; c.mt = (T)P.mt;
-        if (iset == 0 || !D.shared_ext) {
-          // ---- a2: external wavefunctions, momentum sums, propagator denominators ----
-          constexpr int nobj = 2 * N + 4 + Ge::NMASK;
-          for (int t = tid; t < ns * nobj; t += NWT) {
-            int sl = t / nobj, o = t % nobj; const double* pm = s.pm + sl * next * 4;
-            if (o < 2 * N) {                         // gluon i, helicity bit hb (0: +1, 1: -1); entry = 2*i + hb
-              int i = o >> 1, hb = o & 1, leg = i < 2 ? i : i + 2; const double* p = pm + 4 * leg;
-              vec4<T> e = polvec<T>((T)p[1], (T)p[2], (T)p[3], hb ? -1 : +1);
-              if (i >= 2) e = conj4(e);              // outgoing gluon carries eps*
-              st4(s.G + (size_t)sl * 4 * nG, nG, 2 * i + hb, e);
-            } else if (o < 2 * N + 2) {              // v(p_tbar, lam), R() entries 0,1
-              int hb = o - 2 * N; const double* p = pm + 12;
-              chi_pair<T> x = make_chi<T>((T)p[1], (T)p[2], (T)p[3]);
-              st4(s.R + (size_t)sl * 4 * nR, nR, hb, spinor_v<T>(x, (T)p[0], c.mt, hb ? -1 : +1));
-            } else if (o < 2 * N + 4) {              // ubar(p_t, lam), L() entries 0,1
-              int hb = o - 2 * N - 2; const double* p = pm + 8;
-              chi_pair<T> x = make_chi<T>((T)p[1], (T)p[2], (T)p[3]);
-              st4(s.L + (size_t)sl * 4 * nL, nL, hb, bar(spinor_u<T>(x, (T)p[0], c.mt, hb ? -1 : +1)));
-            } else {                                 // gluon subset `mask`
-              int mask = o - 2 * N - 4;
-              TK k[4] = {0, 0, 0, 0};
-#pragma unroll
-              for (int i = 0; i < N; i++) if (mask >> i & 1) { int leg = i < 2 ? i : i + 2; TK sg = i < 2 ? TK(1) : TK(-1);
-                for (int mu = 0; mu < 4; mu++) k[mu] += sg * (TK)pm[4 * leg + mu]; }
-              TK k2 = mdot_rr<TK>(k, k);
-              TK qr[4], ql[4]; for (int mu = 0; mu < 4; mu++) { qr[mu] = k[mu] - (TK)pm[12 + mu]; ql[mu] = (TK)pm[8 + mu] - k[mu]; }
-              TK m2 = (TK)P.mt * (TK)P.mt;
-              T* K = s.K + ((size_t)sl * Ge::NMASK + mask) * 4; for (int mu = 0; mu < 4; mu++) K[mu] = (T)k[mu];
-              s.iK2[sl * Ge::NMASK + mask] = (__popc(mask) >= 2) ? (T)(TK(1) / k2) : T(0);
-              s.dR[sl * Ge::NMASK + mask] = (T)(TK(1) / (mdot_rr<TK>(qr, qr) - m2));
-              s.dL[sl * Ge::NMASK + mask] = (T)(TK(1) / (mdot_rr<TK>(ql, ql) - m2));
-            }
-          }
+        if (iset > 0 && !D.shared_ext) {
+          // a set with another top mass: external spinors and denominators are redone for it (reading R12)
+          group_externals<N, T, TK>(tid, NWT, ns, ev0, nev, stride, mom, P.mt, s.pm, s.G, nG, s.R, nR, s.L, nL, s.K, s.iK2, s.dR, s.dL, false, [] {});
           bar_sync(BAR_WORK, NWT);
         }
         // ---- a3: current levels ----
@@ -772,9 +824,21 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
     if constexpr (HANDOVER) asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REG_COL));
     const int ctid = threadIdx.x - NWT, cwarp = ctid >> 5, lane = ctid & 31;
     unsigned step = 0;
+    // a1 + a2 of an event group into the staging buffers (parameter set 0; masses of the other sets: see the workers)
+    auto stage = [&](long long g) {
+      group_externals<N, T, TK>(ctid, NCT, ns, g * ns, nev, stride, mom, D.set[0].mt, s.pmS, s.GS, 2 * N, s.RS, 2, s.LS, 2, s.KS, s.iK2S, s.dRS, s.dLS, true,
+                                [] { bar_sync(BAR_COLOUR, NCT); });
+      __threadfence_block();
+      bar_arrive(BAR_STAGE_FULL, NTH);
+    };
+    if (STAGE && (long long)blockIdx.x < ngroups) stage(blockIdx.x);
     for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
       const long long ev0 = grp * ns;
       for (int t = ctid; t < ns * BG_NSMAX; t += NCT) s.acc[t] = 0.0;
+      if constexpr (STAGE) {
+        bar_sync(BAR_STAGE_EMPTY, NTH);                        // the workers have taken this group's staged data
+        if (grp + gridDim.x < ngroups) stage(grp + gridDim.x); // the next group's fixed work overlaps the workers' currents and amplitudes
+      }
       bar_sync(BAR_COLOUR, NCT);
 #pragma unroll 1
       for (int iset = 0; iset < D.nsets; iset++) {
