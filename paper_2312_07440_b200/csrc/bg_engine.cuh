@@ -709,7 +709,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
   // a1/a2 of the next group on the colour warps: pays when the colour warps are mostly idle and the per-group fixed work is small
   // next to the currents (n >= 4); for n <= 3 four colour warps are slower at it than eight workers (measured: 5.4 -> 5.9 ms)
   constexpr bool STAGE = (N >= 4);
-  constexpr bool HANDOVER = sizeof(T) == 8 && NW % 4 == 0 && NCW % 4 == 0;
+  constexpr bool HANDOVER = NW % 4 == 0 && NCW % 4 == 0;
   // the CTA's pool is what it was launched with: (registers per thread under the launch bounds) x warps; an inc beyond it never returns
   constexpr int REG_LAUNCH = (65536 / CTAS / NTH) / 8 * 8 > 255 ? 248 : (65536 / CTAS / NTH) / 8 * 8, REG_POOL = REG_LAUNCH * (NW + NCW);
   constexpr int REG_COL = 56, REG_WORK = ((REG_POOL - NCW * REG_COL) / NW) / 8 * 8 > 232 ? 232 : ((REG_POOL - NCW * REG_COL) / NW) / 8 * 8;
@@ -919,25 +919,29 @@ static size_t smem_need_n(int n, const BgSched& S, int nslot, bool dbl) {
 }
 // Warp split: one CTA per SM, 8 worker warps (FP64 / FP32 pipe) + 4 colour warps (DMMA) = 3 warps x 168 registers per SM
 // sub-partition.  Measured on B200 against 10+2, 6+2, 12+4 and (n = 3) two CTAs of 4+2 warps per SM: best or within 4 % of best
-// for every process.  (The kernel is parametrised on the split and on the CTAs per SM.)
-template <int N> struct BgCfg { static constexpr int NW = 8, NCW = 4, CTAS = 1; };
-static int bg_nw(int n) { return n <= 3 ? BgCfg<3>::NW : BgCfg<5>::NW; }
-static int bg_ctas(int n) { return n <= 3 ? BgCfg<3>::CTAS : BgCfg<5>::CTAS; }
+// for every process.  (The kernel is parametrised on the split and on the CTAs per SM.)  FP32/mixed n = 4: 12 worker warps with 152
+// registers (hand-over from the colour warps) and 8 event slots: 6.35 -> 5.70 ms (16 workers at 104 registers: 6.47).  n = 5 stays at 8:
+// one event slot gives 240 amplitude tasks per batch, a second slot does not fit beside the FP64 amplitude buffers.
+#ifndef RWGT_NW32_N4
+#define RWGT_NW32_N4 12
+#endif
+template <int N, typename T> struct BgCfg { static constexpr int NW = (N == 4 && sizeof(T) == 4) ? RWGT_NW32_N4 : 8, NCW = 4, CTAS = 1; };
+static int bg_nw(int n, bool dbl) { return (n == 4 && !dbl) ? BgCfg<4, float>::NW : 8; }
+static int bg_ctas(int) { return 1; }
 
 template <int N> static cudaError_t bg_set_attr(size_t s64, size_t s32) {
-  typedef BgCfg<N> Cf;
-  cudaError_t e = cudaFuncSetAttribute(bg_kernel<N, double, false, Cf::NW, Cf::NCW, Cf::CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s64);
+  typedef BgCfg<N, double> Cd; typedef BgCfg<N, float> Cf;
+  cudaError_t e = cudaFuncSetAttribute(bg_kernel<N, double, false, Cd::NW, Cd::NCW, Cd::CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s64);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, false, Cf::NW, Cf::NCW, Cf::CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, true, Cf::NW, Cf::NCW, Cf::CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
   return e;
 }
 template <int N> static void bg_launch(int precision, int grid, size_t s64, size_t s32, cudaStream_t st, const double* mom, const double* w,
                                        double* a, double* b, double* o, long long nev, long long stride, long long ostride, const BgDev& D) {
-  typedef BgCfg<N> Cf;
-  const int nth = (Cf::NW + Cf::NCW) * 32;
-  if (precision == RWGT_FP64) bg_kernel<N, double, false, Cf::NW, Cf::NCW, Cf::CTAS><<<grid, nth, s64, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
-  else if (precision == RWGT_FP32) bg_kernel<N, float, false, Cf::NW, Cf::NCW, Cf::CTAS><<<grid, nth, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
-  else bg_kernel<N, float, true, Cf::NW, Cf::NCW, Cf::CTAS><<<grid, nth, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
+  typedef BgCfg<N, double> Cd; typedef BgCfg<N, float> Cf;
+  if (precision == RWGT_FP64) bg_kernel<N, double, false, Cd::NW, Cd::NCW, Cd::CTAS><<<grid, (Cd::NW + Cd::NCW) * 32, s64, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
+  else if (precision == RWGT_FP32) bg_kernel<N, float, false, Cf::NW, Cf::NCW, Cf::CTAS><<<grid, (Cf::NW + Cf::NCW) * 32, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
+  else bg_kernel<N, float, true, Cf::NW, Cf::NCW, Cf::CTAS><<<grid, (Cf::NW + Cf::NCW) * 32, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
 }
 
 static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::string& err) {
@@ -968,7 +972,7 @@ static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::stri
   B->sm_count = prop.multiProcessorCount; size_t maxsm = prop.sharedMemPerBlockOptin;
   // event slots per CTA: as many as make the amplitude phase fill the 256 worker threads (npair * 4 tasks per slot and batch)
   auto pick = [&](bool dbl, int& nslot, size_t& bytes) {
-    int cap = std::max(1, std::min(64, (bg_nw(n) * 32) / (S.npair * (n == 2 ? 2 : 4)))); nslot = 0;
+    int cap = std::max(1, std::min(64, (bg_nw(n, dbl) * 32) / (S.npair * (n == 2 ? 2 : 4)))); nslot = 0;
     // with k CTAs per SM each gets 1/k of the SM's shared memory (1 KB per CTA is reserved by the system)
     size_t budget = std::min(maxsm, prop.sharedMemPerMultiprocessor / bg_ctas(n) - 1024);
     for (int e = cap; e >= 1; e--) if (smem_need_n(n, S, e, dbl) <= budget) { nslot = e; break; }
