@@ -399,14 +399,15 @@ template <int N, typename T> __host__ __device__ inline size_t carve(Smem<T>& s,
   s.iK2 = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
   s.dR = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
   s.dL = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
-  s.pmS = (double*)(base + off); off += sizeof(double) * ns * (N + 2) * 4; al();
-  s.GS = (cx<T>*)(base + off); off += sizeof(T) * (size_t)ns * 8 * (2 * N); al();
-  s.RS = (cx<T>*)(base + off); off += sizeof(T) * (size_t)ns * 8 * 2; al();
-  s.LS = (cx<T>*)(base + off); off += sizeof(T) * (size_t)ns * 8 * 2; al();
-  s.KS = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK * 4; al();
-  s.iK2S = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
-  s.dRS = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
-  s.dLS = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
+  const int nst = (N >= 4) ? ns : 0;                         // staging exists only where the colour warps prefetch (bg_kernel: STAGE)
+  s.pmS = (double*)(base + off); off += sizeof(double) * nst * (N + 2) * 4; al();
+  s.GS = (cx<T>*)(base + off); off += sizeof(T) * (size_t)nst * 8 * (2 * N); al();
+  s.RS = (cx<T>*)(base + off); off += sizeof(T) * (size_t)nst * 8 * 2; al();
+  s.LS = (cx<T>*)(base + off); off += sizeof(T) * (size_t)nst * 8 * 2; al();
+  s.KS = (T*)(base + off); off += sizeof(T) * nst * Ge::NMASK * 4; al();
+  s.iK2S = (T*)(base + off); off += sizeof(T) * nst * Ge::NMASK; al();
+  s.dRS = (T*)(base + off); off += sizeof(T) * nst * Ge::NMASK; al();
+  s.dLS = (T*)(base + off); off += sizeof(T) * nst * Ge::NMASK; al();
   s.W = (uint32_t*)(base + off); off += sizeof(uint32_t) * nwords; al();
   return off;
 }
@@ -925,8 +926,14 @@ static size_t smem_need_n(int n, const BgSched& S, int nslot, bool dbl) {
 #ifndef RWGT_NW32_N4
 #define RWGT_NW32_N4 12
 #endif
-template <int N, typename T> struct BgCfg { static constexpr int NW = (N == 4 && sizeof(T) == 4) ? RWGT_NW32_N4 : 8, NCW = 4, CTAS = 1; };
-static int bg_nw(int n, bool dbl) { return (n == 4 && !dbl) ? BgCfg<4, float>::NW : 8; }
+#ifndef RWGT_NW64_N4
+#define RWGT_NW64_N4 8
+#endif
+#ifndef RWGT_NW32_N3
+#define RWGT_NW32_N3 12
+#endif
+template <int N, typename T> struct BgCfg { static constexpr int NW = (N == 4) ? (sizeof(T) == 4 ? RWGT_NW32_N4 : RWGT_NW64_N4) : (N == 3 && sizeof(T) == 4) ? RWGT_NW32_N3 : 8, NCW = 4, CTAS = 1; };
+static int bg_nw(int n, bool dbl) { return n == 4 ? (dbl ? BgCfg<4, double>::NW : BgCfg<4, float>::NW) : (n == 3 && !dbl) ? BgCfg<3, float>::NW : 8; }
 static int bg_ctas(int) { return 1; }
 
 template <int N> static cudaError_t bg_set_attr(size_t s64, size_t s32) {
