@@ -44,6 +44,9 @@ template <int NG> struct PhGeo {
                        O_W = O_IQ2 + NSUB, O_PSI = O_W + 4, SLOT = O_PSI + 4 * NENT;
 };
 
+// barrier over the cooperating group: the whole CTA (CG == NTH) or one warp (CG == 32)
+template <int CG, int NTH> __device__ __forceinline__ void gsync() { if constexpr (CG == NTH) __syncthreads(); else __syncwarp(); }
+
 // y += B x for a 2x2 complex block B = (m[0] m[1]; m[2] m[3])
 __device__ __forceinline__ void block_acc(cx<double>& y0, cx<double>& y1, const cx<double>* m, cx<double> x0, cx<double> x1) {
   cfma(y0, m[0], x0); cfma(y0, m[1], x1); cfma(y1, m[2], x0); cfma(y1, m[3], x1);
@@ -53,11 +56,11 @@ __device__ __forceinline__ void block_acc(cx<double>& y0, cx<double>& y1, const 
 // for every other member the block is shared and the two spinors are neighbours (entry + 2^(K-2)); this halves the shared-memory
 // wavefronts per block product, which is what bounds this kernel.
 // s_child[S][r] = (first entry of S without its r-th member) << 8 | (2 * that member's label).
-template <int NG, int K, int E, int NTH>
+template <int NG, int K, int E, int CG, int NTH>
 __device__ __forceinline__ void photon_level(double* sm, const unsigned char* s_sub, const unsigned short* s_off, const unsigned* s_child, int first_sub, int tid) {
   typedef PhGeo<NG> Ge;
   constexpr int NENT = Ge::NENT, KL = K - 1, per = binom(NG, K) << KL;
-  for (int t = tid; t < E * per; t += NTH) {
+  for (int t = tid; t < E * per; t += CG) {
     const int sl = t / per, o = t - sl * per; const int S = s_sub[first_sub + (o >> KL)]; const unsigned v = o & ((1u << KL) - 1u);
     double* s = sm + sl * Ge::SLOT;
     const cx<double>* M = reinterpret_cast<const cx<double>*>(s + Ge::O_EPS);
@@ -89,17 +92,19 @@ __device__ __forceinline__ void photon_level(double* sm, const unsigned char* s_
     const int eo = s_off[S] + (int)v;
     stc(T + eo, o0); stc(T + NENT + eo, o1); stc(T + eo + (1 << KL), u0); stc(T + NENT + eo + (1 << KL), u1);
   }
-  __syncthreads();
+  gsync<CG, NTH>();
 }
-template <int NG, int K, int E, int NTH>
+template <int NG, int K, int E, int CG, int NTH>
 __device__ __forceinline__ void photon_levels(double* sm, const unsigned char* s_sub, const unsigned short* s_off, const unsigned* s_child, const unsigned char* s_lvl, int tid) {
   if constexpr (K < NG) {
-    photon_level<NG, K, E, NTH>(sm, s_sub, s_off, s_child, s_lvl[K], tid);
-    photon_levels<NG, K + 1, E, NTH>(sm, s_sub, s_off, s_child, s_lvl, tid);
+    photon_level<NG, K, E, CG, NTH>(sm, s_sub, s_off, s_child, s_lvl[K], tid);
+    photon_levels<NG, K + 1, E, CG, NTH>(sm, s_sub, s_off, s_child, s_lvl, tid);
   }
 }
 
-template <int NG, int E, int NTH>
+// E events per cooperating group of CG threads (CG == NTH: the CTA, levels separated by __syncthreads; CG == 32: each warp works on
+// its own E events and only ever waits for itself)
+template <int NG, int E, int CG, int NTH>
 __global__ void __launch_bounds__(NTH) epem_photons_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
                                                            double* __restrict__ me_old, double* __restrict__ me_new,
                                                            double* __restrict__ w_new, long long nev, long long stride, long long ostride,
@@ -107,13 +112,13 @@ __global__ void __launch_bounds__(NTH) epem_photons_kernel(const double* __restr
   typedef PhGeo<NG> Ge;
   constexpr int next = NG + 2, NSUB = Ge::NSUB, NENT = Ge::NENT;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  double* sm = reinterpret_cast<double*>(smem_raw);
+  const int tid = (CG == NTH) ? (int)threadIdx.x : (int)(threadIdx.x & 31u);                        // index within the group
+  double* sm = reinterpret_cast<double*>(smem_raw) + (CG == NTH ? 0 : (threadIdx.x >> 5) * E * Ge::SLOT);   // the group's event slots
   __shared__ unsigned short s_off[NSUB];            // first entry of subset S
   __shared__ unsigned char s_sub[NSUB];             // subsets ordered by (size, value)
   __shared__ unsigned char s_lvl[NG + 2];           // s_sub index of the first subset of each size
   __shared__ unsigned s_child[NSUB * NG];           // (first entry of S without its r-th member) << 8 | 2 * member label
-  const int tid = threadIdx.x;
-  if (tid == 0) {
+  if (threadIdx.x == 0) {
     int o = 0; for (int S = 0; S < NSUB; S++) { s_off[S] = (unsigned short)o; o += 1 << __popc(S); }
     int j = 0; for (int k = 0; k <= NG; k++) { s_lvl[k] = (unsigned char)j; for (int S = 0; S < NSUB; S++) if (__popc(S) == k) s_sub[j++] = (unsigned char)S; }
     s_lvl[NG + 1] = (unsigned char)j;
@@ -121,16 +126,17 @@ __global__ void __launch_bounds__(NTH) epem_photons_kernel(const double* __restr
   }
   __syncthreads();
   const long long ngroups = (nev + E - 1) / E;
-  for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
+  constexpr int GPB = NTH / CG;                                      // groups per CTA
+  for (long long grp = (long long)blockIdx.x * GPB + (CG == NTH ? 0 : threadIdx.x >> 5); grp < ngroups; grp += (long long)gridDim.x * GPB) {
     const long long ev0 = grp * E;
     // ---- a1: momenta (coalesced over the events of the group) ----
-    for (int t = tid; t < E * next * 4; t += NTH) {
+    for (int t = tid; t < E * next * 4; t += CG) {
       int sl = t % E, comp = t / E; long long ev = ev0 + sl; if (ev >= nev) ev = nev - 1;
       sm[sl * Ge::SLOT + Ge::O_PM + comp] = __ldg(mom + (size_t)comp * stride + ev);
     }
-    __syncthreads();
+    gsync<CG, NTH>();
     // ---- a2: external wavefunctions, momenta and inverse virtualities of the electron line ----
-    for (int t = tid; t < E * Ge::NEXTOBJ; t += NTH) {
+    for (int t = tid; t < E * Ge::NEXTOBJ; t += CG) {
       int sl = t / Ge::NEXTOBJ, o = t % Ge::NEXTOBJ; double* s = sm + sl * Ge::SLOT; const double* pm = s + Ge::O_PM;
       if (o < 2 * NG) {                            // photon i, helicity bit hb (0: +1, 1: -1): the block (eps0 - sigma.eps*) = [[m, -r], [-l, p]]
         int i = o >> 1, hb = o & 1; const double* k = pm + 4 * (i + 2);
@@ -153,13 +159,13 @@ __global__ void __launch_bounds__(NTH) epem_photons_kernel(const double* __restr
         s[Ge::O_IQ2 + S] = (S != 0 && S != NSUB - 1) ? 1.0 / mdot_rr(q, q) : 0.0;
       }
     }
-    __syncthreads();
+    gsync<CG, NTH>();
     // ---- a3: current levels k = 1 .. NG-1 ----
-    photon_levels<NG, 1, E, NTH>(sm, s_sub, s_off, s_child, s_lvl, tid);
+    photon_levels<NG, 1, E, CG, NTH>(sm, s_sub, s_off, s_child, s_lvl, tid);
     // ---- a4-a7: the 2^NG amplitudes of an event, two per thread (both helicities of the last photon) in 2^(NG-1) consecutive lanes,
     //             helicity sum by a fixed shuffle tree, eq. 3 ----
     constexpr int NFIN = E << (NG - 1), NFIN_W = (NFIN + 31) / 32 * 32;       // whole warps take part in the shuffles
-    for (int t0 = tid; t0 < NFIN_W; t0 += NTH) {
+    for (int t0 = tid; t0 < NFIN_W; t0 += CG) {
       const bool live = t0 < NFIN; const int t = live ? t0 : 0;
       const int sl = t >> (NG - 1); const unsigned v = t & (NSUB / 2 - 1);
       const double* s = sm + sl * Ge::SLOT;
@@ -196,7 +202,7 @@ __global__ void __launch_bounds__(NTH) epem_photons_kernel(const double* __restr
         }
       }
     }
-    __syncthreads();
+    gsync<CG, NTH>();
   }
 }
 
@@ -214,25 +220,30 @@ static double photon_flops_per_event(int ng) {
 
 // host side: E = 8 events per CTA, 256 threads (the 8 x 32 final amplitudes of n = 5 are one task per thread), 3 CTAs per SM.
 // Measured on B200 (n = 5, 131072 events), one variant per thread: E/threads 16/512 0.503 ms, 12/384 0.449, 8/256 0.410, 6/192 0.405,
-// 4/128 0.408; two variants per thread: 8/256 0.398, 6/128 0.401, 12/256 0.421, 8/128 0.428, 16/256 0.565.
+// 4/128 0.408; two variants per thread: 8/256 0.398, 6/128 0.401, 12/256 0.421, 8/128 0.428, 16/256 0.565; warp-cooperative groups
+// (CG = 32, no CTA barriers) with E events per warp / threads per CTA: 2/128 0.414, 2/64 0.415, 1/128 0.474, 4/64 0.608.  Every variant
+// lands at ~0.40 ms: the shared-memory data pipe (72-75 % of its wavefront peak; an LDS.128 costs four wavefronts whether or not lanes
+// share addresses, and every 2x2 block product reads 6 of them for 16 DFMAs) is the bound, not barriers or occupancy.
 #ifndef RWGT_PH_E
 #define RWGT_PH_E 8
+#define RWGT_PH_CG 256
 #define RWGT_PH_NTH 256
 #endif
-constexpr int PH_E = RWGT_PH_E, PH_NTH = RWGT_PH_NTH;
+constexpr int PH_E = RWGT_PH_E, PH_CG = RWGT_PH_CG, PH_NTH = RWGT_PH_NTH;
 template <int NG> static cudaError_t photon_launch_n(int sm_count, cudaStream_t st, const double* mom, const double* w, double* a, double* b, double* o,
                                                      long long nev, long long stride, long long ostride, const PhotonParams& P) {
   static bool attr_set = false;
-  const size_t smem = sizeof(double) * PH_E * PhGeo<NG>::SLOT;
+  constexpr int GPB = PH_NTH / PH_CG;
+  const size_t smem = sizeof(double) * GPB * PH_E * PhGeo<NG>::SLOT;
   if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(epem_photons_kernel<NG, PH_E, PH_NTH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(epem_photons_kernel<NG, PH_E, PH_CG, PH_NTH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     attr_set = true;
   }
-  const long long ngroups = (nev + PH_E - 1) / PH_E;
+  const long long ngroups = (nev + PH_E - 1) / PH_E, nblocks = (ngroups + GPB - 1) / GPB;
   const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(2048 / PH_NTH, (size_t)(227 * 1024) / (smem + 2048)));
-  const int grid = (int)std::min<long long>(ngroups, (long long)sm_count * per_sm);
-  epem_photons_kernel<NG, PH_E, PH_NTH><<<grid, PH_NTH, smem, st>>>(mom, w, a, b, o, nev, stride, ostride, P);
+  const int grid = (int)std::min<long long>(nblocks, (long long)sm_count * per_sm);
+  epem_photons_kernel<NG, PH_E, PH_CG, PH_NTH><<<grid, PH_NTH, smem, st>>>(mom, w, a, b, o, nev, stride, ostride, P);
   return cudaSuccess;
 }
 static cudaError_t photon_launch(int ng, int sm_count, cudaStream_t st, const double* mom, const double* w, double* a, double* b, double* o,
