@@ -922,7 +922,8 @@ static size_t smem_need_n(int n, const BgSched& S, int nslot, bool dbl) {
 // sub-partition.  Measured on B200 against 10+2, 6+2, 12+4 and (n = 3) two CTAs of 4+2 warps per SM: best or within 4 % of best
 // for every process.  (The kernel is parametrised on the split and on the CTAs per SM.)  FP32/mixed n = 4: 12 worker warps with 152
 // registers (hand-over from the colour warps) and 8 event slots: 6.35 -> 5.70 ms (16 workers at 104 registers: 6.47).  n = 5 stays at 8:
-// one event slot gives 240 amplitude tasks per batch, a second slot does not fit beside the FP64 amplitude buffers.
+// one event slot gives 240 amplitude tasks per batch, a second slot does not fit beside the FP64 amplitude buffers.  FP32/mixed n = 3:
+// 12 workers 3.79 -> 3.16 ms.  FP64 with 12 workers at 152 registers is slower (n = 4: 10.9 -> 11.9 ms, n = 3: 5.39 -> 5.50 ms).
 #ifndef RWGT_NW32_N4
 #define RWGT_NW32_N4 12
 #endif
@@ -932,8 +933,11 @@ static size_t smem_need_n(int n, const BgSched& S, int nslot, bool dbl) {
 #ifndef RWGT_NW32_N3
 #define RWGT_NW32_N3 12
 #endif
-template <int N, typename T> struct BgCfg { static constexpr int NW = (N == 4) ? (sizeof(T) == 4 ? RWGT_NW32_N4 : RWGT_NW64_N4) : (N == 3 && sizeof(T) == 4) ? RWGT_NW32_N3 : 8, NCW = 4, CTAS = 1; };
-static int bg_nw(int n, bool dbl) { return n == 4 ? (dbl ? BgCfg<4, double>::NW : BgCfg<4, float>::NW) : (n == 3 && !dbl) ? BgCfg<3, float>::NW : 8; }
+#ifndef RWGT_NW64_N3
+#define RWGT_NW64_N3 8
+#endif
+template <int N, typename T> struct BgCfg { static constexpr int NW = (N == 4) ? (sizeof(T) == 4 ? RWGT_NW32_N4 : RWGT_NW64_N4) : (N == 3) ? (sizeof(T) == 4 ? RWGT_NW32_N3 : RWGT_NW64_N3) : 8, NCW = 4, CTAS = 1; };
+static int bg_nw(int n, bool dbl) { return n == 4 ? (dbl ? BgCfg<4, double>::NW : BgCfg<4, float>::NW) : n == 3 ? (dbl ? BgCfg<3, double>::NW : BgCfg<3, float>::NW) : 8; }
 static int bg_ctas(int) { return 1; }
 
 template <int N> static cudaError_t bg_set_attr(size_t s64, size_t s32) {

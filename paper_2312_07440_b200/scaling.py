@@ -2,7 +2,7 @@
 against the number of events for one parameter set; Fig. 3: runtime against the number of parameter sets), run
 through this library on one GPU.  As in the paper every point is the mean of 5 runs with its min/max.
 
-    python -m paper_2312_07440_b200.scaling [--max-log2 20] [--sets 1,2,4,8,16] [--fig3-events 131072]
+    python -m paper_2312_07440_b200.scaling [--config 6] [--max-log2 20] [--sets 1,2,4,8,16] [--fig3-events 131072]
 
 Columns: device = rwgt_run_multi on device-resident buffers (CUDA events); host = rwgt_run_multi_host on pinned host buffers,
 host<->device copies inside the timed call (the transfer overhead the paper describes for small n).
@@ -22,10 +22,11 @@ def main() -> None:
     ap.add_argument("--max-log2", type=int, default=20)
     ap.add_argument("--sets", default="1,2,4,8,16")
     ap.add_argument("--fig3-events", type=int, default=131072)
+    ap.add_argument("--config", type=int, default=6, help="6 = the paper's process; 1..5 = the BASELINE.json configs (SURVEY 8(d) D3 sweep)")
     args = ap.parse_args()
     import torch
     from . import binding as B, events as ev
-    c = ev.config(6)
+    c = ev.config(args.config)
     nmax = max(1 << args.max_log2, args.fig3_events)
     m0, w0 = ev.generate(c, min(nmax, c.n_events))
     reps = (nmax + m0.shape[2] - 1) // m0.shape[2]
@@ -34,7 +35,11 @@ def main() -> None:
     rng = np.random.default_rng(c.seed)
 
     def new_sets(k):
-        return [ev.params(alpha_em=float(a)) for a in rng.uniform(0.5, 2.0, size=k) / 132.5]
+        if c.index == 6:      # a random electroweak coupling per set
+            return [ev.params(alpha_em=float(a)) for a in rng.uniform(0.5, 2.0, size=k) / 132.5]
+        if c.index == 1:
+            return [ev.params(GammaZ=float(g), sin2_thetaW=float(x)) for g, x in zip(rng.uniform(2.3, 2.7, size=k), rng.uniform(0.22, 0.24, size=k))]
+        return [ev.params(ggg_scale=float(1 + x), gggg_scale=float(1 + x)) for x in rng.uniform(-0.2, 0.2, size=k)]
 
     def measure(n, K):
         sets = new_sets(K)
@@ -64,6 +69,7 @@ def main() -> None:
         B.rwgt_destroy(h)
         return dev, host
 
+    print(f"# {c.process} (config {c.index}), FP64\n")
     print("## Runtime against the number of events, one parameter set (PAPER.md:105 Fig. 2), ms: mean (min-max) of 5\n")
     print("| events | device ms | host-buffer ms | device events/s | host-buffer events/s |\n|---|---|---|---|---|")
     for lg in range(0, args.max_log2 + 1, 2):
