@@ -143,8 +143,9 @@ __global__ void __launch_bounds__(128) gg_ttx_kernel(const double* __restrict__ 
   me_old[i] = a; me_new[i] = b; w_new[i] = W * (b / a);
 }
 
-// K > 1 new sets of equal top mass: the helicity amplitudes X12, X21, Y are formed once, every set is one more
-// pair of real FMAs and one more colour form (PAPER.md:87 step 7).  sums[k] for k < nsets.
+// K > 1 new sets of equal top mass: the 8 x 3 helicity amplitudes X12, X21, Y are formed once by the same fully unrolled code as
+// in ggttx_sums and kept (registers / L1-resident local memory); every set is then one more pair of real FMAs and one more colour form
+// per helicity (PAPER.md:87 step 7).  sums[k] for k < nsets.
 __device__ __forceinline__ void ggttx_sums_multi(const double (*p)[4], double m, const double* s3, int nsets, double* sums) {
   const double* k1 = p[0]; const double* k2 = p[1];
   double q1[4], q2[4], kk[4];
@@ -153,34 +154,37 @@ __device__ __forceinline__ void ggttx_sums_multi(const double (*p)[4], double m,
   double m2 = m * m;
   double d1 = -1.0 / (mdot_rr(q1, q1) - m2), d2 = -1.0 / (mdot_rr(q2, q2) - m2), ds = -1.0 / mdot_rr(kk, kk);
   chi_pair<double> xt = make_chi(p[2][1], p[2][2], p[2][3]), xb = make_chi(p[3][1], p[3][2], p[3][3]);
-#pragma unroll
-  for (int k = 0; k < SMALL_NSMAX; k++) sums[k] = 0;
+  cx<double> aX12[8], aX21[8], aY[8];
   vec4<double> e1 = polvec(k1[1], k1[2], k1[3], +1);
-#pragma unroll 1
+#pragma unroll
   for (int i2 = 0; i2 < 2; i2++) {
     vec4<double> e2 = polvec(k2[1], k2[2], k2[3], i2 ? -1 : +1);
     vec4<double> l3; for (int mu = 0; mu < 4; mu++) l3.c[mu] = mk<double>(0, 0);
     L3_acc(l3, e1, k1, e2, k2);
     for (int mu = 0; mu < 4; mu++) l3.c[mu] = ds * l3.c[mu];
-#pragma unroll 1
+#pragma unroll
     for (int ib = 0; ib < 2; ib++) {
       spn<double> v = spinor_v(xb, p[3][0], m, ib ? -1 : +1);
       spn<double> psi1 = slash_r_plus_m(q1, m, slash_c(e1, v)), psi2 = slash_r_plus_m(q2, m, slash_c(e2, v));
       spn<double> c12 = slash_c(e1, psi2), c21 = slash_c(e2, psi1), cy = slash_c(l3, v);
-#pragma unroll 1
+#pragma unroll
       for (int it = 0; it < 2; it++) {
         spn<double> ub = bar(spinor_u(xt, p[2][0], m, it ? -1 : +1));
-        cx<double> X12 = d2 * rowcol(ub, c12), X21 = d1 * rowcol(ub, c21), Y = rowcol(ub, cy);
-#pragma unroll
-        for (int k = 0; k < SMALL_NSMAX; k++) if (k < nsets) {
-          cx<double> A1 = X12, A2 = X21; rfma(A1, s3[k], Y); rfma(A2, -s3[k], Y);
-          sums[k] += 16.0 * (norm2(A1) + norm2(A2)) - 4.0 * (A1.re * A2.re + A1.im * A2.im);
-        }
+        const int h = (i2 * 2 + ib) * 2 + it;
+        aX12[h] = d2 * rowcol(ub, c12); aX21[h] = d1 * rowcol(ub, c21); aY[h] = rowcol(ub, cy);
       }
     }
   }
+#pragma unroll 1
+  for (int k = 0; k < nsets; k++) {
+    const double sk = s3[k]; double acc = 0;
 #pragma unroll
-  for (int k = 0; k < SMALL_NSMAX; k++) sums[k] *= 2.0 / 3.0;
+    for (int h = 0; h < 8; h++) {
+      cx<double> A1 = aX12[h], A2 = aX21[h]; rfma(A1, sk, aY[h]); rfma(A2, -sk, aY[h]);
+      acc += 16.0 * (norm2(A1) + norm2(A2)) - 4.0 * (A1.re * A2.re + A1.im * A2.im);
+    }
+    sums[k] = acc * (2.0 / 3.0);
+  }
 }
 
 __global__ void __launch_bounds__(128) gg_ttx_multi_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
