@@ -50,7 +50,7 @@ def test_multi_set_fp64_parity_every_event(idx, n):
     assert np.array_equal(got[1 + k_same], got[0]) and np.array_equal(got[1 + K + k_same], w)
 
 
-@pytest.mark.parametrize("idx,n", [(2, 515), (3, 301)])
+@pytest.mark.parametrize("idx,n", [(2, 515), (3, 301), (4, 47), (5, 7)])
 def test_multi_set_with_different_top_masses(idx, n):
     """A set with another top mass makes the library redo externals, momentum sums and denominators for that set
     (reading R12).  The comparison with the oracle is only defined for momenta on the mass shell of the set's own m_t
