@@ -49,14 +49,18 @@ __global__ void __launch_bounds__(256, 3) epem_mupmum_kernel(const double* __res
   chi_pair<double> x1 = make_chi(p[0][1], p[0][2], p[0][3]), x2 = make_chi(p[1][1], p[1][2], p[1][3]);
   chi_pair<double> x3 = make_chi(p[2][1], p[2][2], p[2][3]), x4 = make_chi(p[3][1], p[3][2], p[3][3]);
   // massless: sqrt(E+|p|) with |p| from the 3-momentum (mass parameter 0, reading Q8)
-  double ce = sqrt((p[0][0] + x1.pabs) * (p[1][0] + x2.pabs)), cm = sqrt((p[2][0] + x3.pabs) * (p[3][0] + x4.pabs));
-  // electron line vbar(p1) gamma^mu u(p2): L = (lam1,lam2) = (+,-), R = (-,+)
-  vec4<double> JeL = bilinear2(x1.m, x2.m, true), JeR = bilinear2(x1.p, x2.p, false);
-  // muon line ubar(p4) gamma^mu v(p3): L = (lam3,lam4) = (+,-), R = (-,+)
-  vec4<double> JmL = bilinear2(x4.m, x3.m, true), JmR = bilinear2(x4.p, x3.p, false);
-  double c2 = ce * cm; c2 *= c2;
-  double dLL = norm2(mdot_cc(JeL, JmL)) * c2, dLR = norm2(mdot_cc(JeL, JmR)) * c2;
-  double dRL = norm2(mdot_cc(JeR, JmL)) * c2, dRR = norm2(mdot_cc(JeR, JmR)) * c2;
+  // spinor normalisations sqrt(E+|p|) of the four legs enter every |amplitude|^2 as the product of the four (E+|p|): no square root
+  const double nrm = ((p[0][0] + x1.pabs) * (p[1][0] + x2.pabs)) * ((p[2][0] + x3.pabs) * (p[3][0] + x4.pabs));
+  // electron line vbar(p1) gamma^mu u(p2): L = (lam1,lam2) = (+,-), R = (-,+); muon line ubar(p4) gamma^mu v(p3) likewise.  The four
+  // current contractions J_e . J_mu are done by the Fierz identities of the Pauli matrices (sigma^mu = (1, sigma), sigmabar^mu = (1, -sigma)):
+  //   (a^+ sigmabar^mu b)(c^+ sigmabar_mu d) = (a^+ sigma^mu b)(c^+ sigma_mu d) = 2 conj(a ^ c) (b ^ d),   x ^ y = x_1 y_2 - x_2 y_1,
+  //   (a^+ sigmabar^mu b)(c^+ sigma_mu d) = 2 (a^+ d)(c^+ b),
+  // i.e. every helicity amplitude is a product of two two-spinor products (bilinear2 above is the explicit current, kept for reference).
+  auto wedge = [](const cx<double>* x, const cx<double>* y) { cx<double> r = x[0] * y[1]; cfms(r, x[1], y[0]); return norm2(r); };
+  auto inner = [](const cx<double>* x, const cx<double>* y) { cx<double> r = conj(x[0]) * y[0]; cfma(r, conj(x[1]), y[1]); return norm2(r); };
+  const double c2 = 4.0 * nrm;
+  double dLL = wedge(x1.m, x4.m) * wedge(x2.m, x3.m) * c2, dRR = wedge(x1.p, x4.p) * wedge(x2.p, x3.p) * c2;
+  double dLR = inner(x1.m, x3.p) * inner(x4.p, x2.m) * c2, dRL = inner(x1.p, x3.m) * inner(x4.m, x2.p) * c2;
   double me0 = 0;
 #pragma unroll 1
   for (int k = 0; k < P.nsets; k++) {

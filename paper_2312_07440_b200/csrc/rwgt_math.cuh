@@ -130,7 +130,7 @@ template <typename T> __device__ __forceinline__ chi_pair<T> make_chi(T px, T py
   if (pabs == T(0)) { r.p[0] = mk<T>(1, 0); r.p[1] = mk<T>(0, 0); r.m[0] = mk<T>(0, 0); r.m[1] = mk<T>(1, 0); return r; }
   if (pt2 == T(0) && pz < T(0)) { r.p[0] = mk<T>(0, 0); r.p[1] = mk<T>(1, 0); r.m[0] = mk<T>(-1, 0); r.m[1] = mk<T>(0, 0); return r; }
   T ppz = (pz >= T(0)) ? pabs + pz : pt2 / (pabs - pz);     // |p|+pz, cancellation-free
-  T N = T(1) / sqrt(T(2) * pabs * ppz);
+  T N = rsqrt(T(2) * pabs * ppz);
   r.p[0] = mk<T>(N * ppz, 0); r.p[1] = mk<T>(N * px, N * py);
   r.m[0] = mk<T>(-N * px, N * py); r.m[1] = mk<T>(N * ppz, 0);
   return r;
