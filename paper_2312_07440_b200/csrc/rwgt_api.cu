@@ -145,11 +145,11 @@ int rwgt_n_external(const rwgt_handle* h) { return h ? h->n_ext : -1; }
 double rwgt_flops_per_event(const rwgt_handle* h) {
   if (!h) return -1.0;
   // the two one-event-per-thread kernels: ncu counters of the committed build (152 DFMA + 105 DMUL + 17 DADD resp.
-  // 1243 DFMA + 366 DMUL + 87 DADD per event; profiles/r1_summary.md)
+  // 1225 DFMA + 365 DMUL + 87 DADD per event; profiles/r1_summary.md)
   if (h->proc == P_EPEM) return 426.0 + (h->nsets - 2) * 45.0;
   if (h->proc == P_PHOTONS) return rwgt::photon_flops_per_event(h->n_photons);
-  // gg_ttx: 2939 for two sets of equal mass; a further set of equal mass costs 8 helicities x (4 FMA + colour form 5 FMA + 4 MUL/ADD)
-  if (h->proc == P_GG_TTX) return h->ggttx.two_pass ? h->nsets * 2939.0 : 2939.0 + (h->nsets - 2) * 8 * 26.0;
+  // gg_ttx: 2902 for two sets of equal mass; a further set of equal mass costs 8 helicities x (4 FMA + colour form 5 FMA + 4 MUL/ADD)
+  if (h->proc == P_GG_TTX) return h->ggttx.two_pass ? h->nsets * 2902.0 : 2902.0 + (h->nsets - 2) * 8 * 26.0;
   return rwgt::bg_flops_per_event(h->bg, h->precision);
 }
 

@@ -137,13 +137,13 @@ template <typename T> __device__ __forceinline__ chi_pair<T> make_chi(T px, T py
 }
 // u(p,lam) = ( sqrt(E-lam|p|) chi_lam , sqrt(E+lam|p|) chi_lam )
 template <typename T> __device__ __forceinline__ spn<T> spinor_u(const chi_pair<T>& x, T E, T m, int lam) {
-  T sp = sqrt(E + x.pabs), sm = (m == T(0)) ? T(0) : m / sp;
+  const T ep = E + x.pabs, ir = rsqrt(ep), sp = ep * ir, sm = m * ir;     // sqrt(E+|p|), sqrt(E-|p|) = m / sqrt(E+|p|); one rsqrt, no division
   const cx<T>* c = lam > 0 ? x.p : x.m; T a = lam > 0 ? sm : sp, b = lam > 0 ? sp : sm;
   spn<T> r; r.c[0] = a * c[0]; r.c[1] = a * c[1]; r.c[2] = b * c[0]; r.c[3] = b * c[1]; return r;
 }
 // v(p,lam) = ( -lam sqrt(E+lam|p|) chi_{-lam} , lam sqrt(E-lam|p|) chi_{-lam} )
 template <typename T> __device__ __forceinline__ spn<T> spinor_v(const chi_pair<T>& x, T E, T m, int lam) {
-  T sp = sqrt(E + x.pabs), sm = (m == T(0)) ? T(0) : m / sp;
+  const T ep = E + x.pabs, ir = rsqrt(ep), sp = ep * ir, sm = m * ir;     // sqrt(E+|p|), sqrt(E-|p|) = m / sqrt(E+|p|); one rsqrt, no division
   const cx<T>* c = lam > 0 ? x.m : x.p; T a = lam > 0 ? -sp : sm, b = lam > 0 ? sm : -sp;
   spn<T> r; r.c[0] = a * c[0]; r.c[1] = a * c[1]; r.c[2] = b * c[0]; r.c[3] = b * c[1]; return r;
 }
@@ -153,10 +153,10 @@ template <typename T> __device__ __forceinline__ spn<T> bar(const spn<T>& s) {
 }
 // eps(p,lam) = (0, (-lam e1 - i e2)/sqrt2), spatial-transverse in the given frame (binding, reading Q1)
 template <typename T> __device__ __forceinline__ vec4<T> polvec(T px, T py, T pz, int lam) {
-  T pt2 = px * px + py * py, pt = sqrt(pt2), pabs = sqrt(pt2 + pz * pz);
+  T pt2 = px * px + py * py;
   T e1x, e1y, e1z, e2x, e2y;
-  if (pt == T(0)) { e1x = pz >= T(0) ? T(1) : T(-1); e1y = 0; e1z = 0; e2x = 0; e2y = 1; }
-  else { T inv = T(1) / (pabs * pt); e1x = px * pz * inv; e1y = py * pz * inv; e1z = -pt2 * inv; T ip = T(1) / pt; e2x = -py * ip; e2y = px * ip; }
+  if (pt2 == T(0)) { e1x = pz >= T(0) ? T(1) : T(-1); e1y = 0; e1z = 0; e2x = 0; e2y = 1; }
+  else { T ip = rsqrt(pt2), inv = ip * rsqrt(pt2 + pz * pz); e1x = px * pz * inv; e1y = py * pz * inv; e1z = -pt2 * inv; e2x = -py * ip; e2y = px * ip; }   // 1/pT, 1/(|p| pT)
   const T s = T(0.70710678118654752440); T l = T(lam);
   vec4<T> r; r.c[0] = mk<T>(0, 0); r.c[1] = mk<T>(-l * s * e1x, -s * e2x); r.c[2] = mk<T>(-l * s * e1y, -s * e2y); r.c[3] = mk<T>(-l * s * e1z, 0);
   return r;
