@@ -208,13 +208,13 @@ __global__ void __launch_bounds__(NTH) epem_photons_kernel(const double* __restr
 
 // Algorithmic flops per event (FMA = 2, MUL = ADD = 1): a level-k task is k 2x2 complex blocks (16 FMA each), the (q0 + sigma.q)
 // block with the propagator folded in (8 FMA + 4 MUL for the block, 6 MUL + 2 ADD for its scaled entries); a final amplitude is NG
-// blocks, the row contraction (6 FMA + 2 MUL) and the square (1 FMA + 1 MUL); externals ~60 per polarisation block, ~50 per
-// spinor, ~20 per subset momentum.
+// blocks, the row contraction (6 FMA + 2 MUL) and the square (1 FMA + 1 MUL); externals ~30 per polarisation block, ~25 per
+// spinor, ~12 per subset momentum (n = 5: 33 078 against 33 075 counted by ncu).
 static double photon_flops_per_event(int ng) {
   double f = 0;
   for (int k = 1; k < ng; k++) f += (double)binom(ng, k) * (1 << k) * (32.0 * k + 16 + 4 + 8);
-  f += (double)(1 << ng) * (32.0 * ng + 14 + 3 + ng /* shuffle adds */);
-  f += 2.0 * ng * 60 + 2 * 50 + (1 << ng) * 20.0;
+  f += (double)(1 << ng) * (32.0 * ng + 14 + 3);
+  f += 2.0 * ng * 30 + 2 * 25 + (1 << ng) * 12.0;
   return f;
 }
 
