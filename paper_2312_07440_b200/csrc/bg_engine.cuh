@@ -660,7 +660,7 @@ __device__ __forceinline__ void group_externals(int t0, int nth, int ns, long lo
   }
   constexpr int nobj = 2 * N + 4 + Ge::NMASK;
   for (int t = t0; t < ns * nobj; t += nth) {
-    int sl = t / nobj, o = t % nobj; const double* pm = pmD + sl * next * 4;
+    int o = t / ns, sl = t - o * ns; const double* pm = pmD + sl * next * 4;      // object-major: the lanes of a warp run the same branch
     if (o < 2 * N) {                         // gluon i, helicity bit hb (0: +1, 1: -1); entry = 2*i + hb
       int i = o >> 1, hb = o & 1, leg = i < 2 ? i : i + 2; const double* p = pm + 4 * leg;
       vec4<T> e = polvec<T>((T)p[1], (T)p[2], (T)p[3], hb ? -1 : +1);
@@ -684,9 +684,12 @@ __device__ __forceinline__ void group_externals(int t0, int nth, int ns, long lo
       TK qr[4], ql[4]; for (int mu = 0; mu < 4; mu++) { qr[mu] = k[mu] - (TK)pm[12 + mu]; ql[mu] = (TK)pm[8 + mu] - k[mu]; }
       TK m2 = (TK)mtd * (TK)mtd;
       T* K = Kd + ((size_t)sl * Ge::NMASK + mask) * 4; for (int mu = 0; mu < 4; mu++) K[mu] = (T)k[mu];
-      iK2d[sl * Ge::NMASK + mask] = (__popc(mask) >= 2) ? (T)(TK(1) / k2) : T(0);
-      dRd[sl * Ge::NMASK + mask] = (T)(TK(1) / (mdot_rr<TK>(qr, qr) - m2));
-      dLd[sl * Ge::NMASK + mask] = (T)(TK(1) / (mdot_rr<TK>(ql, ql) - m2));
+      // only the denominators some current uses (warp-uniform conditions): gluon propagators of >= 2 gluons, quark propagators
+      // behind 1..RMAX (right) resp. 1..LMAX (left) gluons
+      const int pc = __popc(mask);
+      iK2d[sl * Ge::NMASK + mask] = (pc >= 2) ? (T)(TK(1) / k2) : T(0);
+      dRd[sl * Ge::NMASK + mask] = (pc >= 1 && pc <= Ge::RMAX) ? (T)(TK(1) / (mdot_rr<TK>(qr, qr) - m2)) : T(0);
+      dLd[sl * Ge::NMASK + mask] = (pc >= 1 && pc <= Ge::LMAX) ? (T)(TK(1) / (mdot_rr<TK>(ql, ql) - m2)) : T(0);
     }
   }
 }
