@@ -368,6 +368,9 @@ template <> struct pair_of<float> { typedef float2 type; };
 template <typename T> __device__ __forceinline__ cx<T> ldc(const cx<T>* p) { typename pair_of<T>::type t = *reinterpret_cast<const typename pair_of<T>::type*>(p); return mk<T>(t.x, t.y); }
 template <typename T> __device__ __forceinline__ void stc(cx<T>* p, cx<T> v) { typename pair_of<T>::type t; t.x = v.re; t.y = v.im; *reinterpret_cast<typename pair_of<T>::type*>(p) = t; }
 
+#ifndef RWGT_STAGE_MIN_N
+#define RWGT_STAGE_MIN_N 4
+#endif
 template <typename T> struct Smem {
   uint32_t* W;    // schedule words (whole CTA)
   double* LF;     // Cholesky factors L+^T, L-^T of the colour blocks in mma-fragment order (whole CTA)
@@ -399,7 +402,7 @@ template <int N, typename T> __host__ __device__ inline size_t carve(Smem<T>& s,
   s.iK2 = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
   s.dR = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
   s.dL = (T*)(base + off); off += sizeof(T) * ns * Ge::NMASK; al();
-  const int nst = (N >= 4) ? ns : 0;                         // staging exists only where the colour warps prefetch (bg_kernel: STAGE)
+  const int nst = (N >= RWGT_STAGE_MIN_N) ? ns : 0;                         // staging exists only where the colour warps prefetch (bg_kernel: STAGE)
   s.pmS = (double*)(base + off); off += sizeof(double) * nst * (N + 2) * 4; al();
   s.GS = (cx<T>*)(base + off); off += sizeof(T) * (size_t)nst * 8 * (2 * N); al();
   s.RS = (cx<T>*)(base + off); off += sizeof(T) * (size_t)nst * 8 * 2; al();
@@ -711,8 +714,9 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
   // register hand-over between the warpgroups: the colour warps need few registers, the workers get the rest
   // (setmaxnreg is a warpgroup instruction: both groups must be whole warpgroups of 4 warps)
   // a1/a2 of the next group on the colour warps: pays when the colour warps are mostly idle and the per-group fixed work is small
-  // next to the currents (n >= 4); for n <= 3 four colour warps are slower at it than eight workers (measured: 5.4 -> 5.9 ms)
-  constexpr bool STAGE = (N >= 4);
+  // next to the currents (n >= 4); for n = 3 four colour warps are slower at it than the workers (measured: 5.4 -> 5.9 ms, and 4.58 -> 4.76 ms
+  // after the externals became object-major)
+  constexpr bool STAGE = (N >= RWGT_STAGE_MIN_N);
   constexpr bool HANDOVER = NW % 4 == 0 && NCW % 4 == 0;
   // the CTA's pool is what it was launched with: (registers per thread under the launch bounds) x warps; an inc beyond it never returns
   constexpr int REG_LAUNCH = (65536 / CTAS / NTH) / 8 * 8 > 255 ? 248 : (65536 / CTAS / NTH) / 8 * 8, REG_POOL = REG_LAUNCH * (NW + NCW);
