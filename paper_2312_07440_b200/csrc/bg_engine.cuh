@@ -856,6 +856,33 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
           bar_sync(BAR_FULL0 + buf, NTH);                      // the workers have filled this buffer
           const double* Abuf = s.A + (size_t)buf * ns * Ge::ABUF;
           // a5: Z = L^T A with FP64 tensor-core mma over the upper-triangular tiles, colour form = sum of squares of Z
+          if constexpr (Ge::MTH == 1 && Ge::KTH == 1) {
+            // n <= 3: one 8x4 tile per half, so a unit is four mma and a shuffle tree, i.e. pure latency.  Four units (slot x half) are
+            // written out side by side so that their chains overlap; each unit's arithmetic and order are the same as in the general path.
+            constexpr int UB = 4;
+            for (int u0 = cwarp * UB; u0 < ns * 2 && !RWGT_EXP_SKIP(1); u0 += NCW * UB) {
+              double part[UB];
+#pragma unroll
+              for (int j = 0; j < UB; j++) {
+                const int u = (u0 + j < ns * 2) ? u0 + j : ns * 2 - 1, sl = u >> 1, h = u & 1;
+                const double* A = Abuf + (size_t)sl * Ge::ABUF + (size_t)(h * Ge::NHK + (lane & 3)) * Ge::ASTR + (lane >> 2);
+                const double a = s.LF[h * 32 + lane];
+                double acc[Ge::NT][2];
+#pragma unroll
+                for (int nt = 0; nt < Ge::NT; nt++) { acc[nt][0] = 0.0; acc[nt][1] = 0.0; dmma884(acc[nt][0], acc[nt][1], a, A[8 * nt]); }
+                double pj = 0.0;
+#pragma unroll
+                for (int nt = 0; nt < Ge::NT; nt++) { pj = fma(acc[nt][0], acc[nt][0], pj); pj = fma(acc[nt][1], acc[nt][1], pj); }
+                part[j] = pj;
+              }
+#pragma unroll
+              for (int d = 16; d >= 1; d >>= 1)
+#pragma unroll
+                for (int j = 0; j < UB; j++) part[j] += __shfl_xor_sync(0xffffffffu, part[j], d);
+#pragma unroll
+              for (int j = 0; j < UB; j++) if (lane == 0 && u0 + j < ns * 2) s.red[((u0 + j) >> 1) * 8 + ((u0 + j) & 1)] = part[j];
+            }
+          } else
           for (int u = cwarp; u < ns * Ge::U && !RWGT_EXP_SKIP(1); u += NCW) {
             int sl = u / Ge::U, unit = u % Ge::U; const int h = unit / Ge::UH, uu = unit % Ge::UH;     // h: 0 = u rows / L+, 1 = v rows / L-
             const double* A = Abuf + (size_t)sl * Ge::ABUF + (size_t)(h * Ge::NHK + (lane & 3)) * Ge::ASTR + (lane >> 2);
