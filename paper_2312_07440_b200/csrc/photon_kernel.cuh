@@ -137,7 +137,7 @@ __global__ void __launch_bounds__(NTH) epem_photons_kernel(const double* __restr
     gsync<CG, NTH>();
     // ---- a2: external wavefunctions, momenta and inverse virtualities of the electron line ----
     for (int t = tid; t < E * Ge::NEXTOBJ; t += CG) {
-      int sl = t / Ge::NEXTOBJ, o = t % Ge::NEXTOBJ; double* s = sm + sl * Ge::SLOT; const double* pm = s + Ge::O_PM;
+      int o = t / E, sl = t - o * E; double* s = sm + sl * Ge::SLOT; const double* pm = s + Ge::O_PM;      // object-major: few branches per warp
       if (o < 2 * NG) {                            // photon i, helicity bit hb (0: +1, 1: -1): the block (eps0 - sigma.eps*) = [[m, -r], [-l, p]]
         int i = o >> 1, hb = o & 1; const double* k = pm + 4 * (i + 2);
         lcv<double> a = lightcone(conj4(polvec<double>(k[1], k[2], k[3], hb ? -1 : +1)));
