@@ -211,3 +211,32 @@ def test_repeated_launches_are_bitwise_identical(idx, n, precision):
     r2 = B.Reweighter(c.process, c.params_old, c.params_new, precision)
     assert torch.equal(r2.run(dm, dw), ref)
     r2.close()
+
+
+def test_rwgt_run_can_be_captured_in_a_cuda_graph():
+    """rwgt_run only enqueues one kernel on the caller's stream (no allocation, no sync, no copy: SURVEY 8(b)), so a launch-bound loop
+    over small event sets can be captured once and replayed."""
+    for idx, n in ((1, 16384), (3, 1001), (6, 257)):
+        c = ev.config(idx)
+        m, w = ev.generate(c, n)
+        dm, dw = torch.from_numpy(m).cuda(), torch.from_numpy(w).cuda()
+        r = B.Reweighter(c.process, c.params_old, c.params_new, "fp64")
+        ref = r.run(dm, dw).clone()
+        out = torch.zeros_like(ref)
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            r.run(dm, dw, out)                      # warm-up on the capture stream
+        torch.cuda.current_stream().wait_stream(side)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g):
+            r.run(dm, dw, out)
+        out.zero_()
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out, ref)
+        dw.mul_(2.0)                                # new inputs in the same buffers
+        g.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(out[2], 2.0 * ref[2]) and torch.equal(out[0], ref[0])
+        r.close()
