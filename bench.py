@@ -195,7 +195,7 @@ def main() -> None:
 
     import torch
     import torch.distributed as dist
-    from paper_2312_07440_b200 import binding as B
+    from paper_2312_07440_b200 import binding as B, microbench as MB
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -249,7 +249,7 @@ def main() -> None:
         return
 
     # ---- roofline of the (single) kernel of a step: the FP64 (FP32) arithmetic pipe ----
-    # FP64 mode: DFMA and DMMA share one pipe on B200 (rwgt_measure_peak kind 7), so the numerator is the vector flops
+    # FP64 mode: DFMA and DMMA share one pipe on B200 (include/rwgt_microbench.h kind 7), so the numerator is the vector flops
     # plus the algorithmic flops of the colour form (a5, run as mma.m8n8k4).  FP32/mixed: the vector flops against the
     # FP32 pipe; the colour form stays on the FP64 pipe and is reported beside it.
     peaks = measured_peaks()
@@ -272,7 +272,7 @@ def main() -> None:
                             "ffma2_chain": 8, "ffma2_3_distinct_sources": 9, "ffma2_1_reused_source": 10})
     for name, kind in kinds.items():
         try:
-            micro[name] = B.rwgt_measure_peak(kind)          # register-resident microbenchmarks, same session
+            micro[name] = MB.rwgt_microbench_peak(kind)     # register-resident microbenchmarks, same session
         except Exception:
             micro[name] = None
     chain_tf = micro.get("fma_chain")

@@ -135,16 +135,6 @@ const char* rwgt_last_error(void);
  * the SU(3) Fierz identity in exact integer arithmetic.  Returns n! or -1. */
 int rwgt_colour_matrix(int n_gluons, double* out);
 
-/* Measurement aid for the roofline: runs a register-resident FMA chain on the current
- * device and writes the sustained rate in TFLOP/s (2 flop per FMA) to *out_tflops (HOST pointer).
- * kind 0: FP64 FMA chain x = fma(x,a,b), 1: FP32 FMA chain, 2: FP64 tensor (mma m8n8k4) chain,
- * 3 / 4: FP64 FMA with three distinct register sources / with one source reused by consecutive FMAs (the operand
- * pattern of real complex arithmetic; register-file read bandwidth makes these slower than kind 0),
- * 5 / 6: the same two patterns in FP32, 7: FP64 FMA chains and DMMA chains concurrently on every SM, summed rate
- * (DFMA and DMMA share one pipe on B200: kind 7 = kind 0 = kind 2), 8 / 9 / 10: packed FP32 fma.rn.f32x2 (FFMA2) chains /
- * three distinct sources / one reused source (what the FP32 and mixed modes issue).  Synchronises the device.  0 or -1. */
-int rwgt_measure_peak(int kind, double* out_tflops);
-
 #ifdef __cplusplus
 }
 #endif

@@ -17,7 +17,7 @@ PRECISIONS = {"fp64": RWGT_FP64, "fp32": RWGT_FP32, "mixed": RWGT_MIXED}
 
 RWGT_MAX_SETS = 16
 EXPORTS = ("rwgt_create", "rwgt_create_multi", "rwgt_n_sets", "rwgt_run_multi", "rwgt_run_multi_host", "rwgt_set_precision", "rwgt_n_external", "rwgt_flops_per_event", "rwgt_run",
-           "rwgt_run_host", "rwgt_destroy", "rwgt_last_error", "rwgt_colour_matrix", "rwgt_measure_peak", "rwgt_tensor_flops_per_event")
+           "rwgt_run_host", "rwgt_destroy", "rwgt_last_error", "rwgt_colour_matrix", "rwgt_tensor_flops_per_event")
 
 
 class rwgt_params(C.Structure):
@@ -55,7 +55,6 @@ def lib():
         L.rwgt_destroy.argtypes = [vp]
         L.rwgt_last_error.restype = C.c_char_p
         L.rwgt_colour_matrix.argtypes = [C.c_int, dp]
-        L.rwgt_measure_peak.argtypes = [C.c_int, C.POINTER(C.c_double)]
         _lib = L
     return _lib
 
@@ -165,13 +164,6 @@ def rwgt_colour_matrix(n_gluons: int) -> np.ndarray:
     return out
 
 
-def rwgt_measure_peak(kind: int) -> float:
-    out = C.c_double()
-    if lib().rwgt_measure_peak(int(kind), C.byref(out)) != 0:
-        raise RuntimeError("rwgt_measure_peak failed")
-    return out.value
-
-
 class Reweighter:
     """Convenience wrapper: one handle, torch device tensors in, torch device tensors out."""
 
@@ -195,10 +187,12 @@ class Reweighter:
         import torch
         n = weights.shape[0]
         assert momenta.is_cuda and momenta.dtype == torch.float64 and momenta.is_contiguous()
-        assert momenta.shape == (self.n_ext, 4, n) and weights.dtype == torch.float64
+        assert momenta.shape == (self.n_ext, 4, n)
+        assert weights.is_cuda and weights.dtype == torch.float64 and weights.is_contiguous() and weights.device == momenta.device
         k = self.k
         if out is None:
             out = torch.empty((1 + 2 * k, n), dtype=torch.float64, device=momenta.device)
+        assert out.is_cuda and out.dtype == torch.float64 and out.device == momenta.device
         assert out.shape == (1 + 2 * k, n) and out.is_contiguous()
         st = torch.cuda.current_stream(momenta.device).cuda_stream
         rwgt_run_multi(self.h, momenta.data_ptr(), weights.data_ptr(), out[0].data_ptr(), out[1].data_ptr(),

@@ -35,18 +35,6 @@
 
 namespace rwgt {
 
-// Diagnostic build only (python -m paper_2312_07440_b200.experiments; never defined for librwgt.so): run-time switches that
-// REMOVE parts of the engine to time the rest.  Results are wrong by construction.  c_exp = {table-entry multiplier (0: every
-// table load reads entry 0, i.e. a conflict-free broadcast), skip colour mma, skip current levels, skip amplitude tasks}.
-#ifdef RWGT_EXPERIMENT
-__constant__ int c_exp[4] = {1, 0, 0, 0};
-#define RWGT_EXP_ENTRY(e) ((e) * c_exp[0])
-#define RWGT_EXP_SKIP(i) (c_exp[i] != 0)
-#else
-#define RWGT_EXP_ENTRY(e) (e)
-#define RWGT_EXP_SKIP(i) false
-#endif
-
 // ------------------------------------------------------------------------------------------------ host: colour matrix
 // C_{ss'} = sum_a Tr(T^{a_s1}..T^{a_sn} T^{a_s'n}..T^{a_s'1}) by repeated use of the SU(N) Fierz identity
 //   T^a_ij T^a_kl = 1/2 (d_il d_jk - 1/N d_ij d_kl), exact integers over (2N)^n.  (Independent of the oracle's
@@ -416,13 +404,13 @@ template <int N, typename T> __host__ __device__ inline size_t carve(Smem<T>& s,
 }
 
 template <typename T> __device__ __forceinline__ vec4<T> ld4(const cx<T>* tab, int stride, int e) {
-  vec4<T> r; e = RWGT_EXP_ENTRY(e);
+  vec4<T> r;
 #pragma unroll
   for (int c = 0; c < 4; c++) r.c[c] = ldc(tab + c * stride + e);
   return r;
 }
 template <typename T> __device__ __forceinline__ spn<T> lds4(const cx<T>* tab, int stride, int e) {
-  spn<T> r; e = RWGT_EXP_ENTRY(e);
+  spn<T> r;
 #pragma unroll
   for (int c = 0; c < 4; c++) r.c[c] = ldc(tab + c * stride + e);
   return r;
@@ -534,7 +522,7 @@ template <int N, int M, typename T, int NWT> __device__ __forceinline__ void lev
   const Smem<T>& s = c.s; constexpr int nG = Ge::NG, nR = Ge::NR, nL = Ge::NL, next = N + 2;
   const int ns = c.ns, nGt = ns * tg, nRt = ns * tr, nLt = ns * tl;
   const uint32_t* TL = s.W + c.D->offT[M];
-  for (int t = c.tid; t < nGt + nRt + nLt && !RWGT_EXP_SKIP(2); t += NWT) {
+  for (int t = c.tid; t < nGt + nRt + nLt; t += NWT) {
     if (HASG && t < nGt) {
      if constexpr (HASG) {
       int sl = t / tg, o = t - sl * tg; uint32_t tw = TL[o]; uint32_t v = tw >> 16;
@@ -782,7 +770,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
           if (step >= 2) bar_sync(BAR_EMPTY0 + buf, NTH);      // colour warps have finished reading this buffer
           double* Abuf = s.A + (size_t)buf * ns * Ge::ABUF;
           constexpr int per = Ge::NPAIR * Ge::NFREE;
-          for (int t = tid; t < ns * per && !RWGT_EXP_SKIP(3); t += NWT) {
+          for (int t = tid; t < ns * per; t += NWT) {
             int sl = t / per, o = t - sl * per; int pair = o / Ge::NFREE, f = o % Ge::NFREE;
             const cx<T>* G = s.G + (size_t)sl * 4 * nG; const cx<T>* R = s.R + (size_t)sl * 4 * nR; const cx<T>* L = s.L + (size_t)sl * 4 * nL;
             const T* K = s.K + (size_t)sl * Ge::NMASK * 4;
@@ -860,7 +848,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
             // n <= 3: one 8x4 tile per half, so a unit is four mma and a shuffle tree, i.e. pure latency.  Four units (slot x half) are
             // written out side by side so that their chains overlap; each unit's arithmetic and order are the same as in the general path.
             constexpr int UB = 4;
-            for (int u0 = cwarp * UB; u0 < ns * 2 && !RWGT_EXP_SKIP(1); u0 += NCW * UB) {
+            for (int u0 = cwarp * UB; u0 < ns * 2; u0 += NCW * UB) {
               double part[UB];
 #pragma unroll
               for (int j = 0; j < UB; j++) {
@@ -883,7 +871,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
               for (int j = 0; j < UB; j++) if (lane == 0 && u0 + j < ns * 2) s.red[((u0 + j) >> 1) * 8 + ((u0 + j) & 1)] = part[j];
             }
           } else
-          for (int u = cwarp; u < ns * Ge::U && !RWGT_EXP_SKIP(1); u += NCW) {
+          for (int u = cwarp; u < ns * Ge::U; u += NCW) {
             int sl = u / Ge::U, unit = u % Ge::U; const int h = unit / Ge::UH, uu = unit % Ge::UH;     // h: 0 = u rows / L+, 1 = v rows / L-
             const double* A = Abuf + (size_t)sl * Ge::ABUF + (size_t)(h * Ge::NHK + (lane & 3)) * Ge::ASTR + (lane >> 2);
             double part = 0.0;
@@ -991,6 +979,7 @@ template <int N> static void bg_launch(int precision, int grid, size_t s64, size
 
 static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::string& err) {
   BgProcess* B = new BgProcess();
+  B->d_words = nullptr; B->d_lfrag = nullptr;
   B->S = build_schedule(n, err);
   if (!err.empty()) { delete B; return nullptr; }
   const BgSched& S = B->S;
@@ -1031,7 +1020,7 @@ static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::stri
   if (e == cudaSuccess) e = cudaMemcpy(B->d_lfrag, S.lfrag.data(), S.lfrag.size() * sizeof(double), cudaMemcpyHostToDevice);
   if (e == cudaSuccess) switch (n) { case 2: e = bg_set_attr<2>(B->smem64, B->smem32); break; case 3: e = bg_set_attr<3>(B->smem64, B->smem32); break;
                                      case 4: e = bg_set_attr<4>(B->smem64, B->smem32); break; default: e = bg_set_attr<5>(B->smem64, B->smem32); }
-  if (e != cudaSuccess) { err = std::string("CUDA: ") + cudaGetErrorString(e); delete B; return nullptr; }
+  if (e != cudaSuccess) { err = std::string("CUDA: ") + cudaGetErrorString(e); cudaFree(B->d_words); cudaFree(B->d_lfrag); delete B; return nullptr; }
   D.words = B->d_words; D.lfrag = B->d_lfrag;
   return B;
 }
@@ -1048,7 +1037,7 @@ static double bg_flops_per_event(const BgProcess* B, int /*precision*/) {
 }
 // Algorithmic flops of the colour form |L+^T u|^2 + |L-^T v|^2 (a5), all parameter sets: per evaluated helicity (2^(n+1) after
 // parity) each of the two reflection blocks (size nh = n!/2) costs nh (nh + 1) / 2 FMAs for the real and for the imaginary part,
-// plus 2 nh FMAs for the sum of squares.  They run as mma.m8n8k4 (DMMA) on the FP64 pipe, which DFMA and DMMA share on B200 (rwgt_measure_peak 7).
+// plus 2 nh FMAs for the sum of squares.  They run as mma.m8n8k4 (DMMA) on the FP64 pipe, which DFMA and DMMA share on B200 (include/rwgt_microbench.h, kind 7).
 static double bg_tensor_flops_per_event(const BgProcess* B) {
   const int n = B->S.n; const double nh = B->S.npair, nhel = (double)(1 << (n + 1));
   return B->D.nsets * nhel * 2.0 * (2.0 * (nh * (nh + 1) / 2) + 2.0 * nh) * 2.0;     // two reflection blocks of size n!/2
@@ -1056,9 +1045,6 @@ static double bg_tensor_flops_per_event(const BgProcess* B) {
 
 static int bg_run(BgProcess* B, int precision, const double* mom, const double* w, double* a, double* b, double* o, long long nev, long long stride, long long ostride, cudaStream_t st) {
   BgDev D = B->D; const bool dbl = (precision == RWGT_FP64);
-#ifdef RWGT_EXPERIMENT
-  { const char* v = getenv("RWGT_EXP"); int f = v ? atoi(v) : 0; int h[4] = {(f & 1) ? 0 : 1, (f >> 1) & 1, (f >> 2) & 1, (f >> 3) & 1}; cudaMemcpyToSymbol(c_exp, h, sizeof(h)); }
-#endif
   D.nslot = dbl ? B->nslot64 : B->nslot32;
   long long ngroups = (nev + D.nslot - 1) / D.nslot; int grid = (int)std::min<long long>(ngroups, (long long)B->sm_count * bg_ctas(B->S.n));
   switch (B->S.n) {

@@ -19,18 +19,6 @@ struct EpemSet {          // per parameter set, prepared on the host
 constexpr int SMALL_NSMAX = 1 + RWGT_MAX_SETS;     // the old set plus up to RWGT_MAX_SETS new ones
 struct EpemParams { EpemSet set[SMALL_NSMAX]; int nsets; };
 
-// chi_a^dagger sigma^mu chi_b (bar=false) or chi_a^dagger sigmabar^mu chi_b (bar=true)
-__device__ __forceinline__ vec4<double> bilinear2(const cx<double>* a, const cx<double>* b, bool barred) {
-  cx<double> a0 = conj(a[0]), a1 = conj(a[1]);
-  cx<double> t00 = a0 * b[0], t11 = a1 * b[1], t01 = a0 * b[1], t10 = a1 * b[0];
-  vec4<double> r; double s = barred ? -1.0 : 1.0;
-  r.c[0] = t00 + t11;
-  r.c[1] = s * (t01 + t10);                                   // sigma_x
-  cx<double> d = t01 - t10; r.c[2] = s * mk<double>(d.im, -d.re);   // sigma_y: -i t01 + i t10
-  r.c[3] = s * (t00 - t11);                                   // sigma_z
-  return r;
-}
-
 // Massless leptons: only the 4 helicity combinations with opposite helicities on each fermion line
 // are non-zero (tests check the oracle's full 16-term sum against this, reading Q5).
 __global__ void __launch_bounds__(256, 3) epem_mupmum_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
@@ -48,14 +36,14 @@ __global__ void __launch_bounds__(256, 3) epem_mupmum_kernel(const double* __res
   double s = mdot_rr(q, q);
   chi_pair<double> x1 = make_chi(p[0][1], p[0][2], p[0][3]), x2 = make_chi(p[1][1], p[1][2], p[1][3]);
   chi_pair<double> x3 = make_chi(p[2][1], p[2][2], p[2][3]), x4 = make_chi(p[3][1], p[3][2], p[3][3]);
-  // massless: sqrt(E+|p|) with |p| from the 3-momentum (mass parameter 0, reading Q8)
-  // spinor normalisations sqrt(E+|p|) of the four legs enter every |amplitude|^2 as the product of the four (E+|p|): no square root
-  const double nrm = ((p[0][0] + x1.pabs) * (p[1][0] + x2.pabs)) * ((p[2][0] + x3.pabs) * (p[3][0] + x4.pabs));
+  // massless legs: spinor normalisation sqrt(2E), energy from the input and mass parameter 0 (reading Q8 / DESIGN.md R8); the four
+  // normalisations enter every |amplitude|^2 as the product of the four 2E: no square root
+  const double nrm = 16.0 * ((p[0][0] * p[1][0]) * (p[2][0] * p[3][0]));
   // electron line vbar(p1) gamma^mu u(p2): L = (lam1,lam2) = (+,-), R = (-,+); muon line ubar(p4) gamma^mu v(p3) likewise.  The four
   // current contractions J_e . J_mu are done by the Fierz identities of the Pauli matrices (sigma^mu = (1, sigma), sigmabar^mu = (1, -sigma)):
   //   (a^+ sigmabar^mu b)(c^+ sigmabar_mu d) = (a^+ sigma^mu b)(c^+ sigma_mu d) = 2 conj(a ^ c) (b ^ d),   x ^ y = x_1 y_2 - x_2 y_1,
   //   (a^+ sigmabar^mu b)(c^+ sigma_mu d) = 2 (a^+ d)(c^+ b),
-  // i.e. every helicity amplitude is a product of two two-spinor products (bilinear2 above is the explicit current, kept for reference).
+  // i.e. every helicity amplitude is a product of two two-spinor products.
   auto wedge = [](const cx<double>* x, const cx<double>* y) { cx<double> r = x[0] * y[1]; cfms(r, x[1], y[0]); return norm2(r); };
   auto inner = [](const cx<double>* x, const cx<double>* y) { cx<double> r = conj(x[0]) * y[0]; cfma(r, conj(x[1]), y[1]); return norm2(r); };
   const double c2 = 4.0 * nrm;

@@ -1,7 +1,10 @@
-// microbench.cuh — register-resident FMA-chain kernels that measure the plain-ALU peaks the roofline of
+// microbench.cu — register-resident FMA-chain kernels that measure the plain-ALU peaks the roofline of
 // bench.py is quoted against (MEASURED_PEAKS.json has no FP64/FP32 FMA peak).
-#pragma once
+// A measurement aid: built into its own library (librwgt_microbench.so, include/rwgt_microbench.h), NOT into librwgt.so.
 #include <cuda_runtime.h>
+#include <cmath>
+
+#include "../../include/rwgt_microbench.h"
 
 namespace rwgt {
 
@@ -155,3 +158,8 @@ static int measure_peak(int kind, double* tflops) {
 }
 
 }  // namespace rwgt
+
+extern "C" int rwgt_microbench_peak(int kind, double* out_tflops) {
+  if (kind < 0 || kind > 10 || !out_tflops) return -1;
+  return rwgt::measure_peak(kind, out_tflops);
+}

@@ -230,16 +230,20 @@ static double photon_flops_per_event(int ng) {
 #define RWGT_PH_NTH 256
 #endif
 constexpr int PH_E = RWGT_PH_E, PH_CG = RWGT_PH_CG, PH_NTH = RWGT_PH_NTH;
+template <int NG> constexpr size_t photon_smem() { return sizeof(double) * (PH_NTH / PH_CG) * PH_E * PhGeo<NG>::SLOT; }
+// once per handle at rwgt_create, on the handle's device (the attribute belongs to the device's copy of the function)
+static cudaError_t photon_prepare(int ng) {
+  switch (ng) {
+    case 2: return cudaFuncSetAttribute(epem_photons_kernel<2, PH_E, PH_CG, PH_NTH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)photon_smem<2>());
+    case 3: return cudaFuncSetAttribute(epem_photons_kernel<3, PH_E, PH_CG, PH_NTH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)photon_smem<3>());
+    case 4: return cudaFuncSetAttribute(epem_photons_kernel<4, PH_E, PH_CG, PH_NTH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)photon_smem<4>());
+    default: return cudaFuncSetAttribute(epem_photons_kernel<5, PH_E, PH_CG, PH_NTH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)photon_smem<5>());
+  }
+}
 template <int NG> static cudaError_t photon_launch_n(int sm_count, cudaStream_t st, const double* mom, const double* w, double* a, double* b, double* o,
                                                      long long nev, long long stride, long long ostride, const PhotonParams& P) {
-  static bool attr_set = false;
   constexpr int GPB = PH_NTH / PH_CG;
-  const size_t smem = sizeof(double) * GPB * PH_E * PhGeo<NG>::SLOT;
-  if (!attr_set) {
-    cudaError_t e = cudaFuncSetAttribute(epem_photons_kernel<NG, PH_E, PH_CG, PH_NTH>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    attr_set = true;
-  }
+  const size_t smem = photon_smem<NG>();
   const long long ngroups = (nev + PH_E - 1) / PH_E, nblocks = (ngroups + GPB - 1) / GPB;
   const int per_sm = (int)std::max<size_t>(1, std::min<size_t>(2048 / PH_NTH, (size_t)(227 * 1024) / (smem + 2048)));
   const int grid = (int)std::min<long long>(nblocks, (long long)sm_count * per_sm);

@@ -12,7 +12,6 @@
 #include "kernels_small.cuh"
 #include "bg_engine.cuh"
 #include "photon_kernel.cuh"
-#include "microbench.cuh"
 
 namespace {
 
@@ -21,6 +20,18 @@ void set_err(const char* fmt, const char* a = "") { std::snprintf(g_err, sizeof(
 
 enum Proc { P_EPEM = 0, P_GG_TTX = 1, P_BG = 2, P_PHOTONS = 3 };
 const double PI = 3.14159265358979323846;
+
+// A handle's tables and kernel attributes live on the device that was current at rwgt_create: every call that launches or
+// copies makes that device current for its duration and restores the caller's device afterwards.
+struct DeviceGuard {
+  int prev = -1; bool ok = true;
+  explicit DeviceGuard(int dev) {
+    if (cudaGetDevice(&prev) != cudaSuccess) { ok = false; return; }
+    if (prev != dev && cudaSetDevice(dev) != cudaSuccess) ok = false;
+    if (prev == dev) prev = -1;
+  }
+  ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
 
 }  // namespace
 
@@ -41,6 +52,7 @@ struct rwgt_handle {
   // device scratch for rwgt_run_host
   double* scratch;
   size_t scratch_bytes;
+  int pipe_ready;                                     // copy streams and events below exist (all of them or none)
   cudaStream_t s_in, s_out;                           // copy streams of rwgt_run_host (created on first use)
   cudaEvent_t ev_in[RWGT_MAX_CHUNKS + 1], ev_k[RWGT_MAX_CHUNKS + 1];
 };
@@ -80,7 +92,7 @@ rwgt_handle* rwgt_create_multi(const char* process, const rwgt_params* params_ol
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) { cudaGetLastError(); set_err("rwgt_create: no CUDA device (this library has no CPU path)"); return nullptr; }
   rwgt_handle* h = new (std::nothrow) rwgt_handle();
   if (!h) { set_err("rwgt_create: out of memory"); return nullptr; }
-  h->proc = -1; h->precision = RWGT_FP64; h->bg = nullptr; h->scratch = nullptr; h->scratch_bytes = 0; h->s_in = nullptr; h->s_out = nullptr;
+  h->proc = -1; h->precision = RWGT_FP64; h->bg = nullptr; h->scratch = nullptr; h->scratch_bytes = 0; h->s_in = nullptr; h->s_out = nullptr; h->pipe_ready = 0;
   h->nsets = 1 + n_new; h->sets[0] = *params_old;
   for (int k = 0; k < n_new; k++) h->sets[1 + k] = params_new[k];
   cudaGetDevice(&h->device);
@@ -101,6 +113,8 @@ rwgt_handle* rwgt_create_multi(const char* process, const rwgt_params* params_ol
     double fact = 1; for (int i = 2; i <= na; i++) fact *= i;
     for (int k = 0; k < h->nsets; k++) h->photons.fac[k] = 2.0 * std::pow(4.0 * PI * h->sets[k].alpha_em, na) / (4.0 * fact);
     cudaDeviceProp prop; cudaGetDeviceProperties(&prop, h->device); h->sm_count = prop.multiProcessorCount;
+    cudaError_t e = rwgt::photon_prepare(na);
+    if (e != cudaSuccess) { set_err("rwgt_create: %s", cudaGetErrorString(e)); delete h; return nullptr; }
     return h;
   }
   else { set_err("rwgt_create: unknown process '%s'", process); delete h; return nullptr; }
@@ -186,6 +200,8 @@ int rwgt_run_multi(rwgt_handle* h, const double* momenta, const double* weights,
   if (!h || n_events < 0) { set_err("rwgt_run: bad handle or n_events < 0"); return -1; }
   if (n_events == 0) return 0;
   if (!momenta || !weights || !out_me_old || !out_me_new || !out_w_new) { set_err("rwgt_run: NULL buffer"); return -1; }
+  DeviceGuard guard(h->device);
+  if (!guard.ok) { set_err("rwgt_run: cannot make the handle's device current"); return -1; }
   return launch_events(h, momenta, weights, out_me_old, out_me_new, out_w_new, n_events, n_events, n_events, (cudaStream_t)stream);
 }
 
@@ -203,41 +219,55 @@ int rwgt_run_multi_host(rwgt_handle* h, const double* momenta, const double* wei
   if (!h || n_events < 0) { set_err("rwgt_run_host: bad handle or n_events < 0"); return -1; }
   if (n_events == 0) return 0;
   if (!momenta || !weights || !out_me_old || !out_me_new || !out_w_new) { set_err("rwgt_run_host: NULL buffer"); return -1; }
+  DeviceGuard guard(h->device);
+  if (!guard.ok) { set_err("rwgt_run_host: cannot make the handle's device current"); return -1; }
   cudaStream_t st = (cudaStream_t)stream;
   const size_t n = (size_t)n_events, planes = (size_t)h->n_ext * 4, nin = planes * n, K = (size_t)h->nsets - 1, need = (nin + (2 + 2 * K) * n) * sizeof(double);
   cudaError_t e = cudaSuccess;
-#define RWGT_CK(call) do { e = (call); if (e != cudaSuccess) { set_err("rwgt_run_host: %s", cudaGetErrorString(e)); return (int)e; } } while (0)
   if (need > h->scratch_bytes) {
     if (h->scratch) cudaFree(h->scratch);
     h->scratch = nullptr; h->scratch_bytes = 0;
-    RWGT_CK(cudaMalloc((void**)&h->scratch, need));
+    e = cudaMalloc((void**)&h->scratch, need);
+    if (e != cudaSuccess) { h->scratch = nullptr; set_err("rwgt_run_host: %s", cudaGetErrorString(e)); return (int)e; }
     h->scratch_bytes = need;
   }
-  if (!h->s_in) {
-    RWGT_CK(cudaStreamCreateWithFlags(&h->s_in, cudaStreamNonBlocking));
-    RWGT_CK(cudaStreamCreateWithFlags(&h->s_out, cudaStreamNonBlocking));
-    for (int c = 0; c <= RWGT_MAX_CHUNKS; c++) {
-      RWGT_CK(cudaEventCreateWithFlags(&h->ev_in[c], cudaEventDisableTiming));
-      RWGT_CK(cudaEventCreateWithFlags(&h->ev_k[c], cudaEventDisableTiming));
+  if (!h->pipe_ready) {
+    // copy streams and events: all or nothing
+    cudaStream_t si = nullptr, so = nullptr; cudaEvent_t ei[RWGT_MAX_CHUNKS + 1] = {}, ek[RWGT_MAX_CHUNKS + 1] = {};
+    e = cudaStreamCreateWithFlags(&si, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&so, cudaStreamNonBlocking);
+    for (int c = 0; c <= RWGT_MAX_CHUNKS && e == cudaSuccess; c++) {
+      e = cudaEventCreateWithFlags(&ei[c], cudaEventDisableTiming);
+      if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ek[c], cudaEventDisableTiming);
     }
+    if (e != cudaSuccess) {
+      for (int c = 0; c <= RWGT_MAX_CHUNKS; c++) { if (ei[c]) cudaEventDestroy(ei[c]); if (ek[c]) cudaEventDestroy(ek[c]); }
+      if (si) cudaStreamDestroy(si); if (so) cudaStreamDestroy(so);
+      set_err("rwgt_run_host: %s", cudaGetErrorString(e)); return (int)e;
+    }
+    h->s_in = si; h->s_out = so;
+    for (int c = 0; c <= RWGT_MAX_CHUNKS; c++) { h->ev_in[c] = ei[c]; h->ev_k[c] = ek[c]; }
+    h->pipe_ready = 1;
   }
   double* d_mom = h->scratch; double* d_w = d_mom + nin; double* d_a = d_w + n; double* d_b = d_a + n; double* d_o = d_b + K * n;
   // chunks of >= 64 Ki events, at most RWGT_MAX_CHUNKS
   long long nchunk = (long long)((n + 65535) / 65536); if (nchunk > RWGT_MAX_CHUNKS) nchunk = RWGT_MAX_CHUNKS; if (nchunk < 1) nchunk = 1;
   long long per = ((long long)n + nchunk - 1) / nchunk;
+  int rc = 0;
+  // on any error: stop issuing, then drain the three streams so that no copy is still touching the caller's buffers on return
+#define RWGT_CK(call) do { if (rc == 0) { e = (call); if (e != cudaSuccess) { set_err("rwgt_run_host: %s", cudaGetErrorString(e)); rc = (int)e; } } } while (0)
   // the scratch may still be in use by earlier work on the caller's stream
   RWGT_CK(cudaEventRecord(h->ev_in[RWGT_MAX_CHUNKS], st));
   RWGT_CK(cudaStreamWaitEvent(h->s_in, h->ev_in[RWGT_MAX_CHUNKS], 0));
-  for (long long c = 0; c < nchunk; c++) {
+  for (long long c = 0; c < nchunk && rc == 0; c++) {
     long long a0 = c * per, cnt = std::min<long long>(per, (long long)n - a0);
-    if (cnt <= 0) { nchunk = c; break; }
+    if (cnt <= 0) break;
     RWGT_CK(cudaMemcpy2DAsync(d_mom + a0, n * sizeof(double), momenta + a0, n * sizeof(double), (size_t)cnt * sizeof(double), planes,
                               cudaMemcpyHostToDevice, h->s_in));
     RWGT_CK(cudaMemcpyAsync(d_w + a0, weights + a0, (size_t)cnt * sizeof(double), cudaMemcpyHostToDevice, h->s_in));
     RWGT_CK(cudaEventRecord(h->ev_in[c], h->s_in));
     RWGT_CK(cudaStreamWaitEvent(st, h->ev_in[c], 0));
-    int rc = launch_events(h, d_mom + a0, d_w + a0, d_a + a0, d_b + a0, d_o + a0, cnt, (long long)n, (long long)n, st);
-    if (rc != 0) return rc;
+    if (rc == 0) rc = launch_events(h, d_mom + a0, d_w + a0, d_a + a0, d_b + a0, d_o + a0, cnt, (long long)n, (long long)n, st);
     RWGT_CK(cudaEventRecord(h->ev_k[c], st));
     RWGT_CK(cudaStreamWaitEvent(h->s_out, h->ev_k[c], 0));
     RWGT_CK(cudaMemcpyAsync(out_me_old + a0, d_a + a0, (size_t)cnt * sizeof(double), cudaMemcpyDeviceToHost, h->s_out));
@@ -249,7 +279,8 @@ int rwgt_run_multi_host(rwgt_handle* h, const double* momenta, const double* wei
   RWGT_CK(cudaStreamWaitEvent(st, h->ev_k[RWGT_MAX_CHUNKS], 0));
   RWGT_CK(cudaStreamSynchronize(st));
 #undef RWGT_CK
-  return 0;
+  if (rc != 0) { cudaStreamSynchronize(h->s_in); cudaStreamSynchronize(st); cudaStreamSynchronize(h->s_out); }
+  return rc;
 }
 
 int rwgt_run_host(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old, double* out_me_new,
@@ -260,19 +291,15 @@ int rwgt_run_host(rwgt_handle* h, const double* momenta, const double* weights, 
 
 int rwgt_destroy(rwgt_handle* h) {
   if (!h) return -1;
+  DeviceGuard guard(h->device);
   if (h->bg) rwgt::bg_destroy(h->bg);
   if (h->scratch) cudaFree(h->scratch);
-  if (h->s_in) {
+  if (h->pipe_ready) {
     cudaStreamDestroy(h->s_in); cudaStreamDestroy(h->s_out);
     for (int c = 0; c <= RWGT_MAX_CHUNKS; c++) { cudaEventDestroy(h->ev_in[c]); cudaEventDestroy(h->ev_k[c]); }
   }
   delete h;
   return 0;
-}
-
-int rwgt_measure_peak(int kind, double* out_tflops) {
-  if (kind < 0 || kind > 10 || !out_tflops) return -1;
-  return rwgt::measure_peak(kind, out_tflops);
 }
 
 int rwgt_colour_matrix(int n_gluons, double* out) {

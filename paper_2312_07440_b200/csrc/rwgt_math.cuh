@@ -95,18 +95,6 @@ template <typename T> __device__ __forceinline__ spn<T> slash_r_plus_m(const T* 
   r.c[3] = m * s.c[3]; rfma(r.c[3], qm, s.c[1]); cfma(r.c[3], ql, s.c[0]);
   return r;
 }
-// row * (a-slash), a complex: psibar-type rows
-template <typename T> __device__ __forceinline__ spn<T> row_slash_c(const spn<T>& w, const vec4<T>& a) {
-  cx<T> ap = a.c[0] + a.c[3], am = a.c[0] - a.c[3];
-  cx<T> ar = mk<T>(a.c[1].re + a.c[2].im, a.c[1].im - a.c[2].re);
-  cx<T> al = mk<T>(a.c[1].re - a.c[2].im, a.c[1].im + a.c[2].re);
-  spn<T> r;   // r_j = sum_i w_i A_ij ; A = [[0,0,am,-ar],[0,0,-al,ap],[ap,ar,0,0],[al,am,0,0]]
-  r.c[0] = w.c[2] * ap; cfma(r.c[0], w.c[3], al);
-  r.c[1] = w.c[2] * ar; cfma(r.c[1], w.c[3], am);
-  r.c[2] = w.c[0] * am; cfms(r.c[2], w.c[1], al);
-  r.c[3] = w.c[1] * ap; cfms(r.c[3], w.c[0], ar);
-  return r;
-}
 // row * (q-slash + m), q real
 template <typename T> __device__ __forceinline__ spn<T> row_slash_r_plus_m(const spn<T>& w, const T* q, T m) {
   T qp = q[0] + q[3], qm = q[0] - q[3];
@@ -135,15 +123,27 @@ template <typename T> __device__ __forceinline__ chi_pair<T> make_chi(T px, T py
   r.m[0] = mk<T>(-N * px, N * py); r.m[1] = mk<T>(N * ppz, 0);
   return r;
 }
-// u(p,lam) = ( sqrt(E-lam|p|) chi_lam , sqrt(E+lam|p|) chi_lam )
+// Spinor normalisation (reading Q8 / DESIGN.md R8): the energy comes from the input, the mass from the PARAMETER SET, and
+// the magnitude of the 3-momentum in the normalisation is the one that follows from these two, P = sqrt((E-m)(E+m));
+// only the direction chi(p_hat) comes from the input 3-momentum.  On the mass shell P = |p|; for a set whose mass differs from
+// the one the events were generated with this is what "the parameter masses in spinors and propagators, E from the input"
+// means, and it equals the oracle's Dirac-representation form (sqrt(E+m) chi, lam sqrt(E-m) chi) exactly:
+// ((sqrt(E+m) -+ lam sqrt(E-m)) / sqrt2)^2 = E -+ lam P.
+template <typename T> __device__ __forceinline__ T shell_norm(T E, T m, T& sm) {
+  const T P = (m == T(0)) ? E : sqrt((E - m) * (E + m));
+  const T ep = E + P, ir = rsqrt(ep);
+  sm = m * ir;                      // sqrt(E-P) = m / sqrt(E+P): no cancellation, no division
+  return ep * ir;                   // sqrt(E+P)
+}
+// u(p,lam) = ( sqrt(E-lam P) chi_lam , sqrt(E+lam P) chi_lam )
 template <typename T> __device__ __forceinline__ spn<T> spinor_u(const chi_pair<T>& x, T E, T m, int lam) {
-  const T ep = E + x.pabs, ir = rsqrt(ep), sp = ep * ir, sm = m * ir;     // sqrt(E+|p|), sqrt(E-|p|) = m / sqrt(E+|p|); one rsqrt, no division
+  T sm; const T sp = shell_norm(E, m, sm);
   const cx<T>* c = lam > 0 ? x.p : x.m; T a = lam > 0 ? sm : sp, b = lam > 0 ? sp : sm;
   spn<T> r; r.c[0] = a * c[0]; r.c[1] = a * c[1]; r.c[2] = b * c[0]; r.c[3] = b * c[1]; return r;
 }
-// v(p,lam) = ( -lam sqrt(E+lam|p|) chi_{-lam} , lam sqrt(E-lam|p|) chi_{-lam} )
+// v(p,lam) = ( -lam sqrt(E+lam P) chi_{-lam} , lam sqrt(E-lam P) chi_{-lam} )
 template <typename T> __device__ __forceinline__ spn<T> spinor_v(const chi_pair<T>& x, T E, T m, int lam) {
-  const T ep = E + x.pabs, ir = rsqrt(ep), sp = ep * ir, sm = m * ir;     // sqrt(E+|p|), sqrt(E-|p|) = m / sqrt(E+|p|); one rsqrt, no division
+  T sm; const T sp = shell_norm(E, m, sm);
   const cx<T>* c = lam > 0 ? x.m : x.p; T a = lam > 0 ? -sp : sm, b = lam > 0 ? sm : -sp;
   spn<T> r; r.c[0] = a * c[0]; r.c[1] = a * c[1]; r.c[2] = b * c[0]; r.c[3] = b * c[1]; return r;
 }
@@ -180,16 +180,6 @@ template <typename T> __device__ __forceinline__ void V4_acc(vec4<T>& acc, const
 #pragma unroll
   for (int i = 0; i < 4; i++) { cfma(acc.c[i], xz, Y.c[i]); cfma(acc.c[i], yz, X.c[i]); cfma(acc.c[i], xy, Z.c[i]); }
 }
-// conditional negation on the integer pipe (sign-bit flip), keeps the FP pipes for arithmetic
-__device__ __forceinline__ double flip_sign(double x, unsigned mask_hi) { return __hiloint2double(__double2hiint(x) ^ (int)mask_hi, __double2loint(x)); }
-__device__ __forceinline__ float flip_sign(float x, unsigned mask_hi) { return __int_as_float(__float_as_int(x) ^ (int)mask_hi); }
-template <typename T> __device__ __forceinline__ vec4<T> cond_neg(const vec4<T>& a, bool neg) {
-  vec4<T> r; const unsigned m = neg ? 0x80000000u : 0u;
-#pragma unroll
-  for (int i = 0; i < 4; i++) { r.c[i].re = flip_sign(a.c[i].re, m); r.c[i].im = flip_sign(a.c[i].im, m); }
-  return r;
-}
-
 // light-cone components of a complex vector: a+ = a0+a3, a- = a0-a3, ar = a1 - i a2, al = a1 + i a2 (what a-slash needs)
 template <typename T> struct lcv { cx<T> p, m, r, l; };
 template <typename T> __device__ __forceinline__ lcv<T> lightcone(const vec4<T>& a) {

@@ -52,13 +52,10 @@ def test_multi_set_fp64_parity_every_event(idx, n):
 
 @pytest.mark.parametrize("idx,n", [(2, 515), (3, 301), (4, 47), (5, 7)])
 def test_multi_set_with_different_top_masses(idx, n):
-    """A set with another top mass makes the library redo externals, momentum sums and denominators for that set
-    (reading R12).  The comparison with the oracle is only defined for momenta on the mass shell of the set's own m_t
-    (reading Q8: off shell, sqrt(E+-m) and sqrt(E+-|p|) spinor normalisations differ), so the masses here differ by
-    one ulp: the separate-externals code path runs, the numbers stay within tolerance of the on-shell oracle."""
+    """Sets with other top masses make the library redo externals, momentum sums and denominators for those sets (R12).
+    The events stay on the old set's mass shell; off shell both sides normalise the spinors from (E, m_t') (reading Q8 / R8)."""
     c = ev.config(idx)
-    up, dn = float(np.nextafter(173.0, 200.0)), float(np.nextafter(173.0, 0.0))
-    sets = [ev.params(mt=up, ggg_scale=1.1, gggg_scale=1.1), c.params_new, ev.params(mt=dn, ggg_scale=0.7)]
+    sets = [ev.params(mt=170.0, ggg_scale=1.1, gggg_scale=1.1), c.params_new, ev.params(mt=178.25, ggg_scale=0.7), ev.params(mt=173.0, alpha_s=0.11)]
     m, w = ev.generate(c, n)
     got = run_multi(c, sets, m, w)
     K = len(sets)

@@ -99,16 +99,88 @@ def test_generic_engine_agrees_with_dedicated_gg_ttx_kernel_and_oracle():
 
 
 @pytest.mark.parametrize("idx", [2, 3])
-def test_mass_change_between_sets_takes_two_passes(idx):
-    """General parameter change (SURVEY §8(f) #4): m_t differs, so nothing but the momenta is shared."""
+def test_general_coupling_change_alpha_s_and_both_scales(idx):
+    """A new set that moves alpha_s and the two scales independently (masses equal: externals stay shared)."""
     c = ev.config(idx)
     m, w = ev.generate(c, 257)
     pn = ev.params(mt=173.0, ggg_scale=1.05, gggg_scale=0.9, alpha_s=0.125)
     po = ev.params(mt=173.0)
-    # keep the events on the old mass shell; the new set only moves alpha_s and the scales (mass shell must match, Q8)
     a, b, wn, _ = orc.reweight(c.process, po, pn, m, w)
     got = gpu_run(c.process, po, pn, m, w)
     assert rel(got, np.stack([a, b, wn])).max() < TOL64
+
+
+@pytest.mark.parametrize("proc_idx_n", [("gg_ttx", 2, 1031), ("gg_ttx@bg", 2, 517), ("gg_ttxg", 3, 301), ("gg_ttxgg", 4, 67), ("gg_ttxggg", 5, 9)])
+@pytest.mark.parametrize("mt_new", [170.0, 176.5])
+def test_top_mass_change_single_new_set(proc_idx_n, mt_new):
+    """SURVEY 8(f) #4 (PAPER.md:87 last sentence: parameters inside the amplitudes): the new set has another top mass.  The events
+    stay on the OLD mass shell (same phase space); spinors and propagators of the new set use m_t' with E from the
+    input (reading Q8 / DESIGN.md R8), in the oracle and in the kernels alike.  One new set: gg_ttx takes gg_ttx_kernel's two_pass
+    branch, the engine its separate-externals path."""
+    proc, idx, n = proc_idx_n
+    c = ev.config(idx)
+    m, w = ev.generate(c, n)
+    pn = ev.params(mt=mt_new, ggg_scale=1.1, gggg_scale=1.1)
+    a, b, wn, _ = orc.reweight(c.process, c.params_old, pn, m, w)
+    got = gpu_run(proc, c.params_old, pn, m, w)
+    assert rel(got, np.stack([a, b, wn])).max() < TOL64
+    assert np.abs(b / a - 1).max() > 1e-3                  # the mass change is macroscopic
+
+
+def _rotation(seed):
+    rng = np.random.default_rng(seed)
+    q, r = np.linalg.qr(rng.normal(size=(3, 3)))
+    q = q @ np.diag(np.sign(np.diag(r)))
+    if np.linalg.det(q) < 0:
+        q[:, 0] = -q[:, 0]
+    return q
+
+
+def _boost(m, beta):
+    """Boost every momentum of m[n_ext,4,n] by the velocity vector beta."""
+    b2 = float(beta @ beta)
+    g = 1.0 / np.sqrt(1.0 - b2)
+    bp = np.einsum("k,pkn->pn", beta, m[:, 1:, :])
+    out = np.empty_like(m)
+    out[:, 0, :] = g * (m[:, 0, :] + bp)
+    out[:, 1:, :] = m[:, 1:, :] + ((g - 1.0) * bp / b2 + g * m[:, 0, :])[:, None, :] * beta[None, :, None]
+    return out
+
+
+@pytest.mark.parametrize("idx,n", [(1, 2003), (2, 2003), (3, 401), (4, 61), (6, 61)])
+def test_rotated_events_against_oracle_incoming_legs_off_axis(idx, n):
+    """The seeded sets have legs 0, 1 exactly on the z axis, so only the exact-axis branches of polvec / make_chi ever see the
+    incoming legs.  A random SO(3) rotation of every event puts them on the generic branch (the library must
+    not assume beams along z); compared with the oracle on the SAME rotated momenta, both parameter sets, and with the
+    unrotated result (rotations are a symmetry of both sets, reading Q1)."""
+    c = ev.config(idx)
+    m, w = ev.generate(c, n)
+    R = _rotation(40 + idx)
+    mr = m.copy()
+    mr[:, 1:, :] = np.einsum("ab,pbn->pan", R, m[:, 1:, :])
+    assert np.abs(mr[0, 1:3, :]).min() > 1.0               # leg 0 has left the axis
+    a, b, wn, _ = orc.reweight(c.process, c.params_old, c.params_new, mr, w)
+    got = gpu_run(c.process, c.params_old, c.params_new, mr, w)
+    assert rel(got, np.stack([a, b, wn])).max() < TOL64
+    g0 = gpu_run(c.process, c.params_old, c.params_new, m, w)
+    assert rel(got, g0).max() < 1e-10
+
+
+@pytest.mark.parametrize("idx,n", [(1, 2003), (2, 2003), (3, 401), (4, 61), (6, 61)])
+def test_boosted_events_against_oracle(idx, n):
+    """A boost along a generic direction: legs 0, 1 off the axis and no longer back to back.  The oracle is evaluated on the same
+    boosted momenta (for cfgs 2-4 the NEW set is frame dependent, reading Q1, so it is compared in the boosted frame only); the old
+    set (and both sets of cfgs 1, 6) must also agree with the unboosted launch."""
+    c = ev.config(idx)
+    m, w = ev.generate(c, n)
+    mb = _boost(m, np.array([0.21, -0.13, 0.32]))
+    a, b, wn, _ = orc.reweight(c.process, c.params_old, c.params_new, mb, w)
+    got = gpu_run(c.process, c.params_old, c.params_new, mb, w)
+    assert rel(got, np.stack([a, b, wn])).max() < TOL64
+    g0 = gpu_run(c.process, c.params_old, c.params_new, m, w)
+    assert rel(got[0], g0[0]).max() < 1e-10
+    if idx in (1, 6):
+        assert rel(got[1], g0[1]).max() < 1e-10
 
 
 def test_edge_cases_empty_single_and_bad_arguments():

@@ -55,12 +55,20 @@ def test_weights_lognormal():
 
 
 def test_library_exports_every_declared_symbol():
-    binding_lib = ctypes.CDLL(binding.LIB_PATH)
-    header = open(os.path.join(ROOT, "include", "rwgt.h")).read()
-    declared = set(re.findall(r"\b(rwgt_[a-z_0-9]+)\s*\(", header)) - {"rwgt_handle", "rwgt_params"}
-    assert declared == set(binding.EXPORTS)
-    for name in declared:
-        assert hasattr(binding_lib, name), name
+    """Every include/*.h against the library that implements it and the binding that wraps it."""
+    from paper_2312_07440_b200 import microbench
+    headers = {"rwgt.h": (binding.LIB_PATH, binding.EXPORTS), "rwgt_microbench.h": (microbench.LIB_PATH, microbench.EXPORTS)}
+    assert set(os.listdir(os.path.join(ROOT, "include"))) == set(headers)
+    for hname, (libpath, exports) in headers.items():
+        so = ctypes.CDLL(libpath)
+        header = open(os.path.join(ROOT, "include", hname)).read()
+        declared = set(re.findall(r"\b(rwgt_[a-z_0-9]+)\s*\(", header)) - {"rwgt_handle", "rwgt_params"}
+        assert declared == set(exports), (hname, declared ^ set(exports))
+        for name in declared:
+            assert hasattr(so, name), name
+            assert hasattr(binding if hname == "rwgt.h" else microbench, name), name
+    # the measurement aid is not part of the product library
+    assert not hasattr(ctypes.CDLL(binding.LIB_PATH), "rwgt_microbench_peak")
 
 
 def test_host_only_entry_points_without_gpu():
