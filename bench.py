@@ -1,10 +1,14 @@
 #!/usr/bin/env python
 """bench.py — reweighted events/s of the LO reweighting hot path (eq. 3; PAPER.md:87 steps 3-6).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--precision fp64] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 5] [--precision fp64] [--impl reference]
+    python bench.py --sweep [--config 6]        # the paper's Fig. 2 / Fig. 3 axes, markdown tables
+    python bench.py --parity-report             # max / median error against tests/golden/full_cfg*.npz, markdown table
 
 A step = one pass of the whole hot path (one rwgt_run launch: a1-a7 of SURVEY §8(a)) over the synthetic
-event set of one BASELINE.json config (default configs[1] = gg -> ttbar, 1,048,576 events).  Prints ONE
+event set of one BASELINE.json config.  Default: configs[4] = gg -> ttbar ggg, 65,536 events, FP64: the largest
+work per step and the config north_star's FMA-peak target is written on.  Every other config / precision is timed
+with the same --steps / --warmup and reported inside the line (roofline.per_config, other_configs).  Prints ONE
 JSON line (rank 0).  N > 1: launched by torchrun, every rank runs the same-size workload with its own seed
 (weak scaling, no data-path collective: events are independent).
 """
@@ -119,9 +123,8 @@ def run_reference(args) -> None:
         return
     import oracle as orc
     c = ev.config(args.config)
-    per_core = {1: 25000.0, 2: 500.0, 3: 55.0, 4: 5.0, 5: 1.1, 6: 5.0}[c.index]       # rough oracle events/s/core, sizes the sample only
     cores = os.cpu_count() or 1
-    n = args.ref_events or max(8, int(per_core * cores * 4.0))                    # ~4 s per step
+    n = args.ref_events or max(8, int(ORACLE_PER_CORE[c.index] * cores * 3.0))    # ~3 s per step
     n = min(n, c.n_events)
     m, w = ev.generate(c, n)
     for _ in range(args.warmup):
@@ -175,19 +178,151 @@ def time_config(torch, B, c, precision, n, steps, warmup, seed_offset, flush_buf
     return res
 
 
+def per_config_entry(cc, prec, rr, max_mhz, hbm_peak):
+    kms = statistics.mean(rr["ms"])
+    dt_ = "f64" if prec == "fp64" else "f32"
+    fpe = rr["flops_per_event"] + (rr["tensor_flops_per_event"] if dt_ == "f64" else 0.0)
+    n = rr["n"]
+    tf = fpe * n / (kms * 1e-3) / 1e12
+    gbs = bytes_per_event(cc) * n / (kms * 1e-3) / 1e9
+    return {"cfg": cc.index, "process": cc.process, "precision": prec, "n": n, "kernel_ms": round(kms, 5), "events_per_s": n / (kms * 1e-3),
+            "alu_tflops": round(tf, 3), "alu_frac": round(tf / alu_peak_tflops(dt_, max_mhz), 4), "hbm_gbs": round(gbs, 1), "hbm_frac": round(gbs / hbm_peak, 4)}
+
+
+def run_sweep(args) -> None:
+    """The paper's two experiments (Fig. 2: runtime against the number of events for one parameter set; PAPER.md:117
+    Fig. 3: runtime against the number of parameter sets), every point the mean (min-max) of 5 runs as in the paper.
+    device = rwgt_run_multi on device-resident buffers (CUDA events); host = rwgt_run_multi_host on pinned host buffers, copies inside the
+    timed call (the transfer overhead the paper describes for small n); file = rwgt_run_file, read + copy + kernel + write."""
+    import tempfile
+    import torch
+    from paper_2312_07440_b200 import binding as B
+    c = ev.config(args.config if args.config else 6)
+    nmax = max(1 << args.max_log2, args.fig3_events)
+    m0, w0 = ev.generate(c, min(nmax, c.n_events))
+    reps = (nmax + m0.shape[2] - 1) // m0.shape[2]
+    m = np.tile(m0, (1, 1, reps))[:, :, :nmax].copy()
+    w = np.tile(w0, reps)[:nmax].copy()
+    rng = np.random.default_rng(c.seed)
+    tmp = tempfile.mkdtemp(prefix="rwgt_sweep_")
+
+    def new_sets(k):
+        if c.index == 6:      # a random electroweak coupling per set (PAPER.md:77)
+            return [ev.params(alpha_em=float(a)) for a in rng.uniform(0.5, 2.0, size=k) / 132.5]
+        if c.index == 1:
+            return [ev.params(GammaZ=float(g), sin2_thetaW=float(x)) for g, x in zip(rng.uniform(2.3, 2.7, size=k), rng.uniform(0.22, 0.24, size=k))]
+        return [ev.params(ggg_scale=float(1 + x), gggg_scale=float(1 + x)) for x in rng.uniform(-0.2, 0.2, size=k)]
+
+    def stats(ts):
+        return f"{np.mean(ts):.4f} ({min(ts):.4f}-{max(ts):.4f})"
+
+    def measure(n, K):
+        sets = new_sets(K)
+        h = B.rwgt_create_multi(c.process, c.params_old, sets)
+        mh = torch.from_numpy(np.ascontiguousarray(m[:, :, :n])).pin_memory()
+        wh = torch.from_numpy(w[:n].copy()).pin_memory()
+        dm, dw = mh.cuda(), wh.cuda()
+        a = torch.empty(n, dtype=torch.float64, device="cuda")
+        b = torch.empty((K, n), dtype=torch.float64, device="cuda")
+        o = torch.empty((K, n), dtype=torch.float64, device="cuda")
+        ha, hb, ho = torch.empty(n, dtype=torch.float64).pin_memory(), torch.empty((K, n), dtype=torch.float64).pin_memory(), torch.empty((K, n), dtype=torch.float64).pin_memory()
+        st = torch.cuda.current_stream().cuda_stream
+        fin, fout = os.path.join(tmp, "in.rwgt"), os.path.join(tmp, "out.rwgt")
+        B.write_event_file(fin, c.process, mh.numpy(), wh.numpy())
+        dev, host, fil = [], [], []
+        for it in range(2 + 5):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            B.rwgt_run_multi(h, dm.data_ptr(), dw.data_ptr(), a.data_ptr(), b.data_ptr(), o.data_ptr(), n, st)
+            e1.record()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            B.rwgt_run_multi_host(h, mh.numpy(), wh.numpy(), ha.numpy(), hb.numpy(), ho.numpy())
+            t1 = time.perf_counter()
+            B.rwgt_run_file(h, fin, fout)
+            t2 = time.perf_counter()
+            if it >= 2:
+                dev.append(e0.elapsed_time(e1)); host.append((t1 - t0) * 1e3); fil.append((t2 - t1) * 1e3)
+        assert np.array_equal(ho.numpy(), o.cpu().numpy())
+        res = B.read_result_file(fout)
+        assert np.array_equal(res["w_new"], ho.numpy())
+        B.rwgt_destroy(h)
+        return dev, host, fil
+
+    print(f"# {c.process} (config {c.index}), FP64\n")
+    print("## Runtime against the number of events, one parameter set (PAPER.md:105 Fig. 2), ms: mean (min-max) of 5\n")
+    print("| events | device ms | host-buffer ms | file ms (read + copy + kernel + write) | device events/s | host-buffer events/s | file events/s |\n|---|---|---|---|---|---|---|")
+    for lg in range(0, args.max_log2 + 1, 2):
+        n = 1 << lg
+        dev, host, fil = measure(n, 1)
+        print(f"| {n} | {stats(dev)} | {stats(host)} | {stats(fil)} | {n / np.mean(dev) * 1e3:.3e} | {n / np.mean(host) * 1e3:.3e} | {n / np.mean(fil) * 1e3:.3e} |", flush=True)
+    n = args.fig3_events
+    print(f"\n## Runtime against the number of parameter sets, {n} events (PAPER.md:117 Fig. 3), ms: mean (min-max) of 5\n")
+    print("| parameter sets | device ms | host-buffer ms | file ms | new weights/s (device) |\n|---|---|---|---|---|")
+    for K in [int(x) for x in args.sets.split(",")]:
+        dev, host, fil = measure(n, K)
+        print(f"| {K} | {stats(dev)} | {stats(host)} | {stats(fil)} | {K * n / np.mean(dev) * 1e3:.3e} |", flush=True)
+
+
+def run_parity_report(args) -> None:
+    """Per config and precision: max / median relative error of |M|^2, |M'|^2, W' of the full-size launch against the stored oracle
+    values tests/golden/full_cfg<N>.npz (written by tests/golden/make_goldens.py from the CPU oracle alone), events over tolerance,
+    worst event.  Reads files only: the oracle is not executed."""
+    import torch
+    from paper_2312_07440_b200 import binding as B
+    tol = {"fp64": (1e-11, 1e-11), "fp32": (1e-4, 1e-6), "mixed": (1e-4, 1e-6)}
+    print("| cfg | process | precision | events compared (of the launch) | output | max rel. err | median rel. err | tolerance (max / median) | events over max tolerance | worst event |")
+    print("|---|---|---|---|---|---|---|---|---|---|")
+    for idx in (1, 2, 3, 4, 5, 6):
+        c = ev.config(idx)
+        f = os.path.join(ROOT, "tests", "golden", f"full_cfg{idx}.npz")
+        if not os.path.exists(f):
+            print(f"| {idx} | {c.process} | - | golden file missing | | | | | | |")
+            continue
+        ref = np.load(f)["out"]
+        ng = ref.shape[1]
+        m, w = ev.generate(c)
+        dm, dw = torch.from_numpy(m).cuda(), torch.from_numpy(w).cuda()
+        for prec in c.precisions + (("mixed",) if "fp32" in c.precisions else ()):
+            r = B.Reweighter(c.process, c.params_old, c.params_new, prec)
+            got = r.run(dm, dw).cpu().numpy()
+            r.close()
+            tmax, tmed = tol[prec]
+            for k, name in enumerate(("|M|^2", "|M'|^2", "W'")):
+                e = np.abs(got[k, :ng] / ref[k] - 1)
+                print(f"| {idx} | {c.process} | {prec} | {ng} ({c.n_events}) | {name} | {e.max():.2e} | {np.median(e):.2e} | {tmax:g} / {tmed:g} | {int((e > tmax).sum())} | {int(e.argmax())} |", flush=True)
+
+
+# rough oracle events/s/core (both parameter sets), measured on this pool's hosts; only sizes the bounded CPU samples
+ORACLE_PER_CORE = {1: 150000.0, 2: 6000.0, 3: 300.0, 4: 25.0, 5: 1.8, 6: 25.0}
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config index 1..5 (default 2 = configs[1]); 6 = the paper's own e+e- -> 5 gamma (PAPER.md:72-77)")
+    ap.add_argument("--config", type=int, default=0, help="BASELINE.json config index 1..5 (default 5 = configs[4], the config north_star's FMA target names); "
+                                                          "6 = the paper's own e+e- -> 5 gamma (PAPER.md:72-77)")
     ap.add_argument("--precision", default="fp64", choices=["fp64", "fp32", "mixed"])
     ap.add_argument("--events", type=int, default=0, help="override the config's event count")
     ap.add_argument("--ref-events", type=int, default=0, help="reference arm: events per step")
-    ap.add_argument("--no-extra", action="store_true", help="skip the per-config summary of the other configs")
+    ap.add_argument("--no-extra", action="store_true", help="skip the other configs / precisions")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--sweep", action="store_true", help="throughput against events / parameter sets (markdown), device, host-buffer and file paths")
+    ap.add_argument("--max-log2", type=int, default=20)
+    ap.add_argument("--sets", default="1,2,4,8,16")
+    ap.add_argument("--fig3-events", type=int, default=131072)
+    ap.add_argument("--parity-report", action="store_true", help="error statistics against tests/golden/full_cfg*.npz (markdown)")
     args = ap.parse_args()
+    if args.sweep:
+        run_sweep(args)
+        return
+    if args.parity_report:
+        run_parity_report(args)
+        return
+    args.config = args.config or 5
     if args.impl == "reference":
         run_reference(args)
         return
@@ -259,11 +394,13 @@ def main() -> None:
     achieved_tf = flops / (kernel_ms * 1e-3) / 1e12
     max_mhz = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
     peak_tf = alu_peak_tflops(dtype, max_mhz)
-    traffic = None
+    hbm_peak = peaks.get("hbm_gbs", 6650.0)
+    traffic, traffic_build = None, None
     try:
-        traffic = json.load(open(os.path.join(ROOT, "profiles", "r1_counts.json")))[f"cfg{c.index}_{args.precision}"]["traffic_bytes"]
-        if n != c.n_events:
-            traffic = None
+        counts = json.load(open(os.path.join(ROOT, "profiles", "counts.json")))
+        ent = counts[f"cfg{c.index}_{args.precision}"]
+        if n == c.n_events:
+            traffic, traffic_build = ent["traffic_bytes"], ent.get("build", counts.get("build"))
     except Exception:
         pass
     micro = {}
@@ -277,17 +414,19 @@ def main() -> None:
             micro[name] = None
     chain_tf = micro.get("fma_chain")
     roofline = {"bound": "alu", "achieved": achieved_tf, "peak": peak_tf, "unit": "TFLOP/s", "frac": achieved_tf / peak_tf, "traffic": traffic,
+                "traffic_source": (f"ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/counts.json, measured on build {traffic_build}") if traffic else None,
                 "peak_source": f"derived: 148 SM x {FP64_LANES_PER_SM if dtype == 'f64' else FP32_LANES_PER_SM} FMA lanes x 2 flop x {max_mhz:g} MHz (max SM clock); DESIGN.md Roofline",
                 "peak_fma_chain_measured": chain_tf, "frac_of_fma_chain_measured": (achieved_tf / chain_tf) if chain_tf else None,
                 "microbench_tflops": micro,
                 "frac_at_clock_under_load": (achieved_tf / alu_peak_tflops(dtype, clocks["sm_mhz"])) if clocks.get("sm_mhz") else None,
                 "flops_per_event": res["flops_per_event"] + (res["tensor_flops_per_event"] if dtype == "f64" else 0.0),
+                "flops_per_event_kind": "algorithmic operation count of the schedule (include/rwgt.h rwgt_flops_per_event); FP32/mixed: model only, FFMA2 is not in ncu's FFMA counters",
                 "vector_flops_per_event": res["flops_per_event"], "colour_form_flops_per_event": res["tensor_flops_per_event"],
                 "kernel_ms": kernel_ms,
                 "colour_form_fp64": {"flops_per_event": res["tensor_flops_per_event"],
                                      "achieved_tflops": col_flops / (kernel_ms * 1e-3) / 1e12,
                                      "note": "mma.m8n8k4 on the FP64 pipe (shared with DFMA); included in `achieved` in FP64 mode only"},
-                "hbm": {"achieved_gbs": bytes_per_event(c) * n / (kernel_ms * 1e-3) / 1e9, "peak_gbs": peaks.get("hbm_gbs", 6650.0),
+                "hbm": {"achieved_gbs": bytes_per_event(c) * n / (kernel_ms * 1e-3) / 1e9, "peak_gbs": hbm_peak,
                         "peak_source": "MEASURED_PEAKS.json" if peaks.get("hbm_gbs") else "fallback"}}
     roofline["hbm"]["frac"] = roofline["hbm"]["achieved_gbs"] / roofline["hbm"]["peak_gbs"]
 
@@ -304,9 +443,8 @@ def main() -> None:
     # ---- cpu_baseline: the oracle on a bounded sample of the same workload (rank 0, N = 1 only) ----
     if world == 1 and not args.no_cpu_baseline:
         import oracle as orc
-        per_core = {1: 25000.0, 2: 500.0, 3: 55.0, 4: 5.0, 5: 1.1, 6: 5.0}[c.index]
         cores = os.cpu_count() or 1
-        ns = min(n, max(8, int(per_core * cores * 12.0)))
+        ns = min(n, max(8, int(ORACLE_PER_CORE[c.index] * cores * 12.0)))
         t0 = time.perf_counter()
         a, b, wn, used = orc.reweight(c.process, c.params_old, c.params_new, m[:, :, :ns].copy(), w[:ns].copy())
         dt = time.perf_counter() - t0
@@ -316,54 +454,46 @@ def main() -> None:
                                 "sample": f"first {ns} events of the same seeded set, both parameter sets, {dt:.1f} s",
                                 "max_rel_err_gpu_vs_oracle_on_sample": err}
 
-    # ---- the other configs / precisions, short runs, same protocol (context for the north_star targets) ----
+    # ---- every config / precision with the same --steps / --warmup (north_star targets: cfgs 4, 5 FMA fraction, cfg 1 HBM) ----
     if world == 1 and not args.no_extra:
+        per_config = [per_config_entry(c, args.precision, dict(res, n=n), max_mhz, hbm_peak)]
         extra = []
         for cc in ev.CONFIGS:
-            for prec in cc.precisions:
+            for prec in cc.precisions + (("mixed",) if "fp32" in cc.precisions else ()):
                 if cc.index == c.index and prec == args.precision:
                     continue
                 try:
-                    rr = time_config(torch, B, cc, prec, cc.n_events, 5, 3, 0, flush_buf)
-                    kms = statistics.mean(rr["ms"])
-                    dt_ = "f64" if prec == "fp64" else "f32"
-                    fpe = rr["flops_per_event"] + (rr["tensor_flops_per_event"] if dt_ == "f64" else 0.0)
-                    tf = fpe * cc.n_events / (kms * 1e-3) / 1e12
-                    extra.append({"workload": workload_name(cc, cc.n_events), "precision": prec, "events_per_s": cc.n_events / (kms * 1e-3),
-                                  "kernel_ms": kms, "alu_tflops": tf, "alu_frac": tf / alu_peak_tflops(dt_, max_mhz),
-                                  "hbm_gbs": bytes_per_event(cc) * cc.n_events / (kms * 1e-3) / 1e9,
-                                  "hbm_frac": bytes_per_event(cc) * cc.n_events / (kms * 1e-3) / 1e9 / roofline["hbm"]["peak_gbs"], "l2": rr["l2"]})
+                    rr = time_config(torch, B, cc, prec, cc.n_events, args.steps, args.warmup, 0, flush_buf)
+                    rr["n"] = cc.n_events
+                    per_config.append(per_config_entry(cc, prec, rr, max_mhz, hbm_peak))
                     rr["rw"].close()
                 except Exception as ex:  # keep the headline line alive
-                    extra.append({"workload": workload_name(cc, cc.n_events), "precision": prec, "error": str(ex)})
-        # K new parameter sets in one pass (PAPER.md:87 step 7, Fig. 3 axis; SURVEY §8(f) NEXT 1): kappa = 0.1 k / K
-        for ci, K in ((2, 8), (4, 8), (5, 4)):
-            try:
-                cc = ev.config(ci)
-                sets = [ev.params(ggg_scale=1 + 0.1 * (k + 1) / K, gggg_scale=1 + 0.1 * (k + 1) / K) for k in range(K)]
-                rr = time_config(torch, B, cc, "fp64", cc.n_events, 5, 3, 0, flush_buf, new_sets=sets)
-                kms = statistics.mean(rr["ms"])
-                fpe = rr["flops_per_event"] + rr["tensor_flops_per_event"]
-                tf = fpe * cc.n_events / (kms * 1e-3) / 1e12
-                extra.append({"workload": workload_name(cc, cc.n_events) + f" with K={K} new parameter sets in one pass", "precision": "fp64",
-                              "events_per_s": cc.n_events / (kms * 1e-3), "new_weights_per_s": K * cc.n_events / (kms * 1e-3), "kernel_ms": kms,
-                              "alu_tflops": tf, "alu_frac": tf / alu_peak_tflops("f64", max_mhz), "l2": rr["l2"]})
-                rr["rw"].close()
-            except Exception as ex:
-                extra.append({"workload": f"cfg{ci} K={K}", "error": str(ex)})
+                    per_config.append({"cfg": cc.index, "precision": prec, "error": str(ex)})
         # cfg 1 is launch-latency-bound at its 16,384 events: the same distribution at n = 2^24 (buffers >> L2)
         try:
             c1 = ev.config(1)
-            rr = time_config(torch, B, c1, "fp64", 1 << 24, 5, 3, 0, flush_buf, tile_from=1 << 20)
-            kms = statistics.mean(rr["ms"]); n1 = 1 << 24
-            gbs = bytes_per_event(c1) * n1 / (kms * 1e-3) / 1e9
-            tf = rr["flops_per_event"] * n1 / (kms * 1e-3) / 1e12
-            extra.append({"workload": workload_name(c1, n1) + " (asymptotic: the seeded set of 2^20 events tiled 16x)", "precision": "fp64",
-                          "events_per_s": n1 / (kms * 1e-3), "kernel_ms": kms, "alu_tflops": tf, "alu_frac": tf / alu_peak_tflops("f64", max_mhz),
-                          "hbm_gbs": gbs, "hbm_frac": gbs / roofline["hbm"]["peak_gbs"], "l2": rr["l2"]})
+            rr = time_config(torch, B, c1, "fp64", 1 << 24, args.steps, args.warmup, 0, flush_buf, tile_from=1 << 20)
+            rr["n"] = 1 << 24
+            e1 = per_config_entry(c1, "fp64", rr, max_mhz, hbm_peak)
+            e1["note"] = "asymptotic size: the seeded set of 2^20 events tiled 16x (buffers >> L2)"
+            per_config.append(e1)
             rr["rw"].close()
         except Exception as ex:
-            extra.append({"workload": "epem_mupmum n=2^24", "error": str(ex)})
+            per_config.append({"cfg": 1, "n": 1 << 24, "error": str(ex)})
+        per_config.sort(key=lambda e: (e.get("cfg", 0), e.get("precision", ""), e.get("n", 0)))
+        roofline["per_config"] = per_config
+        # K new parameter sets in one pass (PAPER.md:87 step 7, Fig. 3 axis; SURVEY §8(f) NEXT 1): kappa = 0.1 k / K
+        for ci, K in ((2, 8), (4, 8), (5, 4), (5, 16)):
+            try:
+                cc = ev.config(ci)
+                sets = [ev.params(ggg_scale=1 + 0.1 * (k + 1) / K, gggg_scale=1 + 0.1 * (k + 1) / K) for k in range(K)]
+                rr = time_config(torch, B, cc, "fp64", cc.n_events, max(3, args.steps // 4), 3, 0, flush_buf, new_sets=sets)
+                kms = statistics.mean(rr["ms"])
+                extra.append({"workload": workload_name(cc, cc.n_events) + f" with K={K} new parameter sets in one pass", "precision": "fp64",
+                              "events_per_s": cc.n_events / (kms * 1e-3), "new_weights_per_s": K * cc.n_events / (kms * 1e-3), "kernel_ms": kms, "l2": rr["l2"]})
+                rr["rw"].close()
+            except Exception as ex:
+                extra.append({"workload": f"cfg{ci} K={K}", "error": str(ex)})
         # cfg 1 at its stated 16,384 events is launch-latency-bound: the same launch captured in a CUDA graph (20 launches per replay)
         try:
             c1 = ev.config(1)

@@ -51,7 +51,8 @@ typedef struct {
  *            leg order in `momenta`: [e+,e-,mu+,mu-] resp. [g,g,t,tbar,(g,(g,(g)))];
  *            legs 0,1 incoming, all momenta physical (E>0).
  * Builds the per-process tables (ordered-current schedule, colour matrix) on the host and
- * copies them and the couplings to the CURRENT device.  Returns NULL on error (unknown
+ * copies them and the couplings to the CURRENT device; every later call on the handle makes that device current for its
+ * duration (and restores the caller's), so streams passed to it must belong to that device.  Returns NULL on error (unknown
  * process, non-positive alpha, sin2_thetaW outside (0,1), Gamma_t != 0, no CUDA device);
  * rwgt_last_error() then describes it.  PAPER.md:87 restricts reweighting to parameters
  * "that can be modified at runtime": old and new share the process. */
@@ -123,6 +124,50 @@ int rwgt_run_host(rwgt_handle* h, const double* momenta, const double* weights, 
 /* rwgt_run_host for K >= 1 new sets: out_me_new, out_w_new are HOST double [K][n_events]. */
 int rwgt_run_multi_host(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old,
                         double* out_me_new, double* out_w_new, long long n_events, void* stream);
+
+/* eq. 2 (§2.1): "the total cross section is the sum of all event weights", sigma ~ sum_k W_k.  Writes the sum of each
+ * of n_rows weight rows to out_sums:
+ *   w         DEVICE double [n_rows][n_events], row r at offset r * n_events: the original weights (n_rows = 1) or the
+ *             out_w_new of rwgt_run_multi (n_rows = K), i.e. the reweighted cross section of every parameter set
+ *   out_sums  DEVICE double [n_rows]
+ * 1 <= n_rows <= 1 + RWGT_MAX_SETS.  One kernel launch on `stream`, no atomics in the arithmetic: a fixed block partition and fixed
+ * summation trees, so the result depends on the values and n_events only (bitwise reproducible); the relative error against the
+ * exact sum is bounded by ~(n_events / 16384 + 30) * 2^-53 * sum|W| / |sum W|.  Uses scratch of the handle: calls on one handle must be
+ * stream-ordered.  No allocation, no synchronisation.  Returns 0, -1 on a bad argument, or the cudaError_t of the launch. */
+int rwgt_sum_weights(rwgt_handle* h, const double* w, int n_rows, long long n_events, double* out_sums, void* stream);
+
+/* Binary event files: the stand-in for the LHE event files the paper's library parses (PAPER.md:87 step 2), which do
+ * not exist here.  Little endian, structure of arrays, the layout rwgt_run takes:
+ *   event file  = rwgt_event_file_header, double momenta[n_ext][4][n_events], double weights[n_events]
+ *   result file = rwgt_result_file_header, double me_old[n_events], me_new[K][n_events], w_new[K][n_events],
+ *                 double sum_w_old, sum_w_new[K]       (eq. 2 of the processed range, old weights and every parameter set) */
+typedef struct {
+  char magic[8];               /* "RWGTEVT1"                                        */
+  unsigned int version;        /* 1                                                 */
+  unsigned int n_ext;          /* external legs per event                           */
+  unsigned long long n_events;
+  char process[32];            /* process name as given to rwgt_create, NUL padded  */
+  unsigned long long reserved;
+} rwgt_event_file_header;
+typedef struct {
+  char magic[8];               /* "RWGTRES1"                                        */
+  unsigned int version;        /* 1                                                 */
+  unsigned int n_sets;         /* K new parameter sets                              */
+  unsigned long long n_events; /* events in this file                               */
+  char process[32];
+  unsigned long long first_event; /* index in the event file of this file's event 0 */
+} rwgt_result_file_header;
+
+/* The whole procedure of PAPER.md:87 (steps 2-8) for events [first_event, first_event + n_events) of the event file `in_path`
+ * (n_events < 0: to the end of the file): parse, copy to the device, evaluate |M|^2 and every |M'_k|^2, eq. 3, copy back, write the
+ * result file `out_path` (created or truncated), including the eq. 2 sums.  The range is cut into chunks; a reader thread fills one
+ * pinned buffer from the file while the previous chunk goes through the overlapped H2D / kernel / D2H pipeline of
+ * rwgt_run_multi_host and a writer thread stores the chunk before.  Pinned buffers and device scratch belong to the handle and are
+ * grown on first use.  Synchronises `stream`.  A rank of a multi-GPU job passes its own contiguous range and result path
+ * (events are independent: no exchange).
+ * Returns 0, -1 (bad argument, unreadable / foreign / truncated event file, range outside the file, write error; see
+ * rwgt_last_error()) or a positive cudaError_t. */
+int rwgt_run_file(rwgt_handle* h, const char* in_path, const char* out_path, long long first_event, long long n_events, void* stream);
 
 /* Frees device tables and scratch. 0 on success, -1 on NULL. */
 int rwgt_destroy(rwgt_handle* h);

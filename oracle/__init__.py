@@ -30,6 +30,8 @@ def lib():
         L.orc_me2_hel.argtypes = [C.c_int, _dp, _dp, _ip, C.c_int, _dp]
         L.orc_amp_epem.argtypes = [_dp, _dp, _ip, _dp]
         L.orc_amp_epem_ng.argtypes = [C.c_int, _dp, _dp, _ip, _dp, _dp]
+        L.orc_cross_section.argtypes = [_dp, C.c_long]
+        L.orc_cross_section.restype = C.c_double
         L.orc_denominator.argtypes = [C.c_int]
         L.orc_denominator.restype = C.c_double
         _lib = L
@@ -140,6 +142,12 @@ def amp_epem(par, p, hel) -> complex:
     out = np.empty(2)
     lib().orc_amp_epem(pp, ppp, ph, out.ctypes.data_as(_dp))
     return complex(out[0], out[1])
+
+
+def cross_section(weights) -> float:
+    """eq. 2: sigma ~ sum_k W_k, the plain left-to-right sum."""
+    w, pw = _d(weights)
+    return lib().orc_cross_section(pw, w.shape[0])
 
 
 def denominator(n: int) -> float:

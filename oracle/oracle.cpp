@@ -14,6 +14,7 @@
 // (route E), colour matrix from explicit Gell-Mann matrices, every helicity combination
 // evaluated from scratch, each parameter set evaluated independently.
 //
+// eq. 2 sigma ~ sum_k W_k: orc_cross_section, the plain sum, pinned against exactly rounded summation.
 // Pins (tests/test_oracle_pins.py): Dirac equation + completeness for u,v; transversality,
 // normalisation, helicity eigen-equation and completeness of eps; e+e- -> mu+mu- closed
 // form and gg -> ttbar closed form; gauge invariance eps->k of
@@ -554,6 +555,11 @@ int orc_reweight(const char* proc, const double* par_old, const double* par_new,
   }
   return used;
 }
+
+// eq. 2 (§2.1): "the total cross section is the sum of all event weights", sigma ~ sum_k W_k.  The plain definition:
+// a left-to-right sum in double.  Pin (tests/test_oracle_pins.py): against Python's exactly rounded math.fsum within the
+// textbook bound (n-1) 2^-53 sum|W| of recursive summation.
+double orc_cross_section(const double* w, long n) { double s = 0.0; for (long k = 0; k < n; k++) s += w[k]; return s; }
 
 // ---- accessors used by the pins -------------------------------------------------------------
 void orc_gamma(int mu, double* out32) {            // mu = 0..3, 5 ; 4x4 complex row-major (re,im)

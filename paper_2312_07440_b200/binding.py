@@ -17,7 +17,7 @@ PRECISIONS = {"fp64": RWGT_FP64, "fp32": RWGT_FP32, "mixed": RWGT_MIXED}
 
 RWGT_MAX_SETS = 16
 EXPORTS = ("rwgt_create", "rwgt_create_multi", "rwgt_n_sets", "rwgt_run_multi", "rwgt_run_multi_host", "rwgt_set_precision", "rwgt_n_external", "rwgt_flops_per_event", "rwgt_run",
-           "rwgt_run_host", "rwgt_destroy", "rwgt_last_error", "rwgt_colour_matrix", "rwgt_tensor_flops_per_event")
+           "rwgt_run_host", "rwgt_destroy", "rwgt_last_error", "rwgt_colour_matrix", "rwgt_tensor_flops_per_event", "rwgt_sum_weights", "rwgt_run_file")
 
 
 class rwgt_params(C.Structure):
@@ -55,6 +55,8 @@ def lib():
         L.rwgt_destroy.argtypes = [vp]
         L.rwgt_last_error.restype = C.c_char_p
         L.rwgt_colour_matrix.argtypes = [C.c_int, dp]
+        L.rwgt_sum_weights.argtypes = [vp, dp, C.c_int, C.c_longlong, dp, vp]
+        L.rwgt_run_file.argtypes = [vp, C.c_char_p, C.c_char_p, C.c_longlong, C.c_longlong, vp]
         _lib = L
     return _lib
 
@@ -152,6 +154,78 @@ def rwgt_run_host(h, momenta: np.ndarray, weights: np.ndarray, out_me_old: np.nd
         raise RuntimeError(f"rwgt_run_host rc={rc}: {rwgt_last_error()}")
 
 
+def rwgt_sum_weights(h, w_ptr: int, n_rows: int, n_events: int, out_sums_ptr: int, stream: int = 0) -> None:
+    """eq. 2: device pointers; w is [n_rows][n_events], out_sums [n_rows]."""
+    rc = lib().rwgt_sum_weights(h, w_ptr, int(n_rows), int(n_events), out_sums_ptr, stream or None)
+    if rc != 0:
+        raise RuntimeError(f"rwgt_sum_weights rc={rc}: {rwgt_last_error()}")
+
+
+def rwgt_run_file(h, in_path: str, out_path: str, first_event: int = 0, n_events: int = -1, stream: int = 0) -> None:
+    """PAPER.md:87 steps 2-8 on a binary SoA event file: read -> H2D -> kernel -> D2H -> write (pipelined in the library)."""
+    rc = lib().rwgt_run_file(h, os.fsencode(in_path), os.fsencode(out_path), int(first_event), int(n_events), stream or None)
+    if rc != 0:
+        raise RuntimeError(f"rwgt_run_file rc={rc}: {rwgt_last_error()}")
+
+
+# ---- event / result files (layout: include/rwgt.h rwgt_event_file_header / rwgt_result_file_header); byte shuffling only ----
+_EVT_HDR = np.dtype([("magic", "S8"), ("version", "<u4"), ("n_ext", "<u4"), ("n_events", "<u8"), ("process", "S32"), ("reserved", "<u8")])
+_RES_HDR = np.dtype([("magic", "S8"), ("version", "<u4"), ("n_sets", "<u4"), ("n_events", "<u8"), ("process", "S32"), ("first_event", "<u8")])
+assert _EVT_HDR.itemsize == 64 and _RES_HDR.itemsize == 64
+
+
+def write_event_file(path: str, process: str, momenta: np.ndarray, weights: np.ndarray) -> None:
+    """momenta[n_ext,4,n] (E,px,py,pz), weights[n], float64: the stand-in for an LHE event file (PAPER.md:87 step 2)."""
+    n_ext, four, n = momenta.shape
+    assert four == 4 and weights.shape == (n,) and momenta.dtype == np.float64 and weights.dtype == np.float64
+    hd = np.zeros(1, dtype=_EVT_HDR)
+    hd["magic"], hd["version"], hd["n_ext"], hd["n_events"], hd["process"] = b"RWGTEVT1", 1, n_ext, n, process.encode()
+    with open(path, "wb") as f:
+        f.write(hd.tobytes())
+        f.write(np.ascontiguousarray(momenta).tobytes())
+        f.write(np.ascontiguousarray(weights).tobytes())
+
+
+def read_event_file(path: str):
+    """-> (process, momenta[n_ext,4,n], weights[n])."""
+    with open(path, "rb") as f:
+        hd = np.frombuffer(f.read(64), dtype=_EVT_HDR)[0]
+        if hd["magic"] != b"RWGTEVT1" or hd["version"] != 1:
+            raise ValueError(f"{path}: not an event file")
+        n_ext, n = int(hd["n_ext"]), int(hd["n_events"])
+        m = np.frombuffer(f.read(n_ext * 4 * n * 8), dtype="<f8").reshape(n_ext, 4, n)
+        w = np.frombuffer(f.read(n * 8), dtype="<f8")
+    return hd["process"].decode(), m, w
+
+
+def event_file_n_events(path: str) -> int:
+    with open(path, "rb") as f:
+        hd = np.frombuffer(f.read(64), dtype=_EVT_HDR)[0]
+    if hd["magic"] != b"RWGTEVT1":
+        raise ValueError(f"{path}: not an event file")
+    return int(hd["n_events"])
+
+
+def event_file_process(path: str) -> str:
+    with open(path, "rb") as f:
+        hd = np.frombuffer(f.read(64), dtype=_EVT_HDR)[0]
+    return hd["process"].decode()
+
+
+def read_result_file(path: str) -> dict:
+    """-> dict(process, first_event, me_old[n], me_new[K,n], w_new[K,n], sum_w_old, sum_w_new[K])."""
+    with open(path, "rb") as f:
+        hd = np.frombuffer(f.read(64), dtype=_RES_HDR)[0]
+        if hd["magic"] != b"RWGTRES1" or hd["version"] != 1:
+            raise ValueError(f"{path}: not a result file")
+        K, n = int(hd["n_sets"]), int(hd["n_events"])
+        body = np.frombuffer(f.read(((1 + 2 * K) * n + 1 + K) * 8), dtype="<f8")
+    rows = body[: (1 + 2 * K) * n].reshape(1 + 2 * K, n)
+    sums = body[(1 + 2 * K) * n:]
+    return {"process": hd["process"].decode(), "first_event": int(hd["first_event"]), "me_old": rows[0], "me_new": rows[1:1 + K],
+            "w_new": rows[1 + K:], "sum_w_old": float(sums[0]), "sum_w_new": sums[1:].copy()}
+
+
 def rwgt_destroy(h) -> None:
     lib().rwgt_destroy(h)
 
@@ -197,6 +271,14 @@ class Reweighter:
         st = torch.cuda.current_stream(momenta.device).cuda_stream
         rwgt_run_multi(self.h, momenta.data_ptr(), weights.data_ptr(), out[0].data_ptr(), out[1].data_ptr(),
                        out[1 + k].data_ptr(), n, st)
+        return out
+
+    def cross_sections(self, w_rows):
+        """eq. 2: sum of every row of a device tensor [rows, n] (e.g. run()[1 + K:], the K reweighted sets)."""
+        import torch
+        assert w_rows.is_cuda and w_rows.dtype == torch.float64 and w_rows.is_contiguous() and w_rows.dim() == 2
+        out = torch.empty(w_rows.shape[0], dtype=torch.float64, device=w_rows.device)
+        rwgt_sum_weights(self.h, w_rows.data_ptr(), w_rows.shape[0], w_rows.shape[1], out.data_ptr(), torch.cuda.current_stream(w_rows.device).cuda_stream)
         return out
 
     def close(self):

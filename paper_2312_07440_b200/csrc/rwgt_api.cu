@@ -12,6 +12,7 @@
 #include "kernels_small.cuh"
 #include "bg_engine.cuh"
 #include "photon_kernel.cuh"
+#include "event_file.cuh"
 
 namespace {
 
@@ -52,6 +53,9 @@ struct rwgt_handle {
   // device scratch for rwgt_run_host
   double* scratch;
   size_t scratch_bytes;
+  char process[32];           // the process name as given to rwgt_create (without any "@" suffix); checked against event files
+  double* sum_partial; unsigned* sum_ticket; double* sum_out;      // device scratch of rwgt_sum_weights (eq. 2), allocated at create
+  rwgt::FileBuffers fb;       // pinned double buffers of rwgt_run_file (allocated on first use)
   int pipe_ready;                                     // copy streams and events below exist (all of them or none)
   cudaStream_t s_in, s_out;                           // copy streams of rwgt_run_host (created on first use)
   cudaEvent_t ev_in[RWGT_MAX_CHUNKS + 1], ev_k[RWGT_MAX_CHUNKS + 1];
@@ -78,6 +82,17 @@ static rwgt::EpemSet make_epem(const rwgt_params& p) {
   return s;
 }
 
+// device scratch every handle owns from the start (nothing is allocated inside rwgt_run / rwgt_sum_weights)
+static rwgt_handle* finish_create(rwgt_handle* h) {
+  const int rows = 1 + RWGT_MAX_SETS;
+  cudaError_t e = cudaMalloc((void**)&h->sum_partial, sizeof(double) * rows * rwgt::SUM_BLOCKS);
+  if (e == cudaSuccess) e = cudaMalloc((void**)&h->sum_ticket, sizeof(unsigned) * rows);
+  if (e == cudaSuccess) e = cudaMalloc((void**)&h->sum_out, sizeof(double) * rows);
+  if (e == cudaSuccess) e = cudaMemset(h->sum_ticket, 0, sizeof(unsigned) * rows);
+  if (e != cudaSuccess) { set_err("rwgt_create: %s", cudaGetErrorString(e)); rwgt_destroy(h); return nullptr; }
+  return h;
+}
+
 extern "C" {
 
 const char* rwgt_last_error(void) { return g_err; }
@@ -93,6 +108,7 @@ rwgt_handle* rwgt_create_multi(const char* process, const rwgt_params* params_ol
   rwgt_handle* h = new (std::nothrow) rwgt_handle();
   if (!h) { set_err("rwgt_create: out of memory"); return nullptr; }
   h->proc = -1; h->precision = RWGT_FP64; h->bg = nullptr; h->scratch = nullptr; h->scratch_bytes = 0; h->s_in = nullptr; h->s_out = nullptr; h->pipe_ready = 0;
+  h->sum_partial = nullptr; h->sum_ticket = nullptr; h->sum_out = nullptr;
   h->nsets = 1 + n_new; h->sets[0] = *params_old;
   for (int k = 0; k < n_new; k++) h->sets[1 + k] = params_new[k];
   cudaGetDevice(&h->device);
@@ -100,6 +116,7 @@ rwgt_handle* rwgt_create_multi(const char* process, const rwgt_params* params_ol
   // "@bg" suffix routes gg_ttx through the generic ordered-current engine (used by the tests to cross-check it)
   bool force_bg = false;
   if (p.size() > 3 && p.compare(p.size() - 3, 3, "@bg") == 0) { force_bg = true; p.resize(p.size() - 3); }
+  std::memset(h->process, 0, sizeof(h->process)); std::strncpy(h->process, p.c_str(), sizeof(h->process) - 1);
   int ng = -1;
   if (p == "epem_mupmum") { h->proc = P_EPEM; h->n_ext = 4; h->n_gluons = 0; }
   else if (p == "gg_ttx") { ng = 2; }
@@ -115,13 +132,13 @@ rwgt_handle* rwgt_create_multi(const char* process, const rwgt_params* params_ol
     cudaDeviceProp prop; cudaGetDeviceProperties(&prop, h->device); h->sm_count = prop.multiProcessorCount;
     cudaError_t e = rwgt::photon_prepare(na);
     if (e != cudaSuccess) { set_err("rwgt_create: %s", cudaGetErrorString(e)); delete h; return nullptr; }
-    return h;
+    return finish_create(h);
   }
   else { set_err("rwgt_create: unknown process '%s'", process); delete h; return nullptr; }
   if (h->proc == P_EPEM) {
     h->epem.nsets = h->nsets;
     for (int k = 0; k < h->nsets; k++) h->epem.set[k] = make_epem(h->sets[k]);
-    return h;
+    return finish_create(h);
   }
   h->n_gluons = ng; h->n_ext = ng + 2;
   if (ng == 2 && !force_bg) {
@@ -132,13 +149,13 @@ rwgt_handle* rwgt_create_multi(const char* process, const rwgt_params* params_ol
       h->ggttx.mt[k] = h->sets[k].mt; h->ggttx.fac[k] = gs2 * gs2 / 256.0; h->ggttx.s3[k] = h->sets[k].ggg_scale;
       if (h->sets[k].mt != h->sets[0].mt) h->ggttx.two_pass = 1;
     }
-    return h;
+    return finish_create(h);
   }
   h->proc = P_BG;
   std::string err;
   h->bg = rwgt::bg_create(ng, h->sets, h->nsets, err);
   if (!h->bg) { set_err("rwgt_create: %s", err.c_str()); delete h; return nullptr; }
-  return h;
+  return finish_create(h);
 }
 
 rwgt_handle* rwgt_create(const char* process, const rwgt_params* params_old, const rwgt_params* params_new) {
@@ -289,11 +306,101 @@ int rwgt_run_host(rwgt_handle* h, const double* momenta, const double* weights, 
   return rwgt_run_multi_host(h, momenta, weights, out_me_old, out_me_new, out_w_new, n_events, stream);
 }
 
+// eq. 2: sigma ~ sum_k W_k, one deterministic device reduction per row
+int rwgt_sum_weights(rwgt_handle* h, const double* w, int n_rows, long long n_events, double* out_sums, void* stream) {
+  if (!h || n_events < 0 || n_rows < 1 || n_rows > 1 + RWGT_MAX_SETS) { set_err("rwgt_sum_weights: bad handle, n_events < 0 or n_rows outside 1..1+RWGT_MAX_SETS"); return -1; }
+  if (!w || !out_sums) { set_err("rwgt_sum_weights: NULL buffer"); return -1; }
+  DeviceGuard guard(h->device);
+  if (!guard.ok) { set_err("rwgt_sum_weights: cannot make the handle's device current"); return -1; }
+  rwgt::sum_rows_kernel<<<dim3(rwgt::SUM_BLOCKS, n_rows), rwgt::SUM_THREADS, 0, (cudaStream_t)stream>>>(w, n_events, n_events, h->sum_partial, h->sum_ticket, out_sums);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { set_err("rwgt_sum_weights: %s", cudaGetErrorString(e)); return (int)e; }
+  return 0;
+}
+
+// PAPER.md:87 steps 2-8 on a binary SoA event file (csrc/event_file.cuh): read -> H2D -> kernel -> D2H -> write, pipelined
+int rwgt_run_file(rwgt_handle* h, const char* in_path, const char* out_path, long long first_event, long long n_events, void* stream) {
+  if (!h || !in_path || !out_path || first_event < 0) { set_err("rwgt_run_file: bad argument"); return -1; }
+  DeviceGuard guard(h->device);
+  if (!guard.ok) { set_err("rwgt_run_file: cannot make the handle's device current"); return -1; }
+  int fin = ::open(in_path, O_RDONLY);
+  if (fin < 0) { set_err("rwgt_run_file: cannot open %s", in_path); return -1; }
+  rwgt_event_file_header hd;
+  if (!rwgt::pread_all(fin, &hd, sizeof(hd), 0) || std::memcmp(hd.magic, "RWGTEVT1", 8) != 0 || hd.version != 1) { ::close(fin); set_err("rwgt_run_file: %s is not an event file (magic/version)", in_path); return -1; }
+  if ((int)hd.n_ext != h->n_ext || std::strncmp(hd.process, h->process, sizeof(hd.process)) != 0) { ::close(fin); set_err("rwgt_run_file: %s holds events of another process", in_path); return -1; }
+  struct stat sb;
+  const long long ntot = (long long)hd.n_events, planes = (long long)h->n_ext * 4, K = h->nsets - 1;
+  if (::fstat(fin, &sb) != 0 || (long long)sb.st_size < (long long)sizeof(hd) + (planes + 1) * ntot * 8) { ::close(fin); set_err("rwgt_run_file: %s is truncated", in_path); return -1; }
+  if (n_events < 0) n_events = ntot - first_event;
+  if (n_events < 0 || first_event + n_events > ntot) { ::close(fin); set_err("rwgt_run_file: event range outside the file"); return -1; }
+  int fout = ::open(out_path, O_CREAT | O_TRUNC | O_RDWR, 0644);
+  if (fout < 0) { ::close(fin); set_err("rwgt_run_file: cannot create %s", out_path); return -1; }
+  rwgt_result_file_header ho; std::memset(&ho, 0, sizeof(ho));
+  std::memcpy(ho.magic, "RWGTRES1", 8); ho.version = 1; ho.n_sets = (uint32_t)K; ho.n_events = (uint64_t)n_events; std::memcpy(ho.process, h->process, sizeof(ho.process));
+  ho.first_event = (uint64_t)first_event;
+  const long long n = n_events; const off_t obase = sizeof(ho);
+  bool io_ok = rwgt::pwrite_all(fout, &ho, sizeof(ho), 0) && ::ftruncate(fout, obase + (off_t)((1 + 2 * K) * n + 1 + K) * 8) == 0;
+  int rc = io_ok ? 0 : -1;
+  if (!io_ok) set_err("rwgt_run_file: cannot write %s", out_path);
+  double sums[1 + RWGT_MAX_SETS]; for (int k = 0; k <= K; k++) sums[k] = 0.0;
+  if (rc == 0 && n > 0) {
+    long long chunk = (n + 7) / 8; if (chunk < 16384) chunk = 16384; if (chunk > (1 << 19)) chunk = 1 << 19; if (chunk > n) chunk = n;
+    chunk = (chunk + 1023) / 1024 * 1024;
+    cudaError_t e = h->fb.ensure(chunk, (int)planes, (int)K);
+    if (e != cudaSuccess) { set_err("rwgt_run_file: %s", cudaGetErrorString(e)); rc = (int)e; }
+    const long long nchunk = (n + chunk - 1) / chunk;
+    // reader: the chunk's planes (ntot apart in the file) into compact planes (cnt apart) of pinned buffer b
+    auto read_chunk = [&](long long c, int b, bool* ok) {
+      const long long a0 = c * chunk, cnt = std::min(chunk, n - a0); bool g = true;
+      for (long long pl = 0; pl <= planes && g; pl++)
+        g = rwgt::pread_all(fin, h->fb.in[b] + pl * cnt, (size_t)cnt * 8, (off_t)sizeof(hd) + (off_t)(pl * ntot + first_event + a0) * 8);
+      *ok = g;
+    };
+    // writer: me_old | me_new[K] | w_new[K] rows (cnt apart in the buffer, n apart in the file)
+    auto write_chunk = [&](long long c, int b, bool* ok) {
+      const long long a0 = c * chunk, cnt = std::min(chunk, n - a0); bool g = true;
+      for (long long r = 0; r < 1 + 2 * K && g; r++) g = rwgt::pwrite_all(fout, h->fb.out[b] + r * cnt, (size_t)cnt * 8, obase + (off_t)(r * n + a0) * 8);
+      *ok = g;
+    };
+    bool rd_ok = true, wr_ok = true;
+    std::thread reader, writer;
+    if (rc == 0) reader = std::thread(read_chunk, 0LL, 0, &rd_ok);
+    for (long long c = 0; c < nchunk && rc == 0; c++) {
+      const int b = (int)(c & 1); const long long a0 = c * chunk, cnt = std::min(chunk, n - a0);
+      reader.join();
+      if (!rd_ok) { set_err("rwgt_run_file: read error on %s", in_path); rc = -1; break; }
+      if (c + 1 < nchunk) reader = std::thread(read_chunk, c + 1, b ^ 1, &rd_ok);
+      double* hi = h->fb.in[b]; double* o = h->fb.out[b];
+      rc = rwgt_run_multi_host(h, hi, hi + planes * cnt, o, o + cnt, o + (1 + K) * cnt, cnt, stream);
+      if (rc == 0) {
+        // eq. 2 on the chunk while it is still in the device scratch (layout of rwgt_run_multi_host): sum W, sum W'_k
+        const size_t nin = (size_t)planes * cnt; double* d_w = h->scratch + nin; double* d_o = d_w + (2 + K) * cnt;
+        rc = rwgt_sum_weights(h, d_w, 1, cnt, h->sum_out, stream);
+        if (rc == 0) rc = rwgt_sum_weights(h, d_o, (int)K, cnt, h->sum_out + 1, stream);
+        double part[1 + RWGT_MAX_SETS];
+        if (rc == 0) { e = cudaMemcpyAsync(part, h->sum_out, sizeof(double) * (1 + K), cudaMemcpyDeviceToHost, (cudaStream_t)stream);
+                       if (e == cudaSuccess) e = cudaStreamSynchronize((cudaStream_t)stream);
+                       if (e != cudaSuccess) { set_err("rwgt_run_file: %s", cudaGetErrorString(e)); rc = (int)e; } }
+        if (rc == 0) for (int k = 0; k <= K; k++) sums[k] += part[k];       // chunk order: deterministic for a given range
+      }
+      if (writer.joinable()) { writer.join(); if (!wr_ok) { set_err("rwgt_run_file: write error on %s", out_path); rc = -1; } }
+      if (rc == 0) writer = std::thread(write_chunk, c, b, &wr_ok);
+    }
+    if (reader.joinable()) reader.join();
+    if (writer.joinable()) { writer.join(); if (!wr_ok && rc == 0) { set_err("rwgt_run_file: write error on %s", out_path); rc = -1; } }
+  }
+  if (rc == 0 && !rwgt::pwrite_all(fout, sums, sizeof(double) * (1 + K), obase + (off_t)((1 + 2 * K) * n) * 8)) { set_err("rwgt_run_file: write error on %s", out_path); rc = -1; }
+  ::close(fin); ::close(fout);
+  return rc;
+}
+
 int rwgt_destroy(rwgt_handle* h) {
   if (!h) return -1;
   DeviceGuard guard(h->device);
   if (h->bg) rwgt::bg_destroy(h->bg);
   if (h->scratch) cudaFree(h->scratch);
+  cudaFree(h->sum_partial); cudaFree(h->sum_ticket); cudaFree(h->sum_out);
+  h->fb.release();
   if (h->pipe_ready) {
     cudaStreamDestroy(h->s_in); cudaStreamDestroy(h->s_out);
     for (int c = 0; c <= RWGT_MAX_CHUNKS; c++) { cudaEventDestroy(h->ev_in[c]); cudaEventDestroy(h->ev_k[c]); }

@@ -129,10 +129,13 @@ template <typename T> __device__ __forceinline__ chi_pair<T> make_chi(T px, T py
 // the one the events were generated with this is what "the parameter masses in spinors and propagators, E from the input"
 // means, and it equals the oracle's Dirac-representation form (sqrt(E+m) chi, lam sqrt(E-m) chi) exactly:
 // ((sqrt(E+m) -+ lam sqrt(E-m)) / sqrt2)^2 = E -+ lam P.
+// If a set's mass exceeds the input energy (E < m: a slow top of the event's own, lighter mass shell) the oracle clamps
+// sqrt(E-m) to 0, i.e. both chiral normalisations are sqrt((E+m)/2); the same here.
 template <typename T> __device__ __forceinline__ T shell_norm(T E, T m, T& sm) {
-  const T P = (m == T(0)) ? E : sqrt((E - m) * (E + m));
-  const T ep = E + P, ir = rsqrt(ep);
-  sm = m * ir;                      // sqrt(E-P) = m / sqrt(E+P): no cancellation, no division
+  const bool on = (E >= m);
+  const T P = (m == T(0)) ? E : sqrt(fmax((E - m) * (E + m), T(0)));
+  const T ep = on ? E + P : T(0.5) * (E + m), ir = rsqrt(ep);
+  sm = (on ? m : ep) * ir;          // sqrt(E-P) = m / sqrt(E+P): no cancellation, no division
   return ep * ir;                   // sqrt(E+P)
 }
 // u(p,lam) = ( sqrt(E-lam P) chi_lam , sqrt(E+lam P) chi_lam )

@@ -140,3 +140,36 @@ def test_bench_reference_arm_prints_contract_line():
     assert line["impl"] == "reference" and line["unit"] == "events/s" and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
     assert line["config"]["workload"].startswith("gg_ttx")
+
+
+def test_event_and_result_file_layout_round_trip(tmp_path):
+    """The binary SoA files that stand in for LHE files (include/rwgt.h): 64-byte headers, planes in rwgt_run's layout."""
+    c = ev.config(4)
+    m, w = ev.generate(c, 33)
+    f = str(tmp_path / "e.rwgt")
+    binding.write_event_file(f, c.process, m, w)
+    assert os.path.getsize(f) == 64 + (c.n_ext * 4 + 1) * 33 * 8
+    raw = open(f, "rb").read()
+    assert raw[:8] == b"RWGTEVT1" and int.from_bytes(raw[8:12], "little") == 1 and int.from_bytes(raw[12:16], "little") == c.n_ext
+    assert int.from_bytes(raw[16:24], "little") == 33 and raw[24:24 + len(c.process)] == c.process.encode()
+    assert np.array_equal(np.frombuffer(raw[64:64 + 33 * 8], dtype="<f8"), m[0, 0])       # first plane: E of leg 0
+    p, m2, w2 = binding.read_event_file(f)
+    assert p == c.process and np.array_equal(m2, m) and np.array_equal(w2, w)
+    assert binding.event_file_n_events(f) == 33 and binding.event_file_process(f) == c.process
+    # a result file as librwgt.so lays it out
+    K, n = 2, 5
+    hd = np.zeros(1, dtype=binding._RES_HDR)
+    hd["magic"], hd["version"], hd["n_sets"], hd["n_events"], hd["process"], hd["first_event"] = b"RWGTRES1", 1, K, n, b"gg_ttxgg", 7
+    body = np.arange((1 + 2 * K) * n + 1 + K, dtype=np.float64)
+    r = str(tmp_path / "r.rwgt")
+    open(r, "wb").write(hd.tobytes() + body.tobytes())
+    res = binding.read_result_file(r)
+    assert res["first_event"] == 7 and res["me_new"].shape == (K, n) and res["w_new"][1, 4] == 24.0 and res["sum_w_old"] == 25.0 and list(res["sum_w_new"]) == [26.0, 27.0]
+
+
+def test_reweight_file_cli_parses_parameter_sets():
+    from paper_2312_07440_b200 import reweight_file
+    p = reweight_file.parse_set("ggg_scale=1.1,mt=170")
+    assert p[ev.PARAM_NAMES.index("ggg_scale")] == 1.1 and p[ev.PARAM_NAMES.index("mt")] == 170.0 and p[ev.PARAM_NAMES.index("alpha_s")] == 0.118
+    with pytest.raises(SystemExit):
+        reweight_file.parse_set("nonsense=1")

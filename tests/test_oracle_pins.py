@@ -434,6 +434,18 @@ def test_eq3_reweight_and_identity_when_params_equal():
     assert np.array_equal(a2, b2) and np.array_equal(wn2, w) and np.array_equal(a2, a)
 
 
+def test_eq2_cross_section_is_the_sum_of_weights():
+    """eq. 2: sigma ~ sum_k W_k.  Pin: Python's exactly rounded math.fsum; recursive summation of n positive terms is
+    within (n - 1) 2^-53 of it (Higham, Accuracy and Stability of Numerical Algorithms, eq. 4.4); W' of eq. 3 summed the same way."""
+    c = ev.config(2)
+    m, w = ev.generate(c, 5000)
+    for x in (w, orc.reweight(c.process, c.params_old, c.params_new, m[:, :, :300].copy(), w[:300].copy())[2]):
+        exact = math.fsum(x)
+        assert abs(orc.cross_section(x) - exact) <= (len(x) - 1) * 2.0 ** -53 * exact
+    assert orc.cross_section(np.array([1.0, 2.0 ** -60, -1.0])) == 0.0          # plain left-to-right, not compensated
+    assert orc.cross_section(np.array([])) == 0.0
+
+
 def test_me2_zero_gives_ieee_result():
     """eq. 3 needs |M|^2 != 0; convention (include/rwgt.h): IEEE inf/nan, no trap."""
     c = ev.config(2)
