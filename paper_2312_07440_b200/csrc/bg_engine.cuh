@@ -155,7 +155,10 @@ template <int N> struct Geo {
   // batch is 16 amplitude columns (4 free gluon configurations x 4 quark helicities) for N >= 3
   static constexpr int NB = (N == 5) ? 2 : (N == 4) ? 1 : 0, NBATCH = 1 << NB;
   static constexpr int NFREE = 1 << (N - 1 - NB), NCOL = NFREE * 4;
-  static constexpr int ASTR = 2 * NCOL + 4;                              // row stride (doubles) of the amplitude buffer, bank-conflict-free
+  // row stride (elements) of the amplitude buffer, bank-conflict-free for the mma B-fragment loads: rows r = lane & 3 must land
+  // 8 32-bit banks apart: 64-bit elements: stride = 4 mod 16 elements, 32-bit elements: stride = 8 mod 32
+  template <typename TA> __host__ __device__ static constexpr int astr() { return 2 * NCOL + (sizeof(TA) == 8 ? 4 : 8); }
+  template <typename TA> __host__ __device__ static constexpr size_t abuf() { return (size_t)(2 * NHK) * astr<TA>(); }   // elements per slot per buffer: rows [u of all pairs | v of all pairs]
   // colour form split by the reflection symmetry C[s][s'] = C[rev s][rev s']: with u = J_s + J_rev(s), v = J_s - J_rev(s) per pair,
   // J^dagger C J = 1/2 u^dagger C+ u + 1/2 v^dagger C- v, C+- = C[s_p][s_q] +- C[s_p][rev s_q]: two NPAIR x NPAIR forms, half the flops
   static constexpr int NHK = pad4(NPAIR);                                // amplitude rows per half (K dimension of the mma, padded to 4)
@@ -168,7 +171,6 @@ template <int N> struct Geo {
   static constexpr int JW = pad4(2 * NL3 + 3 * NV4);                     // words of the n-gluon current's references
   static constexpr int QH = C + NJ + NJ * C, QW = pad4((QH + 1) / 2);    // halfwords / words of one quark-line reference block
   static constexpr int STRIDEF = 4 + JW + 2 * QW;
-  static constexpr size_t ABUF = (size_t)(2 * NHK) * ASTR;               // doubles per slot per buffer: rows [u of all pairs | v of all pairs]
   static constexpr int NG = c_nG(N), NR = c_nR(N), NL = c_nL(N);   // entries of the current tables (checked against the schedule)
 };
 __host__ __device__ constexpr int gdesc_words(int m) { return pad4(2 + 2 * (m - 1) + 3 * (m - 1) * (m - 2) / 2); }
@@ -373,12 +375,13 @@ template <typename T> struct Smem {
   // staging copy of everything step a1/a2 produces for the NEXT event group (written by the colour warps while the workers run the
   // current group): momenta, external wavefunctions (table entries 0..2N-1 of G, 0..1 of R and L), momentum sums, denominators
   double* pmS; cx<T>* GS; cx<T>* RS; cx<T>* LS; T* KS; T* iK2S; T* dRS; T* dLS;
-  double* A;      // [2][nslot][2 NHK][ASTR] double-buffered rows u = J_s + J_rev(s), v = J_s - J_rev(s) (re,im interleaved), always double
+  T* A;           // [2][nslot][2 NHK][astr] double-buffered rows u = J_s + J_rev(s), v = J_s - J_rev(s) (re,im interleaved), formed in double,
+                  // stored in T (the colour form itself always runs in double)
 };
 template <int N, typename T> __host__ __device__ inline size_t carve(Smem<T>& s, unsigned char* base, int ns, int nwords) {
   typedef Geo<N> Ge; size_t off = 0; constexpr int nG = Ge::NG, nR = Ge::NR, nL = Ge::NL;
   auto al = [&]() { off = (off + 15) / 16 * 16; };
-  s.A = (double*)(base + off); off += sizeof(double) * 2 * (size_t)ns * Ge::ABUF; al();
+  s.A = (T*)(base + off); off += sizeof(T) * 2 * (size_t)ns * Ge::template abuf<T>(); al();
   s.LF = (double*)(base + off); off += sizeof(double) * 2 * Ge::KSH * 32; al();
   s.pm = (double*)(base + off); off += sizeof(double) * ns * (N + 2) * 4; al();
   s.acc = (double*)(base + off); off += sizeof(double) * ns * BG_NSMAX; al();
@@ -637,11 +640,15 @@ template <int N, int WHICH, typename T> struct QuarkLine {
 // external wavefunctions (gluon i, helicity bit hb -> entry 2 i + hb of G; v(p_tbar) -> entries 0,1 of R; ubar(p_t) -> 0,1 of L),
 // momentum sums of the gluon subsets and the inverse propagator denominators.  sG / sR / sL: entries per component plane of the
 // destination tables.  SYNC(): a barrier over the calling threads between the two steps.
-template <int N, typename T, typename TK, typename SYNC>
+template <typename T, typename TE, typename V> __device__ __forceinline__ void st4cvt(cx<T>* tab, int stride, int e, const V& v) {
+#pragma unroll
+  for (int c = 0; c < 4; c++) stc(tab + c * stride + e, mk<T>((T)v.c[c].re, (T)v.c[c].im));
+}
+template <int N, typename T, typename TK, typename TE, typename SYNC>
 __device__ __forceinline__ void group_externals(int t0, int nth, int ns, long long ev0, long long nev, long long stride, const double* __restrict__ mom,
                                                 double mtd, double* pmD, cx<T>* Gd, int sG, cx<T>* Rd, int sR, cx<T>* Ld, int sL, T* Kd, T* iK2d, T* dRd, T* dLd,
                                                 bool load, SYNC sync) {
-  typedef Geo<N> Ge; constexpr int next = N + 2; const T mt = (T)mtd;
+  typedef Geo<N> Ge; constexpr int next = N + 2;
   if (load) {
     for (int t = t0; t < ns * next * 4; t += nth) {
       int sl = t % ns, comp = t / ns; long long ev = ev0 + sl; if (ev >= nev) ev = nev - 1;
@@ -654,17 +661,17 @@ __device__ __forceinline__ void group_externals(int t0, int nth, int ns, long lo
     int o = t / ns, sl = t - o * ns; const double* pm = pmD + sl * next * 4;      // object-major: the lanes of a warp run the same branch
     if (o < 2 * N) {                         // gluon i, helicity bit hb (0: +1, 1: -1); entry = 2*i + hb
       int i = o >> 1, hb = o & 1, leg = i < 2 ? i : i + 2; const double* p = pm + 4 * leg;
-      vec4<T> e = polvec<T>((T)p[1], (T)p[2], (T)p[3], hb ? -1 : +1);
+      vec4<TE> e = polvec<TE>((TE)p[1], (TE)p[2], (TE)p[3], hb ? -1 : +1);
       if (i >= 2) e = conj4(e);              // outgoing gluon carries eps*
-      st4(Gd + (size_t)sl * 4 * sG, sG, 2 * i + hb, e);
+      st4cvt<T, TE>(Gd + (size_t)sl * 4 * sG, sG, 2 * i + hb, e);
     } else if (o < 2 * N + 2) {              // v(p_tbar, lam), R() entries 0,1
       int hb = o - 2 * N; const double* p = pm + 12;
-      chi_pair<T> x = make_chi<T>((T)p[1], (T)p[2], (T)p[3]);
-      st4(Rd + (size_t)sl * 4 * sR, sR, hb, spinor_v<T>(x, (T)p[0], mt, hb ? -1 : +1));
+      chi_pair<TE> x = make_chi<TE>((TE)p[1], (TE)p[2], (TE)p[3]);
+      st4cvt<T, TE>(Rd + (size_t)sl * 4 * sR, sR, hb, spinor_v<TE>(x, make_shell<TE>((TE)p[0], (TE)mtd), hb ? -1 : +1));
     } else if (o < 2 * N + 4) {              // ubar(p_t, lam), L() entries 0,1
       int hb = o - 2 * N - 2; const double* p = pm + 8;
-      chi_pair<T> x = make_chi<T>((T)p[1], (T)p[2], (T)p[3]);
-      st4(Ld + (size_t)sl * 4 * sL, sL, hb, bar(spinor_u<T>(x, (T)p[0], mt, hb ? -1 : +1)));
+      chi_pair<TE> x = make_chi<TE>((TE)p[1], (TE)p[2], (TE)p[3]);
+      st4cvt<T, TE>(Ld + (size_t)sl * 4 * sL, sL, hb, bar(spinor_u<TE>(x, make_shell<TE>((TE)p[0], (TE)mtd), hb ? -1 : +1)));
     } else {                                 // gluon subset `mask`
       int mask = o - 2 * N - 4;
       TK k[4] = {0, 0, 0, 0};
@@ -692,8 +699,11 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 // One persistent CTA per SM.  Warps 0..NW-1 ("workers") build the currents and the colour-flow amplitudes of one helicity
 // batch after the other on the FP64 pipe; the last NCW warps ("colour") turn finished batches into |L^T J|^2 on the FP64
 // tensor pipe (a separate pipe, so the two overlap) and write the outputs.  The two amplitude buffers are handed over with
-// named barriers.  MIXED: T = float but momentum sums / propagator denominators are formed in double before rounding to T.
-template <int N, typename T, bool MIXED, int NW, int NCW, int CTAS>
+// named barriers.  MX (T = float only): 1 = momentum sums / propagator denominators are formed in double before rounding to T (the
+// FP32 mode: with float denominators gg -> ttggg misses the 1e-4 / 1e-6 tolerances on 8,192 events, profiles/r2_parity.md);
+// 2 = the external wavefunctions too (the mixed mode).  Everything downstream of the amplitudes (u, v rows, colour form,
+// helicity sum, eq. 3) runs in double in every mode.
+template <int N, typename T, int MX, int NW, int NCW, int CTAS>
 __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
                                                                double* __restrict__ me_old, double* __restrict__ me_new,
                                                                double* __restrict__ w_new, long long nev, long long stride, long long ostride, BgDev D) {
@@ -714,11 +724,13 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
   Ctx<T> c; c.D = &D; c.ns = D.nslot;
   carve<N, T>(c.s, smem_raw, D.nslot, D.nwords);
   const Smem<T>& s = c.s;
-  typedef typename std::conditional<MIXED, double, T>::type TK;
+  typedef typename std::conditional<MX >= 1, double, T>::type TK;
+  typedef typename std::conditional<MX >= 2, double, T>::type TE;
   constexpr int next = N + 2, nG = Ge::NG, nR = Ge::NR, nL = Ge::NL; const int ns = D.nslot;
   const long long ngroups = (nev + ns - 1) / ns;
   // once per CTA: zero both amplitude buffers (their padding rows are never written again)
-  for (int t = threadIdx.x; t < 2 * ns * (int)Ge::ABUF; t += NTH) s.A[t] = 0.0;
+  constexpr int ASTR = Ge::template astr<T>(); constexpr size_t ABUF = Ge::template abuf<T>();
+  for (int t = threadIdx.x; t < 2 * ns * (int)ABUF; t += NTH) s.A[t] = T(0);
   for (int t = threadIdx.x; t < 2 * Ge::KSH * 32; t += NTH) s.LF[t] = __ldg(D.lfrag + t);
   __syncthreads();
   if (threadIdx.x < NWT) {
@@ -732,7 +744,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
       if constexpr (!STAGE) {
         // ---- a1/a2 by the workers themselves ----
         bar_sync(BAR_WORK, NWT);
-        group_externals<N, T, TK>(tid, NWT, ns, ev0, nev, stride, mom, D.set[0].mt, s.pm, s.G, nG, s.R, nR, s.L, nL, s.K, s.iK2, s.dR, s.dL, true,
+        group_externals<N, T, TK, TE>(tid, NWT, ns, ev0, nev, stride, mom, D.set[0].mt, s.pm, s.G, nG, s.R, nR, s.L, nL, s.K, s.iK2, s.dR, s.dL, true,
                                   [] { bar_sync(BAR_WORK, NWT); });
       } else {
       // ---- a1/a2 were done for this group by the colour warps (staging buffers): copy them into the tables ----
@@ -756,7 +768,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
         c.g3 = (T)P.g3; c.g4 = (T)P.g4; c.gq = (T)P.gq; c.mt = (T)P.mt;
         if (iset > 0 && !D.shared_ext) {
           // a set with another top mass: external spinors and denominators are redone for it (reading R12)
-          group_externals<N, T, TK>(tid, NWT, ns, ev0, nev, stride, mom, P.mt, s.pm, s.G, nG, s.R, nR, s.L, nL, s.K, s.iK2, s.dR, s.dL, false, [] {});
+          group_externals<N, T, TK, TE>(tid, NWT, ns, ev0, nev, stride, mom, P.mt, s.pm, s.G, nG, s.R, nR, s.L, nL, s.K, s.iK2, s.dR, s.dL, false, [] {});
           bar_sync(BAR_WORK, NWT);
         }
         // ---- a3: current levels ----
@@ -768,7 +780,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
         for (int batch = 0; batch < Ge::NBATCH; batch++, step++) {
           const int buf = step & 1;
           if (step >= 2) bar_sync(BAR_EMPTY0 + buf, NTH);      // colour warps have finished reading this buffer
-          double* Abuf = s.A + (size_t)buf * ns * Ge::ABUF;
+          T* Abuf = s.A + (size_t)buf * ns * ABUF;
           constexpr int per = Ge::NPAIR * Ge::NFREE;
           for (int t = tid; t < ns * per; t += NWT) {
             int sl = t / per, o = t - sl * per; int pair = o / Ge::NFREE, f = o % Ge::NFREE;
@@ -798,15 +810,15 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
               QuarkLine<N, 1, T>::run(A1, wq, brevm<N>(v), Jn, G, R, L);
             }
             // rows u = J_s + J_rev(s) and v = J_s - J_rev(s) of the pair (formed in double)
-            double* Au = Abuf + (size_t)sl * Ge::ABUF + (size_t)w0 * Ge::ASTR; double* Av = Au + (size_t)Ge::NHK * Ge::ASTR;
+            T* Au = Abuf + (size_t)sl * ABUF + (size_t)w0 * ASTR; T* Av = Au + (size_t)Ge::NHK * ASTR;
 #pragma unroll
             for (int ht = 0; ht < 2; ht++)
 #pragma unroll
               for (int hb = 0; hb < 2; hb++) {
                 const int col = f * 4 + ht * 2 + hb;
                 const double ar = (double)A0[ht][hb].re, ai = (double)A0[ht][hb].im, br = (double)A1[ht][hb].re, bi = (double)A1[ht][hb].im;
-                *reinterpret_cast<double2*>(Au + 2 * col) = make_double2(ar + br, ai + bi);
-                *reinterpret_cast<double2*>(Av + 2 * col) = make_double2(ar - br, ai - bi);
+                stc(reinterpret_cast<cx<T>*>(Au + 2 * col), mk<T>((T)(ar + br), (T)(ai + bi)));
+                stc(reinterpret_cast<cx<T>*>(Av + 2 * col), mk<T>((T)(ar - br), (T)(ai - bi)));
               }
           }
           __threadfence_block();
@@ -822,7 +834,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
     unsigned step = 0;
     // a1 + a2 of an event group into the staging buffers (parameter set 0; masses of the other sets: see the workers)
     auto stage = [&](long long g) {
-      group_externals<N, T, TK>(ctid, NCT, ns, g * ns, nev, stride, mom, D.set[0].mt, s.pmS, s.GS, 2 * N, s.RS, 2, s.LS, 2, s.KS, s.iK2S, s.dRS, s.dLS, true,
+      group_externals<N, T, TK, TE>(ctid, NCT, ns, g * ns, nev, stride, mom, D.set[0].mt, s.pmS, s.GS, 2 * N, s.RS, 2, s.LS, 2, s.KS, s.iK2S, s.dRS, s.dLS, true,
                                 [] { bar_sync(BAR_COLOUR, NCT); });
       __threadfence_block();
       bar_arrive(BAR_STAGE_FULL, NTH);
@@ -842,7 +854,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
         for (int batch = 0; batch < Ge::NBATCH; batch++, step++) {
           const int buf = step & 1;
           bar_sync(BAR_FULL0 + buf, NTH);                      // the workers have filled this buffer
-          const double* Abuf = s.A + (size_t)buf * ns * Ge::ABUF;
+          const T* Abuf = s.A + (size_t)buf * ns * ABUF;
           // a5: Z = L^T A with FP64 tensor-core mma over the upper-triangular tiles, colour form = sum of squares of Z
           if constexpr (Ge::MTH == 1 && Ge::KTH == 1) {
             // n <= 3: one 8x4 tile per half, so a unit is four mma and a shuffle tree, i.e. pure latency.  Four units (slot x half) are
@@ -853,11 +865,11 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
 #pragma unroll
               for (int j = 0; j < UB; j++) {
                 const int u = (u0 + j < ns * 2) ? u0 + j : ns * 2 - 1, sl = u >> 1, h = u & 1;
-                const double* A = Abuf + (size_t)sl * Ge::ABUF + (size_t)(h * Ge::NHK + (lane & 3)) * Ge::ASTR + (lane >> 2);
+                const T* A = Abuf + (size_t)sl * ABUF + (size_t)(h * Ge::NHK + (lane & 3)) * ASTR + (lane >> 2);
                 const double a = s.LF[h * 32 + lane];
                 double acc[Ge::NT][2];
 #pragma unroll
-                for (int nt = 0; nt < Ge::NT; nt++) { acc[nt][0] = 0.0; acc[nt][1] = 0.0; dmma884(acc[nt][0], acc[nt][1], a, A[8 * nt]); }
+                for (int nt = 0; nt < Ge::NT; nt++) { acc[nt][0] = 0.0; acc[nt][1] = 0.0; dmma884(acc[nt][0], acc[nt][1], a, (double)A[8 * nt]); }
                 double pj = 0.0;
 #pragma unroll
                 for (int nt = 0; nt < Ge::NT; nt++) { pj = fma(acc[nt][0], acc[nt][0], pj); pj = fma(acc[nt][1], acc[nt][1], pj); }
@@ -873,7 +885,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
           } else
           for (int u = cwarp; u < ns * Ge::U; u += NCW) {
             int sl = u / Ge::U, unit = u % Ge::U; const int h = unit / Ge::UH, uu = unit % Ge::UH;     // h: 0 = u rows / L+, 1 = v rows / L-
-            const double* A = Abuf + (size_t)sl * Ge::ABUF + (size_t)(h * Ge::NHK + (lane & 3)) * Ge::ASTR + (lane >> 2);
+            const T* A = Abuf + (size_t)sl * ABUF + (size_t)(h * Ge::NHK + (lane & 3)) * ASTR + (lane >> 2);
             double part = 0.0;
 #pragma unroll 1
             for (int half = 0; half < 2; half++) {
@@ -884,19 +896,19 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
               for (int nt = 0; nt < Ge::NT; nt++) { acc[nt][0] = 0.0; acc[nt][1] = 0.0; }
               const double* F = s.LF + (h * Ge::KSH + mt * Ge::KTH - mt * (mt - 1)) * 32 + lane;
               const int nk = Ge::KTH - 2 * mt;
-              const double* Br = A + (size_t)(8 * mt) * Ge::ASTR;
+              const T* Br = A + (size_t)(8 * mt) * ASTR;
               // operands of k-step kk + 1 are fetched from shared memory while the mma of k-step kk issue
-              double a_cur = F[0], b_cur[Ge::NT];
+              double a_cur = F[0]; T b_cur[Ge::NT];
 #pragma unroll
               for (int nt = 0; nt < Ge::NT; nt++) b_cur[nt] = Br[8 * nt];
 #pragma unroll 2
               for (int kk = 0; kk < nk; kk++) {
                 const int kn = (kk + 1 < nk) ? kk + 1 : kk;
-                const double a_nxt = F[kn * 32]; double b_nxt[Ge::NT];
+                const double a_nxt = F[kn * 32]; T b_nxt[Ge::NT];
 #pragma unroll
-                for (int nt = 0; nt < Ge::NT; nt++) b_nxt[nt] = Br[(size_t)(4 * kn) * Ge::ASTR + 8 * nt];
+                for (int nt = 0; nt < Ge::NT; nt++) b_nxt[nt] = Br[(size_t)(4 * kn) * ASTR + 8 * nt];
 #pragma unroll
-                for (int nt = 0; nt < Ge::NT; nt++) dmma884(acc[nt][0], acc[nt][1], a_cur, b_cur[nt]);
+                for (int nt = 0; nt < Ge::NT; nt++) dmma884(acc[nt][0], acc[nt][1], a_cur, (double)b_cur[nt]);
                 a_cur = a_nxt;
 #pragma unroll
                 for (int nt = 0; nt < Ge::NT; nt++) b_cur[nt] = b_nxt[nt];
@@ -958,23 +970,29 @@ static size_t smem_need_n(int n, const BgSched& S, int nslot, bool dbl) {
 #ifndef RWGT_NW64_N3
 #define RWGT_NW64_N3 8
 #endif
-template <int N, typename T> struct BgCfg { static constexpr int NW = (N == 4) ? (sizeof(T) == 4 ? RWGT_NW32_N4 : RWGT_NW64_N4) : (N == 3) ? (sizeof(T) == 4 ? RWGT_NW32_N3 : RWGT_NW64_N3) : 8, NCW = 4, CTAS = 1; };
-static int bg_nw(int n, bool dbl) { return n == 4 ? (dbl ? BgCfg<4, double>::NW : BgCfg<4, float>::NW) : n == 3 ? (dbl ? BgCfg<3, double>::NW : BgCfg<3, float>::NW) : 8; }
+#ifndef RWGT_NW32_N5
+#define RWGT_NW32_N5 8
+#endif
+#ifndef RWGT_SLOTS32_N5
+#define RWGT_SLOTS32_N5 2
+#endif
+template <int N, typename T> struct BgCfg { static constexpr int NW = (N == 4) ? (sizeof(T) == 4 ? RWGT_NW32_N4 : RWGT_NW64_N4) : (N == 3) ? (sizeof(T) == 4 ? RWGT_NW32_N3 : RWGT_NW64_N3) : (N == 5 && sizeof(T) == 4) ? RWGT_NW32_N5 : 8, NCW = 4, CTAS = 1; };
+static int bg_nw(int n, bool dbl) { return n == 4 ? (dbl ? BgCfg<4, double>::NW : BgCfg<4, float>::NW) : n == 3 ? (dbl ? BgCfg<3, double>::NW : BgCfg<3, float>::NW) : n == 5 ? (dbl ? BgCfg<5, double>::NW : BgCfg<5, float>::NW) : 8; }
 static int bg_ctas(int) { return 1; }
 
 template <int N> static cudaError_t bg_set_attr(size_t s64, size_t s32) {
   typedef BgCfg<N, double> Cd; typedef BgCfg<N, float> Cf;
-  cudaError_t e = cudaFuncSetAttribute(bg_kernel<N, double, false, Cd::NW, Cd::NCW, Cd::CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s64);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, false, Cf::NW, Cf::NCW, Cf::CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
-  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, true, Cf::NW, Cf::NCW, Cf::CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
+  cudaError_t e = cudaFuncSetAttribute(bg_kernel<N, double, 0, Cd::NW, Cd::NCW, Cd::CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s64);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, 1, Cf::NW, Cf::NCW, Cf::CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, 2, Cf::NW, Cf::NCW, Cf::CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
   return e;
 }
 template <int N> static void bg_launch(int precision, int grid, size_t s64, size_t s32, cudaStream_t st, const double* mom, const double* w,
                                        double* a, double* b, double* o, long long nev, long long stride, long long ostride, const BgDev& D) {
   typedef BgCfg<N, double> Cd; typedef BgCfg<N, float> Cf;
-  if (precision == RWGT_FP64) bg_kernel<N, double, false, Cd::NW, Cd::NCW, Cd::CTAS><<<grid, (Cd::NW + Cd::NCW) * 32, s64, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
-  else if (precision == RWGT_FP32) bg_kernel<N, float, false, Cf::NW, Cf::NCW, Cf::CTAS><<<grid, (Cf::NW + Cf::NCW) * 32, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
-  else bg_kernel<N, float, true, Cf::NW, Cf::NCW, Cf::CTAS><<<grid, (Cf::NW + Cf::NCW) * 32, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
+  if (precision == RWGT_FP64) bg_kernel<N, double, 0, Cd::NW, Cd::NCW, Cd::CTAS><<<grid, (Cd::NW + Cd::NCW) * 32, s64, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
+  else if (precision == RWGT_FP32) bg_kernel<N, float, 1, Cf::NW, Cf::NCW, Cf::CTAS><<<grid, (Cf::NW + Cf::NCW) * 32, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
+  else bg_kernel<N, float, 2, Cf::NW, Cf::NCW, Cf::CTAS><<<grid, (Cf::NW + Cf::NCW) * 32, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
 }
 
 static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::string& err) {
@@ -1007,6 +1025,7 @@ static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::stri
   // event slots per CTA: as many as make the amplitude phase fill the 256 worker threads (npair * 4 tasks per slot and batch)
   auto pick = [&](bool dbl, int& nslot, size_t& bytes) {
     int cap = std::max(1, std::min(64, (bg_nw(n, dbl) * 32) / (S.npair * (n == 2 ? 2 : 4)))); nslot = 0;
+    if (n == 5 && !dbl) cap = RWGT_SLOTS32_N5;       // float amplitude buffers: a second event slot fits (two rounds of amplitude tasks per batch)
     // with k CTAs per SM each gets 1/k of the SM's shared memory (1 KB per CTA is reserved by the system)
     size_t budget = std::min(maxsm, prop.sharedMemPerMultiprocessor / bg_ctas(n) - 1024);
     for (int e = cap; e >= 1; e--) if (smem_need_n(n, S, e, dbl) <= budget) { nslot = e; break; }

@@ -86,7 +86,8 @@ __device__ __forceinline__ void ggttx_sums(const double (*p)[4], double m, doubl
   for (int mu = 0; mu < 4; mu++) { q1[mu] = k1[mu] - p[3][mu]; q2[mu] = k2[mu] - p[3][mu]; kk[mu] = k1[mu] + k2[mu]; }
   double m2 = m * m;
   double d1 = -1.0 / (mdot_rr(q1, q1) - m2), d2 = -1.0 / (mdot_rr(q2, q2) - m2), ds = -1.0 / mdot_rr(kk, kk);
-  chi_pair<double> xt = make_chi(p[2][1], p[2][2], p[2][3]), xb = make_chi(p[3][1], p[3][2], p[3][3]);
+  chi_pair<double> xt = make_chi_raw(p[2][1], p[2][2], p[2][3]), xb = make_chi_raw(p[3][1], p[3][2], p[3][3]);
+  const shell<double> nt = make_shell(p[2][0], m, xt.n2), nb = make_shell(p[3][0], m, xb.n2);
   sum_a = 0; sum_b = 0;
   const int l1 = +1;
   vec4<double> e1 = polvec(k1[1], k1[2], k1[3], l1);
@@ -99,12 +100,12 @@ __device__ __forceinline__ void ggttx_sums(const double (*p)[4], double m, doubl
     for (int mu = 0; mu < 4; mu++) l3.c[mu] = ds * l3.c[mu];
 #pragma unroll
     for (int ib = 0; ib < 2; ib++) {
-      spn<double> v = spinor_v(xb, p[3][0], m, ib ? -1 : +1);
+      spn<double> v = spinor_v(xb, nb, ib ? -1 : +1);
       spn<double> psi1 = slash_r_plus_m(q1, m, slash_c(e1, v)), psi2 = slash_r_plus_m(q2, m, slash_c(e2, v));
       spn<double> c12 = slash_c(e1, psi2), c21 = slash_c(e2, psi1), cy = slash_c(l3, v);
 #pragma unroll
       for (int it = 0; it < 2; it++) {
-        spn<double> ub = bar(spinor_u(xt, p[2][0], m, it ? -1 : +1));
+        spn<double> ub = bar(spinor_u(xt, nt, it ? -1 : +1));
         cx<double> X12 = d2 * rowcol(ub, c12), X21 = d1 * rowcol(ub, c21), Y = rowcol(ub, cy);
         cx<double> A1 = X12, A2 = X21; rfma(A1, sa, Y); rfma(A2, -sa, Y);
         sum_a += 16.0 * (norm2(A1) + norm2(A2)) - 4.0 * (A1.re * A2.re + A1.im * A2.im);
@@ -145,7 +146,8 @@ __device__ __forceinline__ void ggttx_sums_multi(const double (*p)[4], double m,
   for (int mu = 0; mu < 4; mu++) { q1[mu] = k1[mu] - p[3][mu]; q2[mu] = k2[mu] - p[3][mu]; kk[mu] = k1[mu] + k2[mu]; }
   double m2 = m * m;
   double d1 = -1.0 / (mdot_rr(q1, q1) - m2), d2 = -1.0 / (mdot_rr(q2, q2) - m2), ds = -1.0 / mdot_rr(kk, kk);
-  chi_pair<double> xt = make_chi(p[2][1], p[2][2], p[2][3]), xb = make_chi(p[3][1], p[3][2], p[3][3]);
+  chi_pair<double> xt = make_chi_raw(p[2][1], p[2][2], p[2][3]), xb = make_chi_raw(p[3][1], p[3][2], p[3][3]);
+  const shell<double> nt = make_shell(p[2][0], m, xt.n2), nb = make_shell(p[3][0], m, xb.n2);
   cx<double> aX12[8], aX21[8], aY[8];
   vec4<double> e1 = polvec(k1[1], k1[2], k1[3], +1);
 #pragma unroll
@@ -156,12 +158,12 @@ __device__ __forceinline__ void ggttx_sums_multi(const double (*p)[4], double m,
     for (int mu = 0; mu < 4; mu++) l3.c[mu] = ds * l3.c[mu];
 #pragma unroll
     for (int ib = 0; ib < 2; ib++) {
-      spn<double> v = spinor_v(xb, p[3][0], m, ib ? -1 : +1);
+      spn<double> v = spinor_v(xb, nb, ib ? -1 : +1);
       spn<double> psi1 = slash_r_plus_m(q1, m, slash_c(e1, v)), psi2 = slash_r_plus_m(q2, m, slash_c(e2, v));
       spn<double> c12 = slash_c(e1, psi2), c21 = slash_c(e2, psi1), cy = slash_c(l3, v);
 #pragma unroll
       for (int it = 0; it < 2; it++) {
-        spn<double> ub = bar(spinor_u(xt, p[2][0], m, it ? -1 : +1));
+        spn<double> ub = bar(spinor_u(xt, nt, it ? -1 : +1));
         const int h = (i2 * 2 + ib) * 2 + it;
         aX12[h] = d2 * rowcol(ub, c12); aX21[h] = d1 * rowcol(ub, c21); aY[h] = rowcol(ub, cy);
       }

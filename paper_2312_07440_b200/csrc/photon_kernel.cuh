@@ -145,11 +145,11 @@ __global__ void __launch_bounds__(NTH) epem_photons_kernel(const double* __restr
         M[0] = a.m; M[1] = -a.r; M[2] = -a.l; M[3] = a.p;
       } else if (o == 2 * NG) {                    // psi_{} = lower components of u(p2, +)
         const double* p = pm + 4; chi_pair<double> x = make_chi<double>(p[1], p[2], p[3]);
-        spn<double> u = spinor_u<double>(x, p[0], 0.0, +1);
+        spn<double> u = spinor_u<double>(x, make_shell<double>(p[0], 0.0), +1);
         cx<double>* T = reinterpret_cast<cx<double>*>(s + Ge::O_PSI); T[0] = u.c[2]; T[NENT] = u.c[3];
       } else if (o == 2 * NG + 1) {                // row of vbar(p1, -) that meets upper components: (lower components of v)^*
         const double* p = pm; chi_pair<double> x = make_chi<double>(p[1], p[2], p[3]);
-        spn<double> v = spinor_v<double>(x, p[0], 0.0, -1);
+        spn<double> v = spinor_v<double>(x, make_shell<double>(p[0], 0.0), -1);
         cx<double>* W = reinterpret_cast<cx<double>*>(s + Ge::O_W); W[0] = conj(v.c[2]); W[1] = conj(v.c[3]);
       } else {                                     // q_S = p2 - K_S
         int S = o - 2 * NG - 2; double q[4] = {pm[4], pm[5], pm[6], pm[7]};

@@ -112,15 +112,26 @@ template <typename T> __device__ __forceinline__ cx<T> rowcol(const spn<T>& w, c
 
 // ---- external wavefunctions -------------------------------------------------------
 // two-component helicity eigenspinors chi_+, chi_- of direction p_vec; exact on the beam axis.
-template <typename T> struct chi_pair { cx<T> p[2], m[2]; T pabs; };
-template <typename T> __device__ __forceinline__ chi_pair<T> make_chi(T px, T py, T pz) {
-  chi_pair<T> r; T pt2 = px * px + py * py; T pabs = sqrt(pt2 + pz * pz); r.pabs = pabs;
+template <typename T> struct chi_pair { cx<T> p[2], m[2]; T pabs, n2; };      // |chi_+-|^2 = n2 (1 once normalised)
+// unnormalised: chi_+ = (|p|+pz, px + i py), chi_- = (-px + i py, |p|+pz), n2 = 2 |p| (|p|+pz); the caller folds 1/sqrt(n2) into
+// the spinor normalisation (make_shell), which saves one reciprocal square root per leg
+template <typename T> __device__ __forceinline__ chi_pair<T> make_chi_raw(T px, T py, T pz) {
+  chi_pair<T> r; T pt2 = px * px + py * py; T pabs = sqrt(pt2 + pz * pz); r.pabs = pabs; r.n2 = T(1);
   if (pabs == T(0)) { r.p[0] = mk<T>(1, 0); r.p[1] = mk<T>(0, 0); r.m[0] = mk<T>(0, 0); r.m[1] = mk<T>(1, 0); return r; }
   if (pt2 == T(0) && pz < T(0)) { r.p[0] = mk<T>(0, 0); r.p[1] = mk<T>(1, 0); r.m[0] = mk<T>(-1, 0); r.m[1] = mk<T>(0, 0); return r; }
   T ppz = (pz >= T(0)) ? pabs + pz : pt2 / (pabs - pz);     // |p|+pz, cancellation-free
-  T N = rsqrt(T(2) * pabs * ppz);
-  r.p[0] = mk<T>(N * ppz, 0); r.p[1] = mk<T>(N * px, N * py);
-  r.m[0] = mk<T>(-N * px, N * py); r.m[1] = mk<T>(N * ppz, 0);
+  r.n2 = T(2) * pabs * ppz;
+  r.p[0] = mk<T>(ppz, 0); r.p[1] = mk<T>(px, py);
+  r.m[0] = mk<T>(-px, py); r.m[1] = mk<T>(ppz, 0);
+  return r;
+}
+template <typename T> __device__ __forceinline__ chi_pair<T> make_chi(T px, T py, T pz) {
+  chi_pair<T> r = make_chi_raw(px, py, pz);
+  if (r.n2 != T(1)) {
+    const T N = rsqrt(r.n2); r.n2 = T(1);
+#pragma unroll
+    for (int i = 0; i < 2; i++) { r.p[i] = N * r.p[i]; r.m[i] = N * r.m[i]; }
+  }
   return r;
 }
 // Spinor normalisation (reading Q8 / DESIGN.md R8): the energy comes from the input, the mass from the PARAMETER SET, and
@@ -131,22 +142,25 @@ template <typename T> __device__ __forceinline__ chi_pair<T> make_chi(T px, T py
 // ((sqrt(E+m) -+ lam sqrt(E-m)) / sqrt2)^2 = E -+ lam P.
 // If a set's mass exceeds the input energy (E < m: a slow top of the event's own, lighter mass shell) the oracle clamps
 // sqrt(E-m) to 0, i.e. both chiral normalisations are sqrt((E+m)/2); the same here.
-template <typename T> __device__ __forceinline__ T shell_norm(T E, T m, T& sm) {
+template <typename T> struct shell { T sp, sm; };       // sqrt(E+P) / sqrt(n2), sqrt(E-P) / sqrt(n2)
+// n2: squared norm of the chi the spinor is built from (make_chi_raw), 1 for a normalised chi
+template <typename T> __device__ __forceinline__ shell<T> make_shell(T E, T m, T n2 = T(1)) {
   const bool on = (E >= m);
   const T P = (m == T(0)) ? E : sqrt(fmax((E - m) * (E + m), T(0)));
-  const T ep = on ? E + P : T(0.5) * (E + m), ir = rsqrt(ep);
-  sm = (on ? m : ep) * ir;          // sqrt(E-P) = m / sqrt(E+P): no cancellation, no division
-  return ep * ir;                   // sqrt(E+P)
+  const T ep = on ? E + P : T(0.5) * (E + m), ir = rsqrt(ep * n2);
+  shell<T> r; r.sp = ep * ir;       // sqrt(E+P) / sqrt(n2)
+  r.sm = (on ? m : ep) * ir;        // sqrt(E-P) = m / sqrt(E+P): no cancellation, no division
+  return r;
 }
 // u(p,lam) = ( sqrt(E-lam P) chi_lam , sqrt(E+lam P) chi_lam )
-template <typename T> __device__ __forceinline__ spn<T> spinor_u(const chi_pair<T>& x, T E, T m, int lam) {
-  T sm; const T sp = shell_norm(E, m, sm);
+template <typename T> __device__ __forceinline__ spn<T> spinor_u(const chi_pair<T>& x, const shell<T>& n, int lam) {
+  const T sp = n.sp, sm = n.sm;
   const cx<T>* c = lam > 0 ? x.p : x.m; T a = lam > 0 ? sm : sp, b = lam > 0 ? sp : sm;
   spn<T> r; r.c[0] = a * c[0]; r.c[1] = a * c[1]; r.c[2] = b * c[0]; r.c[3] = b * c[1]; return r;
 }
 // v(p,lam) = ( -lam sqrt(E+lam P) chi_{-lam} , lam sqrt(E-lam P) chi_{-lam} )
-template <typename T> __device__ __forceinline__ spn<T> spinor_v(const chi_pair<T>& x, T E, T m, int lam) {
-  T sm; const T sp = shell_norm(E, m, sm);
+template <typename T> __device__ __forceinline__ spn<T> spinor_v(const chi_pair<T>& x, const shell<T>& n, int lam) {
+  const T sp = n.sp, sm = n.sm;
   const cx<T>* c = lam > 0 ? x.m : x.p; T a = lam > 0 ? -sp : sm, b = lam > 0 ? sm : -sp;
   spn<T> r; r.c[0] = a * c[0]; r.c[1] = a * c[1]; r.c[2] = b * c[0]; r.c[3] = b * c[1]; return r;
 }
@@ -176,6 +190,20 @@ template <typename T> __device__ __forceinline__ void L3_acc(vec4<T>& acc, const
 #pragma unroll
   for (int i = 0; i < 4; i++) { rfma(acc.c[i], d[i], ab); cfma(acc.c[i], c1, JB.c[i]); cfma(acc.c[i], c2, JA.c[i]); }
 }
+// FP32: the three real momentum combinations as packed pairs (2 FADD2 + 4 FFMA2 instead of 4 FADD + 8 FFMA)
+__device__ __forceinline__ void L3_acc(vec4<float>& acc, const vec4<float>& JA, const float* KA, const vec4<float>& JB, const float* KB) {
+  const f32x2 two = pk2(2.0f, 2.0f), mtwo = pk2(-2.0f, -2.0f);
+  float d[4], u[4], w[4];
+#pragma unroll
+  for (int h = 0; h < 2; h++) {
+    const f32x2 ka = pk2(KA[2 * h], KA[2 * h + 1]), kb = pk2(KB[2 * h], KB[2 * h + 1]), nkb = pk2(-KB[2 * h], -KB[2 * h + 1]);
+    const cx<float> dd = upk2(add2(ka, nkb)), uu = upk2(fma2(two, kb, ka)), ww = upk2(fma2(mtwo, ka, nkb));
+    d[2 * h] = dd.re; d[2 * h + 1] = dd.im; u[2 * h] = uu.re; u[2 * h + 1] = uu.im; w[2 * h] = ww.re; w[2 * h + 1] = ww.im;
+  }
+  cx<float> ab = mdot_cc(JA, JB), c1 = mdot_rc(u, JA), c2 = mdot_rc(w, JB);
+#pragma unroll
+  for (int i = 0; i < 4; i++) { rfma(acc.c[i], d[i], ab); cfma(acc.c[i], c1, JB.c[i]); cfma(acc.c[i], c2, JA.c[i]); }
+}
 // acc += V4(X,Y,Z), colour-ordered quartic structure V4 = 2 (X.Z) Y - (Y.Z) X - (X.Y) Z.  Trilinear: sign by negating X.
 template <typename T> __device__ __forceinline__ void V4_acc(vec4<T>& acc, const vec4<T>& X, const vec4<T>& Y, const vec4<T>& Z) {
   cx<T> xz = mdot_cc(X, Z), yz = mdot_cc(Y, Z), xy = mdot_cc(X, Y);
@@ -194,6 +222,19 @@ template <typename T> __device__ __forceinline__ lcv<T> lightcone(const vec4<T>&
 template <typename T> __device__ __forceinline__ lcv<T> lightcone_neg(const vec4<T>& a) {
   lcv<T> r; r.p = mk<T>(-a.c[0].re - a.c[3].re, -a.c[0].im - a.c[3].im); r.m = mk<T>(a.c[3].re - a.c[0].re, a.c[3].im - a.c[0].im);
   r.r = mk<T>(-a.c[1].re - a.c[2].im, a.c[2].re - a.c[1].im); r.l = mk<T>(a.c[2].im - a.c[1].re, -a.c[1].im - a.c[2].re);
+  return r;
+}
+// packed FP32 forms: every component is one add.rn.f32x2 (the swap / negation of a2 rides on operand modifiers)
+__device__ __forceinline__ lcv<float> lightcone(const vec4<float>& a) {
+  lcv<float> r; const f32x2 a0 = pk2(a.c[0].re, a.c[0].im), a1 = pk2(a.c[1].re, a.c[1].im);
+  r.p = upk2(add2(a0, pk2(a.c[3].re, a.c[3].im))); r.m = upk2(add2(a0, pk2(-a.c[3].re, -a.c[3].im)));
+  r.r = upk2(add2(a1, pk2(a.c[2].im, -a.c[2].re))); r.l = upk2(add2(a1, pk2(-a.c[2].im, a.c[2].re)));
+  return r;
+}
+__device__ __forceinline__ lcv<float> lightcone_neg(const vec4<float>& a) {
+  lcv<float> r; const f32x2 n0 = pk2(-a.c[0].re, -a.c[0].im), n1 = pk2(-a.c[1].re, -a.c[1].im);
+  r.p = upk2(add2(n0, pk2(-a.c[3].re, -a.c[3].im))); r.m = upk2(add2(n0, pk2(a.c[3].re, a.c[3].im)));
+  r.r = upk2(add2(n1, pk2(-a.c[2].im, a.c[2].re))); r.l = upk2(add2(n1, pk2(a.c[2].im, -a.c[2].re)));
   return r;
 }
 // X += a-slash * s      (8 complex FMAs)
