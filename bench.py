@@ -294,7 +294,7 @@ def run_parity_report(args) -> None:
 
 
 # rough oracle events/s/core (both parameter sets), measured on this pool's hosts; only sizes the bounded CPU samples
-ORACLE_PER_CORE = {1: 150000.0, 2: 6000.0, 3: 300.0, 4: 25.0, 5: 1.8, 6: 25.0}
+ORACLE_PER_CORE = {1: 150000.0, 2: 6000.0, 3: 300.0, 4: 25.0, 5: 1.8, 6: 25.0, 7: 3000.0, 8: 150.0}
 
 
 def main() -> None:

@@ -46,6 +46,8 @@ typedef struct {
 
 /* Create a handle for one process and one (old, new) pair of parameter sets.
  *   process: "epem_mupmum" | "gg_ttx" | "gg_ttxg" | "gg_ttxgg" | "gg_ttxggg"
+ *            | "qqx_ttx" | "qqx_ttxg"   (q qbar -> t tbar (+ g), massless quark, leg order [q,qbar,t,tbar,(g)]: a structurally
+ *              different amplitude for the final states of gg_ttx / gg_ttxg; FP64 only)
  *            | "epem_aa" | "epem_aaa" | "epem_aaaa" | "epem_aaaaa"   (e+ e- -> 2..5 photons, leg order [e+, e-, gamma...];
  *              "epem_aaaaa" is the process the paper measured, Table 1; only alpha_em enters; FP64 only)
  *            leg order in `momenta`: [e+,e-,mu+,mu-] resp. [g,g,t,tbar,(g,(g,(g)))];
@@ -124,6 +126,25 @@ int rwgt_run_host(rwgt_handle* h, const double* momenta, const double* weights, 
 /* rwgt_run_host for K >= 1 new sets: out_me_new, out_w_new are HOST double [K][n_events]. */
 int rwgt_run_multi_host(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old,
                         double* out_me_new, double* out_w_new, long long n_events, void* stream);
+
+/* LO multiprocess (real-emission contributions "can be treated as LO multiprocesses", last sentence:
+ * "reweighting between structurally different amplitude routines"): ONE event list whose events belong to different processes with
+ * the same number of external legs, e.g. "gg_ttxg,qqx_ttxg".  `processes`: comma-separated names (QCD processes only), at most
+ * RWGT_MAX_PROCESSES; parameter sets as in rwgt_create_multi, shared by all members.  NULL on error. */
+#define RWGT_MAX_PROCESSES 4
+rwgt_handle* rwgt_create_multiprocess(const char* processes, const rwgt_params* params_old, const rwgt_params* params_new, int n_new);
+
+/* Number of member processes (1 for a handle of rwgt_create / rwgt_create_multi); -1 on NULL. */
+int rwgt_n_processes(const rwgt_handle* h);
+
+/* rwgt_run_multi for a multiprocess handle.  Buffers as in rwgt_run_multi (DEVICE, K = rwgt_n_sets(h)); in addition
+ *   process_id  HOST int [n_events]: index of event i's process in the list given at create.
+ * The library partitions the event indices by process on the host (stable), copies the index lists to the device on `stream`
+ * (4 bytes per event; pinned staging and device list belong to the handle and grow on demand, which allocates and waits for
+ * `stream`) and launches one kernel per member process that has events; each kernel reads its events through its index list and
+ * writes the outputs at the events' own positions.  Returns 0, -1 (bad argument, id outside the list), or a cudaError_t. */
+int rwgt_run_multiprocess(rwgt_handle* h, const double* momenta, const double* weights, const int* process_id, double* out_me_old,
+                          double* out_me_new, double* out_w_new, long long n_events, void* stream);
 
 /* eq. 2 (§2.1): "the total cross section is the sum of all event weights", sigma ~ sum_k W_k.  Writes the sum of each
  * of n_rows weight rows to out_sums:

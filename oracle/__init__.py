@@ -32,6 +32,7 @@ def lib():
         L.orc_amp_epem_ng.argtypes = [C.c_int, _dp, _dp, _ip, _dp, _dp]
         L.orc_cross_section.argtypes = [_dp, C.c_long]
         L.orc_cross_section.restype = C.c_double
+        L.orc_me2_hel_qq.argtypes = [C.c_int, _dp, _dp, _ip, _dp, _dp]
         L.orc_denominator.argtypes = [C.c_int]
         L.orc_denominator.restype = C.c_double
         _lib = L
@@ -148,6 +149,21 @@ def cross_section(weights) -> float:
     """eq. 2: sigma ~ sum_k W_k, the plain left-to-right sum."""
     w, pw = _d(weights)
     return lib().orc_cross_section(pw, w.shape[0])
+
+
+def me2_hel_qq(ng: int, par, p, hel, eps_override=None) -> float:
+    """Colour-summed |M_h|^2 (no averaging) of q qbar -> t tbar (ng = 0) or q qbar -> t tbar g (ng = 1); p[4+ng,4], hel[4+ng] = +-1."""
+    par, pp = _d(par)
+    p, ppp = _d(p)
+    hel, ph = _i(hel)
+    out = C.c_double()
+    if eps_override is not None:
+        eo = np.ascontiguousarray(eps_override, dtype=np.complex128).reshape(4)
+        peo = eo.view(np.float64).ctypes.data_as(_dp)
+    else:
+        peo = None
+    assert lib().orc_me2_hel_qq(ng, pp, ppp, ph, peo, C.byref(out)) == 0
+    return out.value
 
 
 def denominator(n: int) -> float:

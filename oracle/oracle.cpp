@@ -26,6 +26,9 @@
 // tests/test_oracle_pins_photons.py by the textbook closed forms at n = 2, 3, the soft-photon theorem linking n + 1 to n up to
 // n = 5, gauge invariance eps -> k of every helicity amplitude, boost/rotation invariance, helicity selection rules and the
 // exact (alpha'/alpha)^n scaling.
+// q qbar -> t tbar (+ g) (a structurally different amplitude): explicit colour on every leg; pinned in
+// tests/test_oracle_pins_qq.py by the textbook closed form of q qbar -> Q Qbar, gauge invariance eps -> k, boost / rotation invariance,
+// the soft-gluon (eikonal) limit with colour correlations, parity.
 // PARITY UNPINNED (stated in DESIGN.md): absolute normalisation 1/(n-2)! of cfgs 4,5 and
 // the explicit-colour check of all helicities at n=5 (too slow).
 //
@@ -506,6 +509,87 @@ static int process_n_photons(const char* proc) {
   return -1;
 }
 
+// ---------------------------------------------------------------- q(p1) qbar(p2) -> t(p3) tbar(p4) [+ g(p5)]
+// A structurally different amplitude for the same final states as cfgs 2, 3 (PAPER.md:87 last sentence: "reweighting between structurally
+// different amplitude routines"; real emissions "can be treated as LO multiprocesses").  Massless light quark, rules of
+// SURVEY C3, explicit SU(3) colour on every leg (the plain definition: sum over all colours of |M|^2):
+//   light line as a gluon source   J_A^{mu c} = (-i/Q^2) vbar(p2) (i g gamma^mu T^c) u(p1),  Q = p1 + p2          (incoming momentum K_A = Q)
+//   with the gluon (colour a, wavefunction e = eps*(p5), K_g = -p5) radiated off the light line
+//     J_B^{mu c} = (-i/Q_B^2) vbar(p2) [ (i g gamma^mu T^c) S0(p1-p5) (i g e-slash T^a) + (i g e-slash T^a) S0(-p2+p5) (i g gamma^mu T^c) ] u(p1)
+//   or off the virtual gluon       J_C^{mu c} = (1/Q_B^2) (-i g3 f^{xac}) L3^mu(J_A^x, K_A; e, K_g),   Q_B = p1 + p2 - p5   (as in route E)
+//   iM_kl = ubar(p3) [ i g (J_B + J_C)-slash^c T^c + (i g e-slash T^a) S(p3+p5) (i g J_A-slash^c T^c) + (i g J_A-slash^c T^c) S(-p4-p5) (i g e-slash T^a) ]_kl v(p4)
+// S(q) = i (q-slash + m_t)/(q^2 - m_t^2), S0 the same with m = 0.  Without the gluon: iM_kl = ubar(p3) (i g J_A-slash^c T^c)_kl v(p4).
+// Averaging: 1/(2*2*3*3) (initial helicities and colours); no identical final-state particles.
+// eps_override: null or 4 complex numbers replacing e (gauge test).  Returns sum over colours of |M|^2 for ONE helicity configuration.
+static double me2_hel_qq(int ng, const Par& P, const double* p, const int* hel, const cd* eps_override) {
+  const SU3& su = SU(); const Gammas& G = GM();
+  const double g = std::sqrt(4.0 * PI * P.alpha_s), g3 = g * P.ggg_scale, mt = P.mt;
+  const double *p1 = p, *p2 = p + 4, *p3 = p + 8, *p4 = p + 12, *p5 = p + 16;
+  Sp u1 = spinor_u(p1, 0.0, hel[0]), vb2 = bar(spinor_v(p2, 0.0, hel[1])), ub3 = bar(spinor_u(p3, mt, hel[2])), v4 = spinor_v(p4, mt, hel[3]);
+  double KA[4], Kg[4] = {0, 0, 0, 0}, QB[4]; for (int mu = 0; mu < 4; mu++) { KA[mu] = p1[mu] + p2[mu]; QB[mu] = KA[mu]; }
+  V4 e = v4zero();
+  if (ng) {
+    e = conjv(polvec(p5, hel[4])); if (eps_override) for (int mu = 0; mu < 4; mu++) e.c[mu] = eps_override[mu];
+    for (int mu = 0; mu < 4; mu++) { Kg[mu] = -p5[mu]; QB[mu] = KA[mu] + Kg[mu]; }
+  }
+  auto prop = [&](const double q[4], double m) { return (I_ / cd(mink2(q) - m * m)) * (slash(realv(q)) + cd(m) * G.one); };
+  const cd ig = I_ * g;
+  // colour-stripped Lorentz pieces of the light line
+  V4 jA, jB1, jB2;                 // vbar gamma^mu u ; vbar gamma^mu S0 e-slash u (colour T^c T^a) ; vbar e-slash S0 gamma^mu u (colour T^a T^c)
+  double q1[4], q2[4]; for (int mu = 0; mu < 4; mu++) { q1[mu] = p1[mu] - p5[mu] * (ng ? 1 : 0); q2[mu] = -p2[mu] + p5[mu] * (ng ? 1 : 0); }
+  for (int mu = 0; mu < 4; mu++) {
+    jA.c[mu] = rowcol(vb2, (ig * G.g[mu]) * u1);
+    if (ng) {
+      jB1.c[mu] = rowcol(vb2, (ig * G.g[mu]) * (prop(q1, 0.0) * ((ig * slash(e)) * u1)));
+      jB2.c[mu] = rowcol(vb2, (ig * slash(e)) * (prop(q2, 0.0) * ((ig * G.g[mu]) * u1)));
+    }
+  }
+  const double QA2 = mink2(KA), QB2 = mink2(QB);
+  double qt[4], qtb[4]; for (int mu = 0; mu < 4; mu++) { qt[mu] = p3[mu] + p5[mu] * (ng ? 1 : 0); qtb[mu] = -p4[mu] - p5[mu] * (ng ? 1 : 0); }
+  double total = 0;
+  const int na = ng ? 8 : 1;
+  for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) for (int a = 0; a < na; a++) {
+    // currents entering the top line, colour component c
+    V4 JA[8], JT[8];
+    for (int c = 0; c < 8; c++) { JA[c] = ((-I_ / QA2) * su.T[c][j][i]) * jA; JT[c] = v4zero(); }
+    if (ng) {
+      for (int c = 0; c < 8; c++) {
+        cd ca = 0, ac = 0; for (int l = 0; l < 3; l++) { ca += su.T[c][j][l] * su.T[a][l][i]; ac += su.T[a][j][l] * su.T[c][l][i]; }
+        JT[c] = (-I_ / QB2) * (ca * jB1 + ac * jB2);
+      }
+      for (int x = 0; x < 8; x++) {
+        V4 l = L3(JA[x], KA, e, Kg);
+        for (int c = 0; c < 8; c++) if (su.f[x][a][c] != 0.0) JT[c] = JT[c] + (cd(1.0 / QB2) * (-I_ * g3 * su.f[x][a][c])) * l;
+      }
+    }
+    for (int k = 0; k < 3; k++) for (int l = 0; l < 3; l++) {
+      cd M = 0;
+      for (int c = 0; c < 8; c++) {
+        if (!ng) { if (su.T[c][k][l] != 0.0) M += su.T[c][k][l] * rowcol(ub3, (ig * slash(JA[c])) * v4); continue; }
+        if (su.T[c][k][l] != 0.0) M += su.T[c][k][l] * rowcol(ub3, (ig * slash(JT[c])) * v4);
+        cd ac = 0, ca = 0; for (int r = 0; r < 3; r++) { ac += su.T[a][k][r] * su.T[c][r][l]; ca += su.T[c][k][r] * su.T[a][r][l]; }
+        if (ac != 0.0) M += ac * rowcol(ub3, (ig * slash(e)) * (prop(qt, mt) * ((ig * slash(JA[c])) * v4)));
+        if (ca != 0.0) M += ca * rowcol(ub3, (ig * slash(JA[c])) * (prop(qtb, mt) * ((ig * slash(e)) * v4)));
+      }
+      total += std::norm(M);
+    }
+  }
+  return total;
+}
+static int process_n_qq(const char* proc) {          // number of radiated gluons, -1 if not a q qbar process
+  if (!std::strcmp(proc, "qqx_ttx")) return 0;
+  if (!std::strcmp(proc, "qqx_ttxg")) return 1;
+  return -1;
+}
+static double me2_qq(int ng, const Par& P, const double* p) {
+  double sum = 0; int hel[5];
+  for (int h = 0; h < (1 << (4 + ng)); h++) {          // full helicity sum
+    for (int i = 0; i < 4 + ng; i++) hel[i] = ((h >> i) & 1) ? 1 : -1;
+    sum += me2_hel_qq(ng, P, p, hel, nullptr);
+  }
+  return sum / 36.0;
+}
+
 // ---------------------------------------------------------------- process table
 static int process_n_gluons(const char* proc) {
   if (!std::strcmp(proc, "gg_ttx")) return 2;
@@ -517,11 +601,13 @@ static int process_n_gluons(const char* proc) {
 static int process_n_ext(const char* proc) {
   if (!std::strcmp(proc, "epem_mupmum")) return 4;
   int na = process_n_photons(proc); if (na > 0) return na + 2;
+  int nq = process_n_qq(proc); if (nq >= 0) return nq + 4;
   int n = process_n_gluons(proc); return n < 0 ? -1 : n + 2;
 }
 static double me2_any(const char* proc, const Par& P, const double* p) {
   if (!std::strcmp(proc, "epem_mupmum")) { double q[4][4]; std::memcpy(q, p, sizeof(q)); return me2_epem(P, q); }
   int na = process_n_photons(proc); if (na > 0) return me2_epem_ng(P, na, p);
+  int nq = process_n_qq(proc); if (nq >= 0) return me2_qq(nq, P, p);
   return me2_qcd_F(process_n_gluons(proc), P, p);
 }
 
@@ -599,6 +685,12 @@ void orc_amp_epem(const double* par, const double* p, const int* hel, double* ou
   double q[4][4]; std::memcpy(q, p, sizeof(q)); cd a = amp_epem(par_from(par), q, hel); out2[0] = a.real(); out2[1] = a.imag();
 }
 double orc_denominator(int n) { return denom_qcd(n); }
+// colour-summed |M_h|^2 of q qbar -> t tbar (+ g) for one helicity configuration; eps_override: null or 4 complex (re,im)
+int orc_me2_hel_qq(int ng, const double* par, const double* p, const int* hel, const double* eps_override, double* out) {
+  if (ng < 0 || ng > 1) return -1;
+  cd ov[4]; if (eps_override) for (int i = 0; i < 4; i++) ov[i] = cd(eps_override[2 * i], eps_override[2 * i + 1]);
+  *out = me2_hel_qq(ng, par_from(par), p, hel, eps_override ? ov : nullptr); return 0;
+}
 // helicity amplitude iM of e+ e- -> n photons for one helicity configuration; eps_override as in orc_jamps
 void orc_amp_epem_ng(int n, const double* par, const double* p, const int* hel, const double* eps_override, double* out2) {
   std::vector<cd> ov;

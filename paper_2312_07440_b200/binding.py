@@ -16,8 +16,10 @@ RWGT_FP64, RWGT_FP32, RWGT_MIXED = 0, 1, 2
 PRECISIONS = {"fp64": RWGT_FP64, "fp32": RWGT_FP32, "mixed": RWGT_MIXED}
 
 RWGT_MAX_SETS = 16
+RWGT_MAX_PROCESSES = 4
 EXPORTS = ("rwgt_create", "rwgt_create_multi", "rwgt_n_sets", "rwgt_run_multi", "rwgt_run_multi_host", "rwgt_set_precision", "rwgt_n_external", "rwgt_flops_per_event", "rwgt_run",
-           "rwgt_run_host", "rwgt_destroy", "rwgt_last_error", "rwgt_colour_matrix", "rwgt_tensor_flops_per_event", "rwgt_sum_weights", "rwgt_run_file")
+           "rwgt_run_host", "rwgt_destroy", "rwgt_last_error", "rwgt_colour_matrix", "rwgt_tensor_flops_per_event", "rwgt_sum_weights", "rwgt_run_file",
+           "rwgt_create_multiprocess", "rwgt_n_processes", "rwgt_run_multiprocess")
 
 
 class rwgt_params(C.Structure):
@@ -55,6 +57,10 @@ def lib():
         L.rwgt_destroy.argtypes = [vp]
         L.rwgt_last_error.restype = C.c_char_p
         L.rwgt_colour_matrix.argtypes = [C.c_int, dp]
+        L.rwgt_create_multiprocess.argtypes = [C.c_char_p, C.POINTER(rwgt_params), C.POINTER(rwgt_params), C.c_int]
+        L.rwgt_create_multiprocess.restype = vp
+        L.rwgt_n_processes.argtypes = [vp]
+        L.rwgt_run_multiprocess.argtypes = [vp, dp, dp, dp, dp, dp, dp, C.c_longlong, vp]
         L.rwgt_sum_weights.argtypes = [vp, dp, C.c_int, C.c_longlong, dp, vp]
         L.rwgt_run_file.argtypes = [vp, C.c_char_p, C.c_char_p, C.c_longlong, C.c_longlong, vp]
         _lib = L
@@ -87,6 +93,30 @@ def rwgt_create_multi(process: str, params_old, params_new_list):
     if not h:
         raise RuntimeError(rwgt_last_error())
     return h
+
+
+def rwgt_create_multiprocess(processes: str, params_old, params_new_list):
+    """LO multiprocess: comma-separated process names sharing n_ext, K new parameter sets."""
+    po = _params(params_old)
+    arr = (rwgt_params * len(params_new_list))(*[_params(p) for p in params_new_list])
+    h = lib().rwgt_create_multiprocess(processes.encode(), C.byref(po), arr, len(params_new_list))
+    if not h:
+        raise RuntimeError(rwgt_last_error())
+    return h
+
+
+def rwgt_n_processes(h) -> int:
+    return lib().rwgt_n_processes(h)
+
+
+def rwgt_run_multiprocess(h, momenta_ptr: int, weights_ptr: int, process_id: np.ndarray, out_me_old_ptr: int, out_me_new_ptr: int,
+                          out_w_new_ptr: int, n_events: int, stream: int = 0) -> None:
+    """Device pointers for the event buffers; process_id is a HOST int32 array [n_events]."""
+    assert process_id.dtype == np.int32 and process_id.flags.c_contiguous and process_id.shape == (int(n_events),)
+    rc = lib().rwgt_run_multiprocess(h, momenta_ptr, weights_ptr, process_id.ctypes.data, out_me_old_ptr, out_me_new_ptr, out_w_new_ptr,
+                                     int(n_events), stream or None)
+    if rc != 0:
+        raise RuntimeError(f"rwgt_run_multiprocess rc={rc}: {rwgt_last_error()}")
 
 
 def rwgt_n_sets(h) -> int:
@@ -245,7 +275,11 @@ class Reweighter:
         """params_new: one parameter set, or a list of K sets (then run() returns 1 + 2K rows:
         |M|^2, K rows |M'_k|^2, K rows W'_k)."""
         multi = isinstance(params_new, list)
-        self.h = rwgt_create_multi(process, params_old, params_new) if multi else rwgt_create(process, params_old, params_new)
+        self.multiprocess = "," in process            # "gg_ttxg,qqx_ttxg": run() then needs process_id
+        if self.multiprocess:
+            self.h = rwgt_create_multiprocess(process, params_old, params_new if multi else [params_new])
+        else:
+            self.h = rwgt_create_multi(process, params_old, params_new) if multi else rwgt_create(process, params_old, params_new)
         self.k = rwgt_n_sets(self.h)
         self.process = process
         self.n_ext = rwgt_n_external(self.h)
@@ -257,7 +291,7 @@ class Reweighter:
     def tensor_flops_per_event(self) -> float:
         return rwgt_tensor_flops_per_event(self.h)
 
-    def run(self, momenta, weights, out=None):
+    def run(self, momenta, weights, out=None, process_id=None):
         import torch
         n = weights.shape[0]
         assert momenta.is_cuda and momenta.dtype == torch.float64 and momenta.is_contiguous()
@@ -269,6 +303,10 @@ class Reweighter:
         assert out.is_cuda and out.dtype == torch.float64 and out.device == momenta.device
         assert out.shape == (1 + 2 * k, n) and out.is_contiguous()
         st = torch.cuda.current_stream(momenta.device).cuda_stream
+        if self.multiprocess:
+            rwgt_run_multiprocess(self.h, momenta.data_ptr(), weights.data_ptr(), np.ascontiguousarray(process_id, dtype=np.int32),
+                                  out[0].data_ptr(), out[1].data_ptr(), out[1 + k].data_ptr(), n, st)
+            return out
         rwgt_run_multi(self.h, momenta.data_ptr(), weights.data_ptr(), out[0].data_ptr(), out[1].data_ptr(),
                        out[1 + k].data_ptr(), n, st)
         return out

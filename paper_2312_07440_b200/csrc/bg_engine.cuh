@@ -345,7 +345,7 @@ struct BgDev {
   int offD[3][6], offT[6], offF;
   const uint32_t* words; const double* lfrag;
   BgSet set[BG_NSMAX];
-  unsigned long long* dbg;
+  const int* idx;        // multiprocess handles: event i of this launch is event idx[i] of the buffers (null: identity)
 };
 
 struct BgProcess {
@@ -645,13 +645,14 @@ template <typename T, typename TE, typename V> __device__ __forceinline__ void s
   for (int c = 0; c < 4; c++) stc(tab + c * stride + e, mk<T>((T)v.c[c].re, (T)v.c[c].im));
 }
 template <int N, typename T, typename TK, typename TE, typename SYNC>
-__device__ __forceinline__ void group_externals(int t0, int nth, int ns, long long ev0, long long nev, long long stride, const double* __restrict__ mom,
+__device__ __forceinline__ void group_externals(int t0, int nth, int ns, long long ev0, long long nev, long long stride, const double* __restrict__ mom, const int* __restrict__ idx,
                                                 double mtd, double* pmD, cx<T>* Gd, int sG, cx<T>* Rd, int sR, cx<T>* Ld, int sL, T* Kd, T* iK2d, T* dRd, T* dLd,
                                                 bool load, SYNC sync) {
   typedef Geo<N> Ge; constexpr int next = N + 2;
   if (load) {
     for (int t = t0; t < ns * next * 4; t += nth) {
       int sl = t % ns, comp = t / ns; long long ev = ev0 + sl; if (ev >= nev) ev = nev - 1;
+      if (idx) ev = idx[ev];
       pmD[(sl * next * 4) + comp] = __ldg(mom + (size_t)comp * stride + ev);
     }
     sync();
@@ -744,7 +745,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
       if constexpr (!STAGE) {
         // ---- a1/a2 by the workers themselves ----
         bar_sync(BAR_WORK, NWT);
-        group_externals<N, T, TK, TE>(tid, NWT, ns, ev0, nev, stride, mom, D.set[0].mt, s.pm, s.G, nG, s.R, nR, s.L, nL, s.K, s.iK2, s.dR, s.dL, true,
+        group_externals<N, T, TK, TE>(tid, NWT, ns, ev0, nev, stride, mom, D.idx, D.set[0].mt, s.pm, s.G, nG, s.R, nR, s.L, nL, s.K, s.iK2, s.dR, s.dL, true,
                                   [] { bar_sync(BAR_WORK, NWT); });
       } else {
       // ---- a1/a2 were done for this group by the colour warps (staging buffers): copy them into the tables ----
@@ -768,7 +769,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
         c.g3 = (T)P.g3; c.g4 = (T)P.g4; c.gq = (T)P.gq; c.mt = (T)P.mt;
         if (iset > 0 && !D.shared_ext) {
           // a set with another top mass: external spinors and denominators are redone for it (reading R12)
-          group_externals<N, T, TK, TE>(tid, NWT, ns, ev0, nev, stride, mom, P.mt, s.pm, s.G, nG, s.R, nR, s.L, nL, s.K, s.iK2, s.dR, s.dL, false, [] {});
+          group_externals<N, T, TK, TE>(tid, NWT, ns, ev0, nev, stride, mom, D.idx, P.mt, s.pm, s.G, nG, s.R, nR, s.L, nL, s.K, s.iK2, s.dR, s.dL, false, [] {});
           bar_sync(BAR_WORK, NWT);
         }
         // ---- a3: current levels ----
@@ -834,7 +835,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
     unsigned step = 0;
     // a1 + a2 of an event group into the staging buffers (parameter set 0; masses of the other sets: see the workers)
     auto stage = [&](long long g) {
-      group_externals<N, T, TK, TE>(ctid, NCT, ns, g * ns, nev, stride, mom, D.set[0].mt, s.pmS, s.GS, 2 * N, s.RS, 2, s.LS, 2, s.KS, s.iK2S, s.dRS, s.dLS, true,
+      group_externals<N, T, TK, TE>(ctid, NCT, ns, g * ns, nev, stride, mom, D.idx, D.set[0].mt, s.pmS, s.GS, 2 * N, s.RS, 2, s.LS, 2, s.KS, s.iK2S, s.dRS, s.dLS, true,
                                 [] { bar_sync(BAR_COLOUR, NCT); });
       __threadfence_block();
       bar_arrive(BAR_STAGE_FULL, NTH);
@@ -931,6 +932,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
       for (int sl = ctid; sl < ns; sl += NCT) {
         long long ev = ev0 + sl;
         if (ev < nev) {
+          if (D.idx) ev = D.idx[ev];
           const double a = s.acc[sl * BG_NSMAX] * D.set[0].fac, W = __ldg(wgt + ev);
           me_old[ev] = a;
           for (int k = 1; k < D.nsets; k++) {
@@ -1002,7 +1004,7 @@ static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::stri
   if (!err.empty()) { delete B; return nullptr; }
   const BgSched& S = B->S;
   BgDev& D = B->D;
-  D.nwords = (int)S.words.size(); D.offF = S.offF; D.dbg = nullptr;
+  D.nwords = (int)S.words.size(); D.offF = S.offF; D.idx = nullptr;
   bool ok = (S.nG == c_nG(n) && S.nR == c_nR(n) && S.nL == c_nL(n) && S.npair == S.nperm / 2);
   for (int m = 2; m <= n - 1; m++) ok = ok && S.ntask[0][m] == c_ntaskG(n, m);
   for (int m = 1; m <= S.rmax; m++) ok = ok && S.ntask[1][m + 1] == c_ntaskQ(n, m);
@@ -1062,8 +1064,8 @@ static double bg_tensor_flops_per_event(const BgProcess* B) {
   return B->D.nsets * nhel * 2.0 * (2.0 * (nh * (nh + 1) / 2) + 2.0 * nh) * 2.0;     // two reflection blocks of size n!/2
 }
 
-static int bg_run(BgProcess* B, int precision, const double* mom, const double* w, double* a, double* b, double* o, long long nev, long long stride, long long ostride, cudaStream_t st) {
-  BgDev D = B->D; const bool dbl = (precision == RWGT_FP64);
+static int bg_run(BgProcess* B, int precision, const double* mom, const double* w, const int* idx, double* a, double* b, double* o, long long nev, long long stride, long long ostride, cudaStream_t st) {
+  BgDev D = B->D; D.idx = idx; const bool dbl = (precision == RWGT_FP64);
   D.nslot = dbl ? B->nslot64 : B->nslot32;
   long long ngroups = (nev + D.nslot - 1) / D.nslot; int grid = (int)std::min<long long>(ngroups, (long long)B->sm_count * bg_ctas(B->S.n));
   switch (B->S.n) {

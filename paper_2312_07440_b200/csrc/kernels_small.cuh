@@ -118,11 +118,12 @@ __device__ __forceinline__ void ggttx_sums(const double (*p)[4], double m, doubl
   sum_a *= 2.0 / 3.0; sum_b *= 2.0 / 3.0;
 }
 
-__global__ void __launch_bounds__(128) gg_ttx_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
+__global__ void __launch_bounds__(128) gg_ttx_kernel(const double* __restrict__ mom, const double* __restrict__ wgt, const int* __restrict__ idx,
                                                      double* __restrict__ me_old, double* __restrict__ me_new,
                                                      double* __restrict__ w_new, long long n, long long stride, long long /*ostride*/, GGttxParams P) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
+  if (idx) i = idx[i];                      // multiprocess handles: the events of this process inside a mixed list
   double p[4][4];
 #pragma unroll
   for (int ip = 0; ip < 4; ip++)
@@ -181,11 +182,12 @@ __device__ __forceinline__ void ggttx_sums_multi(const double (*p)[4], double m,
   }
 }
 
-__global__ void __launch_bounds__(128) gg_ttx_multi_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
+__global__ void __launch_bounds__(128) gg_ttx_multi_kernel(const double* __restrict__ mom, const double* __restrict__ wgt, const int* __restrict__ idx,
                                                            double* __restrict__ me_old, double* __restrict__ me_new,
                                                            double* __restrict__ w_new, long long n, long long stride, long long ostride, GGttxParams P) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
+  if (idx) i = idx[i];
   double p[4][4];
 #pragma unroll
   for (int ip = 0; ip < 4; ip++)

@@ -12,6 +12,7 @@
 #include "kernels_small.cuh"
 #include "bg_engine.cuh"
 #include "photon_kernel.cuh"
+#include "qq_kernels.cuh"
 #include "event_file.cuh"
 
 namespace {
@@ -19,7 +20,7 @@ namespace {
 thread_local char g_err[512] = "";
 void set_err(const char* fmt, const char* a = "") { std::snprintf(g_err, sizeof(g_err), fmt, a); }
 
-enum Proc { P_EPEM = 0, P_GG_TTX = 1, P_BG = 2, P_PHOTONS = 3 };
+enum Proc { P_EPEM = 0, P_GG_TTX = 1, P_BG = 2, P_PHOTONS = 3, P_QQ = 4, P_MULTI = 5 };
 const double PI = 3.14159265358979323846;
 
 // A handle's tables and kernel attributes live on the device that was current at rwgt_create: every call that launches or
@@ -49,6 +50,10 @@ struct rwgt_handle {
   rwgt::GGttxParams ggttx;
   rwgt::PhotonParams photons; // e+ e- -> n_photons gamma
   int n_photons, sm_count;
+  rwgt::QQParams qq;          // q qbar -> t tbar (+ g); n_gluons = number of radiated gluons
+  int nsub;                   // P_MULTI ("LO multiprocess"): sub-handles, one per process of the mixed event list
+  rwgt_handle* sub[RWGT_MAX_PROCESSES];
+  int* d_idx; int* h_idx; long long idx_cap;     // per-process event index lists (device, pinned host), grown on demand
   rwgt::BgProcess* bg;        // ordered-current engine (n_gluons >= 3, or gg_ttx when forced)
   // device scratch for rwgt_run_host
   double* scratch;
@@ -109,6 +114,7 @@ rwgt_handle* rwgt_create_multi(const char* process, const rwgt_params* params_ol
   if (!h) { set_err("rwgt_create: out of memory"); return nullptr; }
   h->proc = -1; h->precision = RWGT_FP64; h->bg = nullptr; h->scratch = nullptr; h->scratch_bytes = 0; h->s_in = nullptr; h->s_out = nullptr; h->pipe_ready = 0;
   h->sum_partial = nullptr; h->sum_ticket = nullptr; h->sum_out = nullptr;
+  h->nsub = 0; h->d_idx = nullptr; h->h_idx = nullptr; h->idx_cap = 0;
   h->nsets = 1 + n_new; h->sets[0] = *params_old;
   for (int k = 0; k < n_new; k++) h->sets[1 + k] = params_new[k];
   cudaGetDevice(&h->device);
@@ -123,6 +129,27 @@ rwgt_handle* rwgt_create_multi(const char* process, const rwgt_params* params_ol
   else if (p == "gg_ttxg") { ng = 3; }
   else if (p == "gg_ttxgg") { ng = 4; }
   else if (p == "gg_ttxggg") { ng = 5; }
+  else if (p == "qqx_ttx" || p == "qqx_ttxg") {
+    // q qbar -> t tbar (+ g): a structurally different amplitude for the final states of gg_ttx / gg_ttxg
+    const int ngl = (p == "qqx_ttxg") ? 1 : 0;
+    h->proc = P_QQ; h->n_gluons = ngl; h->n_ext = 4 + ngl; h->qq.nsets = h->nsets; h->qq.two_pass = 0;
+    for (int k = 0; k < h->nsets; k++) {
+      const double g2 = 4.0 * PI * h->sets[k].alpha_s;
+      h->qq.mt[k] = h->sets[k].mt; h->qq.r[k] = h->sets[k].ggg_scale;
+      h->qq.fac[k] = ngl ? 2.0 * g2 * g2 * g2 / 36.0 : 2.0 * 2.0 * g2 * g2 / 36.0;
+      if (h->sets[k].mt != h->sets[0].mt) h->qq.two_pass = 1;
+    }
+    // colour matrix of the four structures C_1 = (T^a T^c)_ji T^c_kl, C_2 = (T^c T^a)_ji T^c_kl, C_3 = T^c_ji (T^a T^c)_kl,
+    // C_4 = T^c_ji (T^c T^a)_kl: G_ab = Tr(L_a(c) L_b(d)^+) Tr(K_a(c) K_b(d)^+), exact integers over 6^3 (labels a = 0, c = 1, d = 2)
+    for (int x = 0; x < 4; x++) for (int y = 0; y < 4; y++) {
+      auto light = [](int s, int lab) { return s == 0 ? std::vector<int>{0, lab} : s == 1 ? std::vector<int>{lab, 0} : std::vector<int>{lab}; };
+      auto top = [](int s, int lab) { return s == 2 ? std::vector<int>{0, lab} : s == 3 ? std::vector<int>{lab, 0} : std::vector<int>{lab}; };
+      std::vector<int> wl = light(x, 1), rl = light(y, 2), wt = top(x, 1), rt = top(y, 2);
+      wl.insert(wl.end(), rl.rbegin(), rl.rend()); wt.insert(wt.end(), rt.rbegin(), rt.rend());
+      h->qq.G[4 * x + y] = (double)rwgt::fierz_reduce({wl, wt}) / 216.0;
+    }
+    return finish_create(h);
+  }
   else if (p == "epem_aa" || p == "epem_aaa" || p == "epem_aaaa" || p == "epem_aaaaa") {
     // e+ e- -> n photons (n = 5: the paper's measured process): only alpha_em enters, as e^(2n)
     const int na = (int)p.size() - 5;
@@ -166,6 +193,10 @@ int rwgt_n_sets(const rwgt_handle* h) { return h ? h->nsets - 1 : -1; }
 
 int rwgt_set_precision(rwgt_handle* h, int mode) {
   if (!h || mode < 0 || mode > 2) { set_err("rwgt_set_precision: bad argument"); return -1; }
+  if (h->proc == P_MULTI) {            // applies to the members that have the mode; the others stay FP64
+    for (int i = 0; i < h->nsub; i++) if (h->sub[i]->proc == P_BG) h->sub[i]->precision = mode;
+    h->precision = mode; return 0;
+  }
   if (h->proc != P_BG && mode != RWGT_FP64) { set_err("rwgt_set_precision: this process is FP64 only"); return -1; }
   h->precision = mode;
   return 0;
@@ -179,6 +210,11 @@ double rwgt_flops_per_event(const rwgt_handle* h) {
   // 1225 DFMA + 365 DMUL + 87 DADD per event; profiles/r1_summary.md)
   if (h->proc == P_EPEM) return 426.0 + (h->nsets - 2) * 45.0;
   if (h->proc == P_PHOTONS) return rwgt::photon_flops_per_event(h->n_photons);
+  // q qbar -> t tbar (g): operation count of qq_kernels.cuh (externals ~300; per gluon helicity b_1, b_2, l ~700; per (gluon, tbar) helicity five
+  // slash chains ~900; per helicity 5 row.col + per set the 4 x 4 colour form ~100)
+  if (h->proc == P_QQ) { const double one = h->n_gluons ? 300.0 + 2 * 700.0 + 4 * 900.0 + 8 * (160.0 + h->nsets * 100.0) : 300.0 + 2 * 64.0 + 4 * 36.0;
+                         return h->qq.two_pass ? h->nsets * one : one; }
+  if (h->proc == P_MULTI) { double f = 0; for (int i = 0; i < h->nsub; i++) f += rwgt_flops_per_event(h->sub[i]); return f / h->nsub; }
   // gg_ttx: 2902 for two sets of equal mass; a further set of equal mass costs 8 helicities x (4 FMA + colour form 5 FMA + 4 MUL/ADD)
   if (h->proc == P_GG_TTX) return h->ggttx.two_pass ? h->nsets * 2902.0 : 2902.0 + (h->nsets - 2) * 8 * 26.0;
   return rwgt::bg_flops_per_event(h->bg, h->precision);
@@ -186,25 +222,31 @@ double rwgt_flops_per_event(const rwgt_handle* h) {
 
 double rwgt_tensor_flops_per_event(const rwgt_handle* h) {
   if (!h) return -1.0;
+  if (h->proc == P_MULTI) { double f = 0; for (int i = 0; i < h->nsub; i++) f += rwgt_tensor_flops_per_event(h->sub[i]); return f / h->nsub; }
   return h->proc == P_BG ? rwgt::bg_tensor_flops_per_event(h->bg) : 0.0;
 }
 
 // one kernel launch over events [0, n) of buffers whose momentum planes are `stride` events apart and whose per-set
 // output planes are `ostride` events apart
 static int launch_events(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old, double* out_me_new,
-                         double* out_w_new, long long n, long long stride, long long ostride, cudaStream_t st) {
+                         double* out_w_new, long long n, long long stride, long long ostride, cudaStream_t st, const int* idx = nullptr) {
+  if (idx && (h->proc == P_EPEM || h->proc == P_PHOTONS)) { set_err("rwgt_run: this process cannot be part of a multiprocess handle"); return -1; }
   if (h->proc == P_EPEM) {
     int bs = 256; long long nb = (n + bs - 1) / bs;
     rwgt::epem_mupmum_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->epem);
   } else if (h->proc == P_GG_TTX) {
     int bs = 128; long long nb = (n + bs - 1) / bs;
-    if (h->nsets == 2) rwgt::gg_ttx_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->ggttx);
-    else rwgt::gg_ttx_multi_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->ggttx);
+    if (h->nsets == 2) rwgt::gg_ttx_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, idx, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->ggttx);
+    else rwgt::gg_ttx_multi_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, idx, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->ggttx);
+  } else if (h->proc == P_QQ) {
+    int bs = 128; long long nb = (n + bs - 1) / bs;
+    if (h->n_gluons) rwgt::qqx_ttx_kernel<1><<<(unsigned)nb, bs, 0, st>>>(momenta, weights, idx, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->qq);
+    else rwgt::qqx_ttx_kernel<0><<<(unsigned)nb, bs, 0, st>>>(momenta, weights, idx, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->qq);
   } else if (h->proc == P_PHOTONS) {
     cudaError_t e = rwgt::photon_launch(h->n_photons, h->sm_count, st, momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->photons);
     if (e != cudaSuccess) { set_err("rwgt_run: %s", cudaGetErrorString(e)); return (int)e; }
   } else {
-    int rc = rwgt::bg_run(h->bg, h->precision, momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, st);
+    int rc = rwgt::bg_run(h->bg, h->precision, momenta, weights, idx, out_me_old, out_me_new, out_w_new, n, stride, ostride, st);
     if (rc != 0) { set_err("rwgt_run: engine launch failed"); return rc; }
   }
   cudaError_t e = cudaGetLastError();
@@ -217,6 +259,7 @@ int rwgt_run_multi(rwgt_handle* h, const double* momenta, const double* weights,
   if (!h || n_events < 0) { set_err("rwgt_run: bad handle or n_events < 0"); return -1; }
   if (n_events == 0) return 0;
   if (!momenta || !weights || !out_me_old || !out_me_new || !out_w_new) { set_err("rwgt_run: NULL buffer"); return -1; }
+  if (h->proc == P_MULTI) { set_err("rwgt_run: multiprocess handle, use rwgt_run_multiprocess"); return -1; }
   DeviceGuard guard(h->device);
   if (!guard.ok) { set_err("rwgt_run: cannot make the handle's device current"); return -1; }
   return launch_events(h, momenta, weights, out_me_old, out_me_new, out_w_new, n_events, n_events, n_events, (cudaStream_t)stream);
@@ -236,6 +279,7 @@ int rwgt_run_multi_host(rwgt_handle* h, const double* momenta, const double* wei
   if (!h || n_events < 0) { set_err("rwgt_run_host: bad handle or n_events < 0"); return -1; }
   if (n_events == 0) return 0;
   if (!momenta || !weights || !out_me_old || !out_me_new || !out_w_new) { set_err("rwgt_run_host: NULL buffer"); return -1; }
+  if (h->proc == P_MULTI) { set_err("rwgt_run_host: multiprocess handle, use rwgt_run_multiprocess"); return -1; }
   DeviceGuard guard(h->device);
   if (!guard.ok) { set_err("rwgt_run_host: cannot make the handle's device current"); return -1; }
   cudaStream_t st = (cudaStream_t)stream;
@@ -304,6 +348,66 @@ int rwgt_run_host(rwgt_handle* h, const double* momenta, const double* weights, 
                   double* out_w_new, long long n_events, void* stream) {
   if (h && h->nsets != 2) { set_err("rwgt_run_host: handle has several new parameter sets, use rwgt_run_multi_host"); return -1; }
   return rwgt_run_multi_host(h, momenta, weights, out_me_old, out_me_new, out_w_new, n_events, stream);
+}
+
+// real-emission contributions "can be treated as LO multiprocesses" -- one event list, several amplitudes
+rwgt_handle* rwgt_create_multiprocess(const char* processes, const rwgt_params* params_old, const rwgt_params* params_new, int n_new) {
+  if (!processes || !params_old || !params_new) { set_err("rwgt_create_multiprocess: NULL argument"); return nullptr; }
+  std::vector<std::string> names; { std::string all(processes), cur; for (char ch : all) { if (ch == ',') { names.push_back(cur); cur.clear(); } else if (ch != ' ') cur += ch; } names.push_back(cur); }
+  if (names.empty() || (int)names.size() > RWGT_MAX_PROCESSES) { set_err("rwgt_create_multiprocess: 1..RWGT_MAX_PROCESSES comma-separated process names"); return nullptr; }
+  rwgt_handle* h = new (std::nothrow) rwgt_handle();
+  if (!h) { set_err("rwgt_create_multiprocess: out of memory"); return nullptr; }
+  h->proc = P_MULTI; h->precision = RWGT_FP64; h->bg = nullptr; h->scratch = nullptr; h->scratch_bytes = 0; h->s_in = nullptr; h->s_out = nullptr; h->pipe_ready = 0;
+  h->sum_partial = nullptr; h->sum_ticket = nullptr; h->sum_out = nullptr; h->nsub = 0; h->d_idx = nullptr; h->h_idx = nullptr; h->idx_cap = 0;
+  h->nsets = 1 + n_new; h->n_gluons = 0; h->n_ext = -1; std::memset(h->process, 0, sizeof(h->process));
+  cudaGetDevice(&h->device);
+  for (const std::string& nm : names) {
+    rwgt_handle* s = rwgt_create_multi(nm.c_str(), params_old, params_new, n_new);       // sets g_err on failure
+    if (s && (s->proc == P_EPEM || s->proc == P_PHOTONS)) { rwgt_destroy(s); s = nullptr; set_err("rwgt_create_multiprocess: '%s' cannot be a member (QCD processes only)", nm.c_str()); }
+    if (s && h->n_ext >= 0 && s->n_ext != h->n_ext) { rwgt_destroy(s); s = nullptr; set_err("rwgt_create_multiprocess: '%s' has another number of external legs than the first process", nm.c_str()); }
+    if (!s) { rwgt_destroy(h); return nullptr; }
+    h->n_ext = s->n_ext; h->sub[h->nsub++] = s;
+  }
+  for (int k = 0; k < h->nsets; k++) h->sets[k] = h->sub[0]->sets[k];
+  std::strncpy(h->process, "multiprocess", sizeof(h->process) - 1);
+  return finish_create(h);
+}
+
+int rwgt_n_processes(const rwgt_handle* h) { return !h ? -1 : (h->proc == P_MULTI ? h->nsub : 1); }
+
+int rwgt_run_multiprocess(rwgt_handle* h, const double* momenta, const double* weights, const int* process_id, double* out_me_old,
+                          double* out_me_new, double* out_w_new, long long n_events, void* stream) {
+  if (!h || h->proc != P_MULTI || n_events < 0) { set_err("rwgt_run_multiprocess: not a multiprocess handle, or n_events < 0"); return -1; }
+  if (n_events == 0) return 0;
+  if (!momenta || !weights || !process_id || !out_me_old || !out_me_new || !out_w_new) { set_err("rwgt_run_multiprocess: NULL buffer"); return -1; }
+  if (n_events > 0x7fffffffLL) { set_err("rwgt_run_multiprocess: more than 2^31-1 events in one call"); return -1; }
+  DeviceGuard guard(h->device);
+  if (!guard.ok) { set_err("rwgt_run_multiprocess: cannot make the handle's device current"); return -1; }
+  cudaStream_t st = (cudaStream_t)stream; cudaError_t e = cudaSuccess;
+  if (n_events > h->idx_cap) {
+    // the pinned list may still be the source of a copy enqueued by an earlier call
+    if (h->h_idx) { cudaStreamSynchronize(st); cudaFreeHost(h->h_idx); h->h_idx = nullptr; }
+    if (h->d_idx) { cudaFree(h->d_idx); h->d_idx = nullptr; }
+    h->idx_cap = 0;
+    e = cudaMalloc((void**)&h->d_idx, sizeof(int) * (size_t)n_events);
+    if (e == cudaSuccess) e = cudaHostAlloc((void**)&h->h_idx, sizeof(int) * (size_t)n_events, cudaHostAllocDefault);
+    if (e != cudaSuccess) { set_err("rwgt_run_multiprocess: %s", cudaGetErrorString(e)); return (int)e; }
+    h->idx_cap = n_events;
+  } else cudaStreamSynchronize(st);               // an earlier call's copy out of h_idx must have finished before it is rewritten
+  // stable partition of the event indices by process (host; 4 bytes per event against >= 136 bytes of momenta)
+  long long count[RWGT_MAX_PROCESSES] = {}, off[RWGT_MAX_PROCESSES + 1] = {};
+  for (long long i = 0; i < n_events; i++) { const int pid = process_id[i]; if (pid < 0 || pid >= h->nsub) { set_err("rwgt_run_multiprocess: process_id outside 0..n_processes-1"); return -1; } count[pid]++; }
+  for (int k = 0; k < h->nsub; k++) off[k + 1] = off[k] + count[k];
+  { long long fill[RWGT_MAX_PROCESSES]; for (int k = 0; k < h->nsub; k++) fill[k] = off[k];
+    for (long long i = 0; i < n_events; i++) h->h_idx[fill[process_id[i]]++] = (int)i; }
+  e = cudaMemcpyAsync(h->d_idx, h->h_idx, sizeof(int) * (size_t)n_events, cudaMemcpyHostToDevice, st);
+  if (e != cudaSuccess) { set_err("rwgt_run_multiprocess: %s", cudaGetErrorString(e)); return (int)e; }
+  for (int k = 0; k < h->nsub; k++) {
+    if (count[k] == 0) continue;
+    int rc = launch_events(h->sub[k], momenta, weights, out_me_old, out_me_new, out_w_new, count[k], n_events, n_events, st, h->d_idx + off[k]);
+    if (rc != 0) return rc;
+  }
+  return 0;
 }
 
 // eq. 2: sigma ~ sum_k W_k, one deterministic device reduction per row
@@ -397,6 +501,9 @@ int rwgt_run_file(rwgt_handle* h, const char* in_path, const char* out_path, lon
 int rwgt_destroy(rwgt_handle* h) {
   if (!h) return -1;
   DeviceGuard guard(h->device);
+  for (int i = 0; i < h->nsub; i++) rwgt_destroy(h->sub[i]);
+  if (h->d_idx) cudaFree(h->d_idx);
+  if (h->h_idx) cudaFreeHost(h->h_idx);
   if (h->bg) rwgt::bg_destroy(h->bg);
   if (h->scratch) cudaFree(h->scratch);
   cudaFree(h->sum_partial); cudaFree(h->sum_ticket); cudaFree(h->sum_out);

@@ -1,4 +1,4 @@
-"""Seeded synthetic event sets for the five BASELINE.json configs (+ the paper's own e+e- -> 5 gamma).
+"""Seeded synthetic event sets for the five BASELINE.json configs (+ the paper's own e+e- -> 5 gamma, + q qbar -> t tbar (g)).
 
 This module is the ONLY code shared by the CPU oracle (tests / cpu_baseline) and
 the CUDA path.  It holds none of the method's arithmetic (no wavefunctions,
@@ -85,6 +85,13 @@ CONFIGS = (
     # cuts are not stated in the paper: 500 GeV as cfg 1, every photon pT > 20 GeV and Delta R > 0.4.
     Config(6, "epem_aaaaa", 131072, 500.0, (0.0,) * 5, 5, True, 20231207 + 6,
            params(), params(alpha_em=1.0 / 128.0), ("fp64",)),
+    # Not BASELINE.json configs: structurally different amplitudes for the final states of cfgs 2 and 3 (PAPER.md:87 last
+    # sentence, "LO multiprocesses"): a massless quark-antiquark pair instead of the two gluons.  Same sqrt(s), masses and
+    # cuts as cfgs 2 / 3; q qbar -> t tbar has no gluon self-coupling, so its new set changes alpha_s (a running-coupling style change).
+    Config(7, "qqx_ttx", 1048576, 1500.0, (_MT, _MT), 0, False, 20231207 + 7,
+           params(), params(alpha_s=0.108), ("fp64",)),
+    Config(8, "qqx_ttxg", 1048576, 1500.0, (_MT, _MT, 0.0), 1, False, 20231207 + 8,
+           params(), params(ggg_scale=1 + _KAPPA, gggg_scale=1 + _KAPPA), ("fp64",)),
 )
 
 
