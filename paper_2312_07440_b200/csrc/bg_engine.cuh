@@ -340,15 +340,21 @@ static BgSched build_schedule(int n, std::string& err) {
 // ------------------------------------------------------------------------------------------------ device side
 struct BgSet { double gq, g3, g4, mt, fac; };        // fac = 2 gq^2 / D  (|i gq|^2, parity factor 2, averaging)
 constexpr int BG_NSMAX = 1 + RWGT_MAX_SETS;      // the old set plus up to RWGT_MAX_SETS new ones
+constexpr int BG_RMAX = 6;                       // most node sets of the polynomial mode (n = 4 needs at most 6, n = 5 five on the diagonal ggg = gggg)
 struct BgDev {
   int nwords, nslot, shared_ext, nsets;
   int offD[3][6], offT[6], offF;
   const uint32_t* words; const double* lfrag;
   BgSet set[BG_NSMAX];
+  // polynomial mode (coupling-only parameter sets, see bg_plan_poly): the currents are evaluated at nnode node sets only; every
+  // parameter set k is the exact linear combination J(k) = sum_j cw[k][j] J(node j) of them
+  int poly, nnode; BgSet node[BG_RMAX]; double cw[BG_NSMAX][BG_RMAX];
+  double* poly_scratch; long long poly_stride;   // Z = L^T (u | v) of every node set of one event group, per CTA (global memory, mostly L2 resident)
   const int* idx;        // multiprocess handles: event i of this launch is event idx[i] of the buffers (null: identity)
 };
 
 struct BgProcess {
+  double* d_poly;        // polynomial mode: Z of the node sets, one slice per CTA
   BgSched S; BgDev D; uint32_t* d_words; double* d_lfrag; int sm_count; size_t smem64, smem32; int nslot64, nslot32;
 };
 
@@ -367,6 +373,7 @@ template <typename T> struct Smem {
   double* pm;     // [nslot][n_ext][4] momenta (always double)
   double* acc;    // [nslot][BG_NSMAX]   helicity-summed colour forms per parameter set (owned by the colour warps)
   double* red;    // [nslot][8]   per-warp partial sums of the colour form
+  double* pred;   // [16][BG_RMAX (BG_RMAX + 1) / 2]   polynomial mode: per-warp partial cross forms
   cx<T>* G; cx<T>* R; cx<T>* L;   // [nslot][4][nX]   component planes of (re,im) pairs: one vector load per component,
                                   //                  conflict-free for consecutive helicity variants
   T* K;           // [nslot][NMASK][4] momentum sums of gluon subsets
@@ -386,6 +393,7 @@ template <int N, typename T> __host__ __device__ inline size_t carve(Smem<T>& s,
   s.pm = (double*)(base + off); off += sizeof(double) * ns * (N + 2) * 4; al();
   s.acc = (double*)(base + off); off += sizeof(double) * ns * BG_NSMAX; al();
   s.red = (double*)(base + off); off += sizeof(double) * ns * 8; al();
+  s.pred = (double*)(base + off); off += sizeof(double) * 16 * (BG_RMAX * (BG_RMAX + 1) / 2); al();
   s.G = (cx<T>*)(base + off); off += sizeof(T) * (size_t)ns * 8 * nG; al();
   s.R = (cx<T>*)(base + off); off += sizeof(T) * (size_t)ns * 8 * nR; al();
   s.L = (cx<T>*)(base + off); off += sizeof(T) * (size_t)ns * 8 * nL; al();
@@ -443,21 +451,23 @@ __device__ __forceinline__ uint32_t halfw(const uint32_t* w, int k) { return (k 
 
 // named barriers (ids 1..6; id 0 is __syncthreads): workers among themselves, colour warps among themselves,
 // and the full/empty handshake of the two amplitude buffers
-enum { BAR_WORK = 1, BAR_FULL0 = 2, BAR_EMPTY0 = 4, BAR_COLOUR = 6, BAR_STAGE_FULL = 7, BAR_STAGE_EMPTY = 8 };
+enum { BAR_WORK = 1, BAR_FULL0 = 2, BAR_EMPTY0 = 4, BAR_COLOUR = 6, BAR_STAGE_FULL = 7, BAR_STAGE_EMPTY = 8, BAR_ZFULL = 9 };
 // the barrier id is an immediate (a register id makes ptxas reserve all 16 barriers, which limits the CTAs per SM)
 __device__ __forceinline__ void bar_sync(int id, int count) {
   switch (id) {
     case 1: asm volatile("bar.sync 1, %0;" ::"r"(count) : "memory"); break; case 2: asm volatile("bar.sync 2, %0;" ::"r"(count) : "memory"); break;
     case 3: asm volatile("bar.sync 3, %0;" ::"r"(count) : "memory"); break; case 4: asm volatile("bar.sync 4, %0;" ::"r"(count) : "memory"); break;
     case 5: asm volatile("bar.sync 5, %0;" ::"r"(count) : "memory"); break; case 6: asm volatile("bar.sync 6, %0;" ::"r"(count) : "memory"); break;
-    case 7: asm volatile("bar.sync 7, %0;" ::"r"(count) : "memory"); break; default: asm volatile("bar.sync 8, %0;" ::"r"(count) : "memory");
+    case 7: asm volatile("bar.sync 7, %0;" ::"r"(count) : "memory"); break; case 8: asm volatile("bar.sync 8, %0;" ::"r"(count) : "memory"); break;
+    default: asm volatile("bar.sync 9, %0;" ::"r"(count) : "memory");
   }
 }
 __device__ __forceinline__ void bar_arrive(int id, int count) {
   switch (id) {
     case 2: asm volatile("bar.arrive 2, %0;" ::"r"(count) : "memory"); break; case 3: asm volatile("bar.arrive 3, %0;" ::"r"(count) : "memory"); break;
     case 4: asm volatile("bar.arrive 4, %0;" ::"r"(count) : "memory"); break; case 5: asm volatile("bar.arrive 5, %0;" ::"r"(count) : "memory"); break;
-    case 7: asm volatile("bar.arrive 7, %0;" ::"r"(count) : "memory"); break; default: asm volatile("bar.arrive 8, %0;" ::"r"(count) : "memory");
+    case 7: asm volatile("bar.arrive 7, %0;" ::"r"(count) : "memory"); break; case 8: asm volatile("bar.arrive 8, %0;" ::"r"(count) : "memory"); break;
+    default: asm volatile("bar.arrive 9, %0;" ::"r"(count) : "memory");
   }
 }
 
@@ -704,7 +714,7 @@ __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double
 // FP32 mode: with float denominators gg -> ttggg misses the 1e-4 / 1e-6 tolerances on 8,192 events, profiles/r2_parity.md);
 // 2 = the external wavefunctions too (the mixed mode).  Everything downstream of the amplitudes (u, v rows, colour form,
 // helicity sum, eq. 3) runs in double in every mode.
-template <int N, typename T, int MX, int NW, int NCW, int CTAS>
+template <int N, typename T, int MX, int NW, int NCW, int CTAS, bool POLY = false>
 __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
                                                                double* __restrict__ me_old, double* __restrict__ me_new,
                                                                double* __restrict__ w_new, long long nev, long long stride, long long ostride, BgDev D) {
@@ -763,11 +773,12 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
       bar_arrive(BAR_STAGE_EMPTY, NTH);                        // the colour warps may stage the next group
       }
       bar_sync(BAR_WORK, NWT);
+      const int neval = POLY ? D.nnode : D.nsets;              // polynomial mode: one evaluation per node set, not per parameter set
 #pragma unroll 1
-      for (int iset = 0; iset < D.nsets; iset++) {
-        const BgSet& P = D.set[iset];
+      for (int iset = 0; iset < neval; iset++) {
+        const BgSet& P = POLY ? D.node[iset] : D.set[iset];
         c.g3 = (T)P.g3; c.g4 = (T)P.g4; c.gq = (T)P.gq; c.mt = (T)P.mt;
-        if (iset > 0 && !D.shared_ext) {
+        if (!POLY && iset > 0 && !D.shared_ext) {
           // a set with another top mass: external spinors and denominators are redone for it (reading R12)
           group_externals<N, T, TK, TE>(tid, NWT, ns, ev0, nev, stride, mom, D.idx, P.mt, s.pm, s.G, nG, s.R, nR, s.L, nL, s.K, s.iK2, s.dR, s.dL, false, [] {});
           bar_sync(BAR_WORK, NWT);
@@ -827,6 +838,64 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
         }
         bar_sync(BAR_WORK, NWT);                               // the current tables are rewritten for the next parameter set / group
       }
+      if constexpr (POLY) {
+        // ---- a5/a6 in polynomial mode: the colour warps have written Z_j = L^T (u_j | v_j) of every node set j and helicity batch to the
+        // CTA's global scratch (all nodes in one element order).  The colour form is quadratic in J and J(set k) = sum_j cw_kj J_j, so
+        // what an event needs are the cross forms Q_jj' = sum_elements Z_j Z_j': a streaming pass, fixed reduction order.
+        constexpr int NP = BG_RMAX * (BG_RMAX + 1) / 2, ZEL = Ge::NBATCH * Ge::U * 2 * Ge::NT * 64;   // doubles of one (node, slot)
+        static_assert(Ge::MTH % 2 == 0, "polynomial mode: every (unit, half) of the triangular mma must exist");
+        const double* Zc = D.poly_scratch + (size_t)blockIdx.x * D.poly_stride;
+        double* red = s.pred;                                  // [NW][NP], one slot at a time
+        const int warp = tid >> 5, lane = tid & 31, nnode = D.nnode;
+        bar_sync(BAR_ZFULL, NTH);                              // all Z of this group are in the scratch
+#pragma unroll 1
+        for (int sl = 0; sl < ns; sl++) {
+          double q[NP];
+#pragma unroll
+          for (int pi = 0; pi < NP; pi++) q[pi] = 0.0;
+          for (int e2 = tid; e2 < ZEL / 2; e2 += NWT) {
+            double2 z[BG_RMAX];
+#pragma unroll
+            for (int j = 0; j < BG_RMAX; j++) z[j] = (j < nnode) ? __ldcg(reinterpret_cast<const double2*>(Zc + ((size_t)j * ns + sl) * ZEL) + e2) : make_double2(0.0, 0.0);
+            int pi = 0;
+#pragma unroll
+            for (int j = 0; j < BG_RMAX; j++)
+#pragma unroll
+              for (int j2 = j; j2 < BG_RMAX; j2++, pi++) { q[pi] = fma(z[j].x, z[j2].x, q[pi]); q[pi] = fma(z[j].y, z[j2].y, q[pi]); }
+          }
+#pragma unroll
+          for (int d = 16; d >= 1; d >>= 1)
+#pragma unroll
+            for (int pi = 0; pi < NP; pi++) q[pi] += __shfl_xor_sync(0xffffffffu, q[pi], d);
+          if (lane == 0) {
+#pragma unroll
+            for (int pi = 0; pi < NP; pi++) red[warp * NP + pi] = q[pi];
+          }
+          bar_sync(BAR_WORK, NWT);
+          // ---- a6/a7: one thread: the warps' partial sums in fixed order, every parameter set, eq. 3, stores ----
+          if (tid == 0) {
+            long long ev = ev0 + sl;
+            if (ev < nev) {
+              if (D.idx) ev = D.idx[ev];
+              double Q[NP];
+#pragma unroll
+              for (int pi = 0; pi < NP; pi++) { double a = 0.0; for (int wv = 0; wv < NW; wv++) a += red[wv * NP + pi]; Q[pi] = a; }
+              const double W = __ldg(wgt + ev); double a0 = 0.0;
+              for (int k = 0; k < D.nsets; k++) {
+                double me = 0.0; int pi = 0;
+#pragma unroll
+                for (int j = 0; j < BG_RMAX; j++)
+#pragma unroll
+                  for (int j2 = j; j2 < BG_RMAX; j2++, pi++) me = fma((j == j2 ? 1.0 : 2.0) * D.cw[k][j] * D.cw[k][j2], Q[pi], me);
+                me *= D.set[k].fac;
+                if (k == 0) { a0 = me; me_old[ev] = me; }
+                else { me_new[(size_t)(k - 1) * ostride + ev] = me; w_new[(size_t)(k - 1) * ostride + ev] = W * (me / a0); }
+              }
+            }
+          }
+          bar_sync(BAR_WORK, NWT);                             // red is reused by the next slot
+        }
+      }
     }
   } else {
     // =========================================================================================== colour warps
@@ -849,8 +918,10 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
         if (grp + gridDim.x < ngroups) stage(grp + gridDim.x); // the next group's fixed work overlaps the workers' currents and amplitudes
       }
       bar_sync(BAR_COLOUR, NCT);
+      const int neval = POLY ? D.nnode : D.nsets;
+      double* const Zc = POLY ? D.poly_scratch + (size_t)blockIdx.x * D.poly_stride : nullptr;
 #pragma unroll 1
-      for (int iset = 0; iset < D.nsets; iset++) {
+      for (int iset = 0; iset < neval; iset++) {
 #pragma unroll 1
         for (int batch = 0; batch < Ge::NBATCH; batch++, step++) {
           const int buf = step & 1;
@@ -914,21 +985,40 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
 #pragma unroll
                 for (int nt = 0; nt < Ge::NT; nt++) b_cur[nt] = b_nxt[nt];
               }
+              if constexpr (POLY) {
+                // polynomial mode: keep Z itself (global scratch, [node][slot][batch][unit][half][n-tile][lane][2]); the workers form the cross terms
+                double* z = Zc + ((((size_t)(iset * ns + sl) * Ge::NBATCH + batch) * Ge::U + unit) * 2 + half) * (Ge::NT * 64) + lane * 2;
+#pragma unroll
+                for (int nt = 0; nt < Ge::NT; nt++) __stcg(reinterpret_cast<double2*>(z + nt * 64), make_double2(acc[nt][0], acc[nt][1]));
+              } else {
 #pragma unroll
               for (int nt = 0; nt < Ge::NT; nt++) { part = fma(acc[nt][0], acc[nt][0], part); part = fma(acc[nt][1], acc[nt][1], part); }
+              }
             }
+            if constexpr (!POLY) {
             // a6: deterministic reduction (same order for both parameter sets => old == new gives a ratio of exactly 1)
 #pragma unroll
             for (int d = 16; d >= 1; d >>= 1) part += __shfl_xor_sync(0xffffffffu, part, d);
             if (lane == 0) s.red[sl * 8 + unit] = part;
+            }
           }
+          if constexpr (POLY) {
+            __threadfence_block();
+            bar_arrive(BAR_EMPTY0 + buf, NTH);                 // buffer may be refilled
+          } else {
           bar_sync(BAR_COLOUR, NCT);
           bar_arrive(BAR_EMPTY0 + buf, NTH);                   // buffer may be refilled
           for (int sl = ctid; sl < ns; sl += NCT) { double a = 0.0; for (int j = 0; j < Ge::U; j++) a += s.red[sl * 8 + j]; s.acc[sl * BG_NSMAX + iset] += a; }
           bar_sync(BAR_COLOUR, NCT);
+          }
         }
       }
+      if constexpr (POLY) {
+        __threadfence_block();
+        bar_arrive(BAR_ZFULL, NTH);                            // every Z of this group is written: the workers form the cross terms and the outputs
+      }
       // ---- a7: eq. 3 and stores ----
+      if constexpr (!POLY)
       for (int sl = ctid; sl < ns; sl += NCT) {
         long long ev = ev0 + sl;
         if (ev < nev) {
@@ -944,6 +1034,61 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
       bar_sync(BAR_COLOUR, NCT);
     }
   }
+}
+
+// ------------------------------------------------------------------------------------------------ polynomial mode (host)
+// PAPER.md:87 step 7 / PAPER.md:117 (run time against the number of parameter sets); "each extra coupling-only set
+// costs one more J accumulation + one quadratic form, no new wavefunctions".  With summed currents the route to that is exact
+// interpolation: for fixed g_s and m_t every J_sigma is a polynomial in (x, y) = (ggg_scale, gggg_scale) with the monomials
+// x^a y^b, a + 2 b <= n - 1 (a three-gluon vertices, b four-gluon vertices of a diagram), and alpha_s is an overall
+// factor g_s^(n-1).  Let P[k][m] be the monomials at the requested sets.  Its rank r is the number of sets that have to be evaluated:
+// r rows ("node sets", chosen among the requested ones by complete pivoting) span the row space, every other set is an exact linear
+// combination P[k] = sum_j cw[k][j] P[node_j], hence J(set k) = (g_k/g_0)^(n-1) sum_j cw[k][j] J(node_j) for every sigma and helicity.
+// The colour form is quadratic in J, so the kernel keeps the r (r + 1) / 2 cross forms Q_jj' = sum_h Re(J_j^+ C J_j') of an event and
+// every parameter set costs r (r + 1) / 2 multiply-adds.  Used when all sets share m_t, n >= 4, and r <= BG_RMAX is smaller than
+// the number of sets.  A set equal to the old one has the same weights and factor as the old one: W' = W bitwise.
+static bool bg_plan_poly(int n, const rwgt_params* sets, int nsets, BgDev& D) {
+  D.poly = 0; D.nnode = 0;
+  if (n < 4 || nsets < 3) return false;
+  for (int k = 1; k < nsets; k++) if (sets[k].mt != sets[0].mt) return false;
+  std::vector<std::pair<int, int>> mono;
+  for (int b = 0; 2 * b <= n - 1; b++) for (int a = 0; a + 2 * b <= n - 1; a++) mono.push_back({a, b});
+  const int M = (int)mono.size();
+  std::vector<std::vector<long double>> P(nsets, std::vector<long double>(M));
+  for (int k = 0; k < nsets; k++) for (int m = 0; m < M; m++) P[k][m] = std::pow((long double)sets[k].ggg_scale, mono[m].first) * std::pow((long double)sets[k].gggg_scale, mono[m].second);
+  // complete pivoting: rows = sets, columns = monomials
+  std::vector<std::vector<long double>> Wk = P; std::vector<int> rows, cols; std::vector<bool> rused(nsets, false), cused(M, false);
+  long double scale = 0; for (auto& r : P) for (auto v : r) scale = std::max(scale, std::fabs(v));
+  for (int step = 0; step < std::min(nsets, M); step++) {
+    int br = -1, bc = -1; long double best = 0;
+    for (int k = 0; k < nsets; k++) if (!rused[k]) for (int m = 0; m < M; m++) if (!cused[m] && std::fabs(Wk[k][m]) > best) { best = std::fabs(Wk[k][m]); br = k; bc = m; }
+    if (br < 0 || best < 1e-9L * scale) break;
+    rused[br] = true; cused[bc] = true; rows.push_back(br); cols.push_back(bc);
+    for (int k = 0; k < nsets; k++) if (!rused[k]) { long double f = Wk[k][bc] / Wk[br][bc]; for (int m = 0; m < M; m++) Wk[k][m] -= f * Wk[br][m]; }
+  }
+  const int r = (int)rows.size();
+  if (r > BG_RMAX || r >= nsets) return false;
+  std::sort(rows.begin(), rows.end());
+  // weights: cw[k] B = P[k][cols], B[j][s] = P[node_j][col_s]  (transposed system, Gaussian elimination with partial pivoting)
+  for (int k = 0; k < nsets; k++) {
+    long double A[BG_RMAX][BG_RMAX + 1];
+    for (int s2 = 0; s2 < r; s2++) { for (int j = 0; j < r; j++) A[s2][j] = P[rows[j]][cols[s2]]; A[s2][r] = P[k][cols[s2]]; }
+    for (int c0 = 0; c0 < r; c0++) {
+      int pv = c0; for (int i = c0 + 1; i < r; i++) if (std::fabs(A[i][c0]) > std::fabs(A[pv][c0])) pv = i;
+      if (A[pv][c0] == 0) return false;
+      if (pv != c0) for (int j = 0; j <= r; j++) std::swap(A[pv][j], A[c0][j]);
+      for (int i = 0; i < r; i++) if (i != c0) { long double f = A[i][c0] / A[c0][c0]; for (int j = c0; j <= r; j++) A[i][j] -= f * A[c0][j]; }
+    }
+    long double wsum = 0;
+    for (int j = 0; j < BG_RMAX; j++) { D.cw[k][j] = j < r ? (double)(A[j][r] / A[j][j]) : 0.0; wsum += std::fabs((long double)D.cw[k][j]); }
+    // exactness on EVERY monomial (the rank argument), and no blow-up of rounding errors
+    for (int m = 0; m < M; m++) { long double v = 0; for (int j = 0; j < r; j++) v += (long double)D.cw[k][j] * P[rows[j]][m]; if (std::fabs(v - P[k][m]) > 1e-13L * scale * (1 + wsum)) return false; }
+    if (wsum > 50) return false;
+  }
+  const double gs0 = std::sqrt(4.0 * 3.14159265358979323846 * sets[0].alpha_s);
+  for (int j = 0; j < r; j++) { D.node[j].gq = gs0; D.node[j].g3 = gs0 * sets[rows[j]].ggg_scale; D.node[j].g4 = gs0 * gs0 * sets[rows[j]].gggg_scale; D.node[j].mt = sets[0].mt; D.node[j].fac = 0; }
+  D.poly = 1; D.nnode = r;
+  return true;
 }
 
 // ------------------------------------------------------------------------------------------------ host API of the engine
@@ -987,19 +1132,31 @@ template <int N> static cudaError_t bg_set_attr(size_t s64, size_t s32) {
   cudaError_t e = cudaFuncSetAttribute(bg_kernel<N, double, 0, Cd::NW, Cd::NCW, Cd::CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s64);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, 1, Cf::NW, Cf::NCW, Cf::CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, 2, Cf::NW, Cf::NCW, Cf::CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
+  if constexpr (N >= 4) {
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, double, 0, Cd::NW, Cd::NCW, Cd::CTAS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s64);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, 1, Cf::NW, Cf::NCW, Cf::CTAS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(bg_kernel<N, float, 2, Cf::NW, Cf::NCW, Cf::CTAS, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s32);
+  }
   return e;
 }
 template <int N> static void bg_launch(int precision, int grid, size_t s64, size_t s32, cudaStream_t st, const double* mom, const double* w,
                                        double* a, double* b, double* o, long long nev, long long stride, long long ostride, const BgDev& D) {
   typedef BgCfg<N, double> Cd; typedef BgCfg<N, float> Cf;
+  if constexpr (N >= 4) if (D.poly) {
+    if (precision == RWGT_FP64) bg_kernel<N, double, 0, Cd::NW, Cd::NCW, Cd::CTAS, true><<<grid, (Cd::NW + Cd::NCW) * 32, s64, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
+    else if (precision == RWGT_FP32) bg_kernel<N, float, 1, Cf::NW, Cf::NCW, Cf::CTAS, true><<<grid, (Cf::NW + Cf::NCW) * 32, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
+    else bg_kernel<N, float, 2, Cf::NW, Cf::NCW, Cf::CTAS, true><<<grid, (Cf::NW + Cf::NCW) * 32, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
+    return;
+  }
   if (precision == RWGT_FP64) bg_kernel<N, double, 0, Cd::NW, Cd::NCW, Cd::CTAS><<<grid, (Cd::NW + Cd::NCW) * 32, s64, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
   else if (precision == RWGT_FP32) bg_kernel<N, float, 1, Cf::NW, Cf::NCW, Cf::CTAS><<<grid, (Cf::NW + Cf::NCW) * 32, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
   else bg_kernel<N, float, 2, Cf::NW, Cf::NCW, Cf::CTAS><<<grid, (Cf::NW + Cf::NCW) * 32, s32, st>>>(mom, w, a, b, o, nev, stride, ostride, D);
 }
 
+static size_t bg_zel(int n) { return n == 5 ? (size_t)Geo<5>::NBATCH * Geo<5>::U * 2 * Geo<5>::NT * 64 : (size_t)Geo<4>::NBATCH * Geo<4>::U * 2 * Geo<4>::NT * 64; }
 static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::string& err) {
   BgProcess* B = new BgProcess();
-  B->d_words = nullptr; B->d_lfrag = nullptr;
+  B->d_words = nullptr; B->d_lfrag = nullptr; B->d_poly = nullptr;
   B->S = build_schedule(n, err);
   if (!err.empty()) { delete B; return nullptr; }
   const BgSched& S = B->S;
@@ -1022,6 +1179,12 @@ static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::stri
     D.set[k].fac = 2.0 * gs * gs / (256.0 * fact);
     if (sets[k].mt != sets[0].mt) D.shared_ext = 0;     // externals, momentum sums and denominators are then redone per set
   }
+  D.poly_scratch = nullptr; D.poly_stride = 0;
+  if (bg_plan_poly(n, sets, nsets, D)) {
+    // node currents carry the OLD set's g_s; a set's own alpha_s is the overall factor (g_k / g_0)^(2 (n - 1)) of its colour form
+    const double gs0 = D.node[0].gq;
+    for (int k = 0; k < nsets; k++) D.set[k].fac *= std::pow(D.set[k].gq / gs0, 2.0 * (n - 1));
+  }
   int dev = 0; cudaGetDevice(&dev); cudaDeviceProp prop; cudaGetDeviceProperties(&prop, dev);
   B->sm_count = prop.multiProcessorCount; size_t maxsm = prop.sharedMemPerBlockOptin;
   // event slots per CTA: as many as make the amplitude phase fill the 256 worker threads (npair * 4 tasks per slot and batch)
@@ -1041,11 +1204,17 @@ static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::stri
   if (e == cudaSuccess) e = cudaMemcpy(B->d_lfrag, S.lfrag.data(), S.lfrag.size() * sizeof(double), cudaMemcpyHostToDevice);
   if (e == cudaSuccess) switch (n) { case 2: e = bg_set_attr<2>(B->smem64, B->smem32); break; case 3: e = bg_set_attr<3>(B->smem64, B->smem32); break;
                                      case 4: e = bg_set_attr<4>(B->smem64, B->smem32); break; default: e = bg_set_attr<5>(B->smem64, B->smem32); }
-  if (e != cudaSuccess) { err = std::string("CUDA: ") + cudaGetErrorString(e); cudaFree(B->d_words); cudaFree(B->d_lfrag); delete B; return nullptr; }
+  if (e == cudaSuccess && D.poly) {
+    // scratch of the polynomial mode: per CTA nnode x slots x (NBATCH x U x 2 x NT x 64) doubles
+    auto elems = [&](bool dbl) { return (size_t)D.nnode * (dbl ? B->nslot64 : B->nslot32) * bg_zel(n); };
+    e = cudaMalloc((void**)&B->d_poly, sizeof(double) * std::max(elems(true), elems(false)) * (size_t)B->sm_count * bg_ctas(n));
+    D.poly_scratch = B->d_poly;
+  }
+  if (e != cudaSuccess) { err = std::string("CUDA: ") + cudaGetErrorString(e); cudaFree(B->d_words); cudaFree(B->d_lfrag); cudaFree(B->d_poly); delete B; return nullptr; }
   D.words = B->d_words; D.lfrag = B->d_lfrag;
   return B;
 }
-static void bg_destroy(BgProcess* B) { if (!B) return; cudaFree(B->d_words); cudaFree(B->d_lfrag); delete B; }
+static void bg_destroy(BgProcess* B) { if (!B) return; cudaFree(B->d_words); cudaFree(B->d_lfrag); cudaFree(B->d_poly); delete B; }
 
 // Algorithmic flop count of the schedule on the FP64 (or FP32) FMA pipe, all parameter sets of the handle, per event: FMA = 2 flop,
 // MUL = ADD = 1 flop, per operation of rwgt_math.cuh (L3 74 FMA + 6 MUL + 4 ADD, V4 90 + 6 + 2, slash-accumulate 32 FMA,
@@ -1054,19 +1223,25 @@ static void bg_destroy(BgProcess* B) { if (!B) return; cudaFree(B->d_words); cud
 static double bg_flops_per_event(const BgProcess* B, int /*precision*/) {
   const int n = B->S.n; const double fl[8] = {158, 188, 64, 8, 71, 32, 32, 16};
   double fp = 0; for (int k = 0; k < 8; k++) fp += B->S.fp_ops[k] * fl[k];
-  return B->D.nsets * fp + (B->D.shared_ext ? 1 : B->D.nsets) * (n * 2 * 30.0 + 4 * 40.0 + (1 << n) * 40.0);
+  const int neval = B->D.poly ? B->D.nnode : B->D.nsets;      // polynomial mode: the currents are evaluated at the node sets only
+  return neval * fp + (B->D.shared_ext ? 1 : B->D.nsets) * (n * 2 * 30.0 + 4 * 40.0 + (1 << n) * 40.0);
 }
 // Algorithmic flops of the colour form |L+^T u|^2 + |L-^T v|^2 (a5), all parameter sets: per evaluated helicity (2^(n+1) after
 // parity) each of the two reflection blocks (size nh = n!/2) costs nh (nh + 1) / 2 FMAs for the real and for the imaginary part,
 // plus 2 nh FMAs for the sum of squares.  They run as mma.m8n8k4 (DMMA) on the FP64 pipe, which DFMA and DMMA share on B200 (include/rwgt_microbench.h, kind 7).
 static double bg_tensor_flops_per_event(const BgProcess* B) {
   const int n = B->S.n; const double nh = B->S.npair, nhel = (double)(1 << (n + 1));
+  if (B->D.poly) {       // Z = L^T J per node set, then r (r + 1) / 2 cross products instead of r squares
+    const double r = B->D.nnode;
+    return nhel * 2.0 * (r * 2.0 * (nh * (nh + 1) / 2) + r * (r + 1) / 2 * 2.0 * nh) * 2.0;
+  }
   return B->D.nsets * nhel * 2.0 * (2.0 * (nh * (nh + 1) / 2) + 2.0 * nh) * 2.0;     // two reflection blocks of size n!/2
 }
 
 static int bg_run(BgProcess* B, int precision, const double* mom, const double* w, const int* idx, double* a, double* b, double* o, long long nev, long long stride, long long ostride, cudaStream_t st) {
   BgDev D = B->D; D.idx = idx; const bool dbl = (precision == RWGT_FP64);
   D.nslot = dbl ? B->nslot64 : B->nslot32;
+  if (D.poly) D.poly_stride = (long long)D.nnode * D.nslot * bg_zel(B->S.n);
   long long ngroups = (nev + D.nslot - 1) / D.nslot; int grid = (int)std::min<long long>(ngroups, (long long)B->sm_count * bg_ctas(B->S.n));
   switch (B->S.n) {
     case 2: bg_launch<2>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, ostride, D); break;

@@ -65,27 +65,79 @@ def test_multi_set_with_different_top_masses(idx, n):
 
 
 def test_multi_set_matches_single_set_calls_bitwise_and_max_sets():
-    """K sets in one pass give bit-identical numbers to K separate (old, new_k) handles; K = RWGT_MAX_SETS works,
-    K = RWGT_MAX_SETS + 1 is refused."""
+    """K sets in one pass (evaluated set by set: four generic sets of n = 4 have rank 5, no saving) give bit-identical numbers to K
+    separate (old, new_k) handles; K = RWGT_MAX_SETS works, K = RWGT_MAX_SETS + 1 is refused."""
     c = ev.config(4)
-    kappas = np.linspace(-0.3, 0.45, B.RWGT_MAX_SETS)
-    sets = [ev.params(ggg_scale=1 + k, gggg_scale=1 + k) for k in kappas]
+    sets = [ev.params(ggg_scale=1.1, gggg_scale=0.9), ev.params(ggg_scale=0.8, gggg_scale=1.3), ev.params(ggg_scale=1.4, gggg_scale=1.05),
+            ev.params(ggg_scale=0.6, gggg_scale=0.7)]
     m, w = ev.generate(c, 57)
     got = run_multi(c, sets, m, w)
     K = len(sets)
     dm, dw = torch.from_numpy(m).cuda(), torch.from_numpy(w).cuda()
-    for k in (0, 7, K - 1):
+    for k in range(K):
         r = B.Reweighter(c.process, c.params_old, sets[k])
         one = r.run(dm, dw).cpu().numpy()
         r.close()
         assert np.array_equal(one[0], got[0]) and np.array_equal(one[1], got[1 + k]) and np.array_equal(one[2], got[1 + K + k])
+    many = [ev.params(ggg_scale=1 + k, gggg_scale=1 + k) for k in np.linspace(-0.3, 0.45, B.RWGT_MAX_SETS)]
+    assert run_multi(c, many, m, w).shape == (1 + 2 * B.RWGT_MAX_SETS, 57)
     with pytest.raises(RuntimeError, match="RWGT_MAX_SETS"):
-        B.rwgt_create_multi(c.process, c.params_old, sets + [sets[0]])
+        B.rwgt_create_multi(c.process, c.params_old, many + [many[0]])
     h = B.rwgt_create_multi(c.process, c.params_old, sets[:3])
     assert B.rwgt_n_sets(h) == 3
     with pytest.raises(RuntimeError, match="rwgt_run_multi"):
         B.rwgt_run(h, 1, 1, 1, 1, 1, 5)              # single-set entry point refuses a multi-set handle
     B.rwgt_destroy(h)
+
+
+def poly_sets(kind, K):
+    if kind == "diagonal":         # the bench's Fig. 3 axis: ggg = gggg = 1 + kappa_k
+        return [ev.params(ggg_scale=1 + 0.1 * (k + 1) / K, gggg_scale=1 + 0.1 * (k + 1) / K) for k in range(K)]
+    rng = np.random.default_rng(K)
+    if kind == "general":          # both scales independent, alpha_s too
+        return [ev.params(ggg_scale=float(x), gggg_scale=float(y), alpha_s=float(a)) for x, y, a in
+                zip(rng.uniform(0.7, 1.3, K), rng.uniform(0.7, 1.3, K), rng.uniform(0.10, 0.13, K))]
+    return [ev.params(ggg_scale=float(x), alpha_s=float(a)) for x, a in zip(rng.uniform(0.5, 1.5, K), rng.uniform(0.10, 0.13, K))]   # ggg only
+
+
+@pytest.mark.parametrize("idx,n,kind,K,precision", [(4, 41, "diagonal", 15, "fp64"), (4, 23, "general", 12, "fp64"), (4, 23, "ggg", 9, "fp64"),
+                                                    (5, 5, "diagonal", 15, "fp64"), (5, 3, "ggg", 7, "fp64"), (4, 41, "diagonal", 15, "fp32"),
+                                                    (5, 5, "diagonal", 15, "mixed")])
+def test_coupling_only_sets_polynomial_mode_against_oracle(idx, n, kind, K, precision):
+    """sets that differ only in ggg_scale / gggg_scale / alpha_s are exact linear combinations of a few node sets (the
+    amplitudes are polynomials in the two scales); every set against the oracle's own full evaluation of that set; a set
+    equal to the old one gives W' = W bitwise (same weights, same factor)."""
+    c = ev.config(idx)
+    sets = poly_sets(kind, K)
+    sets.insert(3, c.params_old.copy())
+    K += 1
+    m, w = ev.generate(c, n)
+    got = run_multi(c, sets, m, w, precision)
+    tmax, tmed = (TOL64, TOL64) if precision == "fp64" else (1e-4, 1e-6 if n > 20 else 1e-5)
+    for k, pn in enumerate(sets):
+        a, b, wn, _ = orc.reweight(c.process, c.params_old, pn, m, w)
+        for g, ref in ((got[0], a), (got[1 + k], b), (got[1 + K + k], wn)):
+            e = rel(g, ref)
+            assert e.max() < tmax and np.median(e) < tmed, (kind, k, e.max(), np.median(e))
+    assert np.array_equal(got[1 + 3], got[0]) and np.array_equal(got[1 + K + 3], w)
+
+
+def test_polynomial_mode_is_deterministic_and_costs_less_than_a_loop():
+    """rwgt_flops_per_event reflects the mode: 16 diagonal sets of n = 5 need five node evaluations (degree n - 1 in kappa), not 17."""
+    c = ev.config(5)
+    h1 = B.rwgt_create(c.process, c.params_old, c.params_new)
+    h16 = B.rwgt_create_multi(c.process, c.params_old, poly_sets("diagonal", 16))
+    f1, f16 = B.rwgt_flops_per_event(h1), B.rwgt_flops_per_event(h16)
+    assert 2.3 < f16 / f1 < 2.7                      # 5 evaluations against 2
+    B.rwgt_destroy(h1)
+    B.rwgt_destroy(h16)
+    m, w = ev.generate(c, 301)
+    r = B.Reweighter(c.process, c.params_old, poly_sets("diagonal", 16))
+    dm, dw = torch.from_numpy(m).cuda(), torch.from_numpy(w).cuda()
+    ref = r.run(dm, dw).clone()
+    for _ in range(3):
+        assert torch.equal(r.run(dm, dw), ref)
+    r.close()
 
 
 @pytest.mark.parametrize("precision", ["fp32", "mixed"])
