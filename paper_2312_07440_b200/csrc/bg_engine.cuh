@@ -33,6 +33,10 @@
 #include "../../include/rwgt.h"
 #include "rwgt_math.cuh"
 
+#ifndef RWGT_NBUF_N3
+#define RWGT_NBUF_N3 1
+#endif
+
 namespace rwgt {
 
 // ------------------------------------------------------------------------------------------------ host: colour matrix
@@ -166,6 +170,11 @@ template <int N> struct Geo {
   static constexpr int KSH = MTH * KTH - MTH * (MTH - 1);                // k-steps of one half (upper-triangular tiles)
   static constexpr int NT = 2 * NCOL / 8;                                // mma n-tiles per batch
   static constexpr int NMASK = 1 << N;
+  // amplitude buffers: two (the colour warps work on one batch while the workers fill the next); n = 3 in FP64 has one batch per
+  // parameter set and a colour form that is shorter than the next set's current levels, so ONE buffer costs nothing there and its space
+  // goes into event slots (21 -> 32 slots, which is what 12 worker warps need for a full round of amplitude tasks): 4.65 -> 4.22 ms.
+  // (FP32: the float levels are shorter than the double colour form, one buffer is slower: 2.45 -> 2.55 ms.)
+  template <typename TA> __host__ __device__ static constexpr int nbuf() { return (N == 3 && sizeof(TA) == 8 && RWGT_NBUF_N3 == 1) ? 1 : 2; }
   static constexpr int NPHASE = (N - 1 > (RMAX > LMAX ? RMAX : LMAX) + 1) ? N - 1 : (RMAX > LMAX ? RMAX : LMAX) + 1;
   static constexpr int NL3 = N - 1, NV4 = (N - 1) * (N - 2) / 2;
   static constexpr int JW = pad4(2 * NL3 + 3 * NV4);                     // words of the n-gluon current's references
@@ -388,7 +397,7 @@ template <typename T> struct Smem {
 template <int N, typename T> __host__ __device__ inline size_t carve(Smem<T>& s, unsigned char* base, int ns, int nwords) {
   typedef Geo<N> Ge; size_t off = 0; constexpr int nG = Ge::NG, nR = Ge::NR, nL = Ge::NL;
   auto al = [&]() { off = (off + 15) / 16 * 16; };
-  s.A = (T*)(base + off); off += sizeof(T) * 2 * (size_t)ns * Ge::template abuf<T>(); al();
+  s.A = (T*)(base + off); off += sizeof(T) * Ge::template nbuf<T>() * (size_t)ns * Ge::template abuf<T>(); al();
   s.LF = (double*)(base + off); off += sizeof(double) * 2 * Ge::KSH * 32; al();
   s.pm = (double*)(base + off); off += sizeof(double) * ns * (N + 2) * 4; al();
   s.acc = (double*)(base + off); off += sizeof(double) * ns * BG_NSMAX; al();
@@ -740,8 +749,8 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
   constexpr int next = N + 2, nG = Ge::NG, nR = Ge::NR, nL = Ge::NL; const int ns = D.nslot;
   const long long ngroups = (nev + ns - 1) / ns;
   // once per CTA: zero both amplitude buffers (their padding rows are never written again)
-  constexpr int ASTR = Ge::template astr<T>(); constexpr size_t ABUF = Ge::template abuf<T>();
-  for (int t = threadIdx.x; t < 2 * ns * (int)ABUF; t += NTH) s.A[t] = T(0);
+  constexpr int ASTR = Ge::template astr<T>(), NBUF = Ge::template nbuf<T>(); constexpr size_t ABUF = Ge::template abuf<T>();
+  for (int t = threadIdx.x; t < NBUF * ns * (int)ABUF; t += NTH) s.A[t] = T(0);
   for (int t = threadIdx.x; t < 2 * Ge::KSH * 32; t += NTH) s.LF[t] = __ldg(D.lfrag + t);
   __syncthreads();
   if (threadIdx.x < NWT) {
@@ -790,8 +799,8 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
         // ---- a3/a4: colour-flow amplitudes, one helicity batch per buffer hand-over ----
 #pragma unroll 1
         for (int batch = 0; batch < Ge::NBATCH; batch++, step++) {
-          const int buf = step & 1;
-          if (step >= 2) bar_sync(BAR_EMPTY0 + buf, NTH);      // colour warps have finished reading this buffer
+          const int buf = step % NBUF;
+          if (step >= NBUF) bar_sync(BAR_EMPTY0 + buf, NTH);      // colour warps have finished reading this buffer
           T* Abuf = s.A + (size_t)buf * ns * ABUF;
           constexpr int per = Ge::NPAIR * Ge::NFREE;
           for (int t = tid; t < ns * per; t += NWT) {
@@ -924,7 +933,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
       for (int iset = 0; iset < neval; iset++) {
 #pragma unroll 1
         for (int batch = 0; batch < Ge::NBATCH; batch++, step++) {
-          const int buf = step & 1;
+          const int buf = step % NBUF;
           bar_sync(BAR_FULL0 + buf, NTH);                      // the workers have filled this buffer
           const T* Abuf = s.A + (size_t)buf * ns * ABUF;
           // a5: Z = L^T A with FP64 tensor-core mma over the upper-triangular tiles, colour form = sum of squares of Z
@@ -1115,7 +1124,7 @@ static size_t smem_need_n(int n, const BgSched& S, int nslot, bool dbl) {
 #define RWGT_NW32_N3 12
 #endif
 #ifndef RWGT_NW64_N3
-#define RWGT_NW64_N3 8
+#define RWGT_NW64_N3 12
 #endif
 #ifndef RWGT_NW32_N5
 #define RWGT_NW32_N5 8
