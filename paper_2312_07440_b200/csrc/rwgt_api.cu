@@ -235,7 +235,7 @@ static int launch_events(rwgt_handle* h, const double* momenta, const double* we
     int bs = 256; long long nb = (n + bs - 1) / bs;
     rwgt::epem_mupmum_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->epem);
   } else if (h->proc == P_GG_TTX) {
-    int bs = 128; long long nb = (n + bs - 1) / bs;
+    int bs = h->nsets == 2 ? rwgt::GGTTX_BS : 128; long long nb = (n + bs - 1) / bs;
     if (h->nsets == 2) rwgt::gg_ttx_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, idx, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->ggttx);
     else rwgt::gg_ttx_multi_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, idx, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->ggttx);
   } else if (h->proc == P_QQ) {
