@@ -712,6 +712,19 @@ __device__ __forceinline__ void group_externals(int t0, int nth, int ns, long lo
   }
 }
 
+// B-fragment operands of one k-step for all NT n-tiles of a lane.  The colour form is a sum of squares over all columns, so the
+// assignment of amplitude columns to (n-tile, lane) is free: FP32 amplitude buffers give lane group n = lane >> 2 the NT = 4 ADJACENT
+// columns 4 n .. 4 n + 3 (one LDS.128, conflict-free with the row stride of astr()); FP64 buffers keep columns n + 8 nt (four
+// conflict-free LDS.64; two LDS.128 would conflict two ways).  bfrag_off() is the lane's column offset, ldB() the loads.
+template <typename T, int NT> __device__ __forceinline__ constexpr bool bfrag_vec() { return sizeof(T) == 4 && NT == 4; }
+template <typename T, int NT> __device__ __forceinline__ int bfrag_off(int lane) { return bfrag_vec<T, NT>() ? (lane >> 2) * NT : (lane >> 2); }
+template <typename T, int NT> __device__ __forceinline__ void ldB(T* b, const T* p) {
+  if constexpr (bfrag_vec<T, NT>()) { const float4 v = *reinterpret_cast<const float4*>(p); b[0] = v.x; b[1] = v.y; b[2] = v.z; b[3] = v.w; }
+  else {
+#pragma unroll
+    for (int nt = 0; nt < NT; nt++) b[nt] = p[8 * nt];
+  }
+}
 __device__ __forceinline__ void dmma884(double& c0, double& c1, double a, double b) {
   asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
@@ -946,11 +959,11 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
 #pragma unroll
               for (int j = 0; j < UB; j++) {
                 const int u = (u0 + j < ns * 2) ? u0 + j : ns * 2 - 1, sl = u >> 1, h = u & 1;
-                const T* A = Abuf + (size_t)sl * ABUF + (size_t)(h * Ge::NHK + (lane & 3)) * ASTR + (lane >> 2);
+                const T* A = Abuf + (size_t)sl * ABUF + (size_t)(h * Ge::NHK + (lane & 3)) * ASTR + bfrag_off<T, Ge::NT>(lane);
                 const double a = s.LF[h * 32 + lane];
-                double acc[Ge::NT][2];
+                double acc[Ge::NT][2]; T bb[Ge::NT]; ldB<T, Ge::NT>(bb, A);
 #pragma unroll
-                for (int nt = 0; nt < Ge::NT; nt++) { acc[nt][0] = 0.0; acc[nt][1] = 0.0; dmma884(acc[nt][0], acc[nt][1], a, (double)A[8 * nt]); }
+                for (int nt = 0; nt < Ge::NT; nt++) { acc[nt][0] = 0.0; acc[nt][1] = 0.0; dmma884(acc[nt][0], acc[nt][1], a, (double)bb[nt]); }
                 double pj = 0.0;
 #pragma unroll
                 for (int nt = 0; nt < Ge::NT; nt++) { pj = fma(acc[nt][0], acc[nt][0], pj); pj = fma(acc[nt][1], acc[nt][1], pj); }
@@ -966,7 +979,7 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
           } else
           for (int u = cwarp; u < ns * Ge::U; u += NCW) {
             int sl = u / Ge::U, unit = u % Ge::U; const int h = unit / Ge::UH, uu = unit % Ge::UH;     // h: 0 = u rows / L+, 1 = v rows / L-
-            const T* A = Abuf + (size_t)sl * ABUF + (size_t)(h * Ge::NHK + (lane & 3)) * ASTR + (lane >> 2);
+            const T* A = Abuf + (size_t)sl * ABUF + (size_t)(h * Ge::NHK + (lane & 3)) * ASTR + bfrag_off<T, Ge::NT>(lane);
             double part = 0.0;
 #pragma unroll 1
             for (int half = 0; half < 2; half++) {
@@ -980,14 +993,12 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
               const T* Br = A + (size_t)(8 * mt) * ASTR;
               // operands of k-step kk + 1 are fetched from shared memory while the mma of k-step kk issue
               double a_cur = F[0]; T b_cur[Ge::NT];
-#pragma unroll
-              for (int nt = 0; nt < Ge::NT; nt++) b_cur[nt] = Br[8 * nt];
+              ldB<T, Ge::NT>(b_cur, Br);
 #pragma unroll 2
               for (int kk = 0; kk < nk; kk++) {
                 const int kn = (kk + 1 < nk) ? kk + 1 : kk;
                 const double a_nxt = F[kn * 32]; T b_nxt[Ge::NT];
-#pragma unroll
-                for (int nt = 0; nt < Ge::NT; nt++) b_nxt[nt] = Br[(size_t)(4 * kn) * ASTR + 8 * nt];
+                ldB<T, Ge::NT>(b_nxt, Br + (size_t)(4 * kn) * ASTR);
 #pragma unroll
                 for (int nt = 0; nt < Ge::NT; nt++) dmma884(acc[nt][0], acc[nt][1], a_cur, (double)b_cur[nt]);
                 a_cur = a_nxt;
