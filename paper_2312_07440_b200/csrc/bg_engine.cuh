@@ -772,12 +772,33 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
     const int tid = threadIdx.x; c.tid = tid;
     for (int t = tid; t < D.nwords; t += NWT) s.W[t] = __ldg(D.words + t);
     unsigned step = 0;
+    // !STAGE (n <= 3): a1 is software-pipelined by the workers themselves: the momenta of the next group travel from HBM into
+    // registers while this group's levels and amplitudes run (the load latency was 6 % of the workers' time at n = 3)
+    constexpr int NPRE = STAGE ? 1 : (64 * next * 4 + NWT - 1) / NWT;        // at most 64 event slots (bg_create: pick)
+    double pre[NPRE];
+    auto fetch = [&](long long g) {
+#pragma unroll
+      for (int j = 0; j < NPRE; j++) {
+        const int t = tid + j * NWT;
+        if (t < ns * next * 4) { int sl = t % ns, comp = t / ns; long long ev = g * ns + sl; if (ev >= nev) ev = nev - 1;
+          if (D.idx) ev = D.idx[ev];
+          pre[j] = __ldg(mom + (size_t)comp * stride + ev); }
+      }
+    };
+    if constexpr (!STAGE) { if ((long long)blockIdx.x < ngroups) fetch(blockIdx.x); }
     for (long long grp = blockIdx.x; grp < ngroups; grp += gridDim.x) {
       const long long ev0 = grp * ns;
       if constexpr (!STAGE) {
         // ---- a1/a2 by the workers themselves ----
         bar_sync(BAR_WORK, NWT);
-        group_externals<N, T, TK, TE>(tid, NWT, ns, ev0, nev, stride, mom, D.idx, D.set[0].mt, s.pm, s.G, nG, s.R, nR, s.L, nL, s.K, s.iK2, s.dR, s.dL, true,
+#pragma unroll
+        for (int j = 0; j < NPRE; j++) {
+          const int t = tid + j * NWT;
+          if (t < ns * next * 4) { int sl = t % ns, comp = t / ns; s.pm[(sl * next * 4) + comp] = pre[j]; }
+        }
+        bar_sync(BAR_WORK, NWT);
+        if (grp + gridDim.x < ngroups) fetch(grp + gridDim.x);
+        group_externals<N, T, TK, TE>(tid, NWT, ns, ev0, nev, stride, mom, D.idx, D.set[0].mt, s.pm, s.G, nG, s.R, nR, s.L, nL, s.K, s.iK2, s.dR, s.dL, false,
                                   [] { bar_sync(BAR_WORK, NWT); });
       } else {
       // ---- a1/a2 were done for this group by the colour warps (staging buffers): copy them into the tables ----

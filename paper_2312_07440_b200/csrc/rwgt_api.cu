@@ -118,6 +118,7 @@ rwgt_handle* rwgt_create_multi(const char* process, const rwgt_params* params_ol
   h->nsets = 1 + n_new; h->sets[0] = *params_old;
   for (int k = 0; k < n_new; k++) h->sets[1 + k] = params_new[k];
   cudaGetDevice(&h->device);
+  { int sms = 0; cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, h->device); h->sm_count = sms > 0 ? sms : 1; }
   std::string p(process);
   // "@bg" suffix routes gg_ttx through the generic ordered-current engine (used by the tests to cross-check it)
   bool force_bg = false;
@@ -156,7 +157,6 @@ rwgt_handle* rwgt_create_multi(const char* process, const rwgt_params* params_ol
     h->proc = P_PHOTONS; h->n_photons = na; h->n_ext = na + 2; h->n_gluons = 0; h->photons.nsets = h->nsets;
     double fact = 1; for (int i = 2; i <= na; i++) fact *= i;
     for (int k = 0; k < h->nsets; k++) h->photons.fac[k] = 2.0 * std::pow(4.0 * PI * h->sets[k].alpha_em, na) / (4.0 * fact);
-    cudaDeviceProp prop; cudaGetDeviceProperties(&prop, h->device); h->sm_count = prop.multiProcessorCount;
     cudaError_t e = rwgt::photon_prepare(na);
     if (e != cudaSuccess) { set_err("rwgt_create: %s", cudaGetErrorString(e)); delete h; return nullptr; }
     return finish_create(h);
@@ -232,7 +232,8 @@ static int launch_events(rwgt_handle* h, const double* momenta, const double* we
                          double* out_w_new, long long n, long long stride, long long ostride, cudaStream_t st, const int* idx = nullptr) {
   if (idx && (h->proc == P_EPEM || h->proc == P_PHOTONS)) { set_err("rwgt_run: this process cannot be part of a multiprocess handle"); return -1; }
   if (h->proc == P_EPEM) {
-    int bs = 256; long long nb = (n + bs - 1) / bs;
+    // small event sets (cfg 1 has 16,384): 64-thread CTAs, so that the grid covers all SMs (256 CTAs instead of 64 on 148 SMs)
+    int bs = (n < 512LL * h->sm_count) ? 64 : 256; long long nb = (n + bs - 1) / bs;
     rwgt::epem_mupmum_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->epem);
   } else if (h->proc == P_GG_TTX) {
     int bs = h->nsets == 2 ? rwgt::GGTTX_BS : 128; long long nb = (n + bs - 1) / bs;
