@@ -395,12 +395,14 @@ def main() -> None:
     max_mhz = clocks.get("sm_max_mhz") or peaks.get("sm_max_mhz") or 1965.0
     peak_tf = alu_peak_tflops(dtype, max_mhz)
     hbm_peak = peaks.get("hbm_gbs", 6650.0)
-    traffic, traffic_build = None, None
+    traffic, traffic_build, ncu_fpe = None, None, None
     try:
         counts = json.load(open(os.path.join(ROOT, "profiles", "counts.json")))
         ent = counts[f"cfg{c.index}_{args.precision}"]
         if n == c.n_events:
             traffic, traffic_build = ent["traffic_bytes"], ent.get("build", counts.get("build"))
+            if dtype == "f64" and ent.get("fp64_vector_flops_per_launch_ncu"):
+                ncu_fpe = ent["fp64_vector_flops_per_launch_ncu"] / n      # executed DFMA x 2 + DMUL + DADD per event, same capture
     except Exception:
         pass
     micro = {}
@@ -422,6 +424,8 @@ def main() -> None:
                 "flops_per_event": res["flops_per_event"] + (res["tensor_flops_per_event"] if dtype == "f64" else 0.0),
                 "flops_per_event_kind": "algorithmic operation count of the schedule (include/rwgt.h rwgt_flops_per_event); FP32/mixed: model only, FFMA2 is not in ncu's FFMA counters",
                 "vector_flops_per_event": res["flops_per_event"], "colour_form_flops_per_event": res["tensor_flops_per_event"],
+                "vector_flops_per_event_ncu": ncu_fpe,
+                "vector_flops_model_over_ncu": (res["flops_per_event"] / ncu_fpe) if ncu_fpe else None,
                 "kernel_ms": kernel_ms,
                 "colour_form_fp64": {"flops_per_event": res["tensor_flops_per_event"],
                                      "achieved_tflops": col_flops / (kernel_ms * 1e-3) / 1e12,

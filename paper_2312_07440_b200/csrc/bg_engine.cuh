@@ -34,7 +34,7 @@
 #include "rwgt_math.cuh"
 
 #ifndef RWGT_NBUF_N3
-#define RWGT_NBUF_N3 1
+#define RWGT_NBUF_N3 2
 #endif
 
 namespace rwgt {
@@ -112,6 +112,7 @@ struct BgSched {
   std::vector<uint32_t> words;
   std::vector<double> lfrag;         // Cholesky factor L^T of the colour matrix in mma-fragment order
   double fp_ops[8];                  // operation counts per event and parameter set: L3, V4, slash, lightcone, prop, rowcol, gstore, gstore2
+  double fp_final[8];                // the part of fp_ops that belongs to the amplitude phase (the rest: current levels)
 };
 
 static int mask_of(const std::vector<int>& t) { int m = 0; for (int x : t) m |= 1 << x; return m; }
@@ -170,10 +171,10 @@ template <int N> struct Geo {
   static constexpr int KSH = MTH * KTH - MTH * (MTH - 1);                // k-steps of one half (upper-triangular tiles)
   static constexpr int NT = 2 * NCOL / 8;                                // mma n-tiles per batch
   static constexpr int NMASK = 1 << N;
-  // amplitude buffers: two (the colour warps work on one batch while the workers fill the next); n = 3 in FP64 has one batch per
-  // parameter set and a colour form that is shorter than the next set's current levels, so ONE buffer costs nothing there and its space
-  // goes into event slots (21 -> 32 slots, which is what 12 worker warps need for a full round of amplitude tasks): 4.65 -> 4.22 ms.
-  // (FP32: the float levels are shorter than the double colour form, one buffer is slower: 2.45 -> 2.55 ms.)
+  // amplitude buffers: two (the colour warps work on one batch while the workers fill the next).  (Round 2, before the fused n = 3 pass:
+  // ONE buffer for n = 3 FP64 put its space into event slots, 21 -> 32, 4.65 -> 4.22 ms with 12 worker warps.  The fused pass writes the
+  // rows of two parameter sets back to back, a single buffer stalls it on the colour form (12 % of the workers' time): two buffers, 8 worker
+  // warps at 224 registers and 21 slots: 3.64 -> 3.32 ms.)
   template <typename TA> __host__ __device__ static constexpr int nbuf() { return (N == 3 && sizeof(TA) == 8 && RWGT_NBUF_N3 == 1) ? 1 : 2; }
   static constexpr int NPHASE = (N - 1 > (RMAX > LMAX ? RMAX : LMAX) + 1) ? N - 1 : (RMAX > LMAX ? RMAX : LMAX) + 1;
   static constexpr int NL3 = N - 1, NV4 = (N - 1) * (N - 2) / 2;
@@ -201,7 +202,7 @@ static BgSched build_schedule(int n, std::string& err) {
   BgSched S; S.n = n;
   for (int k = 0; k < 3; k++) for (int m = 0; m < 6; m++) { S.offD[k][m] = 0; S.ntask[k][m] = 0; }
   for (int m = 0; m < 6; m++) S.offT[m] = 0;
-  for (int k = 0; k < 8; k++) S.fp_ops[k] = 0;
+  for (int k = 0; k < 8; k++) { S.fp_ops[k] = 0; S.fp_final[k] = 0; }
   S.c = (n + 1) / 2; S.lmax = S.c - 1; S.rmax = n - S.c;
   TupleTables T; std::vector<std::vector<int>> tl;
   int nG = 0, nR = 0, nL = 0;
@@ -316,8 +317,9 @@ static BgSched build_schedule(int n, std::string& err) {
   }
   {
     double nf = (double)S.npair * (double)(1 << (n - 1));
-    S.fp_ops[0] += nf * (n - 1); S.fp_ops[1] += nf * ((n - 1) * (n - 2) / 2); S.fp_ops[n > 2 ? 6 : 7] += nf;
-    S.fp_ops[3] += nf * (1 + 2 * (NJ * C - 1)); S.fp_ops[2] += nf * 2 * 2 * NJ * C; S.fp_ops[5] += nf * 2 * NJ * 4;
+    S.fp_final[0] = nf * (n - 1); S.fp_final[1] = nf * ((n - 1) * (n - 2) / 2); S.fp_final[n > 2 ? 6 : 7] = nf;
+    S.fp_final[3] = nf * (1 + 2 * (NJ * C - 1)); S.fp_final[2] = nf * 2 * 2 * NJ * C; S.fp_final[5] = nf * 2 * NJ * 4;
+    for (int k = 0; k < 8; k++) S.fp_ops[k] += S.fp_final[k];
   }
   // Colour form.  C commutes with the reversal s -> rev(s) (a trace and its transpose), so in the basis u_p = J_{s_p} + J_{rev s_p},
   // v_p = J_{s_p} - J_{rev s_p} it is block diagonal: J^dagger C J = u^dagger (C+/2) u + v^dagger (C-/2) v with
@@ -352,6 +354,7 @@ constexpr int BG_NSMAX = 1 + RWGT_MAX_SETS;      // the old set plus up to RWGT_
 constexpr int BG_RMAX = 6;                       // most node sets of the polynomial mode (n = 4 needs at most 6, n = 5 five on the diagonal ggg = gggg)
 struct BgDev {
   int nwords, nslot, shared_ext, nsets;
+  int fuse;              // n = 3, parameter sets of equal top mass: ONE pass over the currents serves all sets, the amplitude phase two sets at a time (QuarkLine3F)
   int offD[3][6], offT[6], offF;
   const uint32_t* words; const double* lfrag;
   BgSet set[BG_NSMAX];
@@ -502,6 +505,13 @@ template <int M, int nG, typename T> struct GluonSum {
         v4<J, K + 1, IDX + 1>(a4, w4, v, G);
       } else v4<J + 1, J + 2, IDX>(a4, w4, v, G);
     }
+  }
+  // the two coupling structures apart: a3 = sum of the L3 terms, a4 = sum of the V4 terms (no coupling applied)
+  static __device__ __forceinline__ void run_split(vec4<T>& a3, vec4<T>& a4, const uint32_t* w, uint32_t v, const cx<T>* G, const T* Kt) {
+#pragma unroll
+    for (int i = 0; i < 4; i++) { a3.c[i] = mk<T>(0, 0); a4.c[i] = mk<T>(0, 0); }
+    l3<1>(a3, w, v, G, Kt);
+    v4<1, 2, 0>(a4, w + 2 * (M - 1), v, G);
   }
   static __device__ __forceinline__ vec4<T> run(const uint32_t* w, uint32_t v, const cx<T>* G, const T* Kt, T g3, T g4) {
     vec4<T> a3, a4;
@@ -655,6 +665,67 @@ template <int N, int WHICH, typename T> struct QuarkLine {
   }
 };
 
+// n = 3, two parameter sets in ONE pass (the amplitude-level form of SURVEY C6's polynomial structure; PAPER.md:87 steps 3-6 for
+// both sets at the price of one).  With the currents of the level phase evaluated at UNIT couplings (gq = g3 = 1) every colour-ordered
+// amplitude of g g -> t tbar g is
+//     J_sigma = gq^2 c0 + gq g3 c1 + g3^2 c2 + g4 c3,
+//     c0 = L(s1) eps-slash(s2) R(s3),   c1 = ubar J-slash(s1 s2) R(s3) + L(s1) J-slash(s2 s3) v,
+//     c2 = -ubar A3-slash v / K^2,      c3 = ubar A4-slash v / K^2      (A3 / A4: the L3 / V4 sums of the three-gluon current),
+// so the four coefficient amplitudes are formed once and each parameter set costs four real-times-complex multiply-adds per amplitude.
+// Acc[s][ht][hb] += sum_m wt[s][m] c_m[ht][hb] for the two sets s; J2 = -A3 / K^2 and J3 = A4 / K^2 are passed in.
+// Reference layout of wq (16-bit): [L(), L(s1), R(s3), R(), block(s1 s2), block(s2), -, block(s2 s3)], as built by build_schedule.
+template <typename T> struct QuarkLine3F {
+  typedef Geo<3> Ge;
+  static constexpr int nG = Ge::NG, nR = Ge::NR, nL = Ge::NL;
+  // Acc[s][ht][.] += wt[s][m] * (X . R_hb) for one top helicity ht
+  static __device__ __forceinline__ void fold(cx<T> (&Acc)[2][2][2], int m, int ht, const spn<T>& X, const spn<T>& Ra, const spn<T>& Rb, const T (&wt)[2][4]) {
+    const cx<T> da = rowcol(X, Ra), db = rowcol(X, Rb);
+#pragma unroll
+    for (int s2 = 0; s2 < 2; s2++) { rfma(Acc[s2][ht][0], wt[s2][m], da); rfma(Acc[s2][ht][1], wt[s2][m], db); }
+  }
+  // X = W a-slash for both top helicities, one after the other (one row spinor live at a time), folded with coefficient m
+  static __device__ __forceinline__ void term(cx<T> (&Acc)[2][2][2], int m, const cx<T>* L, int el, int dl, const lcv<T>& Jl, const spn<T>& Ra, const spn<T>& Rb, const T (&wt)[2][4]) {
+#pragma unroll
+    for (int ht = 0; ht < 2; ht++) {
+      spn<T> X;
+#pragma unroll
+      for (int i = 0; i < 4; i++) X.c[i] = mk<T>(0, 0);
+      row_slash_acc(X, lds4(L, nL, el + ht * dl), Jl);
+      fold(Acc, m, ht, X, Ra, Rb, wt);
+    }
+  }
+  // the term both colour orderings of a pair share: c2, c3 = ubar (three-gluon current) v, J(reversed) = +J for three gluons
+  static __device__ __forceinline__ void common(cx<T> (&Acc)[2][2][2], const uint32_t* wq, const vec4<T>& J2, const vec4<T>& J3, const cx<T>* R, const cx<T>* L, const T (&wt)[2][4]) {
+#pragma unroll
+    for (int s2 = 0; s2 < 2; s2++)
+#pragma unroll
+      for (int a = 0; a < 2; a++)
+#pragma unroll
+        for (int b = 0; b < 2; b++) Acc[s2][a][b] = mk<T>(0, 0);
+    const int el0 = (int)halfw(wq, 0), er3 = (int)halfw(wq, 3);
+    const spn<T> R3a = lds4(R, nR, er3), R3b = lds4(R, nR, er3 + 1);
+    term(Acc, 2, L, el0, 1, lightcone(J2), R3a, R3b, wt);
+    term(Acc, 3, L, el0, 1, lightcone(J3), R3a, R3b, wt);
+  }
+  // c0 and c1 of one colour ordering, added to Acc (which the caller initialises with the common term)
+  static __device__ __forceinline__ void run(cx<T> (&Acc)[2][2][2], const uint32_t* wq, uint32_t v, const cx<T>* G, const cx<T>* R, const cx<T>* L, const T (&wt)[2][4]) {
+    const int el0 = (int)halfw(wq, 0), el1 = (int)halfw(wq, 1) + (int)fieldv<1, 0>(v);
+    {
+      const int er2 = (int)halfw(wq, 2) + (int)fieldv<1, 2>(v);
+      const spn<T> R2a = lds4(R, nR, er2), R2b = lds4(R, nR, er2 + 2);
+      // c0: L(s1) eps-slash(s2) . R(s3)
+      term(Acc, 0, L, el1, 2, lightcone(ld4(G, nG, (int)((halfw(wq, 5) & 0x7fffu) + fieldv<1, 1>(v)))), R2a, R2b, wt);
+      // c1, first part: ubar J-slash(s1 s2) . R(s3)
+      term(Acc, 1, L, el0, 1, lightcone(ld4(G, nG, (int)((halfw(wq, 4) & 0x7fffu) + fieldv<2, 0>(v)))), R2a, R2b, wt);
+    }
+    {   // c1, second part: L(s1) J-slash(s2 s3) . v
+      const int er3 = (int)halfw(wq, 3);
+      const spn<T> R3a = lds4(R, nR, er3), R3b = lds4(R, nR, er3 + 1);
+      term(Acc, 1, L, el1, 2, lightcone(ld4(G, nG, (int)((halfw(wq, 7) & 0x7fffu) + fieldv<2, 1>(v)))), R3a, R3b, wt);
+    }
+  }
+};
+
 // Steps a1 + a2 for one event group, by `nth` threads (index t0): momenta (coalesced over the events of the group) into pm, then
 // external wavefunctions (gluon i, helicity bit hb -> entry 2 i + hb of G; v(p_tbar) -> entries 0,1 of R; ubar(p_t) -> 0,1 of L),
 // momentum sums of the gluon subsets and the inverse propagator denominators.  sG / sR / sL: entries per component plane of the
@@ -774,7 +845,8 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
     unsigned step = 0;
     // !STAGE (n <= 3): a1 is software-pipelined by the workers themselves: the momenta of the next group travel from HBM into
     // registers while this group's levels and amplitudes run (the load latency was 6 % of the workers' time at n = 3)
-    constexpr int NPRE = STAGE ? 1 : (64 * next * 4 + NWT - 1) / NWT;        // at most 64 event slots (bg_create: pick)
+    constexpr int MAXSLOT = (N == 2) ? 64 : NWT / (Ge::NPAIR * 4);           // bg_create: pick
+    constexpr int NPRE = STAGE ? 1 : (MAXSLOT * next * 4 + NWT - 1) / NWT;
     double pre[NPRE];
     auto fetch = [&](long long g) {
 #pragma unroll
@@ -816,7 +888,81 @@ __global__ void __launch_bounds__((NW + NCW) * 32, CTAS) bg_kernel(const double*
       bar_arrive(BAR_STAGE_EMPTY, NTH);                        // the colour warps may stage the next group
       }
       bar_sync(BAR_WORK, NWT);
-      const int neval = POLY ? D.nnode : D.nsets;              // polynomial mode: one evaluation per node set, not per parameter set
+      bool fused = false;
+      if constexpr (N == 3 && !POLY) if (D.fuse) {
+        // ---- n = 3, two sets of equal mass: one pass at unit couplings, four coefficient amplitudes, both sets folded from them ----
+        fused = true;
+        c.g3 = T(1); c.g4 = T(0); c.gq = T(1); c.mt = (T)D.set[0].mt;
+        level_phase<N, 2, T, NWT>(c);
+        constexpr int per = Ge::NPAIR * Ge::NFREE;             // one helicity batch for n = 3; at most one task per thread (bg_create: ns * per <= NWT)
+        const bool live = tid < ns * per;
+        const int sl = live ? tid / per : 0, o = live ? tid - sl * per : 0, pair = o / Ge::NFREE, f = o % Ge::NFREE;
+        const cx<T>* G = s.G + (size_t)sl * 4 * nG; const cx<T>* R = s.R + (size_t)sl * 4 * nR; const cx<T>* L = s.L + (size_t)sl * 4 * nL;
+        const uint32_t* w = s.W + D.offF + pair * Ge::STRIDEF;
+        const uint32_t w0 = w[0], packed = w[1];
+        uint32_t v = 0;
+#pragma unroll
+        for (int j = 0; j < N; j++) v |= ((((uint32_t)f << 1) >> ((packed >> (3 * j)) & 7u)) & 1u) << j;   // helicity bits by position; gluon 0: + (parity)
+        // the parameter sets two at a time: the coefficient amplitudes of a chunk are formed once and folded with the chunk's weights
+        // (the split three-gluon current is re-formed per chunk: it is dead after the common term, which keeps 32 registers free)
+#pragma unroll 1
+        for (int k0 = 0; k0 < D.nsets; k0 += 2) {
+          const int nk = (k0 + 1 < D.nsets) ? 2 : 1;
+          T wt[2][4];
+#pragma unroll
+          for (int s2 = 0; s2 < 2; s2++) { const BgSet& P = D.set[k0 + (s2 < nk ? s2 : 0)]; wt[s2][0] = (T)(P.gq * P.gq); wt[s2][1] = (T)(P.gq * P.g3); wt[s2][2] = (T)(P.g3 * P.g3); wt[s2][3] = (T)P.g4; }
+          cx<T> A0[2][2][2], A1[2][2][2];
+          if (live) {
+            {
+              vec4<T> J2, J3;
+              {
+                uint32_t jw[Ge::JW]; ldw<Ge::JW>(jw, w + 4);
+                GluonSum<N, nG, T>::run_split(J2, J3, jw, v, G, s.K + (size_t)sl * Ge::NMASK * 4);
+                const T sc = s.iK2[sl * Ge::NMASK + Ge::NMASK - 1];
+#pragma unroll
+                for (int i = 0; i < 4; i++) { J2.c[i] = (-sc) * J2.c[i]; J3.c[i] = sc * J3.c[i]; }
+              }
+              uint32_t wq[Ge::QW]; ldw<Ge::QW>(wq, w + 4 + Ge::JW);
+              QuarkLine3F<T>::common(A0, wq, J2, J3, R, L, wt);  // the same for the ordering and its reversal
+#pragma unroll
+              for (int s2 = 0; s2 < 2; s2++)
+#pragma unroll
+                for (int a = 0; a < 2; a++)
+#pragma unroll
+                  for (int b = 0; b < 2; b++) A1[s2][a][b] = A0[s2][a][b];
+              QuarkLine3F<T>::run(A0, wq, v, G, R, L, wt);
+            }
+            {
+              uint32_t wq[Ge::QW]; ldw<Ge::QW>(wq, w + 4 + Ge::JW + Ge::QW);
+              QuarkLine3F<T>::run(A1, wq, brevm<N>(v), G, R, L, wt);
+            }
+          }
+#pragma unroll
+          for (int s2 = 0; s2 < 2; s2++) {
+            if (s2 < nk) {
+              const int buf = step % NBUF;
+              if (step >= NBUF) bar_sync(BAR_EMPTY0 + buf, NTH);    // colour warps have finished reading this buffer
+              if (live) {
+                T* Au = s.A + (size_t)buf * ns * ABUF + (size_t)sl * ABUF + (size_t)w0 * ASTR; T* Av = Au + (size_t)Ge::NHK * ASTR;
+#pragma unroll
+                for (int ht = 0; ht < 2; ht++)
+#pragma unroll
+                  for (int hb = 0; hb < 2; hb++) {
+                    const int col = f * 4 + ht * 2 + hb;
+                    const double ar = (double)A0[s2][ht][hb].re, ai = (double)A0[s2][ht][hb].im, br = (double)A1[s2][ht][hb].re, bi = (double)A1[s2][ht][hb].im;
+                    stc(reinterpret_cast<cx<T>*>(Au + 2 * col), mk<T>((T)(ar + br), (T)(ai + bi)));
+                    stc(reinterpret_cast<cx<T>*>(Av + 2 * col), mk<T>((T)(ar - br), (T)(ai - bi)));
+                  }
+              }
+              __threadfence_block();
+              bar_arrive(BAR_FULL0 + buf, NTH);                  // hand this set's amplitudes to the colour warps
+              step++;
+            }
+          }
+        }
+        bar_sync(BAR_WORK, NWT);                               // the current tables are rewritten for the next group
+      }
+      const int neval = fused ? 0 : (POLY ? D.nnode : D.nsets);   // polynomial mode: one evaluation per node set, not per parameter set
 #pragma unroll 1
       for (int iset = 0; iset < neval; iset++) {
         const BgSet& P = POLY ? D.node[iset] : D.set[iset];
@@ -1156,7 +1302,7 @@ static size_t smem_need_n(int n, const BgSched& S, int nslot, bool dbl) {
 #define RWGT_NW32_N3 12
 #endif
 #ifndef RWGT_NW64_N3
-#define RWGT_NW64_N3 12
+#define RWGT_NW64_N3 8
 #endif
 #ifndef RWGT_NW32_N5
 #define RWGT_NW32_N5 8
@@ -1221,6 +1367,7 @@ static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::stri
     if (sets[k].mt != sets[0].mt) D.shared_ext = 0;     // externals, momentum sums and denominators are then redone per set
   }
   D.poly_scratch = nullptr; D.poly_stride = 0;
+  D.fuse = (n == 3 && D.shared_ext) ? 1 : 0;
   if (bg_plan_poly(n, sets, nsets, D)) {
     // node currents carry the OLD set's g_s; a set's own alpha_s is the overall factor (g_k / g_0)^(2 (n - 1)) of its colour form
     const double gs0 = D.node[0].gq;
@@ -1264,8 +1411,18 @@ static void bg_destroy(BgProcess* B) { if (!B) return; cudaFree(B->d_words); cud
 static double bg_flops_per_event(const BgProcess* B, int /*precision*/) {
   const int n = B->S.n; const double fl[8] = {158, 188, 64, 8, 71, 32, 32, 16};
   double fp = 0; for (int k = 0; k < 8; k++) fp += B->S.fp_ops[k] * fl[k];
+  const double ext = n * 2 * 30.0 + 4 * 40.0 + (1 << n) * 40.0;
+  if (B->D.fuse) {
+    // n = 3 fused pass: the current levels once; per amplitude thread (pair x gluon helicities) the split three-gluon current
+    // (2 L3 + V4 + two scalings), the term the two orderings of a pair share (2 light-cone forms, 4 row-slash products, 8 row.col products of
+    // 30 flops, 2 folds of 4 amplitudes into 2 sets at 4 flops), per colour ordering 3 / 6 / 12 / 3 of the same, and the u / v rows of both sets
+    double lev = 0; for (int k = 0; k < 8; k++) lev += (B->S.fp_ops[k] - B->S.fp_final[k]) * fl[k];
+    const double nf = (double)B->S.npair * (double)(1 << (n - 1));
+    const double per_thread = 2 * fl[0] + fl[1] + 16.0 + (2 * fl[3] + 4 * fl[2] + 8 * 30.0 + 2 * 2 * 4 * 4.0) + 2.0 * (3 * fl[3] + 6 * fl[2] + 12 * 30.0 + 3 * 2 * 4 * 4.0) + 2 * 4 * 4.0;
+    return lev + ((B->D.nsets + 1) / 2) * nf * per_thread + ext;
+  }
   const int neval = B->D.poly ? B->D.nnode : B->D.nsets;      // polynomial mode: the currents are evaluated at the node sets only
-  return neval * fp + (B->D.shared_ext ? 1 : B->D.nsets) * (n * 2 * 30.0 + 4 * 40.0 + (1 << n) * 40.0);
+  return neval * fp + (B->D.shared_ext ? 1 : B->D.nsets) * ext;
 }
 // Algorithmic flops of the colour form |L+^T u|^2 + |L-^T v|^2 (a5), all parameter sets: per evaluated helicity (2^(n+1) after
 // parity) each of the two reflection blocks (size nh = n!/2) costs nh (nh + 1) / 2 FMAs for the real and for the imaginary part,
