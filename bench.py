@@ -487,7 +487,7 @@ def main() -> None:
         per_config.sort(key=lambda e: (e.get("cfg", 0), e.get("precision", ""), e.get("n", 0)))
         roofline["per_config"] = per_config
         # K new parameter sets in one pass (PAPER.md:87 step 7, Fig. 3 axis): kappa = 0.1 k / K
-        for ci, K in ((2, 8), (4, 8), (5, 4), (5, 16)):
+        for ci, K in ((2, 8), (3, 8), (4, 8), (5, 4), (5, 16)):
             try:
                 cc = ev.config(ci)
                 sets = [ev.params(ggg_scale=1 + 0.1 * (k + 1) / K, gggg_scale=1 + 0.1 * (k + 1) / K) for k in range(K)]

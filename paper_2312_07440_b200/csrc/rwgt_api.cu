@@ -206,13 +206,15 @@ int rwgt_n_external(const rwgt_handle* h) { return h ? h->n_ext : -1; }
 
 double rwgt_flops_per_event(const rwgt_handle* h) {
   if (!h) return -1.0;
-  // the two one-event-per-thread kernels: ncu counters of the committed build (152 DFMA + 105 DMUL + 17 DADD resp.
-  // 1225 DFMA + 365 DMUL + 87 DADD per event; profiles/r1_summary.md)
+  // the two one-event-per-thread kernels: executed counts (2 DFMA + DMUL + DADD thread instructions per event) of an ncu capture; the
+  // current build's capture is in profiles/counts.json (435 and 2,935) and bench.py prints model / ncu beside the roofline, so a stale
+  // constant shows
   if (h->proc == P_EPEM) return 426.0 + (h->nsets - 2) * 45.0;
   if (h->proc == P_PHOTONS) return rwgt::photon_flops_per_event(h->n_photons);
-  // q qbar -> t tbar (g): operation count of qq_kernels.cuh (externals ~300; per gluon helicity b_1, b_2, l ~700; per (gluon, tbar) helicity five
-  // slash chains ~900; per helicity 5 row.col + per set the 4 x 4 colour form ~100)
-  if (h->proc == P_QQ) { const double one = h->n_gluons ? 300.0 + 2 * 700.0 + 4 * 900.0 + 8 * (160.0 + h->nsets * 100.0) : 300.0 + 2 * 64.0 + 4 * 36.0;
+  // q qbar -> t tbar (g): operation count of qq_kernels.cuh (externals ~300; per gluon helicity b_1, b_2, l ~550; per (gluon, tbar) helicity five
+  // slash chains ~700; per helicity 5 row.col ~130 + per set the 4 x 4 colour form ~70), calibrated to the executed count (the compiler folds the
+  // zero components of eps and of the massless spinors): ncu 6,398 flops per event for two sets (profiles/counts.json, cfg8_fp64), 582 without the gluon
+  if (h->proc == P_QQ) { const double one = h->n_gluons ? 300.0 + 2 * 550.0 + 4 * 700.0 + 8 * (130.0 + h->nsets * 70.0) : 300.0 + 2 * 64.0 + 4 * 36.0;
                          return h->qq.two_pass ? h->nsets * one : one; }
   if (h->proc == P_MULTI) { double f = 0; for (int i = 0; i < h->nsub; i++) f += rwgt_flops_per_event(h->sub[i]); return f / h->nsub; }
   // gg_ttx: 2902 for two sets of equal mass; a further set of equal mass costs 8 helicities x (4 FMA + colour form 5 FMA + 4 MUL/ADD)
