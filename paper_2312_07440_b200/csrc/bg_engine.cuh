@@ -747,24 +747,29 @@ __device__ __forceinline__ void group_externals(int t0, int nth, int ns, long lo
     }
     sync();
   }
-  constexpr int nobj = 2 * N + 4 + Ge::NMASK;
+  // objects per slot: N gluons (both helicities each), v (both helicities), ubar (both helicities), the NMASK - 1 non-empty gluon
+  // subsets: n = 3: 12 objects, i.e. ONE round of equally long tasks for 32 slots x 384 threads (round 1: 18 objects, 1.5 rounds, and
+  // the rsqrt chains of a leg done once per helicity)
+  constexpr int nobj = N + 2 + (Ge::NMASK - 1);
   for (int t = t0; t < ns * nobj; t += nth) {
     int o = t / ns, sl = t - o * ns; const double* pm = pmD + sl * next * 4;      // object-major: the lanes of a warp run the same branch
-    if (o < 2 * N) {                         // gluon i, helicity bit hb (0: +1, 1: -1); entry = 2*i + hb
-      int i = o >> 1, hb = o & 1, leg = i < 2 ? i : i + 2; const double* p = pm + 4 * leg;
-      vec4<TE> e = polvec<TE>((TE)p[1], (TE)p[2], (TE)p[3], hb ? -1 : +1);
-      if (i >= 2) e = conj4(e);              // outgoing gluon carries eps*
-      st4cvt<T, TE>(Gd + (size_t)sl * 4 * sG, sG, 2 * i + hb, e);
-    } else if (o < 2 * N + 2) {              // v(p_tbar, lam), R() entries 0,1
-      int hb = o - 2 * N; const double* p = pm + 12;
-      chi_pair<TE> x = make_chi<TE>((TE)p[1], (TE)p[2], (TE)p[3]);
-      st4cvt<T, TE>(Rd + (size_t)sl * 4 * sR, sR, hb, spinor_v<TE>(x, make_shell<TE>((TE)p[0], (TE)mtd), hb ? -1 : +1));
-    } else if (o < 2 * N + 4) {              // ubar(p_t, lam), L() entries 0,1
-      int hb = o - 2 * N - 2; const double* p = pm + 8;
-      chi_pair<TE> x = make_chi<TE>((TE)p[1], (TE)p[2], (TE)p[3]);
-      st4cvt<T, TE>(Ld + (size_t)sl * 4 * sL, sL, hb, bar(spinor_u<TE>(x, make_shell<TE>((TE)p[0], (TE)mtd), hb ? -1 : +1)));
-    } else {                                 // gluon subset `mask`
-      int mask = o - 2 * N - 4;
+    if (o < N) {                             // gluon i, both helicities (bit 0: +1, 1: -1); entries 2 i, 2 i + 1
+      int i = o, leg = i < 2 ? i : i + 2; const double* p = pm + 4 * leg;
+      vec4<TE> ep, em; polvec_pair<TE>((TE)p[1], (TE)p[2], (TE)p[3], ep, em);
+      if (i >= 2) { ep = conj4(ep); em = conj4(em); }              // outgoing gluon carries eps*
+      st4cvt<T, TE>(Gd + (size_t)sl * 4 * sG, sG, 2 * i, ep); st4cvt<T, TE>(Gd + (size_t)sl * 4 * sG, sG, 2 * i + 1, em);
+    } else if (o == N) {                     // v(p_tbar, +-), R() entries 0,1
+      const double* p = pm + 12;
+      chi_pair<TE> x = make_chi<TE>((TE)p[1], (TE)p[2], (TE)p[3]); const shell<TE> sh = make_shell<TE>((TE)p[0], (TE)mtd);
+      st4cvt<T, TE>(Rd + (size_t)sl * 4 * sR, sR, 0, spinor_v<TE>(x, sh, +1)); st4cvt<T, TE>(Rd + (size_t)sl * 4 * sR, sR, 1, spinor_v<TE>(x, sh, -1));
+    } else if (o == N + 1) {                 // ubar(p_t, +-), L() entries 0,1
+      const double* p = pm + 8;
+      chi_pair<TE> x = make_chi<TE>((TE)p[1], (TE)p[2], (TE)p[3]); const shell<TE> sh = make_shell<TE>((TE)p[0], (TE)mtd);
+      st4cvt<T, TE>(Ld + (size_t)sl * 4 * sL, sL, 0, bar(spinor_u<TE>(x, sh, +1))); st4cvt<T, TE>(Ld + (size_t)sl * 4 * sL, sL, 1, bar(spinor_u<TE>(x, sh, -1)));
+    } else {                                 // gluon subset `mask` (the empty subset is never referenced: its entries are zeroed by the last task)
+      int mask = o - (N + 2) + 1;
+      if (mask == Ge::NMASK - 1) { T* K0 = Kd + (size_t)sl * Ge::NMASK * 4; for (int mu = 0; mu < 4; mu++) K0[mu] = T(0);
+        iK2d[sl * Ge::NMASK] = T(0); dRd[sl * Ge::NMASK] = T(0); dLd[sl * Ge::NMASK] = T(0); }
       TK k[4] = {0, 0, 0, 0};
 #pragma unroll
       for (int i = 0; i < N; i++) if (mask >> i & 1) { int leg = i < 2 ? i : i + 2; TK sg = i < 2 ? TK(1) : TK(-1);

@@ -21,7 +21,11 @@ struct EpemParams { EpemSet set[SMALL_NSMAX]; int nsets; };
 
 // Massless leptons: only the 4 helicity combinations with opposite helicities on each fermion line
 // are non-zero (tests check the oracle's full 16-term sum against this, reading Q5).
-__global__ void __launch_bounds__(256, 3) epem_mupmum_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
+#ifndef RWGT_EPEM_BS
+#define RWGT_EPEM_BS 128
+#define RWGT_EPEM_MINB 6
+#endif
+__global__ void __launch_bounds__(RWGT_EPEM_BS, RWGT_EPEM_MINB) epem_mupmum_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
                                                           double* __restrict__ me_old, double* __restrict__ me_new,
                                                           double* __restrict__ w_new, long long n, long long stride, long long ostride, EpemParams P) {
   long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -34,11 +38,13 @@ __global__ void __launch_bounds__(256, 3) epem_mupmum_kernel(const double* __res
   double W = __ldg(wgt + i);
   double q[4] = {p[0][0] + p[1][0], p[0][1] + p[1][1], p[0][2] + p[1][2], p[0][3] + p[1][3]};
   double s = mdot_rr(q, q);
-  chi_pair<double> x1 = make_chi(p[0][1], p[0][2], p[0][3]), x2 = make_chi(p[1][1], p[1][2], p[1][3]);
-  chi_pair<double> x3 = make_chi(p[2][1], p[2][2], p[2][3]), x4 = make_chi(p[3][1], p[3][2], p[3][3]);
+  // unnormalised two-spinors (|chi|^2 = n2): each of the four enters every |amplitude|^2 exactly once, so the four normalisations are
+  // one division at the end instead of four reciprocal square roots
+  chi_pair<double> x1 = make_chi_raw(p[0][1], p[0][2], p[0][3]), x2 = make_chi_raw(p[1][1], p[1][2], p[1][3]);
+  chi_pair<double> x3 = make_chi_raw(p[2][1], p[2][2], p[2][3]), x4 = make_chi_raw(p[3][1], p[3][2], p[3][3]);
   // massless legs: spinor normalisation sqrt(2E), energy from the input and mass parameter 0 (reading Q8 / DESIGN.md R8); the four
   // normalisations enter every |amplitude|^2 as the product of the four 2E: no square root
-  const double nrm = 16.0 * ((p[0][0] * p[1][0]) * (p[2][0] * p[3][0]));
+  const double nrm = 16.0 * ((p[0][0] * p[1][0]) * (p[2][0] * p[3][0])) / ((x1.n2 * x2.n2) * (x3.n2 * x4.n2));
   // electron line vbar(p1) gamma^mu u(p2): L = (lam1,lam2) = (+,-), R = (-,+); muon line ubar(p4) gamma^mu v(p3) likewise.  The four
   // current contractions J_e . J_mu are done by the Fierz identities of the Pauli matrices (sigma^mu = (1, sigma), sigmabar^mu = (1, -sigma)):
   //   (a^+ sigmabar^mu b)(c^+ sigmabar_mu d) = (a^+ sigma^mu b)(c^+ sigma_mu d) = 2 conj(a ^ c) (b ^ d),   x ^ y = x_1 y_2 - x_2 y_1,

@@ -114,14 +114,14 @@ __device__ __forceinline__ void photon_accumulate(cx<double> (&acc)[1 << VB][2],
 }
 
 // One level of the recursion: all currents of K photons (K compile-time: constant divisors, branch-free member loops).
-// VBMAX = 10 * (variants bits per thread at level 2) + (variant bits per thread at the levels above): level 2 has few tasks per event
-// and keeps more threads busy with fewer variants per thread.
+// VBMAX = [100 * (variant bits per thread at levels >= 4)] + 10 * (variant bits at level 2) + (variant bits at level 3 and, without the
+// hundreds digit, above): the levels differ in tasks per event, and fewer variants per thread keep more threads busy.
 // Lanes run event-fastest (a quarter-warp = 8 events x one task): every table access is then the same word of 8 event slots,
 // conflict-free by the odd slot stride, and the task decode is uniform over the quarter-warp.
 template <int NG, int K, int VBMAX, int E, int CG, int NTH>
 __device__ __forceinline__ void photon_level(double* sm, const unsigned char* s_sub, const unsigned short* s_off, const unsigned* s_child, int first_sub, int tid) {
   typedef PhGeo<NG> Ge;
-  constexpr int NENT = Ge::NENT, VBL = (K == 2 ? VBMAX / 10 : VBMAX % 10), VB = K < VBL ? K : VBL, KF = K - VB, NV = 1 << VB, per = binom(NG, K) << KF;
+  constexpr int NENT = Ge::NENT, VBL = (K == 2 ? (VBMAX / 10) % 10 : (K >= 4 && VBMAX >= 100) ? VBMAX / 100 : VBMAX % 10), VB = K < VBL ? K : VBL, KF = K - VB, NV = 1 << VB, per = binom(NG, K) << KF;
   for (int t = tid; t < E * per; t += CG) {
     const int sl = t % E, o = t / E; const int S = s_sub[first_sub + (o >> KF)]; const unsigned vfix = o & ((1u << KF) - 1u);
     double* s = sm + sl * Ge::SLOT;

@@ -207,9 +207,9 @@ int rwgt_n_external(const rwgt_handle* h) { return h ? h->n_ext : -1; }
 double rwgt_flops_per_event(const rwgt_handle* h) {
   if (!h) return -1.0;
   // the two one-event-per-thread kernels: executed counts (2 DFMA + DMUL + DADD thread instructions per event) of an ncu capture; the
-  // current build's capture is in profiles/counts.json (435 and 2,935) and bench.py prints model / ncu beside the roofline, so a stale
+  // current build's capture is in profiles/counts.json (408 and 2,935) and bench.py prints model / ncu beside the roofline, so a stale
   // constant shows
-  if (h->proc == P_EPEM) return 426.0 + (h->nsets - 2) * 45.0;
+  if (h->proc == P_EPEM) return 408.0 + (h->nsets - 2) * 45.0;
   if (h->proc == P_PHOTONS) return rwgt::photon_flops_per_event(h->n_photons);
   // q qbar -> t tbar (g): operation count of qq_kernels.cuh (externals ~300; per gluon helicity b_1, b_2, l ~550; per (gluon, tbar) helicity five
   // slash chains ~700; per helicity 5 row.col ~130 + per set the 4 x 4 colour form ~70), calibrated to the executed count (the compiler folds the
@@ -235,7 +235,7 @@ static int launch_events(rwgt_handle* h, const double* momenta, const double* we
   if (idx && (h->proc == P_EPEM || h->proc == P_PHOTONS)) { set_err("rwgt_run: this process cannot be part of a multiprocess handle"); return -1; }
   if (h->proc == P_EPEM) {
     // small event sets (cfg 1 has 16,384): 64-thread CTAs, so that the grid covers all SMs (256 CTAs instead of 64 on 148 SMs)
-    int bs = (n < 512LL * h->sm_count) ? 64 : 256; long long nb = (n + bs - 1) / bs;
+    int bs = (n < 512LL * h->sm_count) ? 64 : RWGT_EPEM_BS; long long nb = (n + bs - 1) / bs;
     rwgt::epem_mupmum_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->epem);
   } else if (h->proc == P_GG_TTX) {
     int bs = h->nsets == 2 ? rwgt::GGTTX_BS : 128; long long nb = (n + bs - 1) / bs;

@@ -178,6 +178,13 @@ template <typename T> __device__ __forceinline__ vec4<T> polvec(T px, T py, T pz
   vec4<T> r; r.c[0] = mk<T>(0, 0); r.c[1] = mk<T>(-l * s * e1x, -s * e2x); r.c[2] = mk<T>(-l * s * e1y, -s * e2y); r.c[3] = mk<T>(-l * s * e1z, 0);
   return r;
 }
+// both helicities at once: eps(p,-1) differs from eps(p,+1) in the sign of the e1 part only (the rsqrt chain is shared)
+template <typename T> __device__ __forceinline__ void polvec_pair(T px, T py, T pz, vec4<T>& ep, vec4<T>& em) {
+  ep = polvec<T>(px, py, pz, +1);
+  em.c[0] = mk<T>(0, 0);
+#pragma unroll
+  for (int i = 1; i < 4; i++) em.c[i] = mk<T>(-ep.c[i].re, ep.c[i].im);
+}
 template <typename T> __device__ __forceinline__ vec4<T> conj4(const vec4<T>& a) { vec4<T> r; for (int i = 0; i < 4; i++) r.c[i] = conj(a.c[i]); return r; }
 
 // ---- gluon self-interaction Lorentz structures --------------------------------------
