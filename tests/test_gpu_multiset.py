@@ -167,3 +167,24 @@ def test_multi_set_host_path_chunked():
     B.rwgt_run_multi_host(h, m, w, a, b, o)
     B.rwgt_destroy(h)
     assert np.array_equal(a, dev[0]) and np.array_equal(b, dev[1:4]) and np.array_equal(o, dev[4:7])
+
+
+@pytest.mark.parametrize("K", [1, 2, 3, 4, 16])
+@pytest.mark.parametrize("precision", ["fp64", "fp32"])
+def test_gg_ttxg_one_pass_for_all_sets_odd_and_even_counts(K, precision):
+    """gg -> ttbar g evaluates the currents once for all sets of equal mass and folds the coefficient amplitudes two sets at a time
+    (QuarkLine3F): odd and even totals (the last chunk of an odd total holds one set), couplings that differ in
+    alpha_s, ggg and gggg scale separately, against the oracle per set; a set equal to the old one reproduces W bitwise."""
+    c = ev.config(3)
+    rng = np.random.default_rng(300 + K)
+    sets = [ev.params(ggg_scale=float(1 + rng.uniform(-0.4, 0.4)), gggg_scale=float(1 + rng.uniform(-0.4, 0.4)), alpha_s=float(rng.uniform(0.09, 0.14)))
+            for _ in range(K)]
+    sets[K // 2] = c.params_old.copy()
+    n = 413
+    m, w = ev.generate(c, n)
+    got = run_multi(c, sets, m, w, precision)
+    tol = TOL64 if precision == "fp64" else 1e-4
+    for k, pn in enumerate(sets):
+        a, b, wn, _ = orc.reweight(c.process, c.params_old, pn, m, w)
+        assert rel(got[0], a).max() < tol and rel(got[1 + k], b).max() < tol and rel(got[1 + K + k], wn).max() < tol, (K, k)
+    assert np.array_equal(got[1 + K // 2], got[0]) and np.array_equal(got[1 + K + K // 2], w)
