@@ -63,7 +63,9 @@ rwgt_handle* rwgt_create(const char* process, const rwgt_params* params_old, con
 /* Several new parameter sets for the same events in one pass (PAPER.md:87 step 7, "Repeat steps 4 - 6 for all parameter
  * sets"; PAPER.md:91 and Fig. 3: run time against the number of parameter sets).  `params_new` points to n_new sets,
  * 1 <= n_new <= RWGT_MAX_SETS.  The event is loaded and its external wavefunctions, momentum sums and propagator
- * denominators are formed ONCE; each set then costs one more evaluation of the currents and one more colour form.
+ * denominators are formed ONCE; each set then costs at most one more evaluation of the currents and one more colour form
+ * (gg_ttxg: one evaluation serves all sets of equal mass; gg_ttxgg / gg_ttxggg: coupling-only sets beyond the rank of their
+ * coupling polynomials cost a colour-form combination each; epem_a...: a multiplication; gg_ttx: two multiply-adds per helicity).
  * Sets may differ in any field; a differing top mass makes the externals of that set be recomputed.
  * rwgt_create(p, old, new) is rwgt_create_multi(p, old, new, 1).  Same error behaviour as rwgt_create. */
 #define RWGT_MAX_SETS 16
@@ -81,7 +83,10 @@ int rwgt_n_external(const rwgt_handle* h);
 
 /* Algorithmic floating-point operations per event that the kernel of this handle executes on
  * the FP64 (FP32 in the FP32/mixed modes) FMA pipe: FMA = 2, MUL = ADD = 1, both parameter
- * sets, all helicities (checked against ncu counters).  Roofline use. */
+ * sets, all helicities.  It is an operation count of the algorithm the kernel runs (for gg -> ttbar g with
+ * sets of equal mass the one-pass form, for coupling-only sets of the larger processes the node evaluations of the polynomial mode).
+ * In FP64 it is checked against the executed 2 DFMA + DMUL + DADD count of an ncu capture (profiles/counts.json; bench.py prints the
+ * ratio); in the FP32 / mixed modes it is the model alone (ncu's FFMA counters do not see the packed FFMA2).  Roofline use. */
 double rwgt_flops_per_event(const rwgt_handle* h);
 
 /* Algorithmic flops per event of the colour form |L^T J|^2 (step a5), which the engine evaluates with FP64 mma.m8n8k4
