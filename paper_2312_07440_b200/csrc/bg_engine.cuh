@@ -1312,12 +1312,22 @@ static size_t smem_need_n(int n, const BgSched& S, int nslot, bool dbl) {
 #ifndef RWGT_NW32_N5
 #define RWGT_NW32_N5 8
 #endif
+// CTAs per SM at n = 3 (the phases of independent CTAs drift apart and could overlap one CTA's per-group fixed work with another's
+// amplitude phase): measured after the one-pass form, 2 CTAs of 4 + 4 warps 3.93 ms FP64 / 2.18 ms FP32 (8 + 4: 1.99 FP32), 3 CTAs 4.92 / 2.11,
+// against 3.36 / 1.67 for one CTA: the colour warpgroups of the extra CTAs cost more registers and shared memory than the overlap returns
+#ifndef RWGT_CTAS64_N3
+#define RWGT_CTAS64_N3 1
+#endif
+#ifndef RWGT_CTAS32_N3
+#define RWGT_CTAS32_N3 1
+#endif
 #ifndef RWGT_SLOTS32_N5
 #define RWGT_SLOTS32_N5 2
 #endif
-template <int N, typename T> struct BgCfg { static constexpr int NW = (N == 4) ? (sizeof(T) == 4 ? RWGT_NW32_N4 : RWGT_NW64_N4) : (N == 3) ? (sizeof(T) == 4 ? RWGT_NW32_N3 : RWGT_NW64_N3) : (N == 5 && sizeof(T) == 4) ? RWGT_NW32_N5 : 8, NCW = 4, CTAS = 1; };
+template <int N, typename T> struct BgCfg { static constexpr int NW = (N == 4) ? (sizeof(T) == 4 ? RWGT_NW32_N4 : RWGT_NW64_N4) : (N == 3) ? (sizeof(T) == 4 ? RWGT_NW32_N3 : RWGT_NW64_N3) : (N == 5 && sizeof(T) == 4) ? RWGT_NW32_N5 : 8, NCW = 4,
+                                                        CTAS = (N == 3) ? (sizeof(T) == 4 ? RWGT_CTAS32_N3 : RWGT_CTAS64_N3) : 1; };
 static int bg_nw(int n, bool dbl) { return n == 4 ? (dbl ? BgCfg<4, double>::NW : BgCfg<4, float>::NW) : n == 3 ? (dbl ? BgCfg<3, double>::NW : BgCfg<3, float>::NW) : n == 5 ? (dbl ? BgCfg<5, double>::NW : BgCfg<5, float>::NW) : 8; }
-static int bg_ctas(int) { return 1; }
+static int bg_ctas(int n, bool dbl) { return n == 3 ? (dbl ? BgCfg<3, double>::CTAS : BgCfg<3, float>::CTAS) : 1; }
 
 template <int N> static cudaError_t bg_set_attr(size_t s64, size_t s32) {
   typedef BgCfg<N, double> Cd; typedef BgCfg<N, float> Cf;
@@ -1385,7 +1395,7 @@ static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::stri
     int cap = std::max(1, std::min(64, (bg_nw(n, dbl) * 32) / (S.npair * (n == 2 ? 2 : 4)))); nslot = 0;
     if (n == 5 && !dbl) cap = RWGT_SLOTS32_N5;       // float amplitude buffers: a second event slot fits (two rounds of amplitude tasks per batch)
     // with k CTAs per SM each gets 1/k of the SM's shared memory (1 KB per CTA is reserved by the system)
-    size_t budget = std::min(maxsm, prop.sharedMemPerMultiprocessor / bg_ctas(n) - 1024);
+    size_t budget = std::min(maxsm, prop.sharedMemPerMultiprocessor / bg_ctas(n, dbl) - 1024);
     for (int e = cap; e >= 1; e--) if (smem_need_n(n, S, e, dbl) <= budget) { nslot = e; break; }
     bytes = nslot ? smem_need_n(n, S, nslot, dbl) : 0;
   };
@@ -1400,7 +1410,7 @@ static BgProcess* bg_create(int n, const rwgt_params* sets, int nsets, std::stri
   if (e == cudaSuccess && D.poly) {
     // scratch of the polynomial mode: per CTA nnode x slots x (NBATCH x U x 2 x NT x 64) doubles
     auto elems = [&](bool dbl) { return (size_t)D.nnode * (dbl ? B->nslot64 : B->nslot32) * bg_zel(n); };
-    e = cudaMalloc((void**)&B->d_poly, sizeof(double) * std::max(elems(true), elems(false)) * (size_t)B->sm_count * bg_ctas(n));
+    e = cudaMalloc((void**)&B->d_poly, sizeof(double) * std::max(elems(true), elems(false)) * (size_t)B->sm_count * std::max(bg_ctas(n, true), bg_ctas(n, false)));
     D.poly_scratch = B->d_poly;
   }
   if (e != cudaSuccess) { err = std::string("CUDA: ") + cudaGetErrorString(e); cudaFree(B->d_words); cudaFree(B->d_lfrag); cudaFree(B->d_poly); delete B; return nullptr; }
@@ -1445,7 +1455,7 @@ static int bg_run(BgProcess* B, int precision, const double* mom, const double* 
   BgDev D = B->D; D.idx = idx; const bool dbl = (precision == RWGT_FP64);
   D.nslot = dbl ? B->nslot64 : B->nslot32;
   if (D.poly) D.poly_stride = (long long)D.nnode * D.nslot * bg_zel(B->S.n);
-  long long ngroups = (nev + D.nslot - 1) / D.nslot; int grid = (int)std::min<long long>(ngroups, (long long)B->sm_count * bg_ctas(B->S.n));
+  long long ngroups = (nev + D.nslot - 1) / D.nslot; int grid = (int)std::min<long long>(ngroups, (long long)B->sm_count * bg_ctas(B->S.n, dbl));
   switch (B->S.n) {
     case 2: bg_launch<2>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, ostride, D); break;
     case 3: bg_launch<3>(precision, grid, B->smem64, B->smem32, st, mom, w, a, b, o, nev, stride, ostride, D); break;
