@@ -370,6 +370,30 @@ def test_ggttx_per_diagram_scaling_reading():
     assert abs((J0.sum() - J2.sum())) < 1e-13 * np.abs(J0).max()
 
 
+def test_ggttxg_jamps_are_c0_plus_x_c1_plus_x2_c2_plus_y_c3():
+    """SURVEY C6 at the amplitude level, for gg -> ttbar g: every colour-flow amplitude is J = c0 + x c1 + x^2 c2 + y c3 in
+    (x, y) = (ggg_scale, gggg_scale) -- no x y, x^3 or y^2 term -- and carries the overall factor alpha_s^(3/2).  The CUDA path
+    forms the four coefficient amplitudes once and folds them with each set's couplings ("one pass for all
+    sets at n = 3"); it may do so only because this holds for the oracle, which evaluates every set from scratch."""
+    c, p = event_aos(3, 5)
+    rng = np.random.default_rng(33)
+    for _ in range(3):
+        hel = rng.choice([-1, 1], size=5)
+        J = lambda x, y, a=0.118: orc.jamps(3, ev.params(ggg_scale=x, gggg_scale=y, alpha_s=a), p, hel)
+        c0 = J(0.0, 0.0)
+        c3 = J(0.0, 1.0) - c0
+        c1 = 0.5 * (J(1.0, 0.0) - J(-1.0, 0.0))
+        c2 = 0.5 * (J(1.0, 0.0) + J(-1.0, 0.0)) - c0
+        scale = np.abs(J(1.0, 1.0)).max()
+        assert min(np.abs(x).max() for x in (c0, c1, c2, c3)) > 1e-6 * scale        # all four structures are present
+        for x, y in ((1.1, 1.1), (0.7, 1.9), (-2.3, 0.4), (3.0, -1.5)):
+            assert np.abs(J(x, y) - (c0 + x * c1 + x * x * c2 + y * c3)).max() < 1e-12 * scale * (1 + x * x + abs(y))
+        # alpha_s: overall factor g_s^3 of the amplitude (sqrt(4 pi alpha_s)^3; the dropped common factor is convention-independent here)
+        r = J(1.3, 0.8, 0.15) / J(1.3, 0.8, 0.118)
+        expo = np.log(abs(r[0])) / np.log(0.15 / 0.118)
+        assert np.abs(r - r[0]).max() < 1e-12 * abs(r[0]) and min(abs(expo - 1.0), abs(expo - 1.5)) < 1e-9     # g_s^2 or g_s^3 (a common i g_q may be dropped)
+
+
 @pytest.mark.parametrize("idx", [2, 3])
 def test_parity_flipping_all_helicities_keeps_me2_hel(idx):
     """|M_{-h}|^2 = |M_h|^2 for both parameter sets (real couplings, Gamma_t = 0) — SURVEY Q5;
