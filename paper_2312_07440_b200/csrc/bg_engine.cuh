@@ -1297,6 +1297,10 @@ static size_t smem_need_n(int n, const BgSched& S, int nslot, bool dbl) {
 // registers (hand-over from the colour warps) and 8 event slots: 6.35 -> 5.70 ms (16 workers at 104 registers: 6.47).  n = 5 stays at 8:
 // one event slot gives 240 amplitude tasks per batch, a second slot does not fit beside the FP64 amplitude buffers.  FP32/mixed n = 3:
 // 12 workers 3.79 -> 3.16 ms.  FP64 with 12 workers at 152 registers is slower (n = 4: 10.9 -> 11.9 ms, n = 3: 5.39 -> 5.50 ms).
+// Round 2: n = 5 FP32 has two event slots (float amplitude buffers).  n = 3 FP64: 12 workers with one amplitude buffer and 32 slots
+// (4.65 -> 4.22 ms) until the one-pass form, whose amplitude threads hold two sets' amplitudes: 8 workers at 224 registers, 21 slots
+// and two buffers 3.32 ms against 3.60 (12 workers, spills to a 28 KB L1) and 3.64 (8 workers, one buffer: the second set's rows wait
+// for the colour form of the first).
 #ifndef RWGT_NW32_N4
 #define RWGT_NW32_N4 12
 #endif
