@@ -173,3 +173,23 @@ def test_reweight_file_cli_parses_parameter_sets():
     assert p[ev.PARAM_NAMES.index("ggg_scale")] == 1.1 and p[ev.PARAM_NAMES.index("mt")] == 170.0 and p[ev.PARAM_NAMES.index("alpha_s")] == 0.118
     with pytest.raises(SystemExit):
         reweight_file.parse_set("nonsense=1")
+
+
+def test_stored_full_set_goldens_are_the_oracle_values():
+    """tests/golden/full_cfg<N>.npz hold every event of every config and are what the GPU parity tests compare with.
+    They are written by tests/golden/make_goldens.py from the CPU oracle alone; this re-evaluates events sampled from the whole range
+    with the oracle (never the CUDA path) and requires the stored numbers back, so a file of any other origin would show."""
+    import oracle as orc
+    gold = os.path.join(os.path.dirname(__file__), "golden")
+    rng = np.random.default_rng(2312_07440)
+    for idx, nsample in ((1, 64), (2, 64), (3, 24), (4, 8), (5, 2), (6, 6)):
+        c = ev.config(idx)
+        g = np.load(os.path.join(gold, f"full_cfg{idx}.npz"))
+        out = g["out"]
+        assert out.shape == (3, c.n_events) and np.all(np.isfinite(out)) and np.all(out[:2] > 0)
+        assert int(g["seed"]) == c.seed and np.array_equal(g["params_old"], c.params_old) and np.array_equal(g["params_new"], c.params_new)
+        m, w = ev.generate(c)
+        pick = np.sort(rng.choice(c.n_events, size=nsample, replace=False))
+        a, b, wn, _ = orc.reweight(c.process, c.params_old, c.params_new, np.ascontiguousarray(m[:, :, pick]), w[pick].copy())
+        for k, ref in enumerate((a, b, wn)):
+            assert np.abs(out[k, pick] / ref - 1).max() < 1e-13, (idx, k)
