@@ -284,7 +284,8 @@ static double photon_flops_per_event(int ng) {
 // into registers and level 1 formed with the externals (two phases and their barriers gone): 0.296; two-buffer current storage +
 // propagator folded into q_S + momenta on the tail of buffer B (6.8 KB per event): 4 CTAs of 8 events x 160 threads 0.272 (128: 0.272,
 // 96: 0.309, 192: 0.299, 256: 0.32, register-limited to 3 CTAs); 2 CTAs of 16 events x 320 threads 0.265 (288: 0.303, 352: 0.286, 384: 0.284);
-// 4 events per CTA (a quarter-warp then holds two tasks, conflicts return): 0.33-0.41.
+// 4 events per CTA (a quarter-warp then holds two tasks, conflicts return): 0.33-0.41; warp-private groups of 8 events (no CTA barriers, four
+// warps per SM fit): 0.37-0.43; three variant bits at level 4: 0.28-0.37.
 #ifndef RWGT_PH_E
 #define RWGT_PH_E 16
 #endif
