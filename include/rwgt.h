@@ -162,6 +162,37 @@ int rwgt_run_multiprocess(rwgt_handle* h, const double* momenta, const double* w
  * stream-ordered.  No allocation, no synchronisation.  Returns 0, -1 on a bad argument, or the cudaError_t of the launch. */
 int rwgt_sum_weights(rwgt_handle* h, const double* w, int n_rows, long long n_events, double* out_sums, void* stream);
 
+/* rwgt_sum_weights for callers that are not allowed to allocate device memory.
+ *
+ * Who that is: a host program that has given all of the GPU's memory to an arena of its own (an event generator or an analysis
+ * framework that hands out every device buffer itself: a cudaMalloc from a plug-in library then fails, or takes memory behind the
+ * arena's back), and a loop that must not stall (cudaMalloc and cudaFree wait for the whole device, so one call in a side thread
+ * stops every stream of the process).  Every other entry point of this library needs a handle, and rwgt_create allocates; this
+ * one needs no handle and calls neither cudaMalloc, cudaFree nor any routine that allocates.
+ *
+ * Same arithmetic as rwgt_sum_weights (eq. 2: sigma ~ sum_k W_k per row; same block partition, same summation trees,
+ * so the two return bitwise the same sums).  The caller still owns input and output:
+ *   w         DEVICE double [n_rows][n_events], row r at offset r * n_events
+ *   out_sums  DEVICE double [n_rows]
+ * on the device that is current at the call.  What differs is where the per-block partial sums and the per-row arrival counters
+ * live: in a fixed array inside the library image (RWGT_STATIC_SCRATCH_BYTES = 9,216 bytes of global memory on every GPU that has
+ * loaded librwgt.so, held until the process exits) instead of a handle's buffers.  That fixes the limit:
+ *   1 <= n_rows <= RWGT_STATIC_SUM_MAX_ROWS (17 = 1 + RWGT_MAX_SETS: the old weights and every parameter set in one call);
+ * more rows are refused with -1 and a message in rwgt_last_error() (split the rows over several calls).  n_events is not limited.
+ *
+ * First call on a device: the library looks up the array's device address (once per device, kept afterwards).  That lookup may
+ * load the library's device code; make this first call during set-up, before any stream capture is open on the thread.
+ * Shared state: every call on a device, from any thread or stream, uses the same array, and the array keeps what the last call
+ * left in it.  The call clears the counters it needs on `stream` before its kernel (one cudaMemsetAsync of 68 bytes), so stale
+ * contents never reach a result; but two calls that can run on the GPU at the same time (different streams without an event
+ * between them, or two host threads) race on the array and return wrong sums.  Keep calls on one device stream-ordered.
+ * No synchronisation.  Returns 0, -1 on a bad argument (NULL buffer, n_events < 0, n_rows outside the limit, more than
+ * RWGT_STATIC_MAX_DEVICES = 64 devices), or the cudaError_t of the address lookup, the clear or the launch. */
+#define RWGT_STATIC_SUM_MAX_ROWS 17
+#define RWGT_STATIC_SCRATCH_BYTES 9216
+#define RWGT_STATIC_MAX_DEVICES 64
+int rwgt_sum_weights_static(const double* w, int n_rows, long long n_events, double* out_sums, void* stream);
+
 /* Binary event files: the stand-in for the LHE event files the paper's library parses (PAPER.md:87 step 2), which do
  * not exist here.  Little endian, structure of arrays, the layout rwgt_run takes:
  *   event file  = rwgt_event_file_header, double momenta[n_ext][4][n_events], double weights[n_events]

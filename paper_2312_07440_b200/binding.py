@@ -19,7 +19,8 @@ RWGT_MAX_SETS = 16
 RWGT_MAX_PROCESSES = 4
 EXPORTS = ("rwgt_create", "rwgt_create_multi", "rwgt_n_sets", "rwgt_run_multi", "rwgt_run_multi_host", "rwgt_set_precision", "rwgt_n_external", "rwgt_flops_per_event", "rwgt_run",
            "rwgt_run_host", "rwgt_destroy", "rwgt_last_error", "rwgt_colour_matrix", "rwgt_tensor_flops_per_event", "rwgt_sum_weights", "rwgt_run_file",
-           "rwgt_create_multiprocess", "rwgt_n_processes", "rwgt_run_multiprocess")
+           "rwgt_create_multiprocess", "rwgt_n_processes", "rwgt_run_multiprocess", "rwgt_sum_weights_static")
+RWGT_STATIC_SUM_MAX_ROWS = 17
 
 
 class rwgt_params(C.Structure):
@@ -62,6 +63,7 @@ def lib():
         L.rwgt_n_processes.argtypes = [vp]
         L.rwgt_run_multiprocess.argtypes = [vp, dp, dp, dp, dp, dp, dp, C.c_longlong, vp]
         L.rwgt_sum_weights.argtypes = [vp, dp, C.c_int, C.c_longlong, dp, vp]
+        L.rwgt_sum_weights_static.argtypes = [dp, C.c_int, C.c_longlong, dp, vp]
         L.rwgt_run_file.argtypes = [vp, C.c_char_p, C.c_char_p, C.c_longlong, C.c_longlong, vp]
         _lib = L
     return _lib
@@ -189,6 +191,17 @@ def rwgt_sum_weights(h, w_ptr: int, n_rows: int, n_events: int, out_sums_ptr: in
     rc = lib().rwgt_sum_weights(h, w_ptr, int(n_rows), int(n_events), out_sums_ptr, stream or None)
     if rc != 0:
         raise RuntimeError(f"rwgt_sum_weights rc={rc}: {rwgt_last_error()}")
+
+
+def rwgt_sum_weights_static(w_ptr: int, n_rows: int, n_events: int, out_sums_ptr: int, stream: int = 0) -> None:
+    """eq. 2 for a caller that may not allocate device memory (all of it belongs to the host program's own arena,
+    or a cudaMalloc's device-wide wait is not affordable): no handle, no allocation; the reduction's scratch is a fixed 9 KB array
+    inside librwgt.so.  Device pointers on the current device; w is [n_rows][n_events], out_sums [n_rows]; n_rows <= 17
+    (RWGT_STATIC_SUM_MAX_ROWS), more raises.  All calls on a device share that array: keep them stream-ordered.  Make the first
+    call on a device at set-up, outside any stream capture (it looks up the array's device address)."""
+    rc = lib().rwgt_sum_weights_static(w_ptr, int(n_rows), int(n_events), out_sums_ptr, stream or None)
+    if rc != 0:
+        raise RuntimeError(f"rwgt_sum_weights_static rc={rc}: {rwgt_last_error()}")
 
 
 def rwgt_run_file(h, in_path: str, out_path: str, first_event: int = 0, n_events: int = -1, stream: int = 0) -> None:

@@ -4,6 +4,7 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -35,6 +36,42 @@ struct DeviceGuard {
   ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
 };
 
+}  // namespace
+
+// ---------------------------------------------------------------------------- scratch of rwgt_sum_weights_static
+// For callers that may not allocate (include/rwgt.h): the block partials and row counters of the eq. 2 reduction in a fixed array of
+// the library image instead of a handle's cudaMalloc'ed buffers.  Layout: double partial[17][SUM_BLOCKS] at byte 0 (8,704 bytes),
+// unsigned ticket[17] at byte 8,704.  One copy per GPU that loads the library; shared by every call on that GPU.
+static_assert(RWGT_STATIC_SUM_MAX_ROWS == 1 + RWGT_MAX_SETS, "one call sums the old weights and every parameter set");
+constexpr size_t STATIC_TICKET_OFFSET = sizeof(double) * RWGT_STATIC_SUM_MAX_ROWS * rwgt::SUM_BLOCKS;
+static_assert(STATIC_TICKET_OFFSET % 256 == 0 && STATIC_TICKET_OFFSET + sizeof(unsigned) * RWGT_STATIC_SUM_MAX_ROWS <= RWGT_STATIC_SCRATCH_BYTES, "static scratch layout");
+static __device__ __align__(256) unsigned char g_static_scratch[RWGT_STATIC_SCRATCH_BYTES];
+
+namespace {
+// In host code `g_static_scratch` names a host-side shadow of the array, not memory a kernel can use: the address a kernel may be
+// given comes from cudaGetSymbolAddress, asked once per device with that device current, and is kept here.
+std::mutex g_static_mutex;
+unsigned char* g_static_ptr[RWGT_STATIC_MAX_DEVICES] = {};
+
+// device address of the static scratch on the CURRENT device (looked up on the first call per device); nullptr + rc on failure
+unsigned char* static_scratch_of_current_device(int* rc) {
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) { set_err("rwgt_sum_weights_static: %s", cudaGetErrorString(e)); *rc = (int)e; return nullptr; }
+  if (dev < 0 || dev >= RWGT_STATIC_MAX_DEVICES) { set_err("rwgt_sum_weights_static: device ordinal beyond RWGT_STATIC_MAX_DEVICES"); *rc = -1; return nullptr; }
+  std::lock_guard<std::mutex> lock(g_static_mutex);
+  if (!g_static_ptr[dev]) {
+    void* p = nullptr;
+    e = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (e != cudaSuccess || !p) {
+      set_err("rwgt_sum_weights_static: cudaGetSymbolAddress: %s", e != cudaSuccess ? cudaGetErrorString(e) : "null address");
+      *rc = e != cudaSuccess ? (int)e : -1; return nullptr;
+    }
+    g_static_ptr[dev] = (unsigned char*)p;
+  }
+  *rc = 0;
+  return g_static_ptr[dev];
+}
 }  // namespace
 
 #define RWGT_MAX_CHUNKS 8
@@ -422,6 +459,28 @@ int rwgt_sum_weights(rwgt_handle* h, const double* w, int n_rows, long long n_ev
   rwgt::sum_rows_kernel<<<dim3(rwgt::SUM_BLOCKS, n_rows), rwgt::SUM_THREADS, 0, (cudaStream_t)stream>>>(w, n_events, n_events, h->sum_partial, h->sum_ticket, out_sums);
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) { set_err("rwgt_sum_weights: %s", cudaGetErrorString(e)); return (int)e; }
+  return 0;
+}
+
+// eq. 2 without a handle and without any allocation (include/rwgt.h): the kernel of rwgt_sum_weights on the library's static scratch
+int rwgt_sum_weights_static(const double* w, int n_rows, long long n_events, double* out_sums, void* stream) {
+  if (n_rows < 1 || n_rows > RWGT_STATIC_SUM_MAX_ROWS) {
+    set_err("rwgt_sum_weights_static: n_rows outside 1..RWGT_STATIC_SUM_MAX_ROWS (17): the static scratch holds 17 rows, sum the rest in a further call");
+    return -1;
+  }
+  if (n_events < 0) { set_err("rwgt_sum_weights_static: n_events < 0"); return -1; }
+  if (!w || !out_sums) { set_err("rwgt_sum_weights_static: NULL buffer"); return -1; }
+  int rc = 0;
+  unsigned char* base = static_scratch_of_current_device(&rc);
+  if (!base) return rc;
+  double* partial = (double*)base;
+  unsigned* ticket = (unsigned*)(base + STATIC_TICKET_OFFSET);
+  // the counters must start at zero whatever an earlier (possibly failed) call left behind; the partials are overwritten before use
+  cudaError_t e = cudaMemsetAsync(ticket, 0, sizeof(unsigned) * RWGT_STATIC_SUM_MAX_ROWS, (cudaStream_t)stream);
+  if (e != cudaSuccess) { set_err("rwgt_sum_weights_static: %s", cudaGetErrorString(e)); return (int)e; }
+  rwgt::sum_rows_kernel<<<dim3(rwgt::SUM_BLOCKS, n_rows), rwgt::SUM_THREADS, 0, (cudaStream_t)stream>>>(w, n_events, n_events, partial, ticket, out_sums);
+  e = cudaGetLastError();
+  if (e != cudaSuccess) { set_err("rwgt_sum_weights_static: %s", cudaGetErrorString(e)); return (int)e; }
   return 0;
 }
 
