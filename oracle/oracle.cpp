@@ -536,7 +536,8 @@ static double me2_hel_qq(int ng, const Par& P, const double* p, const int* hel, 
   const cd ig = I_ * g;
   // colour-stripped Lorentz pieces of the light line
   V4 jA, jB1, jB2;                 // vbar gamma^mu u ; vbar gamma^mu S0 e-slash u (colour T^c T^a) ; vbar e-slash S0 gamma^mu u (colour T^a T^c)
-  double q1[4], q2[4]; for (int mu = 0; mu < 4; mu++) { q1[mu] = p1[mu] - p5[mu] * (ng ? 1 : 0); q2[mu] = -p2[mu] + p5[mu] * (ng ? 1 : 0); }
+  double k5[4]; for (int mu = 0; mu < 4; mu++) k5[mu] = ng ? p5[mu] : 0.0;      // p5 lies outside the caller's buffer when there is no gluon: never read it then
+  double q1[4], q2[4]; for (int mu = 0; mu < 4; mu++) { q1[mu] = p1[mu] - k5[mu]; q2[mu] = -p2[mu] + k5[mu]; }
   for (int mu = 0; mu < 4; mu++) {
     jA.c[mu] = rowcol(vb2, (ig * G.g[mu]) * u1);
     if (ng) {
@@ -545,7 +546,7 @@ static double me2_hel_qq(int ng, const Par& P, const double* p, const int* hel, 
     }
   }
   const double QA2 = mink2(KA), QB2 = mink2(QB);
-  double qt[4], qtb[4]; for (int mu = 0; mu < 4; mu++) { qt[mu] = p3[mu] + p5[mu] * (ng ? 1 : 0); qtb[mu] = -p4[mu] - p5[mu] * (ng ? 1 : 0); }
+  double qt[4], qtb[4]; for (int mu = 0; mu < 4; mu++) { qt[mu] = p3[mu] + k5[mu]; qtb[mu] = -p4[mu] - k5[mu]; }
   double total = 0;
   const int na = ng ? 8 : 1;
   for (int i = 0; i < 3; i++) for (int j = 0; j < 3; j++) for (int a = 0; a < na; a++) {
