@@ -192,4 +192,6 @@ def test_stored_full_set_goldens_are_the_oracle_values():
         pick = np.sort(rng.choice(c.n_events, size=nsample, replace=False))
         a, b, wn, _ = orc.reweight(c.process, c.params_old, c.params_new, np.ascontiguousarray(m[:, :, pick]), w[pick].copy())
         for k, ref in enumerate((a, b, wn)):
-            assert np.abs(out[k, pick] / ref - 1).max() < 1e-13, (idx, k)
+            # 2e-15: the oracle re-run gives the stored value back to the last bits (bit-exact for cfgs 1, 2, 6; a few ulp from the
+            # summation order over threads for cfgs 3-5), whereas the FP64 kernels sit 1e-14..3e-13 away from it (profiles/r2_parity.md)
+            assert np.abs(out[k, pick] / ref - 1).max() < 2e-15, (idx, k)
