@@ -86,7 +86,9 @@ int rwgt_n_external(const rwgt_handle* h);
  * sets, all helicities.  It is an operation count of the algorithm the kernel runs (for gg -> ttbar g with
  * sets of equal mass the one-pass form, for coupling-only sets of the larger processes the node evaluations of the polynomial mode).
  * In FP64 it is checked against the executed 2 DFMA + DMUL + DADD count of an ncu capture (profiles/counts.json; bench.py prints the
- * ratio); in the FP32 / mixed modes it is the model alone (ncu's FFMA counters do not see the packed FFMA2).  Roofline use. */
+ * ratio); in the FP32 / mixed modes it is the model alone (ncu's FFMA counters do not see the packed FFMA2).  Roofline use.
+ * Multiprocess handle: the unweighted mean over the member processes (the mix of an event list is not known before run time);
+ * weight the members' own counts (one handle per process) with the list's composition for a roofline figure. */
 double rwgt_flops_per_event(const rwgt_handle* h);
 
 /* Algorithmic flops per event of the colour form |L^T J|^2 (step a5), which the engine evaluates with FP64 mma.m8n8k4
@@ -115,7 +117,13 @@ int rwgt_run(rwgt_handle* h, const double* momenta, const double* weights, doubl
 /* The same launch for a handle with K = rwgt_n_sets(h) new parameter sets:
  *   out_me_new, out_w_new  DEVICE double [K][n_events]: set k at offset k * n_events
  * (out_me_old stays [n_events]).  rwgt_run is this call restricted to K == 1 (it returns -1 for K > 1, so that a
- * caller who sized the outputs for one set cannot be overrun). */
+ * caller who sized the outputs for one set cannot be overrun).
+ * Ordering: a handle of gg_ttxgg / gg_ttxggg created with three or more coupling-only sets runs in the polynomial mode, whose
+ * kernel keeps intermediate colour vectors in device scratch that belongs to the HANDLE (one slice per CTA, allocated at create).
+ * Two launches of one such handle that can overlap on the GPU (different streams with no event between them, or two host
+ * threads) overwrite each other's scratch and return wrong weights without an error.  Rule for every handle: enqueue the run
+ * calls of ONE handle on one stream, or order them with events; use one handle per stream for concurrent launches (handles are
+ * independent).  Handles outside the polynomial mode hold no mutable device state in rwgt_run / rwgt_run_multi. */
 int rwgt_run_multi(rwgt_handle* h, const double* momenta, const double* weights, double* out_me_old,
                    double* out_me_new, double* out_w_new, long long n_events, void* stream);
 
@@ -134,8 +142,11 @@ int rwgt_run_multi_host(rwgt_handle* h, const double* momenta, const double* wei
 
 /* LO multiprocess (real-emission contributions "can be treated as LO multiprocesses", last sentence:
  * "reweighting between structurally different amplitude routines"): ONE event list whose events belong to different processes with
- * the same number of external legs, e.g. "gg_ttxg,qqx_ttxg".  `processes`: comma-separated names (QCD processes only), at most
- * RWGT_MAX_PROCESSES; parameter sets as in rwgt_create_multi, shared by all members.  NULL on error. */
+ * the same number of external legs, e.g. "gg_ttxg,qqx_ttxg".  `processes`: comma-separated names, at most RWGT_MAX_PROCESSES;
+ * QCD processes only: the epem_* kernels take no event index list, and an e+ e- sample never shares an event list with a hadronic
+ * one, so such a member is refused.  Parameter sets as in rwgt_create_multi, shared by all members.  NULL on error.
+ * rwgt_set_precision on such a handle sets the mode of the members that have FP32 / mixed kernels (gg_ttxg, gg_ttxgg, gg_ttxggg);
+ * the other members stay FP64, and a mode other than RWGT_FP64 is refused (-1) when no member has one. */
 #define RWGT_MAX_PROCESSES 4
 rwgt_handle* rwgt_create_multiprocess(const char* processes, const rwgt_params* params_old, const rwgt_params* params_new, int n_new);
 
@@ -217,7 +228,8 @@ typedef struct {
 
 /* The whole procedure of PAPER.md:87 (steps 2-8) for events [first_event, first_event + n_events) of the event file `in_path`
  * (n_events < 0: to the end of the file): parse, copy to the device, evaluate |M|^2 and every |M'_k|^2, eq. 3, copy back, write the
- * result file `out_path` (created or truncated), including the eq. 2 sums.  The range is cut into chunks; a reader thread fills one
+ * result file `out_path`, including the eq. 2 sums (the file is written as "<out_path>.tmp" and renamed when complete, so a failed
+ * call leaves no result file of this call behind and an existing `out_path` as it was; `out_path` must not be the event file).  The range is cut into chunks; a reader thread fills one
  * pinned buffer from the file while the previous chunk goes through the overlapped H2D / kernel / D2H pipeline of
  * rwgt_run_multi_host and a writer thread stores the chunk before.  Pinned buffers and device scratch belong to the handle and are
  * grown on first use.  Synchronises `stream`.  A rank of a multi-GPU job passes its own contiguous range and result path

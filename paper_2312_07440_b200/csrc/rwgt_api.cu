@@ -231,6 +231,9 @@ int rwgt_n_sets(const rwgt_handle* h) { return h ? h->nsets - 1 : -1; }
 int rwgt_set_precision(rwgt_handle* h, int mode) {
   if (!h || mode < 0 || mode > 2) { set_err("rwgt_set_precision: bad argument"); return -1; }
   if (h->proc == P_MULTI) {            // applies to the members that have the mode; the others stay FP64
+    int with_mode = 0;
+    for (int i = 0; i < h->nsub; i++) with_mode += (h->sub[i]->proc == P_BG);
+    if (mode != RWGT_FP64 && with_mode == 0) { set_err("rwgt_set_precision: every member process of this handle is FP64 only"); return -1; }
     for (int i = 0; i < h->nsub; i++) if (h->sub[i]->proc == P_BG) h->sub[i]->precision = mode;
     h->precision = mode; return 0;
   }
@@ -495,12 +498,23 @@ int rwgt_run_file(rwgt_handle* h, const char* in_path, const char* out_path, lon
   if (!rwgt::pread_all(fin, &hd, sizeof(hd), 0) || std::memcmp(hd.magic, "RWGTEVT1", 8) != 0 || hd.version != 1) { ::close(fin); set_err("rwgt_run_file: %s is not an event file (magic/version)", in_path); return -1; }
   if ((int)hd.n_ext != h->n_ext || std::strncmp(hd.process, h->process, sizeof(hd.process)) != 0) { ::close(fin); set_err("rwgt_run_file: %s holds events of another process", in_path); return -1; }
   struct stat sb;
-  const long long ntot = (long long)hd.n_events, planes = (long long)h->n_ext * 4, K = h->nsets - 1;
-  if (::fstat(fin, &sb) != 0 || (long long)sb.st_size < (long long)sizeof(hd) + (planes + 1) * ntot * 8) { ::close(fin); set_err("rwgt_run_file: %s is truncated", in_path); return -1; }
+  const long long planes = (long long)h->n_ext * 4, K = h->nsets - 1;
+  // n_events comes from the file: bound it by the file's size BEFORE multiplying (a huge value must not wrap the product)
+  if (::fstat(fin, &sb) != 0 || (long long)sb.st_size < (long long)sizeof(hd) ||
+      hd.n_events > (unsigned long long)(((long long)sb.st_size - (long long)sizeof(hd)) / 8) / (unsigned long long)(planes + 1)) {
+    ::close(fin); set_err("rwgt_run_file: %s is truncated", in_path); return -1;
+  }
+  const long long ntot = (long long)hd.n_events;
   if (n_events < 0) n_events = ntot - first_event;
-  if (n_events < 0 || first_event + n_events > ntot) { ::close(fin); set_err("rwgt_run_file: event range outside the file"); return -1; }
-  int fout = ::open(out_path, O_CREAT | O_TRUNC | O_RDWR, 0644);
-  if (fout < 0) { ::close(fin); set_err("rwgt_run_file: cannot create %s", out_path); return -1; }
+  if (n_events < 0 || first_event > ntot || n_events > ntot - first_event) { ::close(fin); set_err("rwgt_run_file: event range outside the file"); return -1; }
+  // the result goes to "<out_path>.tmp" and takes its name only when it is complete: a failed call leaves no well-formed result
+  // file behind (and an existing out_path untouched); input and output must be different files
+  struct stat so;
+  if (::stat(out_path, &so) == 0 && so.st_dev == sb.st_dev && so.st_ino == sb.st_ino) { ::close(fin); set_err("rwgt_run_file: %s is the event file itself", out_path); return -1; }
+  const std::string tmp_path = std::string(out_path) + ".tmp";
+  if (::stat(tmp_path.c_str(), &so) == 0 && so.st_dev == sb.st_dev && so.st_ino == sb.st_ino) { ::close(fin); set_err("rwgt_run_file: %s.tmp is the event file itself", out_path); return -1; }
+  int fout = ::open(tmp_path.c_str(), O_CREAT | O_TRUNC | O_RDWR, 0644);
+  if (fout < 0) { ::close(fin); set_err("rwgt_run_file: cannot create %s.tmp", out_path); return -1; }
   rwgt_result_file_header ho; std::memset(&ho, 0, sizeof(ho));
   std::memcpy(ho.magic, "RWGTRES1", 8); ho.version = 1; ho.n_sets = (uint32_t)K; ho.n_events = (uint64_t)n_events; std::memcpy(ho.process, h->process, sizeof(ho.process));
   ho.first_event = (uint64_t)first_event;
@@ -556,7 +570,10 @@ int rwgt_run_file(rwgt_handle* h, const char* in_path, const char* out_path, lon
     if (writer.joinable()) { writer.join(); if (!wr_ok && rc == 0) { set_err("rwgt_run_file: write error on %s", out_path); rc = -1; } }
   }
   if (rc == 0 && !rwgt::pwrite_all(fout, sums, sizeof(double) * (1 + K), obase + (off_t)((1 + 2 * K) * n) * 8)) { set_err("rwgt_run_file: write error on %s", out_path); rc = -1; }
-  ::close(fin); ::close(fout);
+  ::close(fin);
+  if (::close(fout) != 0 && rc == 0) { set_err("rwgt_run_file: write error on %s", out_path); rc = -1; }
+  if (rc == 0 && ::rename(tmp_path.c_str(), out_path) != 0) { set_err("rwgt_run_file: cannot rename the finished result to %s", out_path); rc = -1; }
+  if (rc != 0) ::unlink(tmp_path.c_str());
   return rc;
 }
 

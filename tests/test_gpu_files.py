@@ -92,6 +92,56 @@ def test_run_file_error_behaviour(tmp_path):
     B.rwgt_destroy(h)
 
 
+def test_run_file_never_destroys_the_input_and_leaves_no_result_after_a_failure(tmp_path):
+    """out_path == in_path is refused with the event file intact; a header whose n_events would wrap the size product counts as
+    truncated; a failed call leaves neither a result file nor its ".tmp", and an earlier result of the same name stays as it was."""
+    c = ev.config(2)
+    m, w = ev.generate(c, 300)
+    fin, fout = str(tmp_path / "e.rwgt"), str(tmp_path / "o.rwgt")
+    B.write_event_file(fin, c.process, m, w)
+    before = open(fin, "rb").read()
+    h = B.rwgt_create(c.process, c.params_old, c.params_new)
+    with pytest.raises(RuntimeError, match="event file itself"):
+        B.rwgt_run_file(h, fin, fin)
+    os.link(fin, str(tmp_path / "alias.rwgt"))                                 # the same inode under another name
+    with pytest.raises(RuntimeError, match="event file itself"):
+        B.rwgt_run_file(h, fin, str(tmp_path / "alias.rwgt"))
+    assert open(fin, "rb").read() == before
+    B.rwgt_run_file(h, fin, fout)                                              # a good result ...
+    good = open(fout, "rb").read()
+    assert not os.path.exists(fout + ".tmp")
+    huge = str(tmp_path / "huge.rwgt")
+    hd = bytearray(before[:64])
+    hd[16:24] = (2 ** 61 + 5).to_bytes(8, "little")                            # (planes + 1) * n * 8 wraps to a small number
+    open(huge, "wb").write(bytes(hd) + before[64:])
+    with pytest.raises(RuntimeError, match="truncated"):
+        B.rwgt_run_file(h, huge, fout)
+    with pytest.raises(RuntimeError, match="range outside"):
+        B.rwgt_run_file(h, fin, fout, 2 ** 62, 2 ** 62)                        # first + n wraps
+    assert open(fout, "rb").read() == good and not os.path.exists(fout + ".tmp")   # ... survives the failed calls
+    os.chmod(tmp_path, 0o500)                                                  # a directory that takes no new file
+    try:
+        if not os.access(str(tmp_path), os.W_OK):                              # (root ignores the mode: nothing to check then)
+            with pytest.raises(RuntimeError, match="cannot create"):
+                B.rwgt_run_file(h, fin, str(tmp_path / "new.rwgt"))
+            assert not os.path.exists(str(tmp_path / "new.rwgt"))
+    finally:
+        os.chmod(tmp_path, 0o700)
+    B.rwgt_destroy(h)
+
+
+def test_set_precision_on_a_multiprocess_handle_without_fp32_members_is_refused():
+    c = ev.config(2)
+    h = B.rwgt_create_multiprocess("gg_ttx,qqx_ttx", c.params_old, [c.params_new])
+    with pytest.raises(RuntimeError, match="FP64 only"):
+        B.rwgt_set_precision(h, B.RWGT_FP32)
+    B.rwgt_set_precision(h, B.RWGT_FP64)
+    B.rwgt_destroy(h)
+    h = B.rwgt_create_multiprocess("gg_ttxg,qqx_ttxg", c.params_old, [c.params_new])
+    B.rwgt_set_precision(h, B.RWGT_MIXED)                                      # gg_ttxg has the mode; qqx_ttxg stays FP64
+    B.rwgt_destroy(h)
+
+
 @pytest.mark.parametrize("n", [1, 63, 64, 65, 16384, 1048576 + 17])
 def test_sum_weights_deterministic_and_accurate(n):
     """eq. 2 on the device: within the documented bound of the exactly rounded sum, identical on repeated launches, equal to the
