@@ -327,10 +327,10 @@ def test_colour_matrix_table():
 
 
 def test_denominators():
-    """Averaging denominator D (reading Q3, SURVEY.md:433: a DEFINITION of what out_me_* contain, not a derived quantity):
-    2 helicities x 2 helicities x 8 colours x 8 colours of the two incoming gluons, times k! for the k identical
-    final-state gluons.  Stated here from the process string, independently of the oracle's own formula; for k <= 1 the
-    closed form of gg -> ttbar pins the 1/256, for k = 2, 3 nothing but this definition does ("parity unpinned": DESIGN.md)."""
+    """Averaging denominator D (reading Q3, SURVEY.md:433: what out_me_* contain): 2 helicities x 2 helicities x 8 colours x 8
+    colours of the two incoming gluons, times k! for the k identical final-state gluons, read here from the process string.
+    This restates the rule; what PINS it is elsewhere: the closed form of gg -> ttbar fixes the 1/256 (k = 0), and the soft-gluon
+    limit |M_n|^2 -> eikonal x |M_{n-1}|^2 / (k+1) fixes D(k+1) / D(k) for k + 1 = 1, 2, 3 (tests/test_oracle_pins_soft.py)."""
     for idx in (2, 3, 4, 5):
         c = ev.config(idx)
         final = c.process.split("_")[1]                  # "ttx", "ttxg", ...
@@ -340,22 +340,37 @@ def test_denominators():
 
 
 # ------------------------------------------------------------------ new-model pins
+def lagrange(xs, ys, x):
+    """value at x of the polynomial of degree len(xs) - 1 through (xs, ys): the Lagrange formula written out, no least squares"""
+    return sum(ys[j] * np.prod([(x - xs[m]) / (xs[j] - xs[m]) for m in range(len(xs)) if m != j]) for j in range(len(xs)))
+
+
+def chebyshev_nodes(lo, hi, count):
+    return 0.5 * (lo + hi) + 0.5 * (hi - lo) * np.cos(np.pi * (2 * np.arange(count) + 1) / (2 * count))
+
+
 @pytest.mark.parametrize("idx", [2, 3, 4, 5])
 def test_me2_is_polynomial_of_degree_2n_minus_2_in_kappa(idx):
+    """|M'|^2 with ggg_scale = gggg_scale = 1 + kappa is a polynomial of degree 2 (n - 1) in kappa (every amplitude has at most
+    n - 1 powers of the scales).  Exact interpolation through 2n - 1 Chebyshev nodes of [-0.3, 0.6] reproduces the oracle at
+    kappa = 0.1 and 0.55 to 1e-9 for every n (np.polyfit on equispaced points lost two digits at n >= 4: that was the fit, not
+    the oracle); one node fewer does not."""
     n = idx
     c, p = event_aos(idx, 4)
     deg = 2 * (n - 1)
-    ks = np.linspace(-0.3, 0.4, deg + 1)
-    vals = [orc.me2(c.process, ev.params(ggg_scale=1 + k, gggg_scale=1 + k), p) for k in ks]
-    coef = np.polyfit(ks, vals, deg)
-    got55 = orc.me2(c.process, ev.params(ggg_scale=1.55, gggg_scale=1.55), p)
-    assert abs(np.polyval(coef, 0.55) / got55 - 1) < (1e-9 if n <= 3 else 1e-7)
-    if n <= 4:
-        got01 = orc.me2(c.process, ev.params(ggg_scale=1.1, gggg_scale=1.1), p)
-        assert abs(np.polyval(coef, 0.1) / got01 - 1) < 1e-9
+
+    def me2_at(k):
+        return orc.me2(c.process, ev.params(ggg_scale=1 + k, gggg_scale=1 + k), p)
+
+    ks = chebyshev_nodes(-0.3, 0.6, deg + 1)
+    vals = [me2_at(k) for k in ks]
+    got55, got01 = me2_at(0.55), me2_at(0.1)
+    assert abs(lagrange(ks, vals, 0.55) / got55 - 1) < 1e-9
+    assert abs(lagrange(ks, vals, 0.1) / got01 - 1) < 1e-9
     # one degree less does NOT fit
-    coef_lo = np.polyfit(ks, vals, deg - 1)
-    assert abs(np.polyval(coef_lo, 0.55) / got55 - 1) > 1e-6
+    ks_lo = chebyshev_nodes(-0.3, 0.6, deg)
+    vals_lo = [me2_at(k) for k in ks_lo]
+    assert max(abs(lagrange(ks_lo, vals_lo, 0.55) / got55 - 1), abs(lagrange(ks_lo, vals_lo, 0.1) / got01 - 1)) > 1e-6
 
 
 def test_ggttx_per_diagram_scaling_reading():
