@@ -110,6 +110,39 @@ def config(index_or_process) -> Config:
     raise KeyError(index_or_process)
 
 
+# ---------------------------------------------------------------------------- named lists of new parameter sets (inputs only)
+# PAPER.md:87 step 7 / Fig. 3: K new sets per pass.  The lists below are what bench.py times with K > 1 and what
+# tests/golden/make_goldens.py --sets evaluates with the oracle; they are inputs (numbers typed in), no arithmetic of the method.
+KSET_LISTS = ("bench4", "bench8", "bench16", "general4", "mass4")
+# which lists each config stores oracle values for (tests/golden/ksets_cfg<N>_<list>.npz)
+KSET_GOLDENS = {3: ("bench8", "mass4"), 4: ("bench8", "general4", "mass4"), 5: ("bench4", "bench16", "general4", "mass4")}
+
+
+def kset_list(cfg: "Config", name: str) -> list:
+    """bench<K>: the coupling-only 'diagonal' lists bench.py times (ggg_scale = gggg_scale = 1 + 0.1 (k+1) / K: polynomial mode at
+    n >= 4, one level pass at n = 3); general4: independent three- and four-gluon scales with the old set among them (rank above
+    the diagonal case); mass4: other top masses (externals and denominators redone per set), the config's new set and the old set."""
+    if name.startswith("bench"):
+        K = int(name[5:])
+        return [params(ggg_scale=1 + 0.1 * (k + 1) / K, gggg_scale=1 + 0.1 * (k + 1) / K) for k in range(K)]
+    if name == "general4":
+        return [params(ggg_scale=1.1, gggg_scale=0.9), params(ggg_scale=0.95, gggg_scale=1.2), cfg.params_old.copy(),
+                params(ggg_scale=1.2, gggg_scale=1.05, alpha_s=0.125)]
+    if name == "mass4":
+        return [params(mt=170.0, ggg_scale=1.1, gggg_scale=1.1), cfg.params_new.copy(), params(mt=176.5, ggg_scale=0.9), cfg.params_old.copy()]
+    raise KeyError(name)
+
+
+def kset_sample(cfg: "Config") -> np.ndarray:
+    """Event indices of the config's full seeded set on which the K-set goldens are stored: a contiguous prefix longer than two
+    rounds of a persistent one-CTA-per-SM launch (148 CTAs x at most 32 / 8 / 2 events in flight per CTA for 3 / 4 / 5 gluons), every
+    stride-th event of the rest (every later round of the launch is hit) and the last events (the ragged tail)."""
+    n = cfg.n_events
+    prefix, strided, tail = {3: (12288, 2048, 256), 4: (2560, 512, 64), 5: (304, 96, 16)}[cfg.index]
+    rest = np.linspace(prefix, n - tail - 1, strided).astype(np.int64)
+    return np.unique(np.concatenate([np.arange(prefix), rest, np.arange(n - tail, n)]))
+
+
 def _splitmix64(counter: np.ndarray, seed: int) -> np.ndarray:
     with np.errstate(over="ignore"):
         z = np.uint64(seed) + (counter.astype(np.uint64) + np.uint64(1)) * _GOLDEN

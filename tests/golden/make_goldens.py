@@ -8,7 +8,15 @@ Calls only oracle/ (the arithmetic) and events.py (the seeded inputs, which hold
 imports or loads the CUDA path.  The event sets are prefix-stable (the first n accepted candidates in counter order), so a
 later call with a larger --events extends an existing file: the events already stored are kept and only the new ones are
 evaluated.  The GPU parity tests (tests/test_gpu_goldens.py) compare FP64, FP32 and mixed launches with these files element
-by element, so no oracle time is spent on the GPU box."""
+by element, so no oracle time is spent on the GPU box.
+
+    python tests/golden/make_goldens.py --config 5 --sets bench16 [--threads 8]
+
+writes tests/golden/ksets_cfg<N>_<list>.npz instead: for the named list of K new parameter sets (events.kset_list: what bench.py
+times with K > 1, lists with other top masses, independent coupling scales) the oracle's |M|^2, |M'_k|^2 and W'_k on the
+events events.kset_sample picks from the config's FULL seeded set (a prefix longer than two rounds of the persistent launch,
+a strided sample of every later round, the tail), one orc.reweight call per set.  tests/test_gpu_ksets.py launches the full
+set and compares these events (VERDICT r2 item 1; PAPER.md:87 step 7, :117)."""
 import argparse
 import os
 import sys
@@ -28,14 +36,40 @@ def path(idx: int) -> str:
     return os.path.join(HERE, f"full_cfg{idx}.npz")
 
 
+def kset_path(idx: int, name: str) -> str:
+    return os.path.join(HERE, f"ksets_cfg{idx}_{name}.npz")
+
+
+def make_ksets(c, name: str, threads: int) -> None:
+    sets = ev.kset_list(c, name)
+    idx = ev.kset_sample(c)
+    m, w = ev.generate(c)
+    ms, ws = np.ascontiguousarray(m[:, :, idx]), w[idx].copy()
+    K = len(sets)
+    me_old, me_new, w_new = np.full(len(idx), np.nan), np.full((K, len(idx)), np.nan), np.full((K, len(idx)), np.nan)
+    t0 = time.time()
+    for k, pn in enumerate(sets):
+        a, b, wn, used = orc.reweight(c.process, c.params_old, pn, ms, ws, nthreads=threads)
+        assert k == 0 or np.array_equal(a, me_old)
+        me_old, me_new[k], w_new[k] = a, b, wn
+        print(f"cfg {c.index} {name}: set {k + 1}/{K}, {len(idx)} events, {time.time() - t0:.0f} s, {used} threads", flush=True)
+    np.savez(kset_path(c.index, name) + ".tmp.npz", idx=idx, sets=np.array(sets), me_old=me_old, me_new=me_new, w_new=w_new, seed=c.seed,
+             process=c.process, params_old=c.params_old)
+    os.replace(kset_path(c.index, name) + ".tmp.npz", kset_path(c.index, name))
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--config", type=int, required=True)
     ap.add_argument("--events", type=int, default=0)
     ap.add_argument("--threads", type=int, default=0)
     ap.add_argument("--chunk", type=int, default=0)
+    ap.add_argument("--sets", default="", help="name of a K-set list (events.KSET_LISTS): write ksets_cfg<N>_<list>.npz")
     args = ap.parse_args()
     c = ev.config(args.config)
+    if args.sets:
+        make_ksets(c, args.sets, args.threads)
+        return
     n = min(args.events or DEFAULT_EVENTS[c.index], c.n_events)
     out = np.full((3, n), np.nan)
     done = 0

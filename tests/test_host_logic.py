@@ -195,3 +195,27 @@ def test_stored_full_set_goldens_are_the_oracle_values():
             # 2e-15: the oracle re-run gives the stored value back to the last bits (bit-exact for cfgs 1, 2, 6; a few ulp from the
             # summation order over threads for cfgs 3-5), whereas the FP64 kernels sit 1e-14..3e-13 away from it (profiles/r2_parity.md)
             assert np.abs(out[k, pick] / ref - 1).max() < 2e-15, (idx, k)
+
+
+def test_stored_k_set_goldens_are_the_oracle_values():
+    """tests/golden/ksets_cfg<N>_<list>.npz (make_goldens.py --sets): the stored lists and event indices are the ones events.py
+    names, and sampled entries re-evaluated with the oracle give the stored numbers back (2e-15, as for the full-set files)."""
+    import oracle as orc
+    gold = os.path.join(os.path.dirname(__file__), "golden")
+    rng = np.random.default_rng(7440)
+    for idx, names in ev.KSET_GOLDENS.items():
+        c = ev.config(idx)
+        m, w = ev.generate(c)
+        sel = ev.kset_sample(c)
+        assert sel[0] == 0 and sel[-1] == c.n_events - 1 and np.all(np.diff(sel) > 0)
+        full = np.load(os.path.join(gold, f"full_cfg{idx}.npz"))["out"]
+        for name in names:
+            g = np.load(os.path.join(gold, f"ksets_cfg{idx}_{name}.npz"))
+            sets = ev.kset_list(c, name)
+            assert np.array_equal(g["idx"], sel) and np.array_equal(g["sets"], np.array(sets)) and int(g["seed"]) == c.seed
+            assert g["me_new"].shape == (len(sets), len(sel)) and np.all(np.isfinite(g["me_new"])) and np.all(g["me_new"] > 0)
+            assert np.abs(g["me_old"] / full[0, sel] - 1).max() < 2e-15
+            pick = np.sort(rng.choice(len(sel), size={3: 6, 4: 2, 5: 1}[idx], replace=False))
+            k = int(rng.integers(len(sets)))
+            a, b, wn, _ = orc.reweight(c.process, c.params_old, sets[k], np.ascontiguousarray(m[:, :, sel[pick]]), w[sel[pick]].copy())
+            assert np.abs(g["me_new"][k, pick] / b - 1).max() < 2e-15 and np.abs(g["w_new"][k, pick] / wn - 1).max() < 2e-15, (idx, name, k)
