@@ -291,6 +291,35 @@ def run_parity_report(args) -> None:
             for k, name in enumerate(("|M|^2", "|M'|^2", "W'")):
                 e = np.abs(got[k, :ng] / ref[k] - 1)
                 print(f"| {idx} | {c.process} | {prec} | {ng} ({c.n_events}) | {name} | {e.max():.2e} | {np.median(e):.2e} | {tmax:g} / {tmed:g} | {int((e > tmax).sum())} | {int(e.argmax())} |", flush=True)
+    # K new parameter sets per pass (PAPER.md:87 step 7): full-size launches with the named lists of events.kset_list against the oracle values of
+    # tests/golden/ksets_cfg<N>_<list>.npz on the multi-round sample events.kset_sample; one row per (cfg, list, precision, set)
+    print()
+    print("| cfg | list | K | precision | set | events compared (of the launch) | max rel. err |M'_k|^2 | median | max rel. err W'_k | median | tolerance (max / median) | over tolerance | old == new bitwise |")
+    print("|---|---|---|---|---|---|---|---|---|---|---|---|---|")
+    for idx, names in ev.KSET_GOLDENS.items():
+        c = ev.config(idx)
+        m, w = ev.generate(c)
+        dm, dw = torch.from_numpy(m).cuda(), torch.from_numpy(w).cuda()
+        for lname in names:
+            f = os.path.join(ROOT, "tests", "golden", f"ksets_cfg{idx}_{lname}.npz")
+            if not os.path.exists(f):
+                print(f"| {idx} | {lname} | - | - | - | golden file missing | | | | | | | |")
+                continue
+            g = np.load(f)
+            sets, sel = ev.kset_list(c, lname), g["idx"]
+            K = len(sets)
+            for prec in ("fp64", "fp32", "mixed"):
+                r = B.Reweighter(c.process, c.params_old, sets, prec)
+                got = r.run(dm, dw).cpu().numpy()
+                r.close()
+                tmax, tmed = tol[prec]
+                for k in range(K):
+                    eb, ew = np.abs(got[1 + k, sel] / g["me_new"][k] - 1), np.abs(got[1 + K + k, sel] / g["w_new"][k] - 1)
+                    same = "-"
+                    if np.array_equal(sets[k], c.params_old):
+                        same = "yes (all events)" if np.array_equal(got[1 + k], got[0]) and np.array_equal(got[1 + K + k], w) else "NO"
+                    print(f"| {idx} | {lname} | {K} | {prec} | {k} | {len(sel)} ({c.n_events}) | {eb.max():.2e} | {np.median(eb):.2e} | {ew.max():.2e} | {np.median(ew):.2e} | "
+                          f"{tmax:g} / {tmed:g} | {int((eb > tmax).sum() + (ew > tmax).sum())} | {same} |", flush=True)
 
 
 # rough oracle events/s/core (both parameter sets), measured on this pool's hosts; only sizes the bounded CPU samples
@@ -486,18 +515,31 @@ def main() -> None:
             per_config.append({"cfg": 1, "n": 1 << 24, "error": str(ex)})
         per_config.sort(key=lambda e: (e.get("cfg", 0), e.get("precision", ""), e.get("n", 0)))
         roofline["per_config"] = per_config
-        # K new parameter sets in one pass (PAPER.md:87 step 7, Fig. 3 axis): kappa = 0.1 k / K
-        for ci, K in ((2, 8), (3, 8), (4, 8), (5, 4), (5, 16)):
+        # K new parameter sets in one pass (PAPER.md:87 step 7, Fig. 3 axis).  bench<K>: kappa = 0.1 (k+1) / K on both
+        # gluon self-couplings (the polynomial mode's best case at n >= 4: rank n-1..n); general4: independent ggg / gggg scales and another
+        # alpha_s (higher rank: the generic case); every line is compared with the oracle values stored for its list on the multi-round sample
+        # of the SAME launch (tests/golden/ksets_*.npz, written by the oracle alone), the old set with every event of full_cfg<N>.npz
+        for ci, lname in ((2, "bench8"), (3, "bench8"), (4, "bench8"), (4, "general4"), (5, "bench4"), (5, "bench16"), (5, "general4")):
             try:
                 cc = ev.config(ci)
-                sets = [ev.params(ggg_scale=1 + 0.1 * (k + 1) / K, gggg_scale=1 + 0.1 * (k + 1) / K) for k in range(K)]
+                sets = ev.kset_list(cc, lname)
+                K = len(sets)
                 rr = time_config(torch, B, cc, "fp64", cc.n_events, max(3, args.steps // 4), 3, 0, flush_buf, new_sets=sets)
                 kms = statistics.mean(rr["ms"])
-                extra.append({"workload": workload_name(cc, cc.n_events) + f" with K={K} new parameter sets in one pass", "precision": "fp64",
-                              "events_per_s": cc.n_events / (kms * 1e-3), "new_weights_per_s": K * cc.n_events / (kms * 1e-3), "kernel_ms": kms, "l2": rr["l2"]})
+                kline = {"workload": workload_name(cc, cc.n_events) + f" with K={K} new parameter sets in one pass (list {lname})", "precision": "fp64",
+                        "events_per_s": cc.n_events / (kms * 1e-3), "new_weights_per_s": K * cc.n_events / (kms * 1e-3), "kernel_ms": kms, "l2": rr["l2"]}
+                gfile = os.path.join(ROOT, "tests", "golden", f"ksets_cfg{ci}_{lname}.npz")
+                if os.path.exists(gfile):
+                    g = np.load(gfile)
+                    got = rr["out"].cpu().numpy()
+                    sel = g["idx"]
+                    err = max(np.abs(got[1:1 + K, sel] / g["me_new"] - 1).max(), np.abs(got[1 + K:, sel] / g["w_new"] - 1).max(), np.abs(got[0, sel] / g["me_old"] - 1).max())
+                    kline["max_rel_err_vs_golden"] = float(err)
+                    kline["golden_events"] = int(len(sel))
+                extra.append(kline)
                 rr["rw"].close()
             except Exception as ex:
-                extra.append({"workload": f"cfg{ci} K={K}", "error": str(ex)})
+                extra.append({"workload": f"cfg{ci} {lname}", "error": str(ex)})
         # cfg 1 at its stated 16,384 events is launch-latency-bound: the same launch captured in a CUDA graph (20 launches per replay)
         try:
             c1 = ev.config(1)

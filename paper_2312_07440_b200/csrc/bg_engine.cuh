@@ -614,10 +614,10 @@ template <int N, int M, typename T, int NWT> __device__ __forceinline__ void lev
 }
 
 // The ordering and its reversal share the term ubar Jn-slash v of the full gluon current (up to the sign (-1)^(n+1)): formed once per
-// pair it saves two row-slash products of 2 x 2 x NJ C.  Measured on B200: gg->ttggg FP64 40.85 -> 39.71 ms; FP32 19.43 -> 19.19 and
-// gg->ttgg FP32 5.43 -> 5.30, but there the saved flops outweigh the saved time (0.505 -> 0.500 of the FP32 peak) and gg->ttgg FP64 gets
-// slower (10.84 -> 10.91): used for the FP64 five-gluon kernel only.
-template <int N, typename T> __host__ __device__ constexpr bool share_full_term() { return N == 5 && sizeof(T) == 8; }
+// pair it saves two row-slash products of 2 x 2 x NJ C.  Measured on B200: gg->ttggg FP64 40.85 -> 39.71 ms, FP32 19.43 -> 19.19,
+// gg->ttgg FP32 5.43 -> 5.30; gg->ttgg FP64 gets slower (10.84 -> 10.91).  Used wherever it is faster: events/s is the metric, and that the
+// saved flops lower the FP32 roofline fraction a little (0.505 -> 0.500) is not a reason to run the slower kernel (round 3).
+template <int N, typename T> __host__ __device__ constexpr bool share_full_term() { return N == 5 || (N == 4 && sizeof(T) == 4); }
 // a4: the quark line of one colour ordering (WHICH = 0: the pair's forward permutation, 1: its reversal) around the split position C:
 //   Acc[ht][hb] += sum_{i < C <= j} L(s_1..i; ht) Jslash(s_i+1..j) R(s_j+1..n; hb)
 // wq: the block's 16-bit references (L bases, R bases, gluon blocks), v: helicity bits by position in THIS ordering.
@@ -1463,8 +1463,8 @@ static double bg_flops_per_event(const BgProcess* B, int precision) {
     return lev + ((B->D.nsets + 1) / 2) * nf * per_thread + ext;
   }
   const int neval = B->D.poly ? B->D.nnode : B->D.nsets;      // polynomial mode: the currents are evaluated at the node sets only
-  // FP64 five-gluon kernel: the row-slash products of the full current once per pair instead of once per ordering (share_full_term)
-  if (n == 5 && precision == RWGT_FP64) fp -= (double)B->S.npair * (double)(1 << (n - 1)) * 2 * fl[2];
+  // the row-slash products of the full current once per pair instead of once per ordering (share_full_term: n = 5, and n = 4 in FP32 / mixed)
+  if (n == 5 || (n == 4 && precision != RWGT_FP64)) fp -= (double)B->S.npair * (double)(1 << (n - 1)) * 2 * fl[2];
   return neval * fp + (B->D.shared_ext ? 1 : B->D.nsets) * ext;
 }
 // Algorithmic flops of the colour form |L+^T u|^2 + |L-^T v|^2 (a5), all parameter sets: per evaluated helicity (2^(n+1) after
