@@ -28,7 +28,7 @@ import numpy as np
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 
-from paper_2312_07440_b200 import events as ev  # noqa: E402
+from paper_2312_07440_b200 import events as ev, sharding  # noqa: E402
 
 # B200 plain-ALU peaks: 148 SMs x 4 SMSP x 16 FP64 (32 FP32) FMA lanes x 2 flop x clock
 SM_COUNT = 148
@@ -387,7 +387,7 @@ def main() -> None:
         barrier()
     clocks = cs.summary()
     total_s = max_over_ranks(sum(res["ms"]) * 1e-3)
-    value = world * n * args.steps / total_s
+    value = sharding.aggregate_throughput([n] * world, args.steps, total_s)      # all ranks' events over the slowest rank's time
     ms_per_step = total_s * 1e3 / args.steps
 
     # ---- e2e: the C-ABI call a user makes with HOST buffers (pinned), copies inside the timed region ----
@@ -404,7 +404,7 @@ def main() -> None:
     for _ in range(e2e_steps):
         B.rwgt_run_host(res["rw"].h, hm, hw, ho[0], ho[1], ho[2], st)     # synchronises the stream itself
     e2e_s = max_over_ranks(time.perf_counter() - t0)
-    e2e_val = world * n * e2e_steps / e2e_s
+    e2e_val = sharding.aggregate_throughput([n] * world, e2e_steps, e2e_s)
     same = bool(np.array_equal(ho, res["out"].cpu().numpy()))
 
     if rank != 0:
@@ -428,8 +428,9 @@ def main() -> None:
     try:
         counts = json.load(open(os.path.join(ROOT, "profiles", "counts.json")))
         ent = counts[f"cfg{c.index}_{args.precision}"]
-        if n == c.n_events:
-            traffic, traffic_build = ent["traffic_bytes"], ent.get("build", counts.get("build"))
+        # the ncu figures describe ONE build of the library: they are reported only when the loaded library is that build
+        if n == c.n_events and ent.get("library_build_id") == B.rwgt_build_id():
+            traffic, traffic_build = ent["traffic_bytes"], ent["library_build_id"]
             if dtype == "f64" and ent.get("fp64_vector_flops_per_launch_ncu"):
                 ncu_fpe = ent["fp64_vector_flops_per_launch_ncu"] / n      # executed DFMA x 2 + DMUL + DADD per event, same capture
     except Exception:

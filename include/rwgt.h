@@ -244,6 +244,11 @@ int rwgt_destroy(rwgt_handle* h);
 /* Thread-local, static storage; never NULL. */
 const char* rwgt_last_error(void);
 
+/* Identity of the build: the first 12 hex digits of the SHA-256 over the library's sources (csrc/*.cu, csrc/*.cuh, include/rwgt.h, in
+ * name order), baked in by paper_2312_07440_b200/build.py; "unknown" for a build made otherwise.  Static storage.  bench.py compares it
+ * with the build id stored beside the ncu counts in profiles/counts.json and drops those figures when the library is another build. */
+const char* rwgt_build_id(void);
+
 /* HOST: writes the n! x n! colour matrix C (row-major, permutations of the gluon labels in
  * lexicographic order) the library uses for a process with n_gluons in 2..5; computed with
  * the SU(3) Fierz identity in exact integer arithmetic.  Returns n! or -1. */

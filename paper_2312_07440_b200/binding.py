@@ -19,7 +19,7 @@ RWGT_MAX_SETS = 16
 RWGT_MAX_PROCESSES = 4
 EXPORTS = ("rwgt_create", "rwgt_create_multi", "rwgt_n_sets", "rwgt_run_multi", "rwgt_run_multi_host", "rwgt_set_precision", "rwgt_n_external", "rwgt_flops_per_event", "rwgt_run",
            "rwgt_run_host", "rwgt_destroy", "rwgt_last_error", "rwgt_colour_matrix", "rwgt_tensor_flops_per_event", "rwgt_sum_weights", "rwgt_run_file",
-           "rwgt_create_multiprocess", "rwgt_n_processes", "rwgt_run_multiprocess", "rwgt_sum_weights_static")
+           "rwgt_create_multiprocess", "rwgt_n_processes", "rwgt_run_multiprocess", "rwgt_sum_weights_static", "rwgt_build_id")
 RWGT_STATIC_SUM_MAX_ROWS = 17
 
 
@@ -57,6 +57,7 @@ def lib():
         L.rwgt_run_host.argtypes = [vp, dp, dp, dp, dp, dp, C.c_longlong, vp]
         L.rwgt_destroy.argtypes = [vp]
         L.rwgt_last_error.restype = C.c_char_p
+        L.rwgt_build_id.restype = C.c_char_p
         L.rwgt_colour_matrix.argtypes = [C.c_int, dp]
         L.rwgt_create_multiprocess.argtypes = [C.c_char_p, C.POINTER(rwgt_params), C.POINTER(rwgt_params), C.c_int]
         L.rwgt_create_multiprocess.restype = vp
@@ -123,6 +124,11 @@ def rwgt_run_multiprocess(h, momenta_ptr: int, weights_ptr: int, process_id: np.
 
 def rwgt_n_sets(h) -> int:
     return lib().rwgt_n_sets(h)
+
+
+def rwgt_build_id() -> str:
+    """SHA-256 prefix of the sources librwgt.so was built from (build.py source_id)."""
+    return lib().rwgt_build_id().decode()
 
 
 def rwgt_set_precision(h, mode) -> None:

@@ -20,6 +20,16 @@ NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a",
               "-Xcompiler", "-fPIC", "-shared", "--fmad=true"]
 
 
+def source_id() -> str:
+    """first 12 hex digits of the SHA-256 over librwgt.so's sources (what rwgt_build_id() returns)"""
+    import hashlib
+    h = hashlib.sha256()
+    srcs, deps = TARGETS[LIB]
+    for f in sorted(srcs + deps, key=os.path.basename):
+        h.update(os.path.basename(f).encode() + b"\0" + open(f, "rb").read())
+    return h.hexdigest()[:12]
+
+
 def up_to_date(lib: str = LIB) -> bool:
     srcs, deps = TARGETS[lib]
     return os.path.exists(lib) and all(os.path.getmtime(lib) >= os.path.getmtime(d) for d in srcs + deps)
@@ -30,7 +40,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
     for lib, (srcs, _) in TARGETS.items():
         if not force and up_to_date(lib):
             continue
-        subprocess.check_call([nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", lib] + srcs)
+        ident = [f'-DRWGT_BUILD_ID="{source_id()}"'] if lib == LIB else []
+        subprocess.check_call([nvcc] + NVCC_FLAGS + ident + (["-Xptxas", "-v"] if verbose else []) + ["-o", lib] + srcs)
     return LIB
 
 

@@ -33,9 +33,7 @@
 #include "../../include/rwgt.h"
 #include "rwgt_math.cuh"
 
-#ifndef RWGT_NBUF_N3
-#define RWGT_NBUF_N3 2
-#endif
+constexpr int RWGT_NBUF_N3 = 2;
 
 namespace rwgt {
 
@@ -376,9 +374,7 @@ template <> struct pair_of<float> { typedef float2 type; };
 template <typename T> __device__ __forceinline__ cx<T> ldc(const cx<T>* p) { typename pair_of<T>::type t = *reinterpret_cast<const typename pair_of<T>::type*>(p); return mk<T>(t.x, t.y); }
 template <typename T> __device__ __forceinline__ void stc(cx<T>* p, cx<T> v) { typename pair_of<T>::type t; t.x = v.re; t.y = v.im; *reinterpret_cast<typename pair_of<T>::type*>(p) = t; }
 
-#ifndef RWGT_STAGE_MIN_N
-#define RWGT_STAGE_MIN_N 4
-#endif
+constexpr int RWGT_STAGE_MIN_N = 4;
 template <typename T> struct Smem {
   uint32_t* W;    // schedule words (whole CTA)
   double* LF;     // Cholesky factors L+^T, L-^T of the colour blocks in mma-fragment order (whole CTA)
@@ -1323,33 +1319,17 @@ static size_t smem_need_n(int n, const BgSched& S, int nslot, bool dbl) {
 // (4.65 -> 4.22 ms) until the one-pass form, whose amplitude threads hold two sets' amplitudes: 8 workers at 224 registers, 21 slots
 // and two buffers 3.32 ms against 3.60 (12 workers, spills to a 28 KB L1) and 3.64 (8 workers, one buffer: the second set's rows wait
 // for the colour form of the first).
-#ifndef RWGT_NW32_N4
-#define RWGT_NW32_N4 12
-#endif
-#ifndef RWGT_NW64_N4
-#define RWGT_NW64_N4 8
-#endif
-#ifndef RWGT_NW32_N3
-#define RWGT_NW32_N3 12
-#endif
-#ifndef RWGT_NW64_N3
-#define RWGT_NW64_N3 8
-#endif
-#ifndef RWGT_NW32_N5
-#define RWGT_NW32_N5 8
-#endif
+constexpr int RWGT_NW32_N4 = 12;
+constexpr int RWGT_NW64_N4 = 8;
+constexpr int RWGT_NW32_N3 = 12;
+constexpr int RWGT_NW64_N3 = 8;
+constexpr int RWGT_NW32_N5 = 8;
 // CTAs per SM at n = 3 (the phases of independent CTAs drift apart and could overlap one CTA's per-group fixed work with another's
 // amplitude phase): measured after the one-pass form, 2 CTAs of 4 + 4 warps 3.93 ms FP64 / 2.18 ms FP32 (8 + 4: 1.99 FP32), 3 CTAs 4.92 / 2.11,
 // against 3.36 / 1.67 for one CTA: the colour warpgroups of the extra CTAs cost more registers and shared memory than the overlap returns
-#ifndef RWGT_CTAS64_N3
-#define RWGT_CTAS64_N3 1
-#endif
-#ifndef RWGT_CTAS32_N3
-#define RWGT_CTAS32_N3 1
-#endif
-#ifndef RWGT_SLOTS32_N5
-#define RWGT_SLOTS32_N5 2
-#endif
+constexpr int RWGT_CTAS64_N3 = 1;
+constexpr int RWGT_CTAS32_N3 = 1;
+constexpr int RWGT_SLOTS32_N5 = 2;
 template <int N, typename T> struct BgCfg { static constexpr int NW = (N == 4) ? (sizeof(T) == 4 ? RWGT_NW32_N4 : RWGT_NW64_N4) : (N == 3) ? (sizeof(T) == 4 ? RWGT_NW32_N3 : RWGT_NW64_N3) : (N == 5 && sizeof(T) == 4) ? RWGT_NW32_N5 : 8, NCW = 4,
                                                         CTAS = (N == 3) ? (sizeof(T) == 4 ? RWGT_CTAS32_N3 : RWGT_CTAS64_N3) : 1; };
 static int bg_nw(int n, bool dbl) { return n == 4 ? (dbl ? BgCfg<4, double>::NW : BgCfg<4, float>::NW) : n == 3 ? (dbl ? BgCfg<3, double>::NW : BgCfg<3, float>::NW) : n == 5 ? (dbl ? BgCfg<5, double>::NW : BgCfg<5, float>::NW) : 8; }

@@ -21,10 +21,8 @@ struct EpemParams { EpemSet set[SMALL_NSMAX]; int nsets; };
 
 // Massless leptons: only the 4 helicity combinations with opposite helicities on each fermion line
 // are non-zero (tests check the oracle's full 16-term sum against this, reading Q5).
-#ifndef RWGT_EPEM_BS
-#define RWGT_EPEM_BS 128
-#define RWGT_EPEM_MINB 6
-#endif
+constexpr int RWGT_EPEM_BS = 128;
+constexpr int RWGT_EPEM_MINB = 6;
 __global__ void __launch_bounds__(RWGT_EPEM_BS, RWGT_EPEM_MINB) epem_mupmum_kernel(const double* __restrict__ mom, const double* __restrict__ wgt,
                                                           double* __restrict__ me_old, double* __restrict__ me_new,
                                                           double* __restrict__ w_new, long long n, long long stride, long long ostride, EpemParams P) {
@@ -126,10 +124,8 @@ __device__ __forceinline__ void ggttx_sums(const double (*p)[4], double m, doubl
 
 // 168 registers with ~1.3 KB of spills at 12 warps per SM beats 254 registers without spills at 8 warps (0.171 -> 0.150 ms for 2^20 events):
 // the kernel is bound by dependent-issue latency (sqrt / division chains), not by the L1-resident spill traffic
-#ifndef RWGT_GGTTX_BS
-#define RWGT_GGTTX_BS 128
-#define RWGT_GGTTX_MINB 3
-#endif
+constexpr int RWGT_GGTTX_BS = 128;
+constexpr int RWGT_GGTTX_MINB = 3;
 constexpr int GGTTX_BS = RWGT_GGTTX_BS;
 __global__ void __launch_bounds__(RWGT_GGTTX_BS, RWGT_GGTTX_MINB) gg_ttx_kernel(const double* __restrict__ mom, const double* __restrict__ wgt, const int* __restrict__ idx,
                                                      double* __restrict__ me_old, double* __restrict__ me_new,

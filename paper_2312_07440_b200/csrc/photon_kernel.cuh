@@ -286,18 +286,10 @@ static double photon_flops_per_event(int ng) {
 // 96: 0.309, 192: 0.299, 256: 0.32, register-limited to 3 CTAs); 2 CTAs of 16 events x 320 threads 0.265 (288: 0.303, 352: 0.286, 384: 0.284);
 // 4 events per CTA (a quarter-warp then holds two tasks, conflicts return): 0.33-0.41; warp-private groups of 8 events (no CTA barriers, four
 // warps per SM fit): 0.37-0.43; three variant bits at level 4: 0.28-0.37.
-#ifndef RWGT_PH_E
-#define RWGT_PH_E 16
-#endif
-#ifndef RWGT_PH_NTH
-#define RWGT_PH_NTH 320
-#endif
-#ifndef RWGT_PH_VB
-#define RWGT_PH_VB 22
-#endif
-#ifndef RWGT_PH_VBF
-#define RWGT_PH_VBF 1
-#endif
+constexpr int RWGT_PH_E = 16;
+constexpr int RWGT_PH_NTH = 320;
+constexpr int RWGT_PH_VB = 22;
+constexpr int RWGT_PH_VBF = 1;
 constexpr int PH_E = RWGT_PH_E, PH_NTH = RWGT_PH_NTH, PH_CG = RWGT_PH_NTH, PH_VB = RWGT_PH_VB, PH_VBF = RWGT_PH_VBF;
 template <int NG> constexpr size_t photon_smem() { return sizeof(double) * (PH_NTH / PH_CG) * PH_E * PhGeo<NG>::SLOT; }
 // once per handle at rwgt_create, on the handle's device (the attribute belongs to the device's copy of the function)

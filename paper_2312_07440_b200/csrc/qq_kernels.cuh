@@ -124,10 +124,8 @@ __device__ __forceinline__ void qq_sums(const double (*p)[4], double m, const QQ
 
 // CTAs of 128 per SM: without the gluon 6 (80 registers, small spills) 0.062 ms for 2^20 events against 0.074 at 140 registers / 3 CTAs
 // (4: 0.064, 8: 0.073); with the gluon the unconstrained 255 registers win (0.339; 168 registers 0.378, 128: 0.472, 96: 0.727)
-#ifndef RWGT_QQ0_MINB
-#define RWGT_QQ0_MINB 6
-#define RWGT_QQ1_MINB 1
-#endif
+constexpr int RWGT_QQ0_MINB = 6;
+constexpr int RWGT_QQ1_MINB = 1;
 template <int NG>
 __global__ void __launch_bounds__(128, NG ? RWGT_QQ1_MINB : RWGT_QQ0_MINB) qqx_ttx_kernel(const double* __restrict__ mom, const double* __restrict__ wgt, const int* __restrict__ idx,
                                                       double* __restrict__ me_old, double* __restrict__ me_new, double* __restrict__ w_new,

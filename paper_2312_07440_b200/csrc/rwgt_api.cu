@@ -139,6 +139,11 @@ extern "C" {
 
 const char* rwgt_last_error(void) { return g_err; }
 
+#ifndef RWGT_BUILD_ID
+#define RWGT_BUILD_ID "unknown"
+#endif
+const char* rwgt_build_id(void) { return RWGT_BUILD_ID; }
+
 rwgt_handle* rwgt_create_multi(const char* process, const rwgt_params* params_old, const rwgt_params* params_new, int n_new) {
   if (!process || !params_old || !params_new) { set_err("rwgt_create: NULL argument"); return nullptr; }
   if (n_new < 1 || n_new > RWGT_MAX_SETS) { set_err("rwgt_create: number of new parameter sets must be in 1..RWGT_MAX_SETS"); return nullptr; }
@@ -275,7 +280,7 @@ static int launch_events(rwgt_handle* h, const double* momenta, const double* we
   if (idx && (h->proc == P_EPEM || h->proc == P_PHOTONS)) { set_err("rwgt_run: this process cannot be part of a multiprocess handle"); return -1; }
   if (h->proc == P_EPEM) {
     // small event sets (cfg 1 has 16,384): 64-thread CTAs, so that the grid covers all SMs (256 CTAs instead of 64 on 148 SMs)
-    int bs = (n < 512LL * h->sm_count) ? 64 : RWGT_EPEM_BS; long long nb = (n + bs - 1) / bs;
+    int bs = (n < 512LL * h->sm_count) ? 64 : rwgt::RWGT_EPEM_BS; long long nb = (n + bs - 1) / bs;
     rwgt::epem_mupmum_kernel<<<(unsigned)nb, bs, 0, st>>>(momenta, weights, out_me_old, out_me_new, out_w_new, n, stride, ostride, h->epem);
   } else if (h->proc == P_GG_TTX) {
     int bs = h->nsets == 2 ? rwgt::GGTTX_BS : 128; long long nb = (n + bs - 1) / bs;
